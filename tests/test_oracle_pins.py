@@ -1,0 +1,417 @@
+"""Pins for the CPU oracle (-m "not gpu").  Each test checks the oracle against
+something the paper or the mathematics fixes, never against itself:
+known-answer vectors, closed forms, exact enumeration, Onsager, invariants.
+Citations are PAPER.md lines; R-numbers are DESIGN.md readings.
+"""
+import itertools
+import math
+import os
+from decimal import Decimal, getcontext
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+
+ISING, BC = oracle.ISING, oracle.BLUME_CAPEL
+
+
+def _pins(golden_dir, name):
+    out = {}
+    with open(os.path.join(golden_dir, name)) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                k, v = line.split()
+                out[k] = float(v)
+    return out
+
+
+# ------------------------------------------------------------------ Philox ---
+def test_philox_known_answers(golden_dir):
+    """PAPER.md:149 names Philox4_32_10; rows = published KAT + SURVEY's keyed values."""
+    n = 0
+    with open(os.path.join(golden_dir, "philox4x32_10_kat.txt")) as f:
+        for line in f:
+            if not line.strip() or line.startswith("#"):
+                continue
+            v = [int(t, 16) for t in line.split()]
+            got = oracle.philox4x32_10(v[0:4], v[4:6])
+            assert [int(x) for x in got] == v[6:10], line
+            n += 1
+    assert n == 7
+
+
+def test_draw_keying():
+    """R3: ctr = (g_lo, g_hi, t, tag), key = seed, word n & 3, g = n >> 2."""
+    seed = 0x0123456789ABCDEF
+    for n, t, tag in [(0, 0, 0), (7, 3, 1), ((1 << 34) + 5, 199, 0), ((1 << 35) - 1, 0, 3)]:
+        g = n >> 2
+        blk = oracle.philox4x32_10([g & 0xFFFFFFFF, g >> 32, t, tag],
+                                   [seed & 0xFFFFFFFF, seed >> 32])
+        assert oracle.draw(seed, n, t, tag) == int(blk[n & 3])
+    # four consecutive sites share one call; the fifth starts a new one
+    a = [oracle.draw(1, n, 7, 1) for n in range(20, 24)]
+    assert a == [int(x) for x in oracle.philox4x32_10([5, 0, 7, 1], [1, 0])]
+
+
+# -------------------------------------------------------------- thresholds ---
+def test_ising_thresholds_closed_form_at_beta_c():
+    """e^{-4 beta}, e^{-8 beta}; at beta_c they are 3-2*sqrt2 and 17-12*sqrt2.
+    floor(2^32 * (3 - 2 sqrt2)) and floor(2^32 (17 - 12 sqrt2)) in exact integer arithmetic."""
+    t4 = 3 * 2**32 - math.isqrt(2**67) - 1          # 2^33 sqrt2 = sqrt(2^67), irrational
+    t8 = 17 * 2**32 - math.isqrt(288 * 2**64) - 1   # 12 sqrt2 2^32 = sqrt(288 2^64)
+    T = oracle.thresholds(ISING, wl.BETA_C)
+    assert (t4, t8) == (736899888, 126432032)
+    assert [int(x) for x in T] == [2**32, 2**32, 2**32, t4, t8]
+
+
+def _exact_T(beta: float, dE: float) -> int:
+    """floor(min(1, exp(-beta dE)) 2^32) with 60-digit decimal arithmetic (independent of libm)."""
+    getcontext().prec = 60
+    x = -(Decimal(float(beta)) * Decimal(float(dE)))
+    if x >= 0:
+        return 2**32
+    return int((x.exp() * Decimal(2**32)).to_integral_value(rounding="ROUND_FLOOR"))
+
+
+@pytest.mark.parametrize("tau", [1.0, 0.5, 0.9, 1.5])
+def test_ising_thresholds_high_precision(tau):
+    beta = wl.BETA_C / tau
+    T = oracle.thresholds(ISING, beta)
+    assert [int(x) for x in T] == [_exact_T(beta, dE) for dE in (-8, -4, 0, 4, 8)]
+
+
+def test_ising_threshold_values_of_the_configs():
+    """Values printed in SURVEY.md Sec. 8(c) for configs 1-3."""
+    assert [int(x) for x in oracle.thresholds(ISING, wl.BETA_C / 0.5)[3:]] == [126432032, 3721811]
+    assert [int(x) for x in oracle.thresholds(ISING, wl.BETA_C / 0.9)[3:]] == [605825050, 85454432]
+
+
+def test_bc_thresholds():
+    """Eq. 2: dE = D dq - ds h; proposal R8; sign of D R10."""
+    beta, D = 1.0 / 1.4, 1.0
+    T = oracle.thresholds(BC, beta, D).reshape(3, 2, 9)
+    by_dE = {1: 2102565417, 2: 1029293363, 3: 503881981, 4: 246671221, 5: 120755839,
+             6: 59115013, 8: 14166974}
+    for s, b, h in itertools.product((-1, 0, 1), (0, 1), range(-4, 5)):
+        sp = {(-1, 0): 0, (-1, 1): 1, (0, 0): 1, (0, 1): -1, (1, 0): -1, (1, 1): 0}[(s, b)]
+        # energy difference straight from the Hamiltonian of a single site in field h
+        dE = (-(sp * h) + D * sp * sp) - (-(s * h) + D * s * s)
+        want = _exact_T(beta, dE)
+        assert int(T[s + 1, b, h + 4]) == want, (s, b, h)
+        if dE > 0 and float(dE).is_integer() and int(dE) in by_dE:
+            assert want == by_dE[int(dE)]
+    # worked examples quoted in SURVEY.md
+    assert int(T[0, 0, 0]) == by_dE[3] and int(T[2, 0, 8]) == by_dE[8] and int(T[1, 1, 8]) == by_dE[5]
+
+
+def test_thresholds_beta_zero_and_large():
+    assert all(int(x) == 2**32 for x in oracle.thresholds(ISING, 0.0))       # R21
+    T = oracle.thresholds(ISING, 50.0)
+    assert int(T[3]) == 0 and int(T[4]) == 0 and int(T[2]) == 2**32          # never / always (R7)
+
+
+# -------------------------------------------------------------------- init ---
+def test_init_mapping_and_statistics():
+    """R11: Ising top bit; BC (3 r) >> 32.  Uniformity within 5 sigma."""
+    L, seed = 128, 1
+    s = oracle.init(ISING, L, seed)
+    assert set(np.unique(s)) == {-1, 1}
+    assert abs(int(s.sum())) < 5 * L
+    for (x, y) in [(0, 0), (1, 0), (5, 7), (127, 127), (64, 3)]:
+        c = (x + y) & 1
+        r = oracle.draw(seed, y * (L // 2) + (x >> 1), 0, 2 + c)
+        assert s[y, x] == (1 if r >> 31 else -1)
+    b = oracle.init(BC, L, seed)
+    assert set(np.unique(b)) == {-1, 0, 1}
+    for v in (-1, 0, 1):
+        assert abs((b == v).sum() - L * L / 3) < 5 * math.sqrt(L * L * 2 / 9)
+    x, y = 9, 4
+    r = oracle.draw(seed, y * (L // 2) + (x >> 1), 0, 2 + ((x + y) & 1))
+    assert b[y, x] == (r * 3 >> 32) - 1
+
+
+# ------------------------------------------------------------- observables ---
+def test_observables_closed_forms():
+    """Eq. 1 / Eq. 2 on crafted lattices (each bond once: 2N bonds)."""
+    L = 16
+    N = L * L
+    up = np.ones((L, L), np.int8)
+    assert oracle.observables(up) == (2 * N, N, N)
+    yy, xx = np.mgrid[0:L, 0:L]
+    neel = np.where((xx + yy) % 2 == 0, 1, -1).astype(np.int8)
+    assert oracle.observables(neel) == (-2 * N, 0, N)
+    one = up.copy()
+    one[3, 5] = -1
+    assert oracle.observables(one) == (2 * N - 8, N - 2, N)
+    zero = np.zeros((L, L), np.int8)
+    assert oracle.observables(zero) == (0, 0, 0)
+    E, e, m, z = oracle.normalised(BC, L, 1.0, oracle.observables(up))
+    assert E == -2 * N + 1.0 * N and e == E / N and m == 1.0 and z == 0.0
+    stripes = np.where((xx // 4) % 2 == 0, 1, -1).astype(np.int8)      # vertical stripes width 4
+    # horizontal bonds: per row L/4 walls -> (L - 2 L/4) ; vertical bonds all +1
+    assert oracle.observables(stripes) == (N + (L - 2 * (L // 4)) * L, 0, N)
+
+
+@pytest.mark.parametrize("model,L,beta,D", [(ISING, 32, wl.BETA_C, 0.0), (BC, 32, 1 / 1.4, 1.0),
+                                            (BC, 9, 0.9, 0.5), (ISING, 7, 0.3, 0.0)])
+def test_tally_equals_recompute(model, L, beta, D):
+    """Invariant named by north_star: incremental dE tally == full recompute of H."""
+    s = oracle.init(model, L, 3)
+    tl = oracle.observables(s)
+    for t in range(40):
+        tl = oracle.sweep(model, s, beta, D, 3, t, tl)
+        assert tl == oracle.observables(s)
+        if model == ISING:
+            assert tl[2] == L * L and set(np.unique(s)) <= {-1, 1}
+        else:
+            assert set(np.unique(s)) <= {-1, 0, 1}
+
+
+def test_sweep_is_one_site_rule_bruteforce():
+    """Re-derive one sweep on a tiny lattice with python ints straight from
+    Eq. 1 energies (dE by recomputing H before/after), in the oracle's visiting order."""
+    L, beta, seed = 6, 0.4, 11
+    s = oracle.init(ISING, L, seed)
+    ref = s.astype(int).copy()
+
+    def H(a):
+        return -sum(a[y][x] * (a[y][(x + 1) % L] + a[(y + 1) % L][x]) for y in range(L) for x in range(L))
+
+    for t in range(3):
+        for c in (0, 1):
+            for y in range(L):
+                for x in range(L):
+                    if (x + y) % 2 != c:
+                        continue
+                    e0 = H(ref)
+                    ref[y][x] *= -1
+                    dE = H(ref) - e0
+                    r = oracle.draw(seed, y * (L // 2) + x // 2, t, c)
+                    if not r < _exact_T(beta, dE):
+                        ref[y][x] *= -1
+        oracle.sweep(ISING, s, beta, 0.0, seed, t)
+        assert (s == ref).all()
+
+
+def test_bc_sweep_bruteforce():
+    L, beta, D, seed = 6, 0.7, 0.8, 5
+    s = oracle.init(BC, L, seed)
+    ref = s.astype(int).copy()
+
+    def H(a):
+        return (-sum(a[y][x] * (a[y][(x + 1) % L] + a[(y + 1) % L][x]) for y in range(L) for x in range(L))
+                + D * sum(a[y][x] ** 2 for y in range(L) for x in range(L)))
+
+    others = {-1: (0, 1), 0: (1, -1), 1: (-1, 0)}        # cyclic in the code s+1 (R8)
+    for t in range(3):
+        for c in (0, 1):
+            for y in range(L):
+                for x in range(L):
+                    if (x + y) % 2 != c:
+                        continue
+                    r = oracle.draw(seed, y * (L // 2) + x // 2, t, c)
+                    old = ref[y][x]
+                    h = ref[(y - 1) % L][x] + ref[(y + 1) % L][x] + ref[y][(x - 1) % L] + ref[y][(x + 1) % L]
+                    new = others[old][r & 1]
+                    dE = (-(new * h) + D * new * new) - (-(old * h) + D * old * old)
+                    e0 = H(ref)
+                    ref[y][x] = new
+                    assert abs((H(ref) - e0) - dE) < 1e-9
+                    if not r < _exact_T(beta, dE):
+                        ref[y][x] = old
+        oracle.sweep(BC, s, beta, D, seed, t)
+        assert (s == ref).all()
+
+
+# ------------------------------------------------------- exact enumeration ---
+def _enumerate(L, values, beta, D):
+    """Exact <E>, <E^2>, <|M|>, <M^2>, <Q>, <B> by brute force over values^(L*L) states."""
+    n = L * L
+    k = len(values)
+    head = min(n, 4 if k == 3 and n > 9 else 0)
+    tail = n - head
+    idx = np.arange(k**tail, dtype=np.int64)
+    tail_spins = np.empty((tail, idx.size), dtype=np.int8)
+    for i in range(tail):
+        tail_spins[i] = np.asarray(values, dtype=np.int8)[(idx // k**i) % k]
+    Z = 0.0
+    acc = np.zeros(6)
+    for hv in itertools.product(values, repeat=head):
+        sp = np.empty((n, idx.size), dtype=np.int8)
+        for i, v in enumerate(hv):
+            sp[i] = v
+        sp[head:] = tail_spins
+        g = sp.reshape(L, L, -1).astype(np.int32)
+        B = (g * (np.roll(g, -1, axis=1) + np.roll(g, -1, axis=0))).sum(axis=(0, 1))
+        M = g.sum(axis=(0, 1))
+        Q = (g * g).sum(axis=(0, 1))
+        E = -B + D * Q
+        w = np.exp(-beta * (E - (-2.0 * n)))
+        Z += w.sum()
+        for j, o in enumerate((E, E * E, np.abs(M), M * M, Q, B)):
+            acc[j] += (w * o).sum()
+    return acc / Z
+
+
+def _mc_mean(model, L, beta, D, n_seeds, burn, meas):
+    """Per-seed time averages of (E, |M|, Q, B) -> mean and standard error across seeds."""
+    rows = []
+    tr = np.zeros(3 * (burn + meas), dtype=np.int64)
+    import ctypes as C
+    lib = oracle.lib()
+    for seed in range(1, n_seeds + 1):
+        s = oracle.init(model, L, seed)
+        tl = np.asarray(oracle.observables(s), dtype=np.int64)
+        lib.orc_run(C.c_int(model), C.c_int64(L), C.c_double(beta), C.c_double(D), C.c_uint64(seed),
+                    C.c_uint32(0), C.c_int64(burn + meas), s.ctypes.data_as(C.POINTER(C.c_int8)),
+                    tl.ctypes.data_as(C.POINTER(C.c_int64)), tr.ctypes.data_as(C.POINTER(C.c_int64)))
+        t = tr.reshape(-1, 3)[burn:]
+        B, M, Q = t[:, 0], t[:, 1], t[:, 2]
+        E = -B + D * Q
+        rows.append([E.mean(), np.abs(M).mean(), Q.mean(), B.mean()])
+    rows = np.asarray(rows)
+    return rows.mean(axis=0), rows.std(axis=0, ddof=1) / math.sqrt(n_seeds)
+
+
+def test_ising_4x4_exact_enumeration(golden_dir):
+    """north_star: long-run <E> vs the exact partition function, 5 standard errors."""
+    pins = _pins(golden_dir, "exact_pins.txt")
+    ex = _enumerate(4, (-1, 1), wl.BETA_C, 0.0)
+    assert abs(ex[0] - pins["ising4x4_betac_E"]) < 1e-7 and abs(ex[1] - pins["ising4x4_betac_E2"]) < 1e-6
+    assert abs(ex[2] - pins["ising4x4_betac_absM"]) < 1e-7 and abs(ex[3] - pins["ising4x4_betac_M2"]) < 1e-6
+    mean, se = _mc_mean(ISING, 4, wl.BETA_C, 0.0, 1024, 100, 400)
+    assert abs(mean[0] - ex[0]) < 5 * se[0], (mean, se, ex)
+    assert abs(mean[1] - ex[2]) < 5 * se[1], (mean, se, ex)
+    assert se[0] < 0.05                                     # the test has power
+
+
+def test_ising_4x4_exact_enumeration_low_T(golden_dir):
+    pins = _pins(golden_dir, "exact_pins.txt")
+    beta = wl.BETA_C / 0.9
+    ex = _enumerate(4, (-1, 1), beta, 0.0)
+    assert abs(ex[0] - pins["ising4x4_beta0.9Tc_E"]) < 1e-7
+    assert abs(ex[2] - pins["ising4x4_beta0.9Tc_absM"]) < 1e-7
+    mean, se = _mc_mean(ISING, 4, beta, 0.0, 1024, 100, 400)
+    assert abs(mean[0] - ex[0]) < 5 * se[0] and abs(mean[1] - ex[2]) < 5 * se[1], (mean, se, ex)
+
+
+def test_bc_3x3_exact_enumeration(golden_dir):
+    """3x3 Blume-Capel, beta = 1/1.4, D = 1 (odd L: sequential in-place sweep, R 'O4')."""
+    pins = _pins(golden_dir, "exact_pins.txt")
+    beta, D = 1 / 1.4, 1.0
+    ex = _enumerate(3, (-1, 0, 1), beta, D)
+    assert abs(ex[0] - pins["bc3x3_E"]) < 1e-7 and abs(ex[4] - pins["bc3x3_Q"]) < 1e-7
+    assert abs(ex[2] - pins["bc3x3_absM"]) < 1e-7 and abs(ex[5] - pins["bc3x3_B"]) < 1e-7
+    mean, se = _mc_mean(BC, 3, beta, D, 1024, 100, 400)
+    for j, k in ((0, 0), (1, 2), (2, 4), (3, 5)):
+        assert abs(mean[j] - ex[k]) < 5 * se[j], (mean, se, ex)
+
+
+def test_bc_4x4_exact_enumeration(golden_dir):
+    """4x4 Blume-Capel (even L: the real checkerboard semantics), 3^16 states."""
+    pins = _pins(golden_dir, "exact_pins.txt")
+    beta, D = 1 / 1.4, 1.0
+    ex = _enumerate(4, (-1, 0, 1), beta, D)
+    assert abs(ex[0] - pins["bc4x4_E"]) < 1e-7 and abs(ex[4] - pins["bc4x4_Q"]) < 1e-7
+    assert abs(ex[2] - pins["bc4x4_absM"]) < 1e-7
+    mean, se = _mc_mean(BC, 4, beta, D, 1024, 100, 400)
+    for j, k in ((0, 0), (1, 2), (2, 4), (3, 5)):
+        assert abs(mean[j] - ex[k]) < 5 * se[j], (mean, se, ex)
+
+
+# ------------------------------------------------------------------ Onsager ---
+def _onsager_u(beta):
+    from scipy.special import ellipk
+    k = 2 * math.sinh(2 * beta) / math.cosh(2 * beta) ** 2
+    return -(1 / math.tanh(2 * beta)) * (1 + (2 / math.pi) * (2 * math.tanh(2 * beta) ** 2 - 1) * ellipk(k * k))
+
+
+def _onsager_m0(beta):
+    return (1 - math.sinh(2 * beta) ** -4) ** 0.125
+
+
+def _blocked(x, nb=20):
+    b = np.asarray(x, dtype=float)[: len(x) // nb * nb].reshape(nb, -1).mean(axis=1)
+    return b.mean(), b.std(ddof=1) / math.sqrt(nb)
+
+
+def test_onsager_closed_form_values(golden_dir):
+    pins = _pins(golden_dir, "exact_pins.txt")
+    assert abs(_onsager_u(wl.BETA_C / 0.9) - pins["onsager_0.9Tc_u"]) < 1e-7
+    assert abs(_onsager_m0(wl.BETA_C / 0.9) - pins["onsager_0.9Tc_m0"]) < 1e-7
+    assert abs(_onsager_u(wl.BETA_C / 0.5) - pins["onsager_0.5Tc_u"]) < 1e-7
+    assert abs(_onsager_m0(wl.BETA_C / 0.5) - pins["onsager_0.5Tc_m0"]) < 1e-7
+    assert abs(_onsager_u(wl.BETA_C / 1.5) - pins["onsager_1.5Tc_u"]) < 1e-7
+
+
+def _run_trace(model, s, beta, D, seed, n):
+    import ctypes as C
+    tr = np.zeros(3 * n, dtype=np.int64)
+    tl = np.asarray(oracle.observables(s), dtype=np.int64)
+    oracle.lib().orc_run(C.c_int(model), C.c_int64(s.shape[0]), C.c_double(beta), C.c_double(D),
+                         C.c_uint64(seed), C.c_uint32(0), C.c_int64(n),
+                         s.ctypes.data_as(C.POINTER(C.c_int8)), tl.ctypes.data_as(C.POINTER(C.c_int64)),
+                         tr.ctypes.data_as(C.POINTER(C.c_int64)))
+    return tr.reshape(-1, 3)
+
+
+def test_onsager_energy_hot_phase():
+    """L = 256, random start at 1.5 Tc: u -> Onsager's exact energy (xi ~ 2 sites)."""
+    L, beta = 256, wl.BETA_C / 1.5
+    s = oracle.init(ISING, L, 2)
+    tr = _run_trace(ISING, s, beta, 0.0, 2, 300 + 1500)[300:]
+    u, se = _blocked(-tr[:, 0] / (L * L))
+    assert abs(u - _onsager_u(beta)) < 5 * se + 2e-4, (u, se, _onsager_u(beta))
+    assert se < 2e-3
+
+
+def test_onsager_energy_and_magnetisation_ordered_phase():
+    """L = 256, cold start (all +1) at 0.9 Tc: u and <|m|> -> Onsager / Yang."""
+    L, beta = 256, wl.BETA_C / 0.9
+    s = np.ones((L, L), np.int8)
+    tr = _run_trace(ISING, s, beta, 0.0, 4, 500 + 2500)[500:]
+    u, se_u = _blocked(-tr[:, 0] / (L * L))
+    m, se_m = _blocked(np.abs(tr[:, 1]) / (L * L))
+    assert abs(u - _onsager_u(beta)) < 5 * se_u + 2e-4, (u, se_u, _onsager_u(beta))
+    assert abs(m - _onsager_m0(beta)) < 5 * se_m + 2e-4, (m, se_m, _onsager_m0(beta))
+    assert se_u < 2e-3 and se_m < 2e-3
+
+
+# --------------------------------------------------------- Schwinger-Dyson ---
+def test_schwinger_dyson_identity():
+    """Eq. 3: (1/N) sum <exp(-2 beta sigma h)> = 1 in equilibrium."""
+    L, beta = 64, 0.35
+    s = oracle.init(ISING, L, 9)
+    tl = oracle.observables(s)
+    vals = []
+    for t in range(600):
+        tl = oracle.sweep(ISING, s, beta, 0.0, 9, t, tl)
+        if t >= 100:
+            v, hist = oracle.schwinger_dyson(s, beta)
+            assert hist.sum() == L * L and hist[1::2].sum() == 0       # sigma*h is even for Ising
+            vals.append(v)
+    mean, se = _blocked(vals)
+    assert abs(mean - 1.0) < 5 * se, (mean, se)
+    assert se < 2e-3
+    # closed forms: all +1 -> every site sigma*h = 4
+    v, hist = oracle.schwinger_dyson(np.ones((8, 8), np.int8), 0.2)
+    assert hist[8] == 64 and abs(v - math.exp(-1.6)) < 1e-15
+
+
+def test_schwinger_dyson_bc():
+    L, beta, D = 48, 0.5, 1.0            # T = 2: disordered phase, short correlations
+    s = oracle.init(BC, L, 5)
+    tl = oracle.observables(s)
+    vals = []
+    for t in range(700):
+        tl = oracle.sweep(BC, s, beta, D, 5, t, tl)
+        if t >= 200:
+            vals.append(oracle.schwinger_dyson(s, beta)[0])
+    mean, se = _blocked(vals)
+    # sigma -> -sigma leaves the Delta*sigma^2 term of Eq. 2 unchanged, so the local
+    # identity sum_sigma w(sigma) exp(-2 beta sigma h) = sum_sigma w(-sigma) holds
+    # exactly in equilibrium ("straightforwardly extends").
+    assert abs(mean - 1.0) < 5 * se, (mean, se)
+    assert se < 3e-3
