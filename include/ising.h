@@ -1,0 +1,160 @@
+/*
+ * include/ising.h -- C ABI of the B200-native checkerboard Metropolis engine
+ * (hot path of arxiv 2502.18624, Bisson et al.; citations are PAPER.md lines).
+ *
+ * One handle = one periodic L x L lattice resident in HBM, stored as two
+ * colour arrays ("two separate buffers arranged in a checkerboard
+ * pattern"), 4 bits per spin, 16 spins per 64-bit word (PAPER.md:57, 93
+ * "Multiple Spin Coding ... four bits per spin"; the 4-bit store is what the
+ * paper keeps for Blume-Capel).
+ *
+ *   site (x, y): x = column, y = row, 0 <= x, y < L, periodic
+ *   colour c = (x + y) & 1; colour 0 ("black") is updated first in a sweep
+ *   inside a colour: k = x >> 1, word m = k >> 4, nibble j = k & 15
+ *   colour array = L rows x (L / 32) uint64 words, row-major
+ *   nibble value: Ising 1 = spin +1, 0 = spin -1;  Blume-Capel s + 1 in {0,1,2}
+ *   colour-site index n = y * (L/2) + k (64 bit) keys the random numbers:
+ *   r(n) = word (n & 3) of Philox4x32-10(ctr = (g_lo, g_hi, t, tag), key = seed),
+ *   g = n >> 2, t = sweep number, tag = colour (update) or 2 + colour (init).
+ *
+ * Pointers: every pointer argument is a HOST pointer unless its name starts
+ * with dev_.  All calls return ISING_OK (0) or a negative error; outputs are
+ * written only on ISING_OK.  Nothing throws or aborts.  ising_last_error()
+ * gives a thread-local message for the last non-OK return on this thread.
+ * A handle is not thread-safe; distinct handles are independent.  Work is
+ * enqueued on the stream given at create; calls documented as "synchronises"
+ * block until that stream has drained.
+ */
+#ifndef ISING_B200_H
+#define ISING_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ising_sim ising_t; /* opaque */
+
+enum { ISING_MODEL_ISING = 0, ISING_MODEL_BLUME_CAPEL = 1 };
+enum { ISING_OK = 0, ISING_EINVAL = -1, ISING_ENOMEM = -2, ISING_ECUDA = -3 };
+
+/* Integer observables are the bit-exact contract; the doubles are formed on
+ * the host from them with one operation each (Eq. 1, Eq. 2):
+ * E = -bond_sum (Ising) or -bond_sum + D*Q (Blume-Capel), J = 1.            */
+typedef struct {
+    int64_t bond_sum;     /* B = sum over the 2N nearest-neighbour bonds of s_x s_y */
+    int64_t M;            /* sum of spins                                            */
+    int64_t Q;            /* sum of squared spins (= N for Ising)                    */
+    int64_t n_sites;      /* N = L*L                                                 */
+    uint64_t sweeps_done; /* t                                                       */
+    double E, e_per_site, m_per_site, zero_density;
+} ising_obs_t;
+
+/* Device bytes a caller-provided buffer must have for (model, L): the two
+ * colour arrays (L*L/2 bytes) plus a small fixed scratch area.  0 if (model, L)
+ * is invalid.                                                               */
+size_t ising_workspace_bytes(int model, int64_t L);
+
+/* Create a simulation (PAPER.md:25 problem statement; Eq. 1 / Eq. 2).
+ *   model       ISING_MODEL_*
+ *   L           linear size, multiple of 64, >= 64 (one 128-bit vector = 32
+ *               same-colour sites of a row)
+ *   beta        1/(k_B T) >= 0, finite;  D = crystal field Delta of Eq. 2
+ *               (finite; ignored for Ising);  seed = Philox key
+ *   dev_buf     device memory of >= ising_workspace_bytes() bytes, 256-byte
+ *               aligned, owned by the caller and alive until ising_destroy;
+ *               NULL: the library allocates (cudaMalloc) and frees it
+ *   cuda_stream a cudaStream_t (e.g. torch's current stream); NULL = default
+ * Builds the acceptance thresholds floor(min(1, exp(-beta dE)) 2^32) in double
+ * (PAPER.md:93 for the Ising probabilities), fills the lattice from the seed
+ * (Ising: top bit of r; Blume-Capel: (3 r) >> 32), sets t = 0.  Asynchronous. */
+int ising_create(int model, int64_t L, double beta, double D, uint64_t seed,
+                 void *dev_buf, size_t dev_bytes, void *cuda_stream, ising_t **out);
+
+/* n >= 0 full sweeps: colour 0 then colour 1 ("two update phases"),
+ * one Philox number per site, accept iff r < T.  Asynchronous:
+ * 2n kernel launches on the handle's stream, no host synchronisation.       */
+int ising_sweep(ising_t *h, int64_t n);
+
+/* Full recompute of B, M, Q by warp-shuffle / block reduction over both colour
+ * arrays.  Synchronises.                                                    */
+int ising_observables(ising_t *h, ising_obs_t *out);
+
+/* Full-source pair sums: sx[r-1] = sum_{x,y} s(x,y) s(x+r,y),
+ * sy[r-1] = sum_{x,y} s(x,y) s(x,y+r), periodic, r = 1..rmax, 1 <= rmax <= L/2.
+ * Host arrays of length rmax.  Synchronises.                                */
+int ising_correlation(ising_t *h, int64_t rmax, int64_t *sx, int64_t *sy);
+
+/* The paper's down-sampled protocol at t = sweeps_done:
+ * all sources for r <= 32; sources {x % 16 == 0, y % 16 == 0} for 32 < r <=
+ * r_c(t) and for r on the logarithmic grid up to L/2.  Arrays of capacity cap;
+ * *count receives the number of distances (also when cap is too small, with
+ * ISING_EINVAL).  Synchronises.                                             */
+int ising_correlation_protocol(ising_t *h, int64_t cap, int64_t *r, int64_t *sx, int64_t *sy,
+                               int64_t *n_src, int64_t *count);
+
+/* Same sums for an explicit strictly positive distance list (each <= L/2) and
+ * a source stride (sources x % stride == 0 and y % stride == 0; stride 1 or a
+ * power of two <= 64).  Synchronises.                                        */
+int ising_correlation_list(ising_t *h, int64_t stride, int64_t count, const int64_t *r,
+                           int64_t *sx, int64_t *sy);
+
+/* Schwinger-Dyson check (Eq. 3): hist[k+4] = number of sites with
+ * s_x h_x = k, k = -4..4; *value = (1/N) sum_k hist[k+4] exp(-2 beta k).
+ * Synchronises.                                                             */
+int ising_schwinger_dyson(ising_t *h, int64_t hist[9], double *value);
+
+/* Unpack rows [y0, y0+ny) to int8 spins, row-major ny x L (host).  Synchronises. */
+int ising_read_lattice(ising_t *h, int64_t y0, int64_t ny, int8_t *host_out);
+/* Unpack the w x hgt window whose top-left site is (x0, y0); coordinates wrap
+ * (any integer x0, y0; 1 <= w, hgt <= L).  Synchronises.                     */
+int ising_read_window(ising_t *h, int64_t x0, int64_t y0, int64_t w, int64_t hgt, int8_t *host_out);
+/* Overwrite rows [y0, y0+ny) from int8 spins (values outside the model's set
+ * give ISING_EINVAL and leave the lattice unchanged).  Synchronises.         */
+int ising_write_lattice(ising_t *h, int64_t y0, int64_t ny, const int8_t *host_in);
+
+/* Raw packed colour array <-> host: words [word0, word0 + nwords) of colour
+ * c (row-major L x L/32).  For checkpoints and the end-to-end benchmark.    */
+int ising_read_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, uint64_t *host_out);
+int ising_write_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, const uint64_t *host_in);
+/* Set the sweep counter t (exact resume: state = lattice + t).               */
+int ising_set_sweeps_done(ising_t *h, uint64_t t);
+
+/* Threshold table dump for the equality assert against the oracle: Ising 5
+ * entries indexed (dE+8)/4; Blume-Capel 54 entries ((s+1)*2+b)*9 + (h+4).
+ * Values in [0, 2^32].  *count = entries; ISING_EINVAL if cap too small.    */
+int ising_thresholds(ising_t *h, uint64_t *out, int cap, int *count);
+
+/* Launch geometry of the update kernel (results never depend on it,
+ * cf. PAPER.md:193): rows walked per thread and threads per block
+ * (multiple of 32, <= 1024).  0 keeps the current value.                    */
+int ising_set_launch(ising_t *h, int rows_per_thread, int block_threads);
+/* Update kernel variant (0 = default; others are equivalent implementations
+ * kept for parity / performance comparison).                                */
+int ising_set_variant(ising_t *h, int variant);
+
+/* Number of kernels this handle has launched since create.                  */
+int64_t ising_launch_count(const ising_t *h);
+/* Block until the handle's stream is idle.                                  */
+int ising_sync(ising_t *h);
+int ising_destroy(ising_t *h);
+const char *ising_last_error(void);
+
+/* Measurement helpers (not part of a simulation): n calls of the Philox-only
+ * kernel with the update kernel's grid (the ALU roof), and a plain
+ * read+write pass over the colour arrays (the HBM roof).  Asynchronous.     */
+int ising_bench_philox_only(ising_t *h, int n);
+int ising_bench_copy(ising_t *h, int n);
+
+/* Debug / test entry: evaluates this library's device Philox4x32-10 for count
+ * (ctr, key) pairs (host arrays: ctr 4*count, key 2*count, out 4*count words).
+ * with_curand != 0 evaluates the CUDA toolkit's curand_Philox4x32_10 instead.  */
+int ising_debug_philox(int64_t count, const uint32_t *ctr, const uint32_t *key, uint32_t *out,
+                       int with_curand);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ISING_B200_H */

@@ -1,0 +1,255 @@
+"""ctypes binding of include/ising.h.  Same names as the C ABI; no arithmetic of
+the method lives here.  torch is used for device memory and streams only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+ISING, BLUME_CAPEL = 0, 1
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libising_b200.so")
+_lib = None
+
+EXPORTS = [
+    "ising_workspace_bytes", "ising_create", "ising_sweep", "ising_observables", "ising_correlation",
+    "ising_correlation_protocol", "ising_correlation_list", "ising_schwinger_dyson", "ising_read_lattice",
+    "ising_read_window", "ising_write_lattice", "ising_read_packed", "ising_write_packed",
+    "ising_set_sweeps_done", "ising_thresholds", "ising_set_launch", "ising_set_variant",
+    "ising_launch_count", "ising_sync", "ising_destroy", "ising_last_error", "ising_bench_philox_only",
+    "ising_bench_copy", "ising_debug_philox",
+]
+
+
+class IsingError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"ising error {code}: {msg}")
+        self.code = code
+
+
+class _Obs(C.Structure):
+    _fields_ = [("bond_sum", C.c_int64), ("M", C.c_int64), ("Q", C.c_int64), ("n_sites", C.c_int64),
+                ("sweeps_done", C.c_uint64), ("E", C.c_double), ("e_per_site", C.c_double),
+                ("m_per_site", C.c_double), ("zero_density", C.c_double)]
+
+
+@dataclass(frozen=True)
+class Observables:
+    bond_sum: int
+    M: int
+    Q: int
+    n_sites: int
+    sweeps_done: int
+    E: float
+    e_per_site: float
+    m_per_site: float
+    zero_density: float
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """dlopen the CUDA library; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise IsingError(-3, f"{_LIB_PATH} is missing: run `python -m paper_2502_18624_b200.build` "
+                             "(or __graft_entry__.build()); there is no CPU fallback")
+    lib = C.CDLL(_LIB_PATH)
+    i64, u64, vp, dbl = C.c_int64, C.c_uint64, C.c_void_p, C.c_double
+    lib.ising_workspace_bytes.restype = C.c_size_t
+    lib.ising_workspace_bytes.argtypes = [C.c_int, i64]
+    lib.ising_create.argtypes = [C.c_int, i64, dbl, dbl, u64, vp, C.c_size_t, vp, C.POINTER(vp)]
+    lib.ising_sweep.argtypes = [vp, i64]
+    lib.ising_observables.argtypes = [vp, C.POINTER(_Obs)]
+    lib.ising_correlation.argtypes = [vp, i64, vp, vp]
+    lib.ising_correlation_protocol.argtypes = [vp, i64, vp, vp, vp, vp, C.POINTER(i64)]
+    lib.ising_correlation_list.argtypes = [vp, i64, i64, vp, vp, vp]
+    lib.ising_schwinger_dyson.argtypes = [vp, vp, C.POINTER(dbl)]
+    lib.ising_read_lattice.argtypes = [vp, i64, i64, vp]
+    lib.ising_read_window.argtypes = [vp, i64, i64, i64, i64, vp]
+    lib.ising_write_lattice.argtypes = [vp, i64, i64, vp]
+    lib.ising_read_packed.argtypes = [vp, C.c_int, i64, i64, vp]
+    lib.ising_write_packed.argtypes = [vp, C.c_int, i64, i64, vp]
+    lib.ising_set_sweeps_done.argtypes = [vp, u64]
+    lib.ising_thresholds.argtypes = [vp, vp, C.c_int, C.POINTER(C.c_int)]
+    lib.ising_set_launch.argtypes = [vp, C.c_int, C.c_int]
+    lib.ising_set_variant.argtypes = [vp, C.c_int]
+    lib.ising_launch_count.restype = i64
+    lib.ising_launch_count.argtypes = [vp]
+    lib.ising_sync.argtypes = [vp]
+    lib.ising_destroy.argtypes = [vp]
+    lib.ising_last_error.restype = C.c_char_p
+    lib.ising_bench_philox_only.argtypes = [vp, C.c_int]
+    lib.ising_bench_copy.argtypes = [vp, C.c_int]
+    lib.ising_debug_philox.argtypes = [i64, vp, vp, vp, C.c_int]
+    _lib = lib
+    return lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise IsingError(rc, load_library().ising_last_error().decode())
+
+
+def workspace_bytes(model: int, L: int) -> int:
+    return int(load_library().ising_workspace_bytes(model, L))
+
+
+def debug_philox(ctr: np.ndarray, key: np.ndarray, with_curand: bool = False) -> np.ndarray:
+    ctr = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+    key = np.ascontiguousarray(key, dtype=np.uint32).reshape(-1, 2)
+    out = np.zeros_like(ctr)
+    _check(load_library().ising_debug_philox(len(ctr), ctr.ctypes.data, key.ctypes.data, out.ctypes.data,
+                                             int(with_curand)))
+    return out
+
+
+class IsingSim:
+    """One lattice on one GPU.  Methods mirror the C ABI one to one."""
+
+    def __init__(self, model: int, L: int, beta: float, D: float = 0.0, seed: int = 1, device="cuda:0",
+                 use_torch_memory: bool = True):
+        import torch
+        if not torch.cuda.is_available():
+            raise IsingError(-3, "no CUDA device: the engine has no CPU fallback")
+        self._lib = load_library()
+        self._torch = torch
+        self.device = torch.device(device)
+        self.model, self.L, self.beta, self.D, self.seed = model, L, float(beta), float(D), seed
+        nbytes = workspace_bytes(model, L)
+        if nbytes == 0:
+            raise IsingError(-1, "invalid (model, L): L must be a multiple of 64, >= 64")
+        self._h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            self._stream = torch.cuda.current_stream(self.device)
+            if use_torch_memory:
+                self._buf = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+                ptr, size = self._buf.data_ptr(), nbytes
+            else:
+                self._buf, ptr, size = None, None, 0
+            _check(self._lib.ising_create(model, L, beta, D, seed, ptr, size, self._stream.cuda_stream,
+                                          C.byref(self._h)))
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            self._lib.ising_destroy(self._h)
+            self._h = None
+            self._buf = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    # -- the path
+    def sweep(self, n: int = 1):
+        _check(self._lib.ising_sweep(self._h, n))
+
+    def sync(self):
+        _check(self._lib.ising_sync(self._h))
+
+    def observables(self) -> Observables:
+        o = _Obs()
+        _check(self._lib.ising_observables(self._h, C.byref(o)))
+        return Observables(*(getattr(o, f[0]) for f in _Obs._fields_))
+
+    def correlation(self, rmax: int):
+        sx = np.zeros(rmax, dtype=np.int64)
+        sy = np.zeros(rmax, dtype=np.int64)
+        _check(self._lib.ising_correlation(self._h, rmax, sx.ctypes.data, sy.ctypes.data))
+        return sx, sy
+
+    def correlation_list(self, stride: int, r):
+        r = np.ascontiguousarray(r, dtype=np.int64)
+        sx = np.zeros(len(r), dtype=np.int64)
+        sy = np.zeros(len(r), dtype=np.int64)
+        _check(self._lib.ising_correlation_list(self._h, stride, len(r), r.ctypes.data, sx.ctypes.data,
+                                                sy.ctypes.data))
+        return sx, sy
+
+    def correlation_protocol(self):
+        n = C.c_int64(0)
+        self._lib.ising_correlation_protocol(self._h, 0, None, None, None, None, C.byref(n))
+        cap = n.value
+        arrs = [np.zeros(cap, dtype=np.int64) for _ in range(4)]
+        _check(self._lib.ising_correlation_protocol(self._h, cap, *(a.ctypes.data for a in arrs), C.byref(n)))
+        return tuple(arrs)
+
+    def schwinger_dyson(self):
+        hist = np.zeros(9, dtype=np.int64)
+        v = C.c_double(0.0)
+        _check(self._lib.ising_schwinger_dyson(self._h, hist.ctypes.data, C.byref(v)))
+        return v.value, hist
+
+    def read_lattice(self, y0: int = 0, ny: int | None = None) -> np.ndarray:
+        ny = self.L - y0 if ny is None else ny
+        out = np.empty((ny, self.L), dtype=np.int8)
+        _check(self._lib.ising_read_lattice(self._h, y0, ny, out.ctypes.data))
+        return out
+
+    def read_window(self, x0: int, y0: int, w: int, h: int) -> np.ndarray:
+        out = np.empty((h, w), dtype=np.int8)
+        _check(self._lib.ising_read_window(self._h, x0, y0, w, h, out.ctypes.data))
+        return out
+
+    def write_lattice(self, spins: np.ndarray, y0: int = 0):
+        spins = np.ascontiguousarray(spins, dtype=np.int8)
+        assert spins.ndim == 2 and spins.shape[1] == self.L
+        _check(self._lib.ising_write_lattice(self._h, y0, spins.shape[0], spins.ctypes.data))
+
+    def read_packed(self, colour: int, word0: int = 0, nwords: int | None = None, out=None):
+        total = self.L * (self.L // 32)
+        nwords = total - word0 if nwords is None else nwords
+        if out is None:
+            out = np.empty(nwords, dtype=np.uint64)
+            ptr = out.ctypes.data
+        else:
+            ptr = out.data_ptr() if hasattr(out, "data_ptr") else out.ctypes.data
+        _check(self._lib.ising_read_packed(self._h, colour, word0, nwords, ptr))
+        return out
+
+    def write_packed(self, colour: int, words, word0: int = 0, nwords: int | None = None):
+        if hasattr(words, "data_ptr"):
+            ptr, n = words.data_ptr(), words.numel() * words.element_size() // 8
+        else:
+            words = np.ascontiguousarray(words, dtype=np.uint64)
+            ptr, n = words.ctypes.data, len(words)
+        _check(self._lib.ising_write_packed(self._h, colour, word0, n if nwords is None else nwords, ptr))
+
+    def set_sweeps_done(self, t: int):
+        _check(self._lib.ising_set_sweeps_done(self._h, t))
+
+    def thresholds(self) -> np.ndarray:
+        out = np.zeros(64, dtype=np.uint64)
+        n = C.c_int(0)
+        _check(self._lib.ising_thresholds(self._h, out.ctypes.data, 64, C.byref(n)))
+        return out[: n.value].copy()
+
+    def set_launch(self, rows_per_thread: int = 0, block_threads: int = 0):
+        _check(self._lib.ising_set_launch(self._h, rows_per_thread, block_threads))
+
+    def set_variant(self, variant: int):
+        _check(self._lib.ising_set_variant(self._h, variant))
+
+    def launch_count(self) -> int:
+        return int(self._lib.ising_launch_count(self._h))
+
+    def bench_philox_only(self, n: int):
+        _check(self._lib.ising_bench_philox_only(self._h, n))
+
+    def bench_copy(self, n: int):
+        _check(self._lib.ising_bench_copy(self._h, n))

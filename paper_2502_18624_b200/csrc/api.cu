@@ -1,0 +1,531 @@
+// C ABI of libising_b200.so (include/ising.h).  Host logic only: argument checks,
+// threshold table (A1), launch sequencing (A11), integer -> double observables.
+#include <math.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <curand_kernel.h>
+
+#include "ising_internal.cuh"
+
+static thread_local std::string g_err;
+
+int set_error(int code, const std::string &msg)
+{
+    g_err = msg;
+    return code;
+}
+
+int cuda_fail(cudaError_t e, const char *what)
+{
+    return set_error(ISING_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+extern "C" const char *ising_last_error(void) { return g_err.c_str(); }
+
+static bool valid_model_L(int model, int64_t L)
+{
+    return (model == ISING_MODEL_ISING || model == ISING_MODEL_BLUME_CAPEL) && L >= 64 && (L % 64) == 0 &&
+           L <= (1ll << 20);
+}
+
+extern "C" size_t ising_workspace_bytes(int model, int64_t L)
+{
+    if (!valid_model_L(model, L)) return 0;
+    return (size_t)L * (size_t)L / 2 + kScratchBytes;
+}
+
+// ------------------------------------------------------------ thresholds ---
+// A1: T = 2^32 if p >= 1 else floor(p 2^32), p = exp(-beta dE) evaluated in double.
+static uint64_t metropolis_threshold(double beta, double dE)
+{
+    const double p = exp(-(beta * dE));
+    if (p >= 1.0) return 1ull << 32;
+    return (uint64_t)floor(ldexp(p, 32));
+}
+
+static void build_thresholds(ising_sim *h)
+{
+    if (h->model == ISING_MODEL_ISING) {
+        // entry i: dE = 4 i - 8, i.e. the spin agrees with i of... dE = 2 s h in {-8,-4,0,4,8}
+        h->n_T = 5;
+        for (int i = 0; i < 5; ++i) h->T[i] = metropolis_threshold(h->beta, 4.0 * i - 8.0);
+        return;
+    }
+    // Blume-Capel (Eq. 2): single-site energy e(s) = -s h + D s^2
+    h->n_T = 54;
+    for (int code = 0; code < 3; ++code)
+        for (int b = 0; b < 2; ++b)
+            for (int S = 0; S <= 8; ++S) {
+                const int s_old = code - 1, s_new = (code + 1 + b) % 3 - 1, field = S - 4;
+                const int d_lin = (s_new - s_old) * field;                 // change of s h
+                const int d_sq = s_new * s_new - s_old * s_old;            // change of s^2
+                volatile double crystal = h->D * (double)d_sq;             // rounded product, no FMA
+                const double dE = crystal - (double)d_lin;
+                h->T[(code * 2 + b) * 9 + S] = metropolis_threshold(h->beta, dE);
+            }
+}
+
+static void build_round_keys(ising_sim *h)
+{
+    uint32_t k0 = (uint32_t)(h->seed & 0xFFFFFFFFull), k1 = (uint32_t)(h->seed >> 32);
+    for (int i = 0; i < 10; ++i) {
+        h->rk.k0[i] = k0; h->rk.k1[i] = k1;
+        k0 += PHILOX_W0; k1 += PHILOX_W1;
+    }
+}
+
+static void default_launch(ising_sim *h)
+{
+    h->rows_per_thread = (h->L >= 4096) ? 32 : (h->L >= 512 ? 8 : 2);
+    h->block_threads = 128;
+}
+
+// ---------------------------------------------------------------- create ---
+extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_t seed, void *dev_buf,
+                            size_t dev_bytes, void *cuda_stream, ising_t **out)
+{
+    if (!out) return set_error(ISING_EINVAL, "ising_create: out is NULL");
+    if (!valid_model_L(model, L))
+        return set_error(ISING_EINVAL, "ising_create: model must be 0/1 and L a multiple of 64 in [64, 2^20]");
+    if (!(beta >= 0.0) || !isfinite(beta)) return set_error(ISING_EINVAL, "ising_create: beta must be finite and >= 0");
+    if (!isfinite(D)) return set_error(ISING_EINVAL, "ising_create: D must be finite");
+    const size_t need = ising_workspace_bytes(model, L);
+    if (dev_buf && dev_bytes < need) return set_error(ISING_EINVAL, "ising_create: dev_bytes < ising_workspace_bytes()");
+    if (dev_buf && ((uintptr_t)dev_buf & 255u)) return set_error(ISING_EINVAL, "ising_create: dev_buf must be 256-byte aligned");
+
+    ising_sim *h = new (std::nothrow) ising_sim();
+    if (!h) return set_error(ISING_ENOMEM, "ising_create: host allocation failed");
+    h->model = model; h->L = L; h->beta = beta; h->D = (model == ISING_MODEL_ISING) ? 0.0 : D; h->seed = seed;
+    h->stream = (cudaStream_t)cuda_stream;
+    char *base = (char *)dev_buf;
+    if (!base) {
+        cudaError_t e = cudaMalloc(&h->owned, need);
+        if (e != cudaSuccess) {
+            delete h;
+            cudaGetLastError();
+            return set_error(e == cudaErrorMemoryAllocation ? ISING_ENOMEM : ISING_ECUDA,
+                             std::string("ising_create: cudaMalloc: ") + cudaGetErrorString(e));
+        }
+        base = (char *)h->owned;
+    }
+    const size_t colour_bytes = (size_t)L * (size_t)L / 4;
+    h->lat[0] = (uint64_t *)base;
+    h->lat[1] = (uint64_t *)(base + colour_bytes);
+    h->d_acc = (long long *)(base + 2 * colour_bytes);                 // 64 int64 = 512 B (+ 4 KiB sink area unused)
+    h->d_bc_table = (uint32_t *)(base + 2 * colour_bytes + 1024);      // 66 uint32
+    build_thresholds(h);
+    build_round_keys(h);
+    default_launch(h);
+    cudaError_t e = cudaMallocHost(&h->h_acc, 64 * sizeof(long long));
+    if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "cudaMallocHost"); }
+    if (model == ISING_MODEL_BLUME_CAPEL) {
+        uint32_t tab[66] = {};
+        uint64_t always = 0;
+        for (int i = 0; i < 54; ++i) {
+            if (h->T[i] >> 32) { always |= 1ull << i; tab[i] = 0xFFFFFFFFu; }
+            else tab[i] = (uint32_t)h->T[i];
+        }
+        tab[64] = (uint32_t)always; tab[65] = (uint32_t)(always >> 32);
+        memcpy(h->h_acc, tab, sizeof(tab));
+        e = cudaMemcpyAsync(h->d_bc_table, h->h_acc, sizeof(tab), cudaMemcpyHostToDevice, h->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+        if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "upload of the Blume-Capel table"); }
+    }
+    e = launch_init(h);
+    if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "init kernel"); }
+    *out = h;
+    return ISING_OK;
+}
+
+extern "C" int ising_destroy(ising_t *h)
+{
+    if (!h) return ISING_OK;
+    cudaStreamSynchronize(h->stream);
+    if (h->io_stage) cudaFree(h->io_stage);
+    if (h->planes) cudaFree(h->planes);
+    if (h->d_corr) cudaFree(h->d_corr);
+    if (h->d_rlist) cudaFree(h->d_rlist);
+    if (h->h_acc) cudaFreeHost(h->h_acc);
+    if (h->owned) cudaFree(h->owned);
+    delete h;
+    return ISING_OK;
+}
+
+extern "C" int ising_sync(ising_t *h)
+{
+    if (!h) return set_error(ISING_EINVAL, "ising_sync: NULL handle");
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return ISING_OK;
+}
+
+extern "C" int64_t ising_launch_count(const ising_t *h) { return h ? h->launches : 0; }
+
+// ----------------------------------------------------------------- sweep ---
+extern "C" int ising_sweep(ising_t *h, int64_t n)
+{
+    if (!h) return set_error(ISING_EINVAL, "ising_sweep: NULL handle");
+    if (n < 0) return set_error(ISING_EINVAL, "ising_sweep: n < 0");
+    if (h->t + (uint64_t)n > 0xFFFFFFFFull) return set_error(ISING_EINVAL, "ising_sweep: sweep counter would exceed 2^32-1");
+    for (int64_t i = 0; i < n; ++i) {
+        for (int c = 0; c < 2; ++c) {
+            cudaError_t e = launch_update(h, c, (uint32_t)h->t);
+            if (e != cudaSuccess) return cuda_fail(e, "update kernel");
+        }
+        h->t++;
+    }
+    return ISING_OK;
+}
+
+extern "C" int ising_set_sweeps_done(ising_t *h, uint64_t t)
+{
+    if (!h) return set_error(ISING_EINVAL, "ising_set_sweeps_done: NULL handle");
+    if (t > 0xFFFFFFFFull) return set_error(ISING_EINVAL, "ising_set_sweeps_done: t > 2^32-1");
+    h->t = t;
+    return ISING_OK;
+}
+
+extern "C" int ising_set_launch(ising_t *h, int rows_per_thread, int block_threads)
+{
+    if (!h) return set_error(ISING_EINVAL, "ising_set_launch: NULL handle");
+    if (rows_per_thread < 0 || (rows_per_thread & 1) || rows_per_thread > 4096)
+        return set_error(ISING_EINVAL, "ising_set_launch: rows_per_thread must be even, in [2, 4096] (0 = keep)");
+    if (block_threads < 0 || (block_threads % 32) || block_threads > 256)
+        return set_error(ISING_EINVAL, "ising_set_launch: block_threads must be a multiple of 32, <= 256 (0 = keep)");
+    if (rows_per_thread) h->rows_per_thread = rows_per_thread;
+    if (block_threads) h->block_threads = block_threads;
+    return ISING_OK;
+}
+
+extern "C" int ising_set_variant(ising_t *h, int variant)
+{
+    if (!h) return set_error(ISING_EINVAL, "ising_set_variant: NULL handle");
+    if (variant < 0 || variant > 0) return set_error(ISING_EINVAL, "ising_set_variant: unknown variant");
+    h->variant = variant;
+    return ISING_OK;
+}
+
+// ----------------------------------------------------------- observables ---
+extern "C" int ising_observables(ising_t *h, ising_obs_t *out)
+{
+    if (!h || !out) return set_error(ISING_EINVAL, "ising_observables: NULL argument");
+    cudaError_t e = launch_observables(h);
+    if (e != cudaSuccess) return cuda_fail(e, "observables kernel");
+    CUDA_TRY(cudaMemcpyAsync(h->h_acc, h->d_acc, 3 * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    ising_obs_t o;
+    o.bond_sum = h->h_acc[0]; o.M = h->h_acc[1]; o.Q = h->h_acc[2];
+    o.n_sites = h->L * h->L; o.sweeps_done = h->t;
+    const double N = (double)h->L * (double)h->L;
+    o.E = (h->model == ISING_MODEL_ISING) ? -(double)o.bond_sum : -(double)o.bond_sum + h->D * (double)o.Q;
+    o.e_per_site = o.E / N;
+    o.m_per_site = (double)o.M / N;
+    o.zero_density = (double)(o.n_sites - o.Q) / N;
+    *out = o;
+    return ISING_OK;
+}
+
+extern "C" int ising_schwinger_dyson(ising_t *h, int64_t hist[9], double *value)
+{
+    if (!h || !hist || !value) return set_error(ISING_EINVAL, "ising_schwinger_dyson: NULL argument");
+    cudaError_t e = launch_sd_hist(h);
+    if (e != cudaSuccess) return cuda_fail(e, "Schwinger-Dyson kernel");
+    CUDA_TRY(cudaMemcpyAsync(h->h_acc + 8, h->d_acc + 8, 9 * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    double acc = 0.0;
+    for (int k = -4; k <= 4; ++k) {
+        hist[k + 4] = h->h_acc[8 + k + 4];
+        acc += (double)hist[k + 4] * exp(-2.0 * h->beta * (double)k);
+    }
+    *value = acc / ((double)h->L * (double)h->L);
+    return ISING_OK;
+}
+
+extern "C" int ising_thresholds(ising_t *h, uint64_t *out, int cap, int *count)
+{
+    if (!h || !count) return set_error(ISING_EINVAL, "ising_thresholds: NULL argument");
+    *count = h->n_T;
+    if (!out || cap < h->n_T) return set_error(ISING_EINVAL, "ising_thresholds: cap too small");
+    memcpy(out, h->T, h->n_T * sizeof(uint64_t));
+    return ISING_OK;
+}
+
+// ------------------------------------------------------------ lattice IO ---
+static int ensure_stage(ising_sim *h, size_t bytes)
+{
+    if (h->io_stage_bytes >= bytes) return ISING_OK;
+    if (h->io_stage) { cudaFree(h->io_stage); h->io_stage = nullptr; h->io_stage_bytes = 0; }
+    cudaError_t e = cudaMalloc(&h->io_stage, bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); return set_error(ISING_ENOMEM, "staging buffer: cudaMalloc failed"); }
+    h->io_stage_bytes = bytes;
+    return ISING_OK;
+}
+
+static const int64_t kStageBytes = 64ll << 20;
+
+extern "C" int ising_read_window(ising_t *h, int64_t x0, int64_t y0, int64_t w, int64_t hgt, int8_t *host_out)
+{
+    if (!h || !host_out) return set_error(ISING_EINVAL, "ising_read_window: NULL argument");
+    if (w < 1 || hgt < 1 || w > h->L || hgt > h->L) return set_error(ISING_EINVAL, "ising_read_window: window size out of range");
+    const int64_t L = h->L;
+    x0 = ((x0 % L) + L) % L; y0 = ((y0 % L) + L) % L;
+    const int64_t rows_per = std::max<int64_t>(1, std::min<int64_t>(hgt, kStageBytes / w));
+    int rc = ensure_stage(h, (size_t)(rows_per * w) + 16);
+    if (rc) return rc;
+    for (int64_t j = 0; j < hgt; j += rows_per) {
+        const int64_t nr = std::min(rows_per, hgt - j);
+        cudaError_t e = launch_unpack(h, x0, (y0 + j) % L, w, nr, (int8_t *)h->io_stage);
+        if (e != cudaSuccess) return cuda_fail(e, "unpack kernel");
+        CUDA_TRY(cudaMemcpyAsync(host_out + j * w, h->io_stage, (size_t)(nr * w), cudaMemcpyDeviceToHost, h->stream));
+        CUDA_TRY(cudaStreamSynchronize(h->stream));
+    }
+    return ISING_OK;
+}
+
+extern "C" int ising_read_lattice(ising_t *h, int64_t y0, int64_t ny, int8_t *host_out)
+{
+    if (!h || !host_out) return set_error(ISING_EINVAL, "ising_read_lattice: NULL argument");
+    if (y0 < 0 || ny < 1 || y0 + ny > h->L) return set_error(ISING_EINVAL, "ising_read_lattice: rows outside [0, L]");
+    return ising_read_window(h, 0, y0, h->L, ny, host_out);
+}
+
+extern "C" int ising_write_lattice(ising_t *h, int64_t y0, int64_t ny, const int8_t *host_in)
+{
+    if (!h || !host_in) return set_error(ISING_EINVAL, "ising_write_lattice: NULL argument");
+    if (y0 < 0 || ny < 1 || y0 + ny > h->L) return set_error(ISING_EINVAL, "ising_write_lattice: rows outside [0, L]");
+    const int64_t L = h->L;
+    const int64_t rows_per = std::max<int64_t>(1, std::min<int64_t>(ny, kStageBytes / L));
+    int rc = ensure_stage(h, (size_t)(rows_per * L) + 16);
+    if (rc) return rc;
+    int *d_bad = (int *)(h->d_acc + 32);
+    const bool one_chunk = ny <= rows_per;
+    // pass 0 validates every chunk, pass 1 writes: the lattice is untouched on bad input
+    for (int pass = 0; pass < 2; ++pass)
+        for (int64_t j = 0; j < ny; j += rows_per) {
+            const int64_t nr = std::min(rows_per, ny - j);
+            if (pass == 0 || !one_chunk)
+                CUDA_TRY(cudaMemcpyAsync(h->io_stage, host_in + j * L, (size_t)(nr * L), cudaMemcpyHostToDevice, h->stream));
+            cudaError_t e = launch_pack(h, y0 + j, nr, (const int8_t *)h->io_stage, d_bad, pass);
+            if (e == cudaErrorInvalidValue)
+                return set_error(ISING_EINVAL, "ising_write_lattice: spin value outside the model's set");
+            if (e != cudaSuccess) return cuda_fail(e, "pack kernel");
+            if (pass == 1) CUDA_TRY(cudaStreamSynchronize(h->stream));   // staging buffer is reused
+        }
+    return ISING_OK;
+}
+
+extern "C" int ising_read_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, uint64_t *host_out)
+{
+    if (!h || !host_out) return set_error(ISING_EINVAL, "ising_read_packed: NULL argument");
+    if ((colour != 0 && colour != 1) || word0 < 0 || nwords < 0 || word0 + nwords > words_per_colour(h->L))
+        return set_error(ISING_EINVAL, "ising_read_packed: range outside the colour array");
+    CUDA_TRY(cudaMemcpyAsync(host_out, h->lat[colour] + word0, (size_t)nwords * 8, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return ISING_OK;
+}
+
+extern "C" int ising_write_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, const uint64_t *host_in)
+{
+    if (!h || !host_in) return set_error(ISING_EINVAL, "ising_write_packed: NULL argument");
+    if ((colour != 0 && colour != 1) || word0 < 0 || nwords < 0 || word0 + nwords > words_per_colour(h->L))
+        return set_error(ISING_EINVAL, "ising_write_packed: range outside the colour array");
+    CUDA_TRY(cudaMemcpyAsync(h->lat[colour] + word0, host_in, (size_t)nwords * 8, cudaMemcpyHostToDevice, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return ISING_OK;
+}
+
+// ----------------------------------------------------------- correlation ---
+static int ensure_planes(ising_sim *h)
+{
+    const size_t pw = (size_t)h->L * (size_t)(h->L / 64);
+    const size_t bytes = pw * 8 * (h->model == ISING_MODEL_ISING ? 2 : 4);
+    if (h->planes_bytes >= bytes) return ISING_OK;
+    cudaError_t e = cudaMalloc((void **)&h->planes, bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); h->planes = nullptr; return set_error(ISING_ENOMEM, "bit planes: cudaMalloc failed"); }
+    h->planes_bytes = bytes;
+    return ISING_OK;
+}
+
+static int ensure_corr(ising_sim *h, int64_t count)
+{
+    const size_t bytes = (size_t)count * 2 * sizeof(long long);
+    if (h->d_corr_bytes < bytes) {
+        if (h->d_corr) cudaFree(h->d_corr);
+        h->d_corr = nullptr; h->d_corr_bytes = 0;
+        cudaError_t e = cudaMalloc((void **)&h->d_corr, bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); return set_error(ISING_ENOMEM, "correlation buffer: cudaMalloc failed"); }
+        h->d_corr_bytes = bytes;
+    }
+    const size_t rb = (size_t)count * sizeof(long long);
+    if (h->d_rlist_bytes < rb) {
+        if (h->d_rlist) cudaFree(h->d_rlist);
+        h->d_rlist = nullptr; h->d_rlist_bytes = 0;
+        cudaError_t e = cudaMalloc((void **)&h->d_rlist, rb);
+        if (e != cudaSuccess) { cudaGetLastError(); return set_error(ISING_ENOMEM, "distance list: cudaMalloc failed"); }
+        h->d_rlist_bytes = rb;
+    }
+    return ISING_OK;
+}
+
+// shared tail: planes already built.  stride 0 = full-source r = 1..count.
+static int run_corr(ising_sim *h, int64_t stride, int64_t count, const int64_t *r, int64_t *sx, int64_t *sy)
+{
+    int rc = ensure_corr(h, count);
+    if (rc) return rc;
+    long long *d_sx = h->d_corr, *d_sy = h->d_corr + count;
+    if (stride > 0)
+        CUDA_TRY(cudaMemcpyAsync(h->d_rlist, r, (size_t)count * sizeof(long long), cudaMemcpyHostToDevice, h->stream));
+    cudaError_t e = launch_corr(h, stride, count, h->d_rlist, d_sx, d_sy);
+    if (e != cudaSuccess) return cuda_fail(e, "correlation kernel");
+    CUDA_TRY(cudaMemcpyAsync(sx, d_sx, (size_t)count * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaMemcpyAsync(sy, d_sy, (size_t)count * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    if (h->model == ISING_MODEL_ISING) {   // popcount of unequal pairs -> pair sum
+        const int64_t s = stride > 0 ? stride : 1;
+        const int64_t n_src = (h->L / s) * (h->L / s);
+        for (int64_t i = 0; i < count; ++i) { sx[i] = n_src - 2 * sx[i]; sy[i] = n_src - 2 * sy[i]; }
+    }
+    return ISING_OK;
+}
+
+extern "C" int ising_correlation(ising_t *h, int64_t rmax, int64_t *sx, int64_t *sy)
+{
+    if (!h || !sx || !sy) return set_error(ISING_EINVAL, "ising_correlation: NULL argument");
+    if (rmax < 1 || rmax > h->L / 2) return set_error(ISING_EINVAL, "ising_correlation: rmax outside [1, L/2]");
+    int rc = ensure_planes(h);
+    if (rc) return rc;
+    cudaError_t e = launch_planes(h);
+    if (e != cudaSuccess) return cuda_fail(e, "bit-plane kernels");
+    return run_corr(h, 0, rmax, nullptr, sx, sy);
+}
+
+static bool valid_stride(int64_t s) { return s == 1 || s == 2 || s == 4 || s == 8 || s == 16 || s == 32 || s == 64; }
+
+extern "C" int ising_correlation_list(ising_t *h, int64_t stride, int64_t count, const int64_t *r, int64_t *sx, int64_t *sy)
+{
+    if (!h || !r || !sx || !sy) return set_error(ISING_EINVAL, "ising_correlation_list: NULL argument");
+    if (!valid_stride(stride)) return set_error(ISING_EINVAL, "ising_correlation_list: stride must be 1 or a power of two <= 64");
+    if (count < 1 || count > 65535) return set_error(ISING_EINVAL, "ising_correlation_list: count outside [1, 65535]");
+    for (int64_t i = 0; i < count; ++i)
+        if (r[i] < 1 || r[i] > h->L / 2) return set_error(ISING_EINVAL, "ising_correlation_list: distance outside [1, L/2]");
+    int rc = ensure_planes(h);
+    if (rc) return rc;
+    cudaError_t e = launch_planes(h);
+    if (e != cudaSuccess) return cuda_fail(e, "bit-plane kernels");
+    return run_corr(h, stride, count, r, sx, sy);
+}
+
+// Sec. 3.3: R = 16, r_c(t) = max{256, floor(g(L) sqrt(t) + 0.5)},
+// g(L) = 6 sqrt(ln(L / 2^16) / 3.3^2 + 1); log grid floor(2^(x/32)), x <= 32 (log2 L - 1).
+static void protocol_distances(int64_t L, uint64_t t, std::vector<int64_t> &dense, std::vector<int64_t> &sparse)
+{
+    const int64_t R = 16, half = L / 2;
+    const double g = 6.0 * sqrt(log((double)L / 65536.0) / (3.3 * 3.3) + 1.0);
+    int64_t rc = (int64_t)floor(g * sqrt((double)t) + 0.5);
+    if (rc < 256) rc = 256;
+    for (int64_t d = 1; d <= std::min(2 * R, half); ++d) dense.push_back(d);
+    for (int64_t d = 2 * R + 1; d <= std::min(rc, half); ++d) sparse.push_back(d);
+    const int64_t xmax = (int64_t)floor(32.0 * (log2((double)L) - 1.0) + 1e-9);
+    int64_t last = std::max(rc, 2 * R);
+    for (int64_t x = 0; x <= xmax; ++x) {
+        const int64_t d = (int64_t)floor(exp2((double)x / 32.0));
+        if (d <= last || d > half) continue;
+        sparse.push_back(d);
+        last = d;
+    }
+}
+
+extern "C" int ising_correlation_protocol(ising_t *h, int64_t cap, int64_t *r, int64_t *sx, int64_t *sy,
+                                          int64_t *n_src, int64_t *count)
+{
+    if (!h || !count) return set_error(ISING_EINVAL, "ising_correlation_protocol: NULL argument");
+    std::vector<int64_t> dense, sparse;
+    protocol_distances(h->L, h->t, dense, sparse);
+    const int64_t nd = (int64_t)dense.size(), ns = (int64_t)sparse.size();
+    *count = nd + ns;
+    if (!r || !sx || !sy || !n_src || cap < nd + ns) return set_error(ISING_EINVAL, "ising_correlation_protocol: cap too small");
+    int rc = ensure_planes(h);
+    if (rc) return rc;
+    cudaError_t e = launch_planes(h);
+    if (e != cudaSuccess) return cuda_fail(e, "bit-plane kernels");
+    rc = run_corr(h, 0, nd, nullptr, sx, sy);                 // all sources, r = 1..2R
+    if (rc) return rc;
+    for (int64_t i = 0; i < nd; ++i) { r[i] = dense[i]; n_src[i] = h->L * h->L; }
+    if (ns > 0) {
+        rc = run_corr(h, 16, ns, sparse.data(), sx + nd, sy + nd);   // one source per 16 x 16 block
+        if (rc) return rc;
+        for (int64_t i = 0; i < ns; ++i) { r[nd + i] = sparse[i]; n_src[nd + i] = (h->L / 16) * (h->L / 16); }
+    }
+    return ISING_OK;
+}
+
+// ----------------------------------------------------- measurement helpers ---
+extern "C" int ising_bench_philox_only(ising_t *h, int n)
+{
+    if (!h || n < 0) return set_error(ISING_EINVAL, "ising_bench_philox_only: bad argument");
+    for (int i = 0; i < n; ++i) {
+        cudaError_t e = launch_philox_only(h, (uint32_t)i);
+        if (e != cudaSuccess) return cuda_fail(e, "philox-only kernel");
+    }
+    return ISING_OK;
+}
+
+extern "C" int ising_bench_copy(ising_t *h, int n)
+{
+    if (!h || n < 0) return set_error(ISING_EINVAL, "ising_bench_copy: bad argument");
+    for (int i = 0; i < n; ++i) {
+        cudaError_t e = launch_copy(h);
+        if (e != cudaSuccess) return cuda_fail(e, "copy kernel");
+    }
+    return ISING_OK;
+}
+
+// ------------------------------------------------------------ debug Philox ---
+__global__ void debug_philox_kernel(int64_t count, const uint32_t *ctr, const uint32_t *key, uint32_t *out, int with_curand)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    uint4 c = make_uint4(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3]);
+    uint4 r;
+    if (with_curand) {
+        r = curand_Philox4x32_10(c, make_uint2(key[2 * i], key[2 * i + 1]));
+    } else {
+        RoundKeys rk;
+        uint32_t k0 = key[2 * i], k1 = key[2 * i + 1];
+        for (int j = 0; j < 10; ++j) { rk.k0[j] = k0; rk.k1[j] = k1; k0 += PHILOX_W0; k1 += PHILOX_W1; }
+        if (with_curand == 0 && (i & 1)) {
+            // odd entries go through the specialised path the update kernel uses
+            PhiloxRow pr = philox_row(c.y, c.z, c.w, rk);
+            r = philox_site4(c.x, pr, rk);
+        } else {
+            r = philox4x32_10(c, rk);
+        }
+    }
+    out[4 * i] = r.x; out[4 * i + 1] = r.y; out[4 * i + 2] = r.z; out[4 * i + 3] = r.w;
+}
+
+cudaError_t launch_debug_philox(int64_t count, const uint32_t *d_ctr, const uint32_t *d_key, uint32_t *d_out,
+                                int with_curand, cudaStream_t s)
+{
+    debug_philox_kernel<<<(unsigned)((count + 127) / 128), 128, 0, s>>>(count, d_ctr, d_key, d_out, with_curand);
+    return cudaGetLastError();
+}
+
+extern "C" int ising_debug_philox(int64_t count, const uint32_t *ctr, const uint32_t *key, uint32_t *out, int with_curand)
+{
+    if (count < 1 || !ctr || !key || !out) return set_error(ISING_EINVAL, "ising_debug_philox: bad argument");
+    uint32_t *d = nullptr;
+    CUDA_TRY(cudaMalloc((void **)&d, (size_t)count * 10 * sizeof(uint32_t)));
+    uint32_t *d_ctr = d, *d_key = d + 4 * count, *d_out = d + 6 * count;
+    cudaError_t e = cudaMemcpy(d_ctr, ctr, (size_t)count * 16, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(d_key, key, (size_t)count * 8, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = launch_debug_philox(count, d_ctr, d_key, d_out, with_curand, 0);
+    if (e == cudaSuccess) e = cudaMemcpy(out, d_out, (size_t)count * 16, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return cuda_fail(e, "ising_debug_philox");
+    return ISING_OK;
+}

@@ -1,0 +1,135 @@
+// Internal declarations shared by the .cu files of libising_b200.so.
+// Nothing here is shared with oracle/ (the CPU checker).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "ising.h"
+
+// ----------------------------------------------------------------- handle ---
+struct RoundKeys {  // Philox key schedule (PAPER.md:149 names the generator): k(i) = seed + i*W
+    uint32_t k0[10], k1[10];
+};
+
+struct ising_sim {
+    int model = 0;
+    int64_t L = 0;
+    double beta = 0, D = 0;
+    uint64_t seed = 0;
+    uint64_t t = 0;  // sweeps done
+    cudaStream_t stream = nullptr;
+    uint64_t *lat[2] = {nullptr, nullptr};  // black, white colour arrays (device)
+    void *owned = nullptr;                  // non-null if the library allocated dev_buf
+    long long *d_acc = nullptr;             // 64 int64 accumulators inside the scratch area
+    long long *h_acc = nullptr;             // pinned mirror
+    uint64_t T[54] = {};                    // thresholds in [0, 2^32]
+    int n_T = 0;
+    uint32_t *d_bc_table = nullptr;         // Blume-Capel: 64-entry uint32 table + flags (scratch)
+    RoundKeys rk;
+    int rows_per_thread = 0, block_threads = 0, variant = 0;
+    int64_t launches = 0;
+    // lazily allocated (cudaMalloc, owned)
+    void *io_stage = nullptr; size_t io_stage_bytes = 0;
+    uint64_t *planes = nullptr; size_t planes_bytes = 0;      // bit planes for the correlation
+    long long *d_corr = nullptr; size_t d_corr_bytes = 0;
+    long long *d_rlist = nullptr; size_t d_rlist_bytes = 0;
+};
+
+static const size_t kScratchBytes = 4096;  // accumulators + BC table at the end of dev_buf
+
+int set_error(int code, const std::string &msg);
+int cuda_fail(cudaError_t e, const char *what);
+#define CUDA_TRY(x)                                            \
+    do {                                                       \
+        cudaError_t e__ = (x);                                 \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #x);     \
+    } while (0)
+
+static inline int64_t words_per_row(int64_t L) { return L / 32; }              // uint64 per colour row
+static inline int64_t words_per_colour(int64_t L) { return L * (L / 32); }
+
+// kernels' host launchers (each returns a cudaError_t from the launch)
+cudaError_t launch_init(ising_sim *h);
+cudaError_t launch_update(ising_sim *h, int colour, uint32_t t);
+cudaError_t launch_observables(ising_sim *h);                       // -> d_acc[0..2] = B, M, Q
+cudaError_t launch_sd_hist(ising_sim *h);                           // -> d_acc[8..16]
+cudaError_t launch_unpack(ising_sim *h, int64_t x0, int64_t y0, int64_t w, int64_t hgt, int8_t *dev_out);
+cudaError_t launch_pack(ising_sim *h, int64_t y0, int64_t ny, const int8_t *dev_in, int *dev_bad, int write);
+cudaError_t launch_planes(ising_sim *h);                            // lattice -> bit planes
+cudaError_t launch_corr(ising_sim *h, int64_t stride, int64_t count, const long long *dev_r,
+                        long long *dev_sx, long long *dev_sy);
+cudaError_t launch_philox_only(ising_sim *h, uint32_t t);
+cudaError_t launch_copy(ising_sim *h);
+cudaError_t launch_debug_philox(int64_t count, const uint32_t *d_ctr, const uint32_t *d_key,
+                                uint32_t *d_out, int with_curand, cudaStream_t s);
+
+// ----------------------------------------------------------------- Philox ---
+#ifdef __CUDACC__
+#define PHILOX_M0 0xD2511F53u
+#define PHILOX_M1 0xCD9E8D57u
+#define PHILOX_W0 0x9E3779B9u
+#define PHILOX_W1 0xBB67AE85u
+
+// Generic Philox4x32-10: ten rounds of
+//   (c0,c1,c2,c3) <- (hi(M1*c2)^c1^k0, lo(M1*c2), hi(M0*c0)^c3^k1, lo(M0*c0)).
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, const RoundKeys &rk)
+{
+#pragma unroll
+    for (int i = 0; i < 10; ++i) {
+        uint64_t p0 = (uint64_t)PHILOX_M0 * c.x;
+        uint64_t p1 = (uint64_t)PHILOX_M1 * c.z;
+        c = make_uint4((uint32_t)(p1 >> 32) ^ c.y ^ rk.k0[i], (uint32_t)p1,
+                       (uint32_t)(p0 >> 32) ^ c.w ^ rk.k1[i], (uint32_t)p0);
+    }
+    return c;
+}
+
+// Per-(row, launch) constants of the counter (g_lo, g_hi, t, tag): everything in
+// rounds 1-2 that does not depend on g_lo.  Saves 2 of the 20 multiplies per call.
+struct PhiloxRow {
+    uint32_t u2;   // tag ^ k1[0]
+    uint32_t v0;   // lo(M1*t) ^ k0[1]
+    uint32_t v1;   // hi(M0*U0) ^ k1[1],  U0 = hi(M1*t) ^ g_hi ^ k0[0]
+    uint32_t v3;   // lo(M0*U0) ^ k1[2]
+};
+
+__device__ __forceinline__ PhiloxRow philox_row(uint32_t g_hi, uint32_t t, uint32_t tag, const RoundKeys &rk)
+{
+    uint64_t p1 = (uint64_t)PHILOX_M1 * t;
+    uint32_t U0 = (uint32_t)(p1 >> 32) ^ g_hi ^ rk.k0[0];
+    uint64_t q0 = (uint64_t)PHILOX_M0 * U0;
+    PhiloxRow r;
+    r.u2 = tag ^ rk.k1[0];
+    r.v0 = (uint32_t)p1 ^ rk.k0[1];
+    r.v1 = (uint32_t)(q0 >> 32) ^ rk.k1[1];
+    r.v3 = (uint32_t)q0 ^ rk.k1[2];
+    return r;
+}
+
+// Same function as philox4x32_10(make_uint4(g_lo, g_hi, t, tag)) with rounds 1-2 specialised.
+__device__ __forceinline__ uint4 philox_site4(uint32_t g_lo, const PhiloxRow &pr, const RoundKeys &rk)
+{
+    // round 1: c = (U0, U1, hi0 ^ u2, lo0), U0/U1 folded into pr
+    uint64_t p0 = (uint64_t)PHILOX_M0 * g_lo;
+    uint32_t c2 = (uint32_t)(p0 >> 32) ^ pr.u2, c3 = (uint32_t)p0;
+    // round 2: c = (hi(M1*c2) ^ U1 ^ k0[1], lo(M1*c2), hi(M0*U0) ^ c3 ^ k1[1], lo(M0*U0))
+    uint64_t p1 = (uint64_t)PHILOX_M1 * c2;
+    uint32_t d0 = (uint32_t)(p1 >> 32) ^ pr.v0, d1 = (uint32_t)p1, d2 = c3 ^ pr.v1;
+    // round 3: c3 of round 2 is uniform and folded with k1[2] into v3
+    p0 = (uint64_t)PHILOX_M0 * d0;
+    p1 = (uint64_t)PHILOX_M1 * d2;
+    uint4 c = make_uint4((uint32_t)(p1 >> 32) ^ d1 ^ rk.k0[2], (uint32_t)p1,
+                         (uint32_t)(p0 >> 32) ^ pr.v3, (uint32_t)p0);
+#pragma unroll
+    for (int i = 3; i < 10; ++i) {
+        p0 = (uint64_t)PHILOX_M0 * c.x;
+        p1 = (uint64_t)PHILOX_M1 * c.z;
+        c = make_uint4((uint32_t)(p1 >> 32) ^ c.y ^ rk.k0[i], (uint32_t)p1,
+                       (uint32_t)(p0 >> 32) ^ c.w ^ rk.k1[i], (uint32_t)p0);
+    }
+    return c;
+}
+#endif  // __CUDACC__

@@ -1,0 +1,169 @@
+// Integer observables (A8 of SURVEY.md Sec. 8(a)) and the Schwinger-Dyson
+// histogram (Eq. 3).  Same register sliding window as the update
+// kernel: each thread walks R rows of one 128-bit column of the BLACK array and
+// sees every bond exactly once (for even L every bond joins a black and a white
+// site).  Warp shuffle -> one int64 atomic per warp per quantity.
+#include "ising_internal.cuh"
+
+#define ONES 0x11111111u
+
+struct ObsParams {
+    const uint4 *ctr, *nbr;   // centre-colour array, neighbour-colour array
+    int centre;               // colour of the centre sites
+    int L, cols, R;
+    long long *acc;
+};
+
+__device__ __forceinline__ uint32_t nibble_sum(uint32_t x)  // sum of the 8 nibbles (each <= 15)
+{
+    uint32_t t = (x & 0x0F0F0F0Fu) + ((x >> 4) & 0x0F0F0F0Fu);
+    return (t * 0x01010101u) >> 24;
+}
+
+__device__ __forceinline__ long long warp_sum(long long v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+
+template <int P>
+__device__ __forceinline__ void side4(const uint4 &sm, uint32_t edge, uint32_t sd[4])
+{
+    if (P == 0) {
+        sd[0] = __funnelshift_l(edge, sm.x, 4); sd[1] = __funnelshift_l(sm.x, sm.y, 4);
+        sd[2] = __funnelshift_l(sm.y, sm.z, 4); sd[3] = __funnelshift_l(sm.z, sm.w, 4);
+    } else {
+        sd[0] = __funnelshift_r(sm.x, sm.y, 4); sd[1] = __funnelshift_r(sm.y, sm.z, 4);
+        sd[2] = __funnelshift_r(sm.z, sm.w, 4); sd[3] = __funnelshift_r(sm.w, edge, 4);
+    }
+}
+
+// MODE 0: B, M, Q.  MODE 1: Schwinger-Dyson histogram of s*h over the centre sites.
+template <int MODEL, int MODE>
+__device__ __forceinline__ void obs_half(uint32_t x, uint32_t up, uint32_t dn, uint32_t sm, uint32_t sd,
+                                         int &B, int &M, int &Q, int hist[9])
+{
+    if (MODEL == ISING_MODEL_ISING) {
+        uint32_t d = (up ^ x) + (dn ^ x) + (sm ^ x) + (sd ^ x);   // unequal neighbours per site
+        if (MODE == 0) {
+            B += 32 - 2 * (int)nibble_sum(d);                      // sum of s*h = sum (4 - 2 d)
+            M += 2 * (__popc(x) + __popc(sm)) - 16;                // black half + the white half of this row
+            Q += 16;
+        } else {
+#pragma unroll
+            for (int k = 0; k <= 4; ++k) {                         // s*h = 4 - 2k
+                uint32_t e = d ^ (ONES * (uint32_t)k);             // nibble == 0 where d == k
+                e = (e | (e >> 1) | (e >> 2)) & ONES;
+                hist[8 - 2 * k] += 8 - __popc(e);
+            }
+        }
+    } else {
+        uint32_t S = up + dn + sm + sd;                            // h + 4 per site
+        uint32_t pos = (x >> 1) & ONES, neg = ~(x | (x >> 1)) & ONES;
+        if (MODE == 0) {
+            int np = __popc(pos), nn = __popc(neg);
+            B += (int)nibble_sum(S & (pos * 15u)) - 4 * np - (int)nibble_sum(S & (neg * 15u)) + 4 * nn;
+            uint32_t wpos = (sm >> 1) & ONES, wneg = ~(sm | (sm >> 1)) & ONES;
+            int wp = __popc(wpos), wn = __popc(wneg);
+            M += np - nn + wp - wn;
+            Q += np + nn + wp + wn;
+        } else {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                int code = (x >> (4 * j)) & 15, h = (int)((S >> (4 * j)) & 15u) - 4;
+                hist[(code - 1) * h + 4] += 1;
+            }
+        }
+    }
+}
+
+template <int MODEL, int MODE>
+__global__ void __launch_bounds__(256) observe_kernel(const __grid_constant__ ObsParams p)
+{
+    // centre sites: colour p.centre (array `ctr`), neighbours in the other array (`nbr`);
+    // row parity of the centre colour is (y + centre) & 1
+    const int cols = p.cols, L = p.L;
+    unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned chunk = tid / (unsigned)cols;
+    int col = (int)(tid - chunk * (unsigned)cols);
+    int y0 = (int)chunk * p.R;
+    int B = 0, M = 0, Q = 0;
+    int hist[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+    if (y0 < L) {
+        int yend = min(L, y0 + p.R);
+        const uint32_t *n32 = reinterpret_cast<const uint32_t *>(p.nbr);
+        const size_t halves = (size_t)cols * 4;
+        const int e0 = (col == 0) ? cols * 4 - 1 : 4 * col - 1;        // parity 0: neighbour k-1
+        const int e1 = (col == cols - 1) ? 0 : 4 * col + 4;            // parity 1: neighbour k+1
+        int ym = (y0 == 0) ? L - 1 : y0 - 1;
+        uint4 up = p.nbr[(size_t)ym * cols + col];
+        uint4 sm = p.nbr[(size_t)y0 * cols + col];
+        for (int y = y0; y < yend; ++y) {
+            int yp = (y + 1 == L) ? 0 : y + 1;
+            uint4 dn = p.nbr[(size_t)yp * cols + col];
+            uint4 x = p.ctr[(size_t)y * cols + col];
+            uint32_t sd[4];
+            if (((y + p.centre) & 1) == 0) side4<0>(sm, n32[(size_t)y * halves + e0], sd);
+            else side4<1>(sm, n32[(size_t)y * halves + e1], sd);
+            obs_half<MODEL, MODE>(x.x, up.x, dn.x, sm.x, sd[0], B, M, Q, hist);
+            obs_half<MODEL, MODE>(x.y, up.y, dn.y, sm.y, sd[1], B, M, Q, hist);
+            obs_half<MODEL, MODE>(x.z, up.z, dn.z, sm.z, sd[2], B, M, Q, hist);
+            obs_half<MODEL, MODE>(x.w, up.w, dn.w, sm.w, sd[3], B, M, Q, hist);
+            up = sm; sm = dn;
+        }
+    }
+    if (MODE == 0) {
+        long long b = warp_sum(B), m = warp_sum(M), q = warp_sum(Q);
+        if ((threadIdx.x & 31) == 0) {
+            atomicAdd((unsigned long long *)&p.acc[0], (unsigned long long)b);
+            atomicAdd((unsigned long long *)&p.acc[1], (unsigned long long)m);
+            atomicAdd((unsigned long long *)&p.acc[2], (unsigned long long)q);
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < 9; ++k) {
+            long long v = warp_sum(hist[k]);
+            if ((threadIdx.x & 31) == 0 && v) atomicAdd((unsigned long long *)&p.acc[8 + k], (unsigned long long)v);
+        }
+    }
+}
+
+template <int MODE>
+static cudaError_t launch_obs(ising_sim *h, int centre)
+{
+    ObsParams p;
+    p.ctr = reinterpret_cast<const uint4 *>(h->lat[centre]);
+    p.nbr = reinterpret_cast<const uint4 *>(h->lat[1 - centre]);
+    p.centre = centre;
+    p.L = (int)h->L; p.cols = (int)(h->L / 64);
+    p.R = (h->L >= 2048) ? 32 : 4;
+    p.acc = h->d_acc;
+    int64_t chunks = (h->L + p.R - 1) / p.R;
+    int64_t threads = chunks * p.cols;
+    int block = 128;
+    unsigned grid = (unsigned)((threads + block - 1) / block);
+    if (h->model == ISING_MODEL_ISING) observe_kernel<ISING_MODEL_ISING, MODE><<<grid, block, 0, h->stream>>>(p);
+    else observe_kernel<ISING_MODEL_BLUME_CAPEL, MODE><<<grid, block, 0, h->stream>>>(p);
+    h->launches++;
+    return cudaGetLastError();
+}
+
+// B, M, Q: centre = black sees every bond once; M and Q also count the white words of
+// the centre row (`sm`), so one pass covers both arrays.
+cudaError_t launch_observables(ising_sim *h)
+{
+    cudaError_t e = cudaMemsetAsync(h->d_acc, 0, 8 * sizeof(long long), h->stream);
+    if (e != cudaSuccess) return e;
+    return launch_obs<0>(h, 0);
+}
+
+// Schwinger-Dyson histogram over ALL sites: one pass centred on each colour.
+cudaError_t launch_sd_hist(ising_sim *h)
+{
+    cudaError_t e = cudaMemsetAsync(h->d_acc + 8, 0, 9 * sizeof(long long), h->stream);
+    if (e != cudaSuccess) return e;
+    e = launch_obs<1>(h, 0);
+    if (e != cudaSuccess) return e;
+    return launch_obs<1>(h, 1);
+}

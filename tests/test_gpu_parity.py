@@ -1,0 +1,302 @@
+"""GPU parity (-m gpu): the CUDA path, called through the C ABI binding, against
+the CPU oracle on the same seeded inputs.  Integer results are compared
+bit-exactly; doubles to rel 1e-12 (north_star)."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+ISING, BC = 0, 1
+
+
+@pytest.fixture(scope="module")
+def eng():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2502_18624_b200 as e
+    e.load_library()           # must fail loudly if the extension is missing
+    return e
+
+
+def _close(a, b):
+    return a == b or abs(a - b) <= 1e-12 * max(abs(a), abs(b))
+
+
+def _check_obs(model, L, D, obs, bmq):
+    assert (obs.bond_sum, obs.M, obs.Q) == tuple(bmq)
+    E, e, m, z = oracle.normalised(model, L, D, bmq)
+    assert _close(obs.E, E) and _close(obs.e_per_site, e) and _close(obs.m_per_site, m) and _close(obs.zero_density, z)
+    assert obs.n_sites == L * L
+
+
+# ------------------------------------------------------------------ Philox ---
+def test_device_philox_matches_oracle_and_curand(eng):
+    rng = np.random.default_rng(0)
+    n = 4096
+    ctr = rng.integers(0, 2**32, size=(n, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2**32, size=(n, 2), dtype=np.uint64).astype(np.uint32)
+    ctr[:4] = [[0, 0, 0, 0], [0xFFFFFFFF] * 4, [0x243F6A88, 0x85A308D3, 0x13198A2E, 0x03707344], [5, 0, 7, 1]]
+    key[:4] = [[0, 0], [0xFFFFFFFF] * 2, [0xA4093822, 0x299F31D0], [1, 0]]
+    ours = eng.debug_philox(ctr, key, with_curand=False)      # even rows generic, odd rows specialised path
+    lib = eng.debug_philox(ctr, key, with_curand=True)        # the toolkit's curand_Philox4x32_10
+    assert (ours == lib).all()
+    for i in list(range(8)) + list(range(100, 164)):
+        assert (ours[i] == oracle.philox4x32_10(ctr[i], key[i])).all()
+    assert [hex(int(v)) for v in ours[0]] == ["0x6627e8d5", "0xe169c58d", "0xbc57ac4c", "0x9b00dbd8"]
+
+
+# -------------------------------------------------------------- thresholds ---
+@pytest.mark.parametrize("i", range(5))
+def test_threshold_tables_equal(eng, i):
+    """north_star: both sides compute the table independently in double and assert equality."""
+    w = wl.config(i)
+    with eng.IsingSim(w.model, 64, w.beta, w.D, w.seed) as sim:
+        assert (sim.thresholds() == oracle.thresholds(w.model, w.beta, w.D)).all()
+
+
+@pytest.mark.parametrize("beta,D", [(0.0, 0.0), (0.3, -2.0), (1.7, 1.966), (25.0, 3.0), (0.5, 0.0)])
+def test_threshold_tables_equal_other_parameters(eng, beta, D):
+    for model in (ISING, BC):
+        with eng.IsingSim(model, 64, beta, D, 3) as sim:
+            assert (sim.thresholds() == oracle.thresholds(model, beta, D)).all()
+
+
+# -------------------------------------------------------------------- init ---
+@pytest.mark.parametrize("model", [ISING, BC])
+@pytest.mark.parametrize("L", [64, 192, 256, 1024])
+def test_init_lattice(eng, model, L):
+    with eng.IsingSim(model, L, 0.4, 0.5, 7) as sim:
+        assert (sim.read_lattice() == oracle.init(model, L, 7)).all()
+
+
+# ------------------------------------------------------------- full parity ---
+def test_config0_ising_L256_every_sweep(eng):
+    """configs[0]: final lattice and E, M after every one of 100 sweeps."""
+    w = wl.config(0)
+    s = oracle.init(w.model, w.L, w.seed)
+    tl = oracle.observables(s)
+    with eng.IsingSim(w.model, w.L, w.beta, w.D, w.seed) as sim:
+        _check_obs(w.model, w.L, w.D, sim.observables(), tl)
+        for t in range(w.sweeps):
+            sim.sweep(1)
+            tl = oracle.sweep(w.model, s, w.beta, w.D, w.seed, t, tl)
+            _check_obs(w.model, w.L, w.D, sim.observables(), tl)
+            if t % 10 == 9:
+                assert (sim.read_lattice() == s).all(), t
+        assert (sim.read_lattice() == s).all()
+        assert sim.observables().sweeps_done == w.sweeps
+
+
+@pytest.mark.parametrize("L,beta,D,seed,n", [(128, 1 / 1.4, 1.0, 1, 50), (320, 0.9, 1.9, 5, 20), (64, 0.3, -1.0, 2, 30)])
+def test_blume_capel_every_sweep(eng, L, beta, D, seed, n):
+    s = oracle.init(BC, L, seed)
+    tl = oracle.observables(s)
+    with eng.IsingSim(BC, L, beta, D, seed) as sim:
+        _check_obs(BC, L, D, sim.observables(), tl)
+        for t in range(n):
+            sim.sweep(1)
+            tl = oracle.sweep(BC, s, beta, D, seed, t, tl)
+            _check_obs(BC, L, D, sim.observables(), tl)
+            assert (sim.read_lattice() == s).all(), t
+
+
+@pytest.mark.parametrize("model,L,beta,D", [(ISING, 2048, wl.BETA_C / 0.9, 0.0), (BC, 1024, 1 / 1.4, 1.0),
+                                            (ISING, 1088, 0.2, 0.0), (ISING, 64, wl.BETA_C, 0.0)])
+def test_several_tiles_and_ragged_tail(eng, model, L, beta, D):
+    """Sizes that span several blocks / row chunks, a non-power-of-two L whose last
+    chunk is ragged, and the minimum L (one 128-bit vector per row)."""
+    seed, n = 11, 6
+    s = oracle.init(model, L, seed)
+    tl = oracle.observables(s)
+    with eng.IsingSim(model, L, beta, D, seed) as sim:
+        sim.sweep(n)
+        for t in range(n):
+            tl = oracle.sweep(model, s, beta, D, seed, t, tl)
+        assert (sim.read_lattice() == s).all()
+        _check_obs(model, L, D, sim.observables(), tl)
+
+
+@pytest.mark.parametrize("model", [ISING, BC])
+def test_result_independent_of_launch_geometry(eng, model):
+    """Analogue of PAPER.md:193 ('identical numerical results regardless of the number of GPUs')."""
+    L, beta, D, seed, n = 512, 0.45, 0.7, 4, 5
+    ref = None
+    for rows, block in [(0, 0), (2, 32), (6, 96), (64, 256), (512, 64), (10, 128)]:
+        with eng.IsingSim(model, L, beta, D, seed) as sim:
+            sim.set_launch(rows, block)
+            sim.sweep(n)
+            lat = sim.read_lattice()
+        if ref is None:
+            ref = lat
+            s = oracle.init(model, L, seed)
+            for t in range(n):
+                oracle.sweep(model, s, beta, D, seed, t)
+            assert (ref == s).all()
+        assert (lat == ref).all(), (rows, block)
+
+
+def test_beta_zero_flips_everything(eng):
+    """R21: beta = 0 -> every threshold is 2^32 -> every spin flips every half sweep."""
+    L = 128
+    with eng.IsingSim(ISING, L, 0.0, 0.0, 3) as sim:
+        a = sim.read_lattice()
+        sim.sweep(1)
+        assert (sim.read_lattice() == -a).all()
+        s = oracle.init(ISING, L, 3)
+        oracle.sweep(ISING, s, 0.0, 0.0, 3, 0)
+        assert (sim.read_lattice() == s).all()
+
+
+def test_large_beta_never_accepts_uphill(eng):
+    L, beta = 128, 40.0
+    s = oracle.init(ISING, L, 8)
+    with eng.IsingSim(ISING, L, beta, 0.0, 8) as sim:
+        for t in range(4):
+            sim.sweep(1)
+            oracle.sweep(ISING, s, beta, 0.0, 8, t)
+        assert (sim.read_lattice() == s).all()
+
+
+def test_resume_from_packed_checkpoint(eng):
+    """state = (lattice, t): restoring both reproduces the trajectory exactly."""
+    L, beta = 256, 0.5
+    with eng.IsingSim(ISING, L, beta, 0.0, 5) as a, eng.IsingSim(ISING, L, beta, 0.0, 5) as b:
+        a.sweep(7)
+        blk, wht = a.read_packed(0), a.read_packed(1)
+        a.sweep(5)
+        b.write_packed(0, blk)
+        b.write_packed(1, wht)
+        b.set_sweeps_done(7)
+        b.sweep(5)
+        assert (a.read_lattice() == b.read_lattice()).all()
+        assert blk.dtype == np.uint64 and len(blk) == L * L // 32
+        assert ((blk & np.uint64(0xEEEEEEEEEEEEEEEE)) == 0).all()       # Ising nibbles are 0/1
+
+
+# ----------------------------------------------------------- lattice IO ------
+@pytest.mark.parametrize("model", [ISING, BC])
+def test_write_read_roundtrip_and_closed_forms(eng, model):
+    L = 128
+    N = L * L
+    rng = np.random.default_rng(1)
+    vals = np.array([-1, 1] if model == ISING else [-1, 0, 1], dtype=np.int8)
+    with eng.IsingSim(model, L, 0.4, 1.0, 1) as sim:
+        a = rng.choice(vals, size=(L, L)).astype(np.int8)
+        sim.write_lattice(a)
+        assert (sim.read_lattice() == a).all()
+        _check_obs(model, L, 1.0, sim.observables(), oracle.observables(a))
+        assert (sim.read_window(L - 5, L - 3, 11, 9) == np.roll(a, (3, 5), axis=(0, 1))[:9, :11]).all()
+        assert (sim.read_lattice(17, 3) == a[17:20]).all()
+        b = a.copy()
+        b[40:44] = rng.choice(vals, size=(4, L))
+        sim.write_lattice(b[40:44], y0=40)
+        assert (sim.read_lattice() == b).all()
+        up = np.ones((L, L), np.int8)
+        sim.write_lattice(up)
+        o = sim.observables()
+        assert (o.bond_sum, o.M, o.Q) == (2 * N, N, N)
+        yy, xx = np.mgrid[0:L, 0:L]
+        sim.write_lattice(np.where((xx + yy) % 2 == 0, 1, -1).astype(np.int8))
+        o = sim.observables()
+        assert (o.bond_sum, o.M, o.Q) == (-2 * N, 0, N)
+        one = up.copy()
+        one[3, 5] = -1
+        sim.write_lattice(one)
+        o = sim.observables()
+        assert (o.bond_sum, o.M, o.Q) == (2 * N - 8, N - 2, N)
+        if model == BC:
+            sim.write_lattice(np.zeros((L, L), np.int8))
+            o = sim.observables()
+            assert (o.bond_sum, o.M, o.Q, o.zero_density) == (0, 0, 0, 1.0)
+        bad = up.copy()
+        bad[7, 9] = 2 if model == BC else 0
+        with pytest.raises(eng.IsingError):
+            sim.write_lattice(bad)
+        assert (sim.read_lattice() == (np.zeros((L, L), np.int8) if model == BC else one)).all()
+
+
+def test_argument_errors(eng):
+    with pytest.raises(eng.IsingError):
+        eng.IsingSim(ISING, 100, 0.4)              # L not a multiple of 64
+    with pytest.raises(eng.IsingError):
+        eng.IsingSim(2, 64, 0.4)                   # unknown model
+    with pytest.raises(eng.IsingError):
+        eng.IsingSim(ISING, 64, -0.1)              # beta < 0
+    with pytest.raises(eng.IsingError):
+        eng.IsingSim(ISING, 64, float("nan"))
+    with pytest.raises(eng.IsingError):
+        eng.IsingSim(BC, 64, 0.5, float("inf"))
+    with eng.IsingSim(ISING, 64, 0.4) as sim:
+        for bad in (lambda: sim.sweep(-1), lambda: sim.correlation(0), lambda: sim.correlation(33),
+                    lambda: sim.read_lattice(60, 8), lambda: sim.set_launch(3, 0), lambda: sim.set_launch(0, 100),
+                    lambda: sim.correlation_list(3, [1]), lambda: sim.correlation_list(1, [40])):
+            with pytest.raises(eng.IsingError):
+                bad()
+        sim.sweep(0)
+        assert sim.observables().sweeps_done == 0
+    sim2 = eng.IsingSim(ISING, 64, 0.4, use_torch_memory=False)     # library-owned memory
+    sim2.sweep(2)
+    s = oracle.init(ISING, 64, 1)
+    for t in range(2):
+        oracle.sweep(ISING, s, 0.4, 0.0, 1, t)
+    assert (sim2.read_lattice() == s).all()
+    sim2.close()
+
+
+# ------------------------------------------------------------- correlation ---
+@pytest.mark.parametrize("model,L", [(ISING, 256), (BC, 256), (ISING, 64), (BC, 192), (ISING, 576)])
+def test_correlation_full_range(eng, model, L):
+    beta, D, seed = (wl.BETA_C / 0.5, 0.0, 1) if model == ISING else (1 / 1.4, 1.0, 1)
+    with eng.IsingSim(model, L, beta, D, seed) as sim:
+        sim.sweep(8)
+        lat = sim.read_lattice()
+        sx, sy = sim.correlation(L // 2)
+        ox, oy = oracle.correlation(lat, L // 2)
+        assert (sx == ox).all() and (sy == oy).all()
+        o = sim.observables()
+        assert sx[0] + sy[0] == o.bond_sum
+        sx3, sy3 = sim.correlation(3)
+        assert (sx3 == ox[:3]).all() and (sy3 == oy[:3]).all()
+
+
+@pytest.mark.parametrize("model", [ISING, BC])
+def test_correlation_list_and_protocol(eng, model):
+    L = 1024
+    beta, D = (wl.BETA_C / 0.5, 0.0) if model == ISING else (1 / 1.4, 1.0)
+    with eng.IsingSim(model, L, beta, D, 2) as sim:
+        sim.sweep(5)
+        lat = sim.read_lattice()
+        r = np.array([1, 2, 31, 32, 33, 100, 257, 511, 512])
+        for stride in (1, 16, 4, 64):
+            sx, sy = sim.correlation_list(stride, r)
+            ox, oy = oracle.correlation_list(lat, stride, r)
+            assert (sx == ox).all() and (sy == oy).all(), stride
+        pr, px, py, pn = sim.correlation_protocol()
+        orr, ox, oy, on = oracle.correlation_protocol(lat, 5)
+        assert (pr == orr).all() and (pn == on).all() and (px == ox).all() and (py == oy).all()
+
+
+def test_protocol_distance_lists_match_oracle(eng):
+    """Host logic of Sec. 3.3 at sizes where the log grid is non-trivial (lists only)."""
+    for L, t in [(4096, 1), (4096, 3000)]:
+        with eng.IsingSim(ISING, L, 0.5, 0.0, 1) as sim:
+            sim.set_sweeps_done(t)
+            pr, px, py, pn = sim.correlation_protocol()
+            orr, ost = oracle.protocol_list(L, t)
+            assert (pr == orr).all()
+            assert (pn == np.where(ost == 1, L * L, (L // 16) ** 2)).all()
+
+
+# --------------------------------------------------------- Schwinger-Dyson ---
+@pytest.mark.parametrize("model", [ISING, BC])
+def test_schwinger_dyson_histogram(eng, model):
+    L, beta, D = 256, 0.4, 0.8
+    with eng.IsingSim(model, L, beta, D, 6) as sim:
+        sim.sweep(12)
+        v, hist = sim.schwinger_dyson()
+        ov, ohist = oracle.schwinger_dyson(sim.read_lattice(), beta)
+        assert (hist == ohist).all() and _close(v, ov)
