@@ -1,0 +1,333 @@
+#!/usr/bin/env python
+"""bench.py -- spin updates/ns of the checkerboard Metropolis hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--L L] [--sweeps-per-step S] [--model ising|bc]
+
+A "step" = S full sweeps (black + white update kernels)
+followed by one observables pass (A8: E, M every S sweeps as in BASELINE.json
+configs[1..3]).  Default workload = configs[2], the one the metric is quoted on:
+Ising L = 2^18, T = 0.9 Tc, seed 1 (32 GiB packed, far larger than L2, so no L2
+flush is needed between iterations).  Prints ONE JSON line (rank 0).
+
+value     = L^2 * S * K / (device time of the K steps), lattice resident in HBM
+e2e       = same through the C ABI with HOST buffers: every step uploads the packed
+            lattice from pinned host memory (ising_write_packed), runs S sweeps and
+            reads the observables back
+roofline  = the Ising update kernel against the measured HBM copy rate
+            (MEASURED_PEAKS.json), algorithmic bytes 0.75 B per site per colour
+            launch; roofline_alu = same kernel against the Philox-only
+            kernel (the integer-ALU roof of "one Philox number per site")
+cpu_baseline = the oracle, as it stands, timed on the host cores on a bounded sample
+
+N > 1 (torchrun): the path does not shard under north_star ("one GPU, no
+sharding"): N independent replicas (seed + rank), weak scaling, no collective on
+the data path; barrier + max-over-ranks timing only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+BYTES_PER_SITE_LAUNCH = 0.75   # per updated site: own nibble read + written, opposite nibble read once
+PAPER_UPDATES_PER_NS = None    # no published number for THIS kernel contract / hardware
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--L", type=int, default=0, help="override the lattice size (default: configs[2], 2^18)")
+    ap.add_argument("--model", default="ising", choices=["ising", "bc"])
+    ap.add_argument("--sweeps-per-step", type=int, default=10)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    return ap.parse_args()
+
+
+def pick_workload(args):
+    base = wl.config(2) if args.model == "ising" else wl.config(3)
+    L = args.L or base.L
+    name = base.name if L == base.L else f"{base.name.split('_L')[0]}_L{L}_override"
+    return base, L, name
+
+
+# ------------------------------------------------------------------ clocks ---
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------- oracle on the host ---
+def time_oracle(model: int, beta: float, D: float, seed: int, seconds: float, L: int = 4096):
+    """The oracle as it stands (oracle/ising_oracle.c, OpenMP over rows) on a bounded
+    sample of the workload: same model / beta / seed, lattice cut to L x L, as many
+    full sweeps as fit in `seconds` (at least 2).  Returns (updates/ns, cores, text)."""
+    import oracle
+    s = oracle.init(model, L, seed)
+    tl = oracle.observables(s)
+    tl = oracle.sweep(model, s, beta, D, seed, 0, tl)          # untimed first touch
+    n, t0 = 0, time.perf_counter()
+    while True:
+        tl = oracle.sweep(model, s, beta, D, seed, 1 + n, tl)
+        n += 1
+        dt = time.perf_counter() - t0
+        if (dt >= seconds and n >= 2) or n >= 100000:
+            break
+    cores = oracle.threads()
+    return L * L * n / (dt * 1e9), cores, f"{n} sweeps of the same model/beta/seed on an L={L} lattice ({dt:.1f} s)"
+
+
+def run_reference(args):
+    """--impl reference: this tier's reference arm is the oracle on the host cores."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    base, L, name = pick_workload(args)
+    model = wl.ISING if args.model == "ising" else wl.BLUME_CAPEL
+    per_step = max(1.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    vals, info, cores = [], "", 0
+    for i in range(args.warmup + args.steps):
+        v, cores, info = time_oracle(model, base.beta, base.D, base.seed, per_step)
+        if i >= args.warmup:
+            vals.append(v)
+    value = sum(vals) / len(vals)
+    line = {
+        "impl": "reference", "metric": "spin updates/ns", "value": value, "unit": "updates/ns",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": per_step * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int8 spins, u32 Philox, f64 thresholds", "data": "synthetic (seeded random start)",
+        "config": {"workload": name, "L": L, "sample": info},
+        "cpu_baseline": {"value": value, "unit": "updates/ns", "cores": cores, "kind": "oracle", "sample": info},
+        "e2e": {"value": value, "unit": "updates/ns", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------- the CUDA path ---
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy rate)", d
+    except (OSError, KeyError, ValueError):
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", {}
+
+
+def mem_available_bytes() -> int:
+    try:
+        with open("/proc/meminfo") as f:
+            for line in f:
+                if line.startswith("MemAvailable:"):
+                    return int(line.split()[1]) * 1024
+    except OSError:
+        pass
+    return 0
+
+
+def run_e2e(eng, torch, model, L, beta, D, seed, S, steps, device):
+    """End to end through the C ABI with HOST buffers: per step upload both packed
+    colour arrays from pinned host memory, run S sweeps, read the observables."""
+    colour_bytes = L * L // 4
+    need = 2 * colour_bytes
+    note = ""
+    if mem_available_bytes() < need + (8 << 30):
+        while L > 4096 and mem_available_bytes() < 2 * (L * L // 4) + (8 << 30):
+            L //= 2
+        colour_bytes = L * L // 4
+        note = f"host memory too small for the 2^18 lattice; e2e measured at L={L}"
+    words = colour_bytes // 8
+    host = [torch.empty(words, dtype=torch.int64).pin_memory() for _ in range(2)]
+    with eng.IsingSim(model, L, beta, D, seed, device=device) as sim:
+        sim.sweep(2)
+        for c in range(2):
+            sim.read_packed(c, 0, words, out=host[c])
+        times = []
+        for i in range(1 + steps):
+            torch.cuda.synchronize(device)
+            t0 = time.perf_counter()
+            for c in range(2):
+                sim.write_packed(c, host[c], 0, words)
+            sim.set_sweeps_done(2)
+            sim.sweep(S)
+            o = sim.observables()                  # synchronises; D2H of B, M, Q
+            torch.cuda.synchronize(device)
+            if i >= 1:
+                times.append(time.perf_counter() - t0)
+        assert o.n_sites == L * L
+    dt = sum(times) / len(times)
+    out = {"value": L * L * S / (dt * 1e9), "unit": "updates/ns", "h2d_bytes_per_step": 2 * colour_bytes,
+           "d2h_bytes_per_step": 24, "L": L, "sweeps_per_step": S, "steps": steps, "ms_per_step": dt * 1e3,
+           "what": "ising_write_packed(both colours, pinned host) + ising_sweep(S) + ising_observables"}
+    if note:
+        out["note"] = note
+    return out
+
+
+def run_ours(args):
+    import torch
+    import paper_2502_18624_b200 as eng
+    eng.load_library()                                     # raises if the CUDA library is missing
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device and no CPU fallback (use --impl reference for the oracle)")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    device = torch.device(f"cuda:{local}")
+    torch.cuda.set_device(device)
+
+    base, L, name = pick_workload(args)
+    model = wl.ISING if args.model == "ising" else wl.BLUME_CAPEL
+    S, K, W = args.sweeps_per_step, args.steps, max(args.warmup, 0)
+    sim = eng.IsingSim(model, L, base.beta, base.D, base.seed + rank, device=device)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(device)
+
+    def step(ev=None):
+        if ev:
+            ev[0].record()
+        sim.sweep(S)
+        if ev:
+            ev[1].record()
+        return sim.observables()
+
+    for _ in range(W):
+        step()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    e_start, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local)
+    launches0 = sim.launch_count()
+    barrier()
+    sampler.start()
+    e_start.record()
+    for k in range(K):
+        obs = step(evs[k])
+    e_end.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = sim.launch_count() - launches0
+    total_ms = e_start.elapsed_time(e_end)
+    sweep_ms = sum(a.elapsed_time(b) for a, b in evs)
+    if dist is not None:
+        t = torch.tensor([total_ms, sweep_ms], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, sweep_ms = float(t[0]), float(t[1])
+
+    # roofs, measured in the same process right after the timed region (rank 0 only matters)
+    n_roof = 2 * S
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    sim.bench_philox_only(2); sim.bench_copy(2); torch.cuda.synchronize(device)
+    ev[0].record(); sim.bench_philox_only(n_roof); ev[1].record(); sim.bench_copy(n_roof); ev[2].record()
+    torch.cuda.synchronize(device)
+    philox_ms = ev[0].elapsed_time(ev[1]) / n_roof
+    copy_ms = ev[1].elapsed_time(ev[2]) / n_roof
+    sim.close()
+
+    sites_per_launch = L * L // 2
+    kern_ms = sweep_ms / (2 * S * K)
+    peak, peak_src, peaks = measured_peaks()
+    achieved = BYTES_PER_SITE_LAUNCH * sites_per_launch / (kern_ms * 1e-3) / 1e9
+    value = world * L * L * S * K / (total_ms * 1e6)
+    line = {
+        "metric": "spin updates/ns", "value": value, "unit": "updates/ns", "n_gpus": world, "steps": K,
+        "warmup": W, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u32 (Philox4x32-10, SWAR on 4-bit spins, integer compare)",
+        "data": "synthetic (seeded random-start quench, the paper's own workload)",
+        "config": {"workload": name, "model": args.model, "L": L, "beta": base.beta, "D": base.D,
+                   "seed": base.seed, "sweeps_per_step": S, "observables_every": S,
+                   "lattice_bytes": L * L // 2, "l2": "inputs larger than L2 (no flush needed)" if L * L // 2 > (256 << 20)
+                   else "lattice fits L2: DRAM figures not meaningful", "parallelism": f"replicas x{world}"},
+        "sweep_only_updates_per_ns": world * L * L * S * K / (sweep_ms * 1e6),
+        "roofline": {"bound": "hbm", "kernel": "update_kernel (one colour phase)", "achieved": achieved,
+                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": BYTES_PER_SITE_LAUNCH * sites_per_launch,
+                     "avg_launch_ms": kern_ms,
+                     "copy_kernel_gbs": BYTES_PER_SITE_LAUNCH * sites_per_launch / (copy_ms * 1e-3) / 1e9},
+        "roofline_alu": {"bound": "alu", "what": "Philox-only kernel, same grid and calls per thread, no lattice traffic",
+                         "achieved": sites_per_launch / (kern_ms * 1e6), "peak": sites_per_launch / (philox_ms * 1e6),
+                         "unit": "updates/ns", "frac": philox_ms / kern_ms},
+        "clocks": clocks, "gpu_launches": launches,
+        "last_observables": {"bond_sum": obs.bond_sum, "M": obs.M, "sweeps_done": obs.sweeps_done},
+        "paper_context": "GB200: 1802 upd/ns (1-bit Ising, 1/2 RNG per spin), 948 upd/ns (Blume-Capel, 1 RNG per spin) -- other hardware/contract",
+    }
+    if rank == 0:
+        if not args.no_e2e:
+            line["e2e"] = run_e2e(eng, torch, model, L, base.beta, base.D, base.seed, S, min(K, 3), device)
+        if not args.no_cpu and world == 1:
+            v, cores, info = time_oracle(model, base.beta, base.D, base.seed, args.cpu_seconds)
+            line["cpu_baseline"] = {"value": v, "unit": "updates/ns", "cores": cores, "kind": "oracle", "sample": info}
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)
