@@ -15,8 +15,10 @@ e2e       = same through the C ABI with HOST buffers: every step uploads the pac
             lattice from pinned host memory (ising_write_packed), runs S sweeps and
             reads the observables back
 roofline  = the Ising update kernel against the measured HBM copy rate
-            (MEASURED_PEAKS.json), algorithmic bytes 0.75 B per site per colour
-            launch; roofline_alu = same kernel against the Philox-only
+            (MEASURED_PEAKS.json), algorithmic bytes 1.5 B per updated site
+            (DESIGN.md: own nibble read + written, opposite nibble read once);
+            `traffic` = dram bytes per launch from the committed ncu capture
+            (profiles/update_kernel_dram.csv) when it was taken at this L; roofline_alu = same kernel against the Philox-only
             kernel (the integer-ALU roof of "one Philox number per site")
 cpu_baseline = the oracle, as it stands, timed on the host cores on a bounded sample
 
@@ -40,7 +42,7 @@ if ROOT not in sys.path:
 
 import workloads as wl  # noqa: E402
 
-BYTES_PER_SITE_LAUNCH = 0.75   # per updated site: own nibble read + written, opposite nibble read once
+BYTES_PER_SITE_LAUNCH = 1.5    # per UPDATED site: own nibble read + written, opposite nibble read once (3 x 4 bit)
 PAPER_UPDATES_PER_NS = None    # no published number for THIS kernel contract / hardware
 
 
@@ -167,6 +169,21 @@ def measured_peaks():
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy rate)", d
     except (OSError, KeyError, ValueError):
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", {}
+
+
+def ncu_traffic(model: str, L: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum per update launch from the committed
+    ncu --set full capture (a number measured under the profiler: reported, never timed)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "update_kernel_dram.csv")) as f:
+            import csv
+            rows = list(csv.reader(ln for ln in f if ln.strip() and not ln.startswith("#")))
+        hdr = rows[0]
+        vals = [float(r[hdr.index("dram_read_bytes")]) + float(r[hdr.index("dram_write_bytes")])
+                for r in rows[1:] if r[hdr.index("model")] == model and int(r[hdr.index("L")]) == L]
+        return sum(vals) / len(vals) if vals else None
+    except (OSError, ValueError, IndexError):
+        return None
 
 
 def mem_available_bytes() -> int:
@@ -302,7 +319,7 @@ def run_ours(args):
                    else "lattice fits L2: DRAM figures not meaningful", "parallelism": f"replicas x{world}"},
         "sweep_only_updates_per_ns": world * L * L * S * K / (sweep_ms * 1e6),
         "roofline": {"bound": "hbm", "kernel": "update_kernel (one colour phase)", "achieved": achieved,
-                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic(args.model, L),
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": BYTES_PER_SITE_LAUNCH * sites_per_launch,
                      "avg_launch_ms": kern_ms,
                      "copy_kernel_gbs": BYTES_PER_SITE_LAUNCH * sites_per_launch / (copy_ms * 1e-3) / 1e9},
