@@ -22,6 +22,8 @@ struct UpdParams {
     uint32_t colour, t;
     uint32_t T4, T8;        // Ising thresholds for dE = 4, 8 (used when < 2^32)
     uint32_t always4, always8;  // ONES if the threshold is 2^32 (beta = 0), else 0
+    uint32_t C4, C8;            // carry form: [r >= T] = carry out of r + (2^32 - T); 0 when T is 0 or 2^32
+    uint32_t Kc;                // (8 - number of thresholds that are 0) in every nibble
     const uint32_t *bc_table;   // Blume-Capel table (device)
     RoundKeys rk;
 };
@@ -84,7 +86,39 @@ __device__ __forceinline__ uint32_t ising_half(uint32_t x, uint32_t up, uint32_t
     return x ^ flip;
 }
 
-template <int P>
+// Carry-chain form of the same rule (default variant).  Per site
+//     g = [r >= T4] + [r >= T8]          (T8 <= T4, so g = 0 iff r < T8 and g <= 1 iff r < T4)
+//     flip iff d >= g                    (d = 0: r < T8;  d = 1: r < T4;  d >= 2: always)
+// [r >= T] is the carry out of r + (2^32 - T): one IADD3 on the ALU pipe, and the carry is
+// shifted into the nibble accumulator G by an IMAD.X (G = 16 G + carry) on the FMA pipe, which
+// has spare dispatch slots next to the Philox IMAD.WIDEs.  T = 2^32 gives
+// C = 0 (never a carry, always flip); T = 0 is folded into Kc (always a "carry").
+__device__ __forceinline__ uint32_t carry2(uint32_t G, uint32_t r, uint32_t C4, uint32_t C8)
+{
+    asm("{\n\t.reg .u32 t;\n\t"
+        "add.cc.u32 t, %1, %2;\n\t"
+        "madc.lo.u32 %0, %0, 16, 0;\n\t"
+        "add.cc.u32 t, %1, %3;\n\t"
+        "addc.u32 %0, %0, 0;\n\t}"
+        : "+r"(G) : "r"(r), "r"(C4), "r"(C8));
+    return G;
+}
+
+__device__ __forceinline__ uint32_t ising_half_carry(uint32_t x, uint32_t up, uint32_t dn, uint32_t sm, uint32_t sd,
+                                                     const uint4 &ra, const uint4 &rb, const UpdParams &p)
+{
+    uint32_t G = 0;                        // nibble j <- g of site j: highest site first
+    G = carry2(G, rb.w, p.C4, p.C8); G = carry2(G, rb.z, p.C4, p.C8);
+    G = carry2(G, rb.y, p.C4, p.C8); G = carry2(G, rb.x, p.C4, p.C8);
+    G = carry2(G, ra.w, p.C4, p.C8); G = carry2(G, ra.z, p.C4, p.C8);
+    G = carry2(G, ra.y, p.C4, p.C8); G = carry2(G, ra.x, p.C4, p.C8);
+    uint32_t n = up + dn + sm + sd;        // neighbours that are +1, per nibble (0..4)
+    uint32_t d = (n ^ (x * 7u)) - x * 3u;  // x = 1: 4 - n = (n ^ 7) - 3;  x = 0: n
+    uint32_t F = d + p.Kc - G;             // per nibble d + 8 - g in [6, 12]: bit 3 set iff d >= g
+    return x ^ ((F >> 3) & ONES);
+}
+
+template <int P, int V>
 __device__ __forceinline__ uint4 ising_row(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
                                            uint32_t edge, uint64_t g0, uint32_t tag, const UpdParams &p)
 {
@@ -97,10 +131,17 @@ __device__ __forceinline__ uint4 ising_row(const uint4 &src, const uint4 &up, co
     uint4 r4 = philox_site4(gl | 4, pr, p.rk), r5 = philox_site4(gl | 5, pr, p.rk);
     uint4 r6 = philox_site4(gl | 6, pr, p.rk), r7 = philox_site4(gl | 7, pr, p.rk);
     uint4 o;
-    o.x = ising_half(src.x, up.x, dn.x, sm.x, sd[0], r0, r1, p);
-    o.y = ising_half(src.y, up.y, dn.y, sm.y, sd[1], r2, r3, p);
-    o.z = ising_half(src.z, up.z, dn.z, sm.z, sd[2], r4, r5, p);
-    o.w = ising_half(src.w, up.w, dn.w, sm.w, sd[3], r6, r7, p);
+    if (V == 0) {
+        o.x = ising_half_carry(src.x, up.x, dn.x, sm.x, sd[0], r0, r1, p);
+        o.y = ising_half_carry(src.y, up.y, dn.y, sm.y, sd[1], r2, r3, p);
+        o.z = ising_half_carry(src.z, up.z, dn.z, sm.z, sd[2], r4, r5, p);
+        o.w = ising_half_carry(src.w, up.w, dn.w, sm.w, sd[3], r6, r7, p);
+    } else {
+        o.x = ising_half(src.x, up.x, dn.x, sm.x, sd[0], r0, r1, p);
+        o.y = ising_half(src.y, up.y, dn.y, sm.y, sd[1], r2, r3, p);
+        o.z = ising_half(src.z, up.z, dn.z, sm.z, sd[2], r4, r5, p);
+        o.w = ising_half(src.w, up.w, dn.w, sm.w, sd[3], r6, r7, p);
+    }
     return o;
 }
 
@@ -157,7 +198,7 @@ __device__ __forceinline__ uint4 bc_row(const uint4 &src, const uint4 &up, const
 }
 
 // ----------------------------------------------------------------- kernel ---
-template <int MODEL, int C>
+template <int MODEL, int C, int V>
 __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ UpdParams p)
 {
     __shared__ uint32_t s_tab[66];
@@ -196,7 +237,7 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
         uint32_t nedge = opp32[(size_t)y1 * halves + e_odd];
         uint4 dn2 = p.opp[(size_t)y2 * cols + col];
         uint4 o;
-        if (MODEL == ISING_MODEL_ISING) o = ising_row<C>(src, up, sm, dn, edge, g0, p.colour, p);
+        if (MODEL == ISING_MODEL_ISING) o = ising_row<C, V>(src, up, sm, dn, edge, g0, p.colour, p);
         else o = bc_row<C>(src, up, sm, dn, edge, g0, p.colour, p, s_tab, always);
         p.own[(size_t)y * cols + col] = o;
         g0 += (uint64_t)(cols * 8);
@@ -207,7 +248,7 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
             nsrc2 = p.own[(size_t)(y + 2) * cols + col];
             nedge2 = opp32[(size_t)(y + 2) * halves + e_even];
         }
-        if (MODEL == ISING_MODEL_ISING) o = ising_row<1 - C>(nsrc, sm, dn, dn2, nedge, g0, p.colour, p);
+        if (MODEL == ISING_MODEL_ISING) o = ising_row<1 - C, V>(nsrc, sm, dn, dn2, nedge, g0, p.colour, p);
         else o = bc_row<1 - C>(nsrc, sm, dn, dn2, nedge, g0, p.colour, p, s_tab, always);
         p.own[(size_t)y1 * cols + col] = o;
         g0 += (uint64_t)(cols * 8);
@@ -226,6 +267,10 @@ cudaError_t launch_update(ising_sim *h, int colour, uint32_t t)
     const uint64_t T4 = h->T[3], T8 = h->T[4];
     p.T4 = (uint32_t)T4; p.T8 = (uint32_t)T8;
     p.always4 = (T4 >> 32) ? ONES : 0u; p.always8 = (T8 >> 32) ? ONES : 0u;
+    // carry constants: 2^32 - T for 0 < T < 2^32; T = 2^32 -> 0 (never a carry); T = 0 -> counted in Kc
+    p.C4 = (T4 == 0 || (T4 >> 32)) ? 0u : (uint32_t)((1ull << 32) - T4);
+    p.C8 = (T8 == 0 || (T8 >> 32)) ? 0u : (uint32_t)((1ull << 32) - T8);
+    p.Kc = ONES * (8u - (T4 == 0 ? 1u : 0u) - (T8 == 0 ? 1u : 0u));
     p.bc_table = h->d_bc_table;
     p.rk = h->rk;
     int64_t chunks = (L + p.R - 1) / p.R;
@@ -233,11 +278,16 @@ cudaError_t launch_update(ising_sim *h, int colour, uint32_t t)
     int block = h->block_threads;
     unsigned grid = (unsigned)((threads + block - 1) / block);
     if (h->model == ISING_MODEL_ISING) {
-        if (colour == 0) update_kernel<ISING_MODEL_ISING, 0><<<grid, block, 0, h->stream>>>(p);
-        else update_kernel<ISING_MODEL_ISING, 1><<<grid, block, 0, h->stream>>>(p);
+        if (h->variant == 0) {
+            if (colour == 0) update_kernel<ISING_MODEL_ISING, 0, 0><<<grid, block, 0, h->stream>>>(p);
+            else update_kernel<ISING_MODEL_ISING, 1, 0><<<grid, block, 0, h->stream>>>(p);
+        } else {
+            if (colour == 0) update_kernel<ISING_MODEL_ISING, 0, 1><<<grid, block, 0, h->stream>>>(p);
+            else update_kernel<ISING_MODEL_ISING, 1, 1><<<grid, block, 0, h->stream>>>(p);
+        }
     } else {
-        if (colour == 0) update_kernel<ISING_MODEL_BLUME_CAPEL, 0><<<grid, block, 0, h->stream>>>(p);
-        else update_kernel<ISING_MODEL_BLUME_CAPEL, 1><<<grid, block, 0, h->stream>>>(p);
+        if (colour == 0) update_kernel<ISING_MODEL_BLUME_CAPEL, 0, 0><<<grid, block, 0, h->stream>>>(p);
+        else update_kernel<ISING_MODEL_BLUME_CAPEL, 1, 0><<<grid, block, 0, h->stream>>>(p);
     }
     h->launches++;
     return cudaGetLastError();

@@ -161,6 +161,25 @@ def test_large_beta_never_accepts_uphill(eng):
         assert (sim.read_lattice() == s).all()
 
 
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("beta", [0.0, 0.1, wl.BETA_C, wl.BETA_C / 0.5, 3.0, 5.5, 5.6, 40.0])
+def test_ising_kernel_variants_and_threshold_edge_cases(eng, variant, beta):
+    """Both implementations of the flip rule (carry chain = default, compare/select) against the
+    oracle, over thresholds that are 2^32 (beta = 0), ordinary, T8 = 0 < T4 (beta = 3: e^-24 2^32 < 1),
+    T4 = 1 (beta = 5.5) and both 0 (beta = 5.6, 40)."""
+    L, seed, n = 256, 21, 8
+    s = oracle.init(ISING, L, seed)
+    tl = oracle.observables(s)
+    with eng.IsingSim(ISING, L, beta, 0.0, seed) as sim:
+        sim.set_variant(variant)
+        assert (sim.thresholds() == oracle.thresholds(ISING, beta)).all()
+        for t in range(n):
+            sim.sweep(1)
+            tl = oracle.sweep(ISING, s, beta, 0.0, seed, t, tl)
+            assert (sim.read_lattice() == s).all(), (variant, beta, t)
+        _check_obs(ISING, L, 0.0, sim.observables(), tl)
+
+
 def test_resume_from_packed_checkpoint(eng):
     """state = (lattice, t): restoring both reproduces the trajectory exactly."""
     L, beta = 256, 0.5
