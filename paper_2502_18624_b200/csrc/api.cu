@@ -117,20 +117,30 @@ extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_
     h->lat[0] = (uint64_t *)base;
     h->lat[1] = (uint64_t *)(base + colour_bytes);
     h->d_acc = (long long *)(base + 2 * colour_bytes);                 // 64 int64 = 512 B (+ 4 KiB sink area unused)
-    h->d_bc_table = (uint32_t *)(base + 2 * colour_bytes + 1024);      // 66 uint32
+    h->d_bc_table = (uint32_t *)(base + 2 * colour_bytes + 1024);      // 212 uint32 (two table forms)
     build_thresholds(h);
     build_round_keys(h);
     default_launch(h);
-    cudaError_t e = cudaMallocHost(&h->h_acc, 64 * sizeof(long long));
+    cudaError_t e = cudaMallocHost(&h->h_acc, 256 * sizeof(long long));
     if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "cudaMallocHost"); }
     if (model == ISING_MODEL_BLUME_CAPEL) {
-        uint32_t tab[66] = {};
+        // [0, 66): thresholds clamped to 2^32-1 + "always" bit mask (compare/select variant).
+        // [80, 80 + 132): carry form for the default variant, two halves of 66 words (264 bytes):
+        // C[b][16 code + S] = 2^32 - T, 0 for T = 2^32 (never a carry -> always accepted).  T = 0 has
+        // no 32-bit carry constant: launch_update then uses the compare/select variant.
+        uint32_t tab[80 + 132] = {};
         uint64_t always = 0;
         for (int i = 0; i < 54; ++i) {
             if (h->T[i] >> 32) { always |= 1ull << i; tab[i] = 0xFFFFFFFFu; }
             else tab[i] = (uint32_t)h->T[i];
         }
         tab[64] = (uint32_t)always; tab[65] = (uint32_t)(always >> 32);
+        for (int code = 0; code < 3; ++code)
+            for (int S = 0; S <= 8; ++S)
+                for (int b = 0; b < 2; ++b) {
+                    const uint64_t T = h->T[(code * 2 + b) * 9 + S];
+                    tab[80 + 66 * b + 16 * code + S] = (T >> 32) ? 0u : (uint32_t)((1ull << 32) - T);
+                }
         memcpy(h->h_acc, tab, sizeof(tab));
         e = cudaMemcpyAsync(h->d_bc_table, h->h_acc, sizeof(tab), cudaMemcpyHostToDevice, h->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);

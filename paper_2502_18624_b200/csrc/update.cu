@@ -197,17 +197,92 @@ __device__ __forceinline__ uint4 bc_row(const uint4 &src, const uint4 &up, const
     return o;
 }
 
+// Carry form (default variant; launch_update falls back to the compare/select variant when a
+// threshold is exactly 0, which the 32-bit carry constant cannot express).  Table entry
+// C[b][16 code + S] = 2^32 - T (0 for T = 2^32) in shared memory (api.cu): the site is REJECTED
+// iff r + C carries.  Per site: one PRMT picks the pre-scaled index byte 4 (16 code + S),
+// b = r & 1, one LDS, one IADD3 (carry) and
+// IMAD.X / IMAD accumulate the reject and proposal nibbles; everything else is word-level.
+__device__ __forceinline__ void bc_site(uint32_t &G, uint32_t &Gb, uint32_t e4, uint32_t r, const unsigned char *tab)
+{
+    // b is produced once and feeds both the table address (b = 1 half of the table starts at
+    // byte 264) and the proposal accumulator through IMADs (FMA pipe); PTX keeps that split.
+    uint32_t b, addr;
+    asm("and.b32 %0, %2, 1;\n\t"
+        "mad.lo.u32 %1, %0, 264, %3;"
+        : "=&r"(b), "=r"(addr) : "r"(r), "r"(e4));
+    const uint32_t Cj = *reinterpret_cast<const uint32_t *>(tab + addr);
+    asm("{\n\t.reg .u32 t;\n\t"
+        "add.cc.u32 t, %1, %2;\n\t"
+        "madc.lo.u32 %0, %0, 16, 0;\n\t}"
+        : "+r"(G) : "r"(r), "r"(Cj));
+    asm("mad.lo.u32 %0, %0, 16, %1;" : "+r"(Gb) : "r"(b));
+}
+
+__device__ __forceinline__ uint32_t bc_half_carry(uint32_t x, uint32_t up, uint32_t dn, uint32_t sm, uint32_t sd,
+                                                  const uint4 &ra, const uint4 &rb, const unsigned char *tab)
+{
+    const uint32_t S = up + dn + sm + sd;                 // neighbour code sum per nibble, 0..8
+    // index bytes 4 (16 code + S) = (code << 6) | (S << 2): even sites from the low nibbles, odd from the high
+    const uint32_t Be = ((S << 2) & 0x3C3C3C3Cu) | ((x << 6) & 0xC3C3C3C3u);
+    const uint32_t Bo = ((S >> 2) & 0x3C3C3C3Cu) | ((x << 2) & 0xC3C3C3C3u);
+    uint32_t G = 0, Gb = 0;                               // reject / proposal-bit nibbles, highest site first
+    bc_site(G, Gb, __byte_perm(Bo, 0, 0x4443), rb.w, tab);
+    bc_site(G, Gb, __byte_perm(Be, 0, 0x4443), rb.z, tab);
+    bc_site(G, Gb, __byte_perm(Bo, 0, 0x4442), rb.y, tab);
+    bc_site(G, Gb, __byte_perm(Be, 0, 0x4442), rb.x, tab);
+    bc_site(G, Gb, __byte_perm(Bo, 0, 0x4441), ra.w, tab);
+    bc_site(G, Gb, __byte_perm(Be, 0, 0x4441), ra.z, tab);
+    bc_site(G, Gb, __byte_perm(Bo, 0, 0x4440), ra.y, tab);
+    bc_site(G, Gb, __byte_perm(Be, 0, 0x4440), ra.x, tab);
+    // accepted sites move by 1 + b (mod 3)
+    const uint32_t acc3 = 0x33333333u - 3u * G;           // 3 where accepted, 0 where rejected
+    const uint32_t y = x + ((ONES + Gb) & acc3);          // 0..4
+    const uint32_t ge3 = ((y + ONES) >> 2) & ONES;
+    return y - 3u * ge3;
+}
+
+template <int P>
+__device__ __forceinline__ uint4 bc_row_carry(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
+                                              uint32_t edge, uint64_t g0, uint32_t tag, const UpdParams &p,
+                                              const unsigned char *tab)
+{
+    uint32_t sd[4];
+    side_words<P>(sm, edge, sd);
+    PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), p.t, tag, p.rk);
+    uint32_t gl = (uint32_t)g0;
+    uint4 o;
+    {
+        uint4 ra = philox_site4(gl | 0, pr, p.rk), rb = philox_site4(gl | 1, pr, p.rk);
+        o.x = bc_half_carry(src.x, up.x, dn.x, sm.x, sd[0], ra, rb, tab);
+    }
+    {
+        uint4 ra = philox_site4(gl | 2, pr, p.rk), rb = philox_site4(gl | 3, pr, p.rk);
+        o.y = bc_half_carry(src.y, up.y, dn.y, sm.y, sd[1], ra, rb, tab);
+    }
+    {
+        uint4 ra = philox_site4(gl | 4, pr, p.rk), rb = philox_site4(gl | 5, pr, p.rk);
+        o.z = bc_half_carry(src.z, up.z, dn.z, sm.z, sd[2], ra, rb, tab);
+    }
+    {
+        uint4 ra = philox_site4(gl | 6, pr, p.rk), rb = philox_site4(gl | 7, pr, p.rk);
+        o.w = bc_half_carry(src.w, up.w, dn.w, sm.w, sd[3], ra, rb, tab);
+    }
+    return o;
+}
+
 // ----------------------------------------------------------------- kernel ---
 template <int MODEL, int C, int V>
 __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ UpdParams p)
 {
-    __shared__ uint32_t s_tab[66];
+    __shared__ __align__(16) uint32_t s_tab[80 + 132];   // both table forms (api.cu)
     uint64_t always = 0;
     if (MODEL == ISING_MODEL_BLUME_CAPEL) {
-        for (int i = threadIdx.x; i < 66; i += blockDim.x) s_tab[i] = p.bc_table[i];
+        for (int i = threadIdx.x; i < 80 + 132; i += blockDim.x) s_tab[i] = p.bc_table[i];
         __syncthreads();
         always = (uint64_t)s_tab[64] | ((uint64_t)s_tab[65] << 32);
     }
+    const unsigned char *ctab = reinterpret_cast<const unsigned char *>(s_tab + 80);
     const int cols = p.cols, L = p.L;
     unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
     unsigned chunk = tid / (unsigned)cols;
@@ -238,6 +313,7 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
         uint4 dn2 = p.opp[(size_t)y2 * cols + col];
         uint4 o;
         if (MODEL == ISING_MODEL_ISING) o = ising_row<C, V>(src, up, sm, dn, edge, g0, p.colour, p);
+        else if (V == 0) o = bc_row_carry<C>(src, up, sm, dn, edge, g0, p.colour, p, ctab);
         else o = bc_row<C>(src, up, sm, dn, edge, g0, p.colour, p, s_tab, always);
         p.own[(size_t)y * cols + col] = o;
         g0 += (uint64_t)(cols * 8);
@@ -249,6 +325,7 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
             nedge2 = opp32[(size_t)(y + 2) * halves + e_even];
         }
         if (MODEL == ISING_MODEL_ISING) o = ising_row<1 - C, V>(nsrc, sm, dn, dn2, nedge, g0, p.colour, p);
+        else if (V == 0) o = bc_row_carry<1 - C>(nsrc, sm, dn, dn2, nedge, g0, p.colour, p, ctab);
         else o = bc_row<1 - C>(nsrc, sm, dn, dn2, nedge, g0, p.colour, p, s_tab, always);
         p.own[(size_t)y1 * cols + col] = o;
         g0 += (uint64_t)(cols * 8);
@@ -286,8 +363,15 @@ cudaError_t launch_update(ising_sim *h, int colour, uint32_t t)
             else update_kernel<ISING_MODEL_ISING, 1, 1><<<grid, block, 0, h->stream>>>(p);
         }
     } else {
-        if (colour == 0) update_kernel<ISING_MODEL_BLUME_CAPEL, 0, 0><<<grid, block, 0, h->stream>>>(p);
-        else update_kernel<ISING_MODEL_BLUME_CAPEL, 1, 0><<<grid, block, 0, h->stream>>>(p);
+        bool never = false;                       // a threshold that is exactly 0
+        for (int i = 0; i < h->n_T; ++i) never = never || h->T[i] == 0;
+        if (h->variant == 0 && !never) {
+            if (colour == 0) update_kernel<ISING_MODEL_BLUME_CAPEL, 0, 0><<<grid, block, 0, h->stream>>>(p);
+            else update_kernel<ISING_MODEL_BLUME_CAPEL, 1, 0><<<grid, block, 0, h->stream>>>(p);
+        } else {
+            if (colour == 0) update_kernel<ISING_MODEL_BLUME_CAPEL, 0, 1><<<grid, block, 0, h->stream>>>(p);
+            else update_kernel<ISING_MODEL_BLUME_CAPEL, 1, 1><<<grid, block, 0, h->stream>>>(p);
+        }
     }
     h->launches++;
     return cudaGetLastError();

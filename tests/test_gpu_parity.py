@@ -180,6 +180,25 @@ def test_ising_kernel_variants_and_threshold_edge_cases(eng, variant, beta):
         _check_obs(ISING, L, 0.0, sim.observables(), tl)
 
 
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("beta,D", [(0.0, 1.0), (1 / 1.4, 1.0), (0.4, -1.5), (2.0, 1.966), (12.0, 0.5), (30.0, 3.0)])
+def test_blume_capel_kernel_variants_and_threshold_edge_cases(eng, variant, beta, D):
+    """Carry-table kernel (default) and compare/select kernel against the oracle: all thresholds
+    2^32 (beta = 0), ordinary tables, negative D, and tables holding exact zeros (beta = 12, 30:
+    the default variant must fall back, see launch_update)."""
+    L, seed, n = 192, 33, 6
+    s = oracle.init(BC, L, seed)
+    tl = oracle.observables(s)
+    with eng.IsingSim(BC, L, beta, D, seed) as sim:
+        sim.set_variant(variant)
+        assert (sim.thresholds() == oracle.thresholds(BC, beta, D)).all()
+        for t in range(n):
+            sim.sweep(1)
+            tl = oracle.sweep(BC, s, beta, D, seed, t, tl)
+            assert (sim.read_lattice() == s).all(), (variant, beta, D, t)
+        _check_obs(BC, L, D, sim.observables(), tl)
+
+
 def test_resume_from_packed_checkpoint(eng):
     """state = (lattice, t): restoring both reproduces the trajectory exactly."""
     L, beta = 256, 0.5
