@@ -236,6 +236,26 @@ def run_e2e(eng, torch, model, L, beta, D, seed, S, steps, device):
     return out
 
 
+def max_over_ranks(values, dist, device):
+    """Element-wise MAX over all ranks of a list of floats (device times in ms); the only
+    cross-rank step of the replicas-only N > 1 run.  dist = None: single process."""
+    if dist is None:
+        return [float(v) for v in values]
+    import torch
+    t = torch.tensor([float(v) for v in values], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_updates_per_ns(world: int, L: int, sweeps: int, steps: int, total_ms: float) -> float:
+    """N independent replicas of the same size: every rank does L^2 * sweeps * steps updates."""
+    return world * L * L * sweeps * steps / (total_ms * 1e6)
+
+
+def replica_seed(base_seed: int, rank: int) -> int:
+    return base_seed + rank
+
+
 def run_ours(args):
     import torch
     import paper_2502_18624_b200 as eng
@@ -256,7 +276,7 @@ def run_ours(args):
     base, L, name = pick_workload(args)
     model = wl.ISING if args.model == "ising" else wl.BLUME_CAPEL
     S, K, W = args.sweeps_per_step, args.steps, max(args.warmup, 0)
-    sim = eng.IsingSim(model, L, base.beta, base.D, base.seed + rank, device=device)
+    sim = eng.IsingSim(model, L, base.beta, base.D, replica_seed(base.seed, rank), device=device)
 
     def barrier():
         if dist is not None:
@@ -288,10 +308,7 @@ def run_ours(args):
     launches = sim.launch_count() - launches0
     total_ms = e_start.elapsed_time(e_end)
     sweep_ms = sum(a.elapsed_time(b) for a, b in evs)
-    if dist is not None:
-        t = torch.tensor([total_ms, sweep_ms], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, sweep_ms = float(t[0]), float(t[1])
+    total_ms, sweep_ms = max_over_ranks([total_ms, sweep_ms], dist, device)
 
     # roofs, measured in the same process right after the timed region (rank 0 only matters)
     n_roof = 2 * S
@@ -307,7 +324,7 @@ def run_ours(args):
     kern_ms = sweep_ms / (2 * S * K)
     peak, peak_src, peaks = measured_peaks()
     achieved = BYTES_PER_SITE_LAUNCH * sites_per_launch / (kern_ms * 1e-3) / 1e9
-    value = world * L * L * S * K / (total_ms * 1e6)
+    value = whole_job_updates_per_ns(world, L, S, K, total_ms)
     line = {
         "metric": "spin updates/ns", "value": value, "unit": "updates/ns", "n_gpus": world, "steps": K,
         "warmup": W, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
