@@ -55,6 +55,9 @@ def parse_args():
     ap.add_argument("--L", type=int, default=0, help="override the lattice size (default: configs[2], 2^18)")
     ap.add_argument("--model", default="ising", choices=["ising", "bc"])
     ap.add_argument("--sweeps-per-step", type=int, default=10)
+    ap.add_argument("--rows-per-thread", type=int, default=0, help="update-kernel launch geometry (0 = library default)")
+    ap.add_argument("--block", type=int, default=0, help="update-kernel threads per block (0 = library default)")
+    ap.add_argument("--variant", type=int, default=0, help="update-kernel variant (0 = default carry form)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
@@ -277,6 +280,10 @@ def run_ours(args):
     model = wl.ISING if args.model == "ising" else wl.BLUME_CAPEL
     S, K, W = args.sweeps_per_step, args.steps, max(args.warmup, 0)
     sim = eng.IsingSim(model, L, base.beta, base.D, replica_seed(base.seed, rank), device=device)
+    if args.rows_per_thread or args.block:
+        sim.set_launch(args.rows_per_thread, args.block)
+    if args.variant:
+        sim.set_variant(args.variant)
 
     def barrier():
         if dist is not None:
@@ -332,6 +339,8 @@ def run_ours(args):
         "data": "synthetic (seeded random-start quench, the paper's own workload)",
         "config": {"workload": name, "model": args.model, "L": L, "beta": base.beta, "D": base.D,
                    "seed": base.seed, "sweeps_per_step": S, "observables_every": S,
+                   "launch": {"rows_per_thread": args.rows_per_thread or "default", "block": args.block or "default",
+                              "variant": args.variant},
                    "lattice_bytes": L * L // 2, "l2": "inputs larger than L2 (no flush needed)" if L * L // 2 > (256 << 20)
                    else "lattice fits L2: DRAM figures not meaningful", "parallelism": f"replicas x{world}"},
         "sweep_only_updates_per_ns": world * L * L * S * K / (sweep_ms * 1e6),
