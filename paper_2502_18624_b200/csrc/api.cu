@@ -158,6 +158,7 @@ extern "C" int ising_destroy(ising_t *h)
     cudaStreamSynchronize(h->stream);
     if (h->io_stage) cudaFree(h->io_stage);
     if (h->planes) cudaFree(h->planes);
+    if (h->comb) cudaFree(h->comb);
     if (h->d_corr) cudaFree(h->d_corr);
     if (h->d_rlist) cudaFree(h->d_rlist);
     if (h->h_acc) cudaFreeHost(h->h_acc);
@@ -360,6 +361,18 @@ static int ensure_planes(ising_sim *h)
     return ISING_OK;
 }
 
+static int ensure_comb(ising_sim *h, int64_t stride)
+{
+    const size_t bytes = (size_t)h->L * (size_t)comb_words_per_row(h->L, stride) * 8 *
+                         (h->model == ISING_MODEL_ISING ? 2 : 4);
+    if (h->comb_bytes >= bytes) return ISING_OK;
+    if (h->comb) { cudaFree(h->comb); h->comb = nullptr; h->comb_bytes = 0; }
+    cudaError_t e = cudaMalloc((void **)&h->comb, bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); h->comb = nullptr; return set_error(ISING_ENOMEM, "comb planes: cudaMalloc failed"); }
+    h->comb_bytes = bytes;
+    return ISING_OK;
+}
+
 static int ensure_corr(ising_sim *h, int64_t count)
 {
     const size_t bytes = (size_t)count * 2 * sizeof(long long);
@@ -386,6 +399,7 @@ static int run_corr(ising_sim *h, int64_t stride, int64_t count, const int64_t *
 {
     int rc = ensure_corr(h, count);
     if (rc) return rc;
+    if (stride >= 2) { rc = ensure_comb(h, stride); if (rc) return rc; }
     long long *d_sx = h->d_corr, *d_sy = h->d_corr + count;
     if (stride > 0)
         CUDA_TRY(cudaMemcpyAsync(h->d_rlist, r, (size_t)count * sizeof(long long), cudaMemcpyHostToDevice, h->stream));

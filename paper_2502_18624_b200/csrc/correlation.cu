@@ -58,34 +58,79 @@ __global__ void __launch_bounds__(128) corr_full_kernel(const uint64_t *__restri
             }
         }
     }
+    // warp shuffle -> shared memory across the block's warps -> one int64 atomic per distance per block
+    __shared__ int red[4][TR];
 #pragma unroll
     for (int k = 0; k < TR; ++k) {
         int v = acc[k];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-        if (lane == 0 && r0 + k <= rmax) atomicAdd((unsigned long long *)&accum[r0 + k - 1], (unsigned long long)(long long)v);
+        if (lane == 0) red[warp][k] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < TR) {
+        const int k = threadIdx.x;
+        long long v = 0;
+        for (int w = 0; w < nwarp; ++w) v += red[w][k];
+        if (r0 + k <= rmax && v) atomicAdd((unsigned long long *)&accum[r0 + k - 1], (unsigned long long)v);
     }
 }
 
 // ----------------------------------------- explicit distance list + stride ---
-// One block per distance.  Sources: rows y % stride == 0, bits x % stride == 0.
+// Sources: rows y % stride == 0, bits x % stride == 0; the partner (x, y + r) sits on the same
+// comb of bits, so for stride >= 2 the planes are first down-sampled to that comb (all rows,
+// L / stride bits per row, zero padded to whole words): 1/stride of the traffic and of the
+// XOR + POPC work.  stride = 1 runs on the full planes.
+
+// bits 0, 2, 4, ... of x gathered into the low 32 bits
+__device__ __forceinline__ uint64_t gather_even(uint64_t x)
+{
+    x &= 0x5555555555555555ull;
+    x = (x | (x >> 1)) & 0x3333333333333333ull;
+    x = (x | (x >> 2)) & 0x0F0F0F0F0F0F0F0Full;
+    x = (x | (x >> 4)) & 0x00FF00FF00FF00FFull;
+    x = (x | (x >> 8)) & 0x0000FFFF0000FFFFull;
+    x = (x | (x >> 16)) & 0x00000000FFFFFFFFull;
+    return x;
+}
+
+// out[y][cw] packs, for j = 0..stride-1, the 64/stride comb bits of in[y][cw * stride + j]
+__global__ void __launch_bounds__(256) comb_kernel(const uint64_t *__restrict__ in, uint64_t *__restrict__ out,
+                                                   int L, int Wq, int Wc, int log2s)
+{
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (int64_t)L * Wc) return;
+    const int y = (int)(idx / Wc), cw = (int)(idx - (int64_t)y * Wc);
+    const int s = 1 << log2s, bits = 64 >> log2s;
+    uint64_t o = 0;
+    for (int j = 0; j < s; ++j) {
+        const int q = cw * s + j;
+        if (q >= Wq) break;
+        uint64_t w = in[(size_t)y * Wq + q];
+        for (int k = 0; k < log2s; ++k) w = gather_even(w);
+        o |= w << (j * bits);
+    }
+    out[idx] = o;
+}
+
+// One block per distance.  W = words per row of the planes handed in (full or comb).
 template <int MODEL>
 __global__ void __launch_bounds__(256) corr_list_kernel(const uint64_t *__restrict__ sg, const uint64_t *__restrict__ nz,
-                                                        int L, int Wq, int stride, uint64_t mask,
+                                                        int L, int W, int stride,
                                                         const long long *__restrict__ rlist, long long *__restrict__ out)
 {
     const int r = (int)rlist[blockIdx.x];
     long long acc = 0;
     const int rows = L / stride;
-    for (int idx = threadIdx.x; idx < rows * Wq; idx += blockDim.x) {
-        int yi = idx / Wq, q = idx - yi * Wq;
+    for (int idx = threadIdx.x; idx < rows * W; idx += blockDim.x) {
+        int yi = idx / W, q = idx - yi * W;
         int y = yi * stride;
         int yb = y + r;
         if (yb >= L) yb -= L;
-        uint64_t a = sg[(size_t)y * Wq + q], b = sg[(size_t)yb * Wq + q];
-        if (MODEL == ISING_MODEL_ISING) acc += __popcll((a ^ b) & mask);
+        uint64_t a = sg[(size_t)y * W + q], b = sg[(size_t)yb * W + q];
+        if (MODEL == ISING_MODEL_ISING) acc += __popcll(a ^ b);
         else {
-            uint64_t both = nz[(size_t)y * Wq + q] & nz[(size_t)yb * Wq + q] & mask;
+            uint64_t both = nz[(size_t)y * W + q] & nz[(size_t)yb * W + q];
             acc += __popcll(both) - 2 * __popcll(both & (a ^ b));
         }
     }
@@ -101,19 +146,6 @@ __global__ void __launch_bounds__(256) corr_list_kernel(const uint64_t *__restri
     }
 }
 
-static uint64_t stride_mask(int64_t s)
-{
-    switch (s) {
-        case 1: return ~0ull;
-        case 2: return 0x5555555555555555ull;
-        case 4: return 0x1111111111111111ull;
-        case 8: return 0x0101010101010101ull;
-        case 16: return 0x0001000100010001ull;
-        case 32: return 0x0000000100000001ull;
-        default: return 1ull;
-    }
-}
-
 // stride == 0: full-source tiled kernel for r = 1..count (dev_r ignored), raw popcount
 // sums are converted to pair sums on the host (api.cu).  stride >= 1: list kernel.
 cudaError_t launch_corr(ising_sim *h, int64_t stride, int64_t count, const long long *dev_r,
@@ -125,15 +157,21 @@ cudaError_t launch_corr(ising_sim *h, int64_t stride, int64_t count, const long 
     const int np = ising ? 1 : 2;
     const uint64_t *sg = h->planes, *nz = ising ? nullptr : h->planes + pw;
     const uint64_t *sgT = h->planes + np * pw, *nzT = ising ? nullptr : h->planes + (np + 1) * pw;
+    // (the four pointers are re-aimed at the comb planes below when stride >= 2)
     if (stride == 0) {
         cudaError_t e = cudaMemsetAsync(dev_sx, 0, count * sizeof(long long), h->stream);
         if (e != cudaSuccess) return e;
         e = cudaMemsetAsync(dev_sy, 0, count * sizeof(long long), h->stream);
         if (e != cudaSuccess) return e;
-        int ytiles = L / TY;
+        // y-tiles are dealt to warps round-robin; enough blocks to fill 148 SMs x 8 even when
+        // only a few distance blocks are asked for (the protocol's r <= 32 is one)
+        const int ytiles = L / TY, gx = (int)((count + TR - 1) / TR);
         int gy = (ytiles + 4 * 32 - 1) / (4 * 32);       // ~32 y-tiles per warp
+        const int want = (148 * 8 + gx - 1) / gx;
+        if (gy < want) gy = want;
+        if (gy > (ytiles + 3) / 4) gy = (ytiles + 3) / 4;
         if (gy < 1) gy = 1;
-        dim3 grid((unsigned)((count + TR - 1) / TR), (unsigned)gy);
+        dim3 grid((unsigned)gx, (unsigned)gy);
         if (ising) {
             corr_full_kernel<ISING_MODEL_ISING><<<grid, 128, 0, h->stream>>>(sg, nz, L, Wq, (int)count, dev_sy);
             corr_full_kernel<ISING_MODEL_ISING><<<grid, 128, 0, h->stream>>>(sgT, nzT, L, Wq, (int)count, dev_sx);
@@ -144,13 +182,28 @@ cudaError_t launch_corr(ising_sim *h, int64_t stride, int64_t count, const long 
         h->launches += 2;
         return cudaGetLastError();
     }
-    uint64_t mask = stride_mask(stride);
+    // list kernel: on the full planes (stride 1) or on their comb (stride >= 2)
+    int W = Wq;
+    if (stride >= 2) {
+        int log2s = 0;
+        while ((1 << log2s) < stride) ++log2s;
+        W = (int)comb_words_per_row(L, stride);
+        const size_t cw = (size_t)L * W;
+        const uint64_t *src[4] = {sg, nz, sgT, nzT};
+        uint64_t *dst[4] = {h->comb, h->comb + cw, h->comb + (ising ? 1 : 2) * cw, h->comb + 3 * cw};
+        for (int k = 0; k < 4; ++k) {
+            if (!src[k]) continue;
+            comb_kernel<<<(unsigned)((cw + 255) / 256), 256, 0, h->stream>>>(src[k], dst[k], L, Wq, W, log2s);
+            h->launches++;
+        }
+        sg = dst[0]; nz = ising ? nullptr : dst[1]; sgT = dst[2]; nzT = ising ? nullptr : dst[3];
+    }
     if (ising) {
-        corr_list_kernel<ISING_MODEL_ISING><<<(unsigned)count, 256, 0, h->stream>>>(sg, nz, L, Wq, (int)stride, mask, dev_r, dev_sy);
-        corr_list_kernel<ISING_MODEL_ISING><<<(unsigned)count, 256, 0, h->stream>>>(sgT, nzT, L, Wq, (int)stride, mask, dev_r, dev_sx);
+        corr_list_kernel<ISING_MODEL_ISING><<<(unsigned)count, 256, 0, h->stream>>>(sg, nz, L, W, (int)stride, dev_r, dev_sy);
+        corr_list_kernel<ISING_MODEL_ISING><<<(unsigned)count, 256, 0, h->stream>>>(sgT, nzT, L, W, (int)stride, dev_r, dev_sx);
     } else {
-        corr_list_kernel<ISING_MODEL_BLUME_CAPEL><<<(unsigned)count, 256, 0, h->stream>>>(sg, nz, L, Wq, (int)stride, mask, dev_r, dev_sy);
-        corr_list_kernel<ISING_MODEL_BLUME_CAPEL><<<(unsigned)count, 256, 0, h->stream>>>(sgT, nzT, L, Wq, (int)stride, mask, dev_r, dev_sx);
+        corr_list_kernel<ISING_MODEL_BLUME_CAPEL><<<(unsigned)count, 256, 0, h->stream>>>(sg, nz, L, W, (int)stride, dev_r, dev_sy);
+        corr_list_kernel<ISING_MODEL_BLUME_CAPEL><<<(unsigned)count, 256, 0, h->stream>>>(sgT, nzT, L, W, (int)stride, dev_r, dev_sx);
     }
     h->launches += 2;
     return cudaGetLastError();

@@ -34,6 +34,7 @@ struct ising_sim {
     // lazily allocated (cudaMalloc, owned)
     void *io_stage = nullptr; size_t io_stage_bytes = 0;
     uint64_t *planes = nullptr; size_t planes_bytes = 0;      // bit planes for the correlation
+    uint64_t *comb = nullptr; size_t comb_bytes = 0;          // planes down-sampled to the source comb (stride >= 2)
     long long *d_corr = nullptr; size_t d_corr_bytes = 0;
     long long *d_rlist = nullptr; size_t d_rlist_bytes = 0;
 };
@@ -50,6 +51,8 @@ int cuda_fail(cudaError_t e, const char *what);
 
 static inline int64_t words_per_row(int64_t L) { return L / 32; }              // uint64 per colour row
 static inline int64_t words_per_colour(int64_t L) { return L * (L / 32); }
+// 64-bit words per row of a plane down-sampled to the bits x % stride == 0 (zero padded)
+static inline int64_t comb_words_per_row(int64_t L, int64_t stride) { return (L / stride + 63) / 64; }
 
 // kernels' host launchers (each returns a cudaError_t from the launch)
 cudaError_t launch_init(ising_sim *h);
