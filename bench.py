@@ -14,12 +14,14 @@ value     = L^2 * S * K / (device time of the K steps), lattice resident in HBM
 e2e       = same through the C ABI with HOST buffers: every step uploads the packed
             lattice from pinned host memory (ising_write_packed), runs S sweeps and
             reads the observables back
-roofline  = the Ising update kernel against the measured HBM copy rate
-            (MEASURED_PEAKS.json), algorithmic bytes 1.5 B per updated site
-            (DESIGN.md: own nibble read + written, opposite nibble read once);
-            `traffic` = dram bytes per launch from the committed ncu capture
-            (profiles/update_kernel_dram.csv) when it was taken at this L; roofline_alu = same kernel against the Philox-only
-            kernel (the integer-ALU roof of "one Philox number per site")
+roofline  = the update kernel against the bound that actually limits it: the integer
+            ALU ("one Philox4x32-10 number per site" = 9.25 dispatch slots per site,
+            DESIGN.md Sec. 5.1); peak derived from unit counts and the max SM clock, with
+            the live pipe-probe rates and the Philox-only kernel's rate beside it
+roofline_hbm = the same kernel against the measured HBM copy rate (MEASURED_PEAKS.json),
+            algorithmic bytes 1.5 B per updated site (own nibble read + written, opposite
+            nibble read once); `traffic` = dram bytes per launch from the committed ncu
+            capture (profiles/update_kernel_dram.csv) when it was taken at this L
 cpu_baseline = the oracle, as it stands, timed on the host cores on a bounded sample
 
 N > 1 (torchrun): the path does not shard under north_star ("one GPU, no
@@ -43,6 +45,7 @@ if ROOT not in sys.path:
 import workloads as wl  # noqa: E402
 
 BYTES_PER_SITE_LAUNCH = 1.5    # per UPDATED site: own nibble read + written, opposite nibble read once (3 x 4 bit)
+PHILOX_SLOTS_PER_SITE = 9.25   # (18 IMAD.WIDE + 19 LOP3) / 4 sites, rounds 1-2 partly hoisted
 PAPER_UPDATES_PER_NS = None    # no published number for THIS kernel contract / hardware
 
 
@@ -55,6 +58,9 @@ def parse_args():
     ap.add_argument("--L", type=int, default=0, help="override the lattice size (default: configs[2], 2^18)")
     ap.add_argument("--model", default="ising", choices=["ising", "bc"])
     ap.add_argument("--sweeps-per-step", type=int, default=10)
+    ap.add_argument("--workload", default="sweep", choices=["sweep", "corr"],
+                    help="sweep: S sweeps + observables (configs[2]/[3]); corr: configs[4], S sweeps + the paper's "
+                         "correlation protocol (A10/A11) per step")
     ap.add_argument("--rows-per-thread", type=int, default=0, help="update-kernel launch geometry (0 = library default)")
     ap.add_argument("--block", type=int, default=0, help="update-kernel threads per block (0 = library default)")
     ap.add_argument("--variant", type=int, default=0, help="update-kernel variant (0 = default carry form)")
@@ -66,6 +72,8 @@ def parse_args():
 
 def pick_workload(args):
     base = wl.config(2) if args.model == "ising" else wl.config(3)
+    if getattr(args, "workload", "sweep") == "corr":
+        base = wl.config(4)
     L = args.L or base.L
     name = base.name if L == base.L else f"{base.name.split('_L')[0]}_L{L}_override"
     return base, L, name
@@ -296,6 +304,8 @@ def run_ours(args):
         sim.sweep(S)
         if ev:
             ev[1].record()
+        if args.workload == "corr":
+            sim.correlation_protocol()             # r <= 32 all sources + stride-16 sources up to L/2
         return sim.observables()
 
     for _ in range(W):
@@ -326,11 +336,28 @@ def run_ours(args):
     philox_ms = ev[0].elapsed_time(ev[1]) / n_roof
     copy_ms = ev[1].elapsed_time(ev[2]) / n_roof
     sim.close()
+    pipes = eng.bench_pipes(float(measured_peaks()[2].get("sm_max_mhz", 0.0))) if rank == 0 else {}
 
     sites_per_launch = L * L // 2
     kern_ms = sweep_ms / (2 * S * K)
     peak, peak_src, peaks = measured_peaks()
     achieved = BYTES_PER_SITE_LAUNCH * sites_per_launch / (kern_ms * 1e-3) / 1e9
+    traffic = ncu_traffic(args.model, L)
+    # ALU roofline: one Philox4x32-10 call = 18 IMAD.WIDE + 19 LOP3 for 4 sites =
+    # 9.25 dispatch slots per site; a slot is 2 clocks of a 16-lane pipe (0.5 warp-instructions per
+    # sub-partition per clock, a wide multiply also taking one); 4 sub-partitions per SM.
+    sm_ghz = float(peaks.get("sm_max_mhz", 1965.0)) / 1e3
+    n_sm = torch.cuda.get_device_properties(device).multi_processor_count
+    alu_peak = n_sm * 4 * sm_ghz * 32 * 0.5 / PHILOX_SLOTS_PER_SITE
+    kern_upd = sites_per_launch / (kern_ms * 1e6)
+    alu_roof = {"bound": "alu", "kernel": "update_kernel (one colour phase)", "achieved": kern_upd, "peak": alu_peak,
+                "unit": "updates/ns", "frac": kern_upd / alu_peak, "traffic": traffic,
+                "peak_source": f"derived: {n_sm} SMs x 4 sub-partitions x {sm_ghz} GHz x 32 lanes x 0.5 slots/clk / "
+                               f"{PHILOX_SLOTS_PER_SITE} slots per site (Philox4x32-10 alone)",
+                "avg_launch_ms": kern_ms,
+                "philox_only_kernel_updates_per_ns": sites_per_launch / (philox_ms * 1e6),
+                "frac_of_philox_only_kernel": philox_ms / kern_ms,
+                "pipe_rates_warp_instr_per_subpartition_clk": pipes}
     value = whole_job_updates_per_ns(world, L, S, K, total_ms)
     line = {
         "metric": "spin updates/ns", "value": value, "unit": "updates/ns", "n_gpus": world, "steps": K,
@@ -339,19 +366,19 @@ def run_ours(args):
         "data": "synthetic (seeded random-start quench, the paper's own workload)",
         "config": {"workload": name, "model": args.model, "L": L, "beta": base.beta, "D": base.D,
                    "seed": base.seed, "sweeps_per_step": S, "observables_every": S,
+                   "step": "S sweeps + observables" if args.workload == "sweep" else "S sweeps + correlation protocol + observables",
                    "launch": {"rows_per_thread": args.rows_per_thread or "default", "block": args.block or "default",
                               "variant": args.variant},
                    "lattice_bytes": L * L // 2, "l2": "inputs larger than L2 (no flush needed)" if L * L // 2 > (256 << 20)
                    else "lattice fits L2: DRAM figures not meaningful", "parallelism": f"replicas x{world}"},
+        "measurement_ms_per_step": (total_ms - sweep_ms) / K,
         "sweep_only_updates_per_ns": world * L * L * S * K / (sweep_ms * 1e6),
-        "roofline": {"bound": "hbm", "kernel": "update_kernel (one colour phase)", "achieved": achieved,
-                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic(args.model, L),
-                     "peak_source": peak_src, "algorithmic_bytes_per_launch": BYTES_PER_SITE_LAUNCH * sites_per_launch,
-                     "avg_launch_ms": kern_ms,
-                     "copy_kernel_gbs": BYTES_PER_SITE_LAUNCH * sites_per_launch / (copy_ms * 1e-3) / 1e9},
-        "roofline_alu": {"bound": "alu", "what": "Philox-only kernel, same grid and calls per thread, no lattice traffic",
-                         "achieved": sites_per_launch / (kern_ms * 1e6), "peak": sites_per_launch / (philox_ms * 1e6),
-                         "unit": "updates/ns", "frac": philox_ms / kern_ms},
+        "roofline": alu_roof,
+        "roofline_hbm": {"bound": "hbm", "kernel": "update_kernel (one colour phase)", "achieved": achieved,
+                         "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+                         "peak_source": peak_src, "algorithmic_bytes_per_launch": BYTES_PER_SITE_LAUNCH * sites_per_launch,
+                         "avg_launch_ms": kern_ms,
+                         "copy_kernel_gbs": BYTES_PER_SITE_LAUNCH * sites_per_launch / (copy_ms * 1e-3) / 1e9},
         "clocks": clocks, "gpu_launches": launches,
         "last_observables": {"bond_sum": obs.bond_sum, "M": obs.M, "sweeps_done": obs.sweeps_done},
         "paper_context": "GB200: 1802 upd/ns (1-bit Ising, 1/2 RNG per spin), 948 upd/ns (Blume-Capel, 1 RNG per spin) -- other hardware/contract",

@@ -17,7 +17,7 @@ EXPORTS = [
     "ising_workspace_bytes", "ising_create", "ising_sweep", "ising_observables", "ising_correlation",
     "ising_correlation_protocol", "ising_correlation_list", "ising_schwinger_dyson", "ising_read_lattice",
     "ising_read_window", "ising_write_lattice", "ising_read_packed", "ising_write_packed",
-    "ising_set_sweeps_done", "ising_thresholds", "ising_set_launch", "ising_set_variant",
+    "ising_set_sweeps_done", "ising_thresholds", "ising_set_launch", "ising_set_variant", "ising_bench_pipes",
     "ising_launch_count", "ising_sync", "ising_destroy", "ising_last_error", "ising_bench_philox_only",
     "ising_bench_copy", "ising_debug_philox",
 ]
@@ -99,6 +99,20 @@ def _check(rc: int):
 
 def workspace_bytes(model: int, L: int) -> int:
     return int(load_library().ising_workspace_bytes(model, L))
+
+
+PIPE_PROBES = ["IMAD.WIDE", "LOP3", "IMAD", "IMAD.WIDE+LOP3", "IMAD.WIDE+2LOP3", "IADD3(carry)+IMAD.X",
+               "IMAD.WIDE+IMAD", "POPC+IADD"]
+
+
+def bench_pipes(sm_mhz: float = 0.0) -> dict:
+    """Issue rates (warp-instructions per SM sub-partition per clock) of the integer-pipe probes."""
+    lib = load_library()
+    lib.ising_bench_pipes.argtypes = [C.c_double, C.c_void_p, C.c_int, C.c_void_p]
+    rates = np.zeros(len(PIPE_PROBES), dtype=np.float64)
+    n = C.c_int(0)
+    _check(lib.ising_bench_pipes(float(sm_mhz), rates.ctypes.data, len(rates), C.addressof(n)))
+    return {k: float(v) for k, v in zip(PIPE_PROBES, rates)}
 
 
 def debug_philox(ctr: np.ndarray, key: np.ndarray, with_curand: bool = False) -> np.ndarray:

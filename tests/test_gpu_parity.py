@@ -318,6 +318,22 @@ def test_correlation_list_and_protocol(eng, model):
         assert (pr == orr).all() and (pn == on).all() and (px == ox).all() and (py == oy).all()
 
 
+@pytest.mark.parametrize("model", [ISING, BC])
+@pytest.mark.parametrize("L", [64, 192, 320])
+def test_correlation_list_small_and_ragged_comb(eng, model, L):
+    """Every stride at sizes where the comb row is a fraction of a 64-bit word (L = 64, stride 64:
+    one bit per row) or a ragged number of words (L = 192, 320)."""
+    beta, D = (0.3, 0.0) if model == ISING else (0.5, 0.4)
+    with eng.IsingSim(model, L, beta, D, 9) as sim:
+        sim.sweep(3)
+        lat = sim.read_lattice()
+        r = np.array(sorted({1, 2, 3, L // 4, L // 2 - 1, L // 2}))
+        for stride in (1, 2, 4, 8, 16, 32, 64):
+            sx, sy = sim.correlation_list(stride, r)
+            ox, oy = oracle.correlation_list(lat, stride, r)
+            assert (sx == ox).all() and (sy == oy).all(), stride
+
+
 def test_protocol_distance_lists_match_oracle(eng):
     """Host logic of Sec. 3.3 at sizes where the log grid is non-trivial (lists only)."""
     for L, t in [(4096, 1), (4096, 3000)]:
