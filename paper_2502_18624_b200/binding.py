@@ -17,7 +17,7 @@ EXPORTS = [
     "ising_workspace_bytes", "ising_create", "ising_sweep", "ising_observables", "ising_correlation",
     "ising_correlation_protocol", "ising_correlation_list", "ising_schwinger_dyson", "ising_read_lattice",
     "ising_read_window", "ising_write_lattice", "ising_read_packed", "ising_write_packed",
-    "ising_set_sweeps_done", "ising_thresholds", "ising_set_launch", "ising_set_variant", "ising_bench_pipes",
+    "ising_set_sweeps_done", "ising_thresholds", "ising_set_launch", "ising_set_variant", "ising_bench_pipes", "ising_set_corr_path",
     "ising_launch_count", "ising_sync", "ising_destroy", "ising_last_error", "ising_bench_philox_only",
     "ising_bench_copy", "ising_debug_philox",
 ]
@@ -258,6 +258,10 @@ class IsingSim:
 
     def set_variant(self, variant: int):
         _check(self._lib.ising_set_variant(self._h, variant))
+
+    def set_corr_path(self, path: int):
+        self._lib.ising_set_corr_path.argtypes = [C.c_void_p, C.c_int]
+        _check(self._lib.ising_set_corr_path(self._h, path))
 
     def launch_count(self) -> int:
         return int(self._lib.ising_launch_count(self._h))

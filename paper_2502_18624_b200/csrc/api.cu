@@ -159,6 +159,7 @@ extern "C" int ising_destroy(ising_t *h)
     if (h->io_stage) cudaFree(h->io_stage);
     if (h->planes) cudaFree(h->planes);
     if (h->comb) cudaFree(h->comb);
+    if (h->gram) cudaFree(h->gram);
     if (h->d_corr) cudaFree(h->d_corr);
     if (h->d_rlist) cudaFree(h->d_rlist);
     if (h->h_acc) cudaFreeHost(h->h_acc);
@@ -416,6 +417,32 @@ static int run_corr(ising_sim *h, int64_t stride, int64_t count, const int64_t *
     return ISING_OK;
 }
 
+static int ensure_gram(ising_sim *h)
+{
+    const size_t bytes = corr_gram_bytes(h);
+    if (h->gram_bytes >= bytes) return ISING_OK;
+    cudaError_t e = cudaMalloc((void **)&h->gram, bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); h->gram = nullptr; return set_error(ISING_ENOMEM, "int8 spin matrix: cudaMalloc failed"); }
+    h->gram_bytes = bytes;
+    return ISING_OK;
+}
+
+// Full-range sums on the tensor cores (corr_gram.cu): planes already built.
+static int run_corr_gram(ising_sim *h, int64_t count, int64_t *sx, int64_t *sy)
+{
+    int rc = ensure_corr(h, count);
+    if (rc) return rc;
+    rc = ensure_gram(h);
+    if (rc) return rc;
+    long long *d_sx = h->d_corr, *d_sy = h->d_corr + count;
+    cudaError_t e = launch_corr_gram(h, count, d_sx, d_sy);
+    if (e != cudaSuccess) return cuda_fail(e, "tensor-core correlation kernels");
+    CUDA_TRY(cudaMemcpyAsync(sx, d_sx, (size_t)count * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaMemcpyAsync(sy, d_sy, (size_t)count * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return ISING_OK;
+}
+
 extern "C" int ising_correlation(ising_t *h, int64_t rmax, int64_t *sx, int64_t *sy)
 {
     if (!h || !sx || !sy) return set_error(ISING_EINVAL, "ising_correlation: NULL argument");
@@ -424,7 +451,19 @@ extern "C" int ising_correlation(ising_t *h, int64_t rmax, int64_t *sx, int64_t 
     if (rc) return rc;
     cudaError_t e = launch_planes(h);
     if (e != cudaSuccess) return cuda_fail(e, "bit-plane kernels");
+    // tensor cores pay off once the band is wide; narrow bands stay on the bit planes
+    const bool tensor = h->corr_path == 2 || (h->corr_path == 0 && rmax >= 512);
+    if (tensor && corr_gram_supported(h, rmax)) return run_corr_gram(h, rmax, sx, sy);
+    if (h->corr_path == 2) return set_error(ISING_EINVAL, "ising_correlation: tensor-core path needs L % 256 == 0 and L >= 512");
     return run_corr(h, 0, rmax, nullptr, sx, sy);
+}
+
+extern "C" int ising_set_corr_path(ising_t *h, int path)
+{
+    if (!h) return set_error(ISING_EINVAL, "ising_set_corr_path: NULL handle");
+    if (path < 0 || path > 2) return set_error(ISING_EINVAL, "ising_set_corr_path: path must be 0 (auto), 1 (bit planes) or 2 (tensor cores)");
+    h->corr_path = path;
+    return ISING_OK;
 }
 
 static bool valid_stride(int64_t s) { return s == 1 || s == 2 || s == 4 || s == 8 || s == 16 || s == 32 || s == 64; }

@@ -1,0 +1,312 @@
+// Full-range correlation on the tensor cores (A9 of SURVEY.md Sec. 8(a)).
+//
+// S_y(r) = sum_y sum_x s(x, y) s(x, (y + r) mod L) = sum_y G[y, (y + r) mod L],  G = A A^T,
+// with A the L x L spin matrix as int8 (-1, 0, +1): a banded Gram matrix, the one dense
+// contraction on the path.  tcgen05.mma kind::i8 accumulates in int32 (exact: |G| <= L), so
+// the sums stay bit-exact integers.  S_x is the same on the transposed matrix.
+//
+// One persistent CTA per SM, warp-specialised: warp 0 = TMA producer (128-byte-swizzled
+// K-major tiles, 4-stage mbarrier ring), warp 1 = MMA issuer (one elected thread, 128 x 256
+// int32 accumulator in TMEM, double buffered), warps 2-5 = epilogue (tcgen05.ld, every
+// element added to the shared-memory bin of its diagonal j - i, bins flushed to the int64
+// result with one atomic per distance per tile).  Tile (I0, J0 = I0 + 256 k) holds the ordered
+// pairs (y = I0 + i, y + r = J0 + j): r = J0 - I0 + j - i, kept when 1 <= r <= rmax.
+#include "ising_internal.cuh"
+
+#include <cuda.h>
+
+namespace {
+
+constexpr int TM = 128, TN = 256, TKB = 128;        // tile rows, tile columns, K bytes per stage
+constexpr int STAGES = 4;
+constexpr int A_BYTES = TM * TKB, B_BYTES = TN * TKB, STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int NBINS = TM + TN - 1;                   // diagonals j - i = -(TM-1) .. TN-1
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 2048 /*bins, barriers*/;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1) : "memory");
+}
+// K-major operand, 128-byte swizzle: 8-row groups of 1024 bytes, descriptor version 1 (sm_100)
+__device__ __forceinline__ uint64_t umma_desc(uint32_t smem_addr)
+{
+    uint64_t d = 0;
+    d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);          // start address, 16-byte units
+    d |= (uint64_t)(1024 >> 4) << 32;                      // stride between 8-row groups
+    d |= (uint64_t)1 << 46;                                // descriptor version
+    d |= (uint64_t)2 << 61;                                // SWIZZLE_128B
+    return d;
+}
+// kind::i8, signed x signed -> int32, both K-major, M = 128, N = 256
+constexpr uint32_t kInstrDesc = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TN >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);
+
+__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n\t}"
+        ::"r"(tmem_d), "l"(da), "l"(db), "r"(kInstrDesc), "r"(accumulate), "r"(0u) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t *bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+struct GramParams {
+    int L, rmax, n_ib, n_jk;          // row blocks, column tiles per row block
+    long long *out;                   // S(r), r = 1..rmax at out[r-1]
+};
+
+}  // namespace
+
+// ------------------------------------------------------------------ kernel ---
+__global__ void __launch_bounds__(192, 1) gram_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ GramParams p)
+{
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    uint8_t *tail = smem + STAGES * STAGE_BYTES;
+    int *bins = reinterpret_cast<int *>(tail);                              // NBINS ints (1532 B)
+    uint64_t *full = reinterpret_cast<uint64_t *>(tail + 1536);             // [STAGES]
+    uint64_t *empty = full + STAGES;                                        // [STAGES]
+    uint64_t *tfull = empty + STAGES;                                       // [2]
+    uint64_t *tempty = tfull + 2;                                           // [2]
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + 2);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_tiles = p.n_ib * p.n_jk, n_kb = p.L / TKB;
+
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 2) {   // TMEM: 512 columns = two 128 x 256 int32 accumulators
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    for (int i = threadIdx.x; i < NBINS; i += blockDim.x) bins[i] = 0;
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            int stage = 0; uint32_t phase = 0;
+            for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+                const int ib = t / p.n_jk, jk = t - ib * p.n_jk;
+                const int I0 = ib * TM;
+                int J0 = I0 + jk * TN; if (J0 >= p.L) J0 -= p.L;
+                int J1 = J0 + TM; if (J1 >= p.L) J1 -= p.L;                 // second half of the B tile (wraps)
+                for (int kb = 0; kb < n_kb; ++kb) {
+                    mbar_wait(&empty[stage], phase ^ 1);
+                    mbar_expect_tx(&full[stage], STAGE_BYTES);
+                    uint8_t *sa = smem + stage * STAGE_BYTES, *sb = sa + A_BYTES;
+                    tma_load_2d(sa, &tmap, &full[stage], kb * TKB, I0);
+                    tma_load_2d(sb, &tmap, &full[stage], kb * TKB, J0);
+                    tma_load_2d(sb + A_BYTES, &tmap, &full[stage], kb * TKB, J1);
+                    if (++stage == STAGES) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer (one thread) =====
+        if (lane == 0) {
+            int stage = 0; uint32_t phase = 0;
+            int as = 0; uint32_t aphase = 0;
+            for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+                mbar_wait(&tempty[as], aphase ^ 1);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t d_tmem = tmem_base + (uint32_t)(as * TN);
+                for (int kb = 0; kb < n_kb; ++kb) {
+                    mbar_wait(&full[stage], phase);
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    const uint32_t sa = smem_u32(smem + stage * STAGE_BYTES), sb = sa + A_BYTES;
+                    const uint64_t da = umma_desc(sa), db = umma_desc(sb);
+#pragma unroll
+                    for (int k = 0; k < TKB / 32; ++k)                       // UMMA_K = 32 int8 = 32 bytes = 2 x 16 B
+                        umma_i8(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), (kb | k) ? 1u : 0u);
+                    umma_commit(&empty[stage]);                              // frees the smem slot when the MMAs retire
+                    if (++stage == STAGES) { stage = 0; phase ^= 1; }
+                }
+                umma_commit(&tfull[as]);                                     // accumulator complete
+                if (++as == 2) { as = 0; aphase ^= 1; }
+            }
+        }
+    } else {
+        // ===== epilogue: warps 2..5, TMEM lane quarter = warp % 4 =====
+        const int q = warp & 3, row = q * 32 + lane;                        // tile row i of this thread
+        const int et = threadIdx.x - 64;                                    // 0..127 among the epilogue threads
+        int as = 0; uint32_t aphase = 0;
+        for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+            const int ib = t / p.n_jk, jk = t - ib * p.n_jk;
+            mbar_wait(&tfull[as], aphase);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * TN);
+#pragma unroll 1
+            for (int c = 0; c < TN / 32; ++c) {
+                uint32_t v[32];
+                asm volatile(
+                    "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                    "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+                    "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+                    : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                      "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+                      "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+                      "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+                    : "r"(taddr + (uint32_t)(c * 32)));
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                // element (row, 32 c + k) lies on diagonal j - i: lanes hit consecutive bins, no conflicts
+                const uint32_t b0 = smem_u32(bins) + 4u * (uint32_t)((TM - 1) + 32 * c - row);
+#pragma unroll
+                for (int k = 0; k < 32; ++k)
+                    asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(b0 + 4u * k), "r"(v[k]) : "memory");
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&tempty[as]);                        // this warp has drained its quarter
+            if (++as == 2) { as = 0; aphase ^= 1; }
+            // flush the diagonal bins of this tile: r = jk * TN + (bin - (TM - 1))
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            for (int b = et; b < NBINS; b += 128) {
+                const int r = jk * TN + b - (TM - 1);
+                const int v = bins[b];
+                bins[b] = 0;
+                if (r >= 1 && r <= p.rmax && v != 0)
+                    atomicAdd(reinterpret_cast<unsigned long long *>(&p.out[r - 1]), (unsigned long long)(long long)v);
+            }
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 2) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+}
+
+// ------------------------------------------------- planes -> int8 matrix ---
+// out[y][64 q + i] = nz bit ? (sg bit ? +1 : -1) : 0   (Ising: nz == nullptr, every site non-zero)
+__global__ void __launch_bounds__(256) expand_kernel(const uint64_t *__restrict__ sg, const uint64_t *__restrict__ nz,
+                                                     int8_t *__restrict__ out, int64_t n_words)
+{
+    const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= n_words) return;
+    const uint64_t s = sg[w], z = nz ? nz[w] : ~0ull;
+    uint4 *o = reinterpret_cast<uint4 *>(out + w * 64);
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        uint32_t v[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            uint32_t word = 0;
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const int bit = 16 * c + 4 * k + b;
+                const uint32_t val = ((z >> bit) & 1ull) ? (((s >> bit) & 1ull) ? 0x01u : 0xFFu) : 0u;
+                word |= val << (8 * b);
+            }
+            v[k] = word;
+        }
+        o[c] = make_uint4(v[0], v[1], v[2], v[3]);
+    }
+}
+
+// ------------------------------------------------------------------- host ---
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_tiled()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+bool corr_gram_supported(const ising_sim *h, int64_t rmax)
+{
+    return (h->L % 256) == 0 && h->L >= 512 && rmax >= 1;
+}
+
+size_t corr_gram_bytes(const ising_sim *h) { return (size_t)h->L * (size_t)h->L; }
+
+// S_y (planes sg/nz) and S_x (transposed planes) for r = 1..count via the int8 Gram kernel.
+// dev_sx / dev_sy receive the pair sums themselves (no popcount conversion needed).
+cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, long long *dev_sy)
+{
+    const int L = (int)h->L, Wq = L / 64;
+    const size_t pw = (size_t)L * Wq;
+    const bool ising = h->model == ISING_MODEL_ISING;
+    const int np = ising ? 1 : 2;
+    EncodeTiledFn enc = encode_tiled();
+    if (!enc) return cudaErrorNotSupported;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    CUtensorMap tmap;
+    const cuuint64_t gdim[2] = {(cuuint64_t)L, (cuuint64_t)L};
+    const cuuint64_t gstride[1] = {(cuuint64_t)L};
+    const cuuint32_t box[2] = {(cuuint32_t)TKB, (cuuint32_t)TM};
+    const cuuint32_t estr[2] = {1, 1};
+    if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, h->gram, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return cudaErrorInvalidValue;
+    int dev = 0, n_sm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    GramParams p;
+    p.L = L; p.rmax = (int)count; p.n_ib = L / TM;
+    p.n_jk = (int)((count + TM + TN - 1) / TN);          // columns I0 .. I0 + 127 + rmax
+    const int n_tiles = p.n_ib * p.n_jk;
+    const int grid = n_tiles < n_sm ? n_tiles : n_sm;
+    for (int axis = 0; axis < 2; ++axis) {              // 0: S_y from the planes, 1: S_x from the transposed planes
+        const uint64_t *sg = h->planes + (axis ? np * pw : 0);
+        const uint64_t *nz = ising ? nullptr : sg + pw;
+        long long *out = axis ? dev_sx : dev_sy;
+        cudaError_t e = cudaMemsetAsync(out, 0, count * sizeof(long long), h->stream);
+        if (e != cudaSuccess) return e;
+        expand_kernel<<<(unsigned)((pw + 255) / 256), 256, 0, h->stream>>>(sg, nz, h->gram, (int64_t)pw);
+        p.out = out;
+        gram_kernel<<<grid, 192, SMEM_BYTES, h->stream>>>(tmap, p);
+        h->launches += 2;
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}

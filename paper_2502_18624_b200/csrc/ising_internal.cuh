@@ -35,6 +35,8 @@ struct ising_sim {
     void *io_stage = nullptr; size_t io_stage_bytes = 0;
     uint64_t *planes = nullptr; size_t planes_bytes = 0;      // bit planes for the correlation
     uint64_t *comb = nullptr; size_t comb_bytes = 0;          // planes down-sampled to the source comb (stride >= 2)
+    int8_t *gram = nullptr; size_t gram_bytes = 0;            // L x L int8 spin matrix for the tensor-core correlation
+    int corr_path = 0;                                        // 0 auto, 1 bit planes (XOR + POPC), 2 tensor cores
     long long *d_corr = nullptr; size_t d_corr_bytes = 0;
     long long *d_rlist = nullptr; size_t d_rlist_bytes = 0;
 };
@@ -64,6 +66,9 @@ cudaError_t launch_pack(ising_sim *h, int64_t y0, int64_t ny, const int8_t *dev_
 cudaError_t launch_planes(ising_sim *h);                            // lattice -> bit planes
 cudaError_t launch_corr(ising_sim *h, int64_t stride, int64_t count, const long long *dev_r,
                         long long *dev_sx, long long *dev_sy);
+bool corr_gram_supported(const ising_sim *h, int64_t rmax);
+size_t corr_gram_bytes(const ising_sim *h);
+cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, long long *dev_sy);
 cudaError_t launch_philox_only(ising_sim *h, uint32_t t);
 cudaError_t launch_copy(ising_sim *h);
 cudaError_t launch_debug_philox(int64_t count, const uint32_t *d_ctr, const uint32_t *d_key,
