@@ -335,6 +335,25 @@ def run_ours(args):
     torch.cuda.synchronize(device)
     philox_ms = ev[0].elapsed_time(ev[1]) / n_roof
     copy_ms = ev[1].elapsed_time(ev[2]) / n_roof
+    tensor_roof = None
+    if args.workload == "corr" and rank == 0:
+        # full-range correlation (A9) on the tensor cores: whole ising_correlation(L/2) call, i.e.
+        # bit planes + transposes + int8 expansion + the two Gram launches + the D2H of the sums
+        sim.correlation(L // 2)
+        ev2 = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize(device)
+        ev2[0].record(); sim.correlation(L // 2); ev2[1].record()
+        torch.cuda.synchronize(device)
+        full_ms = ev2[0].elapsed_time(ev2[1])
+        n_jk = (L // 2 + 128 + 255) // 256
+        macs = 2.0 * (L // 128) * n_jk * 128 * 256 * L          # both axes, tiles actually multiplied
+        peak_t = 2.0 * float(measured_peaks()[2].get("bf16_tflops", 0.0)) or None
+        tops = 2.0 * macs / (full_ms * 1e-3) / 1e12
+        tensor_roof = {"bound": "tensor", "kernel": "gram_kernel (tcgen05 kind::i8), whole ising_correlation(L/2) call",
+                       "achieved": tops, "peak": peak_t, "unit": "TOP/s (int8)",
+                       "frac": (tops / peak_t) if peak_t else None, "traffic": None, "ms_per_call": full_ms,
+                       "peak_source": "2 x MEASURED_PEAKS.json bf16_tflops (nominal int8 : bf16 ratio)",
+                       "useful_pair_products": 2.0 * (L // 2) * L * L}
     sim.close()
     pipes = eng.bench_pipes(float(measured_peaks()[2].get("sm_max_mhz", 0.0))) if rank == 0 else {}
 
@@ -379,6 +398,7 @@ def run_ours(args):
                          "peak_source": peak_src, "algorithmic_bytes_per_launch": BYTES_PER_SITE_LAUNCH * sites_per_launch,
                          "avg_launch_ms": kern_ms,
                          "copy_kernel_gbs": BYTES_PER_SITE_LAUNCH * sites_per_launch / (copy_ms * 1e-3) / 1e9},
+        "roofline_tensor": tensor_roof,
         "clocks": clocks, "gpu_launches": launches,
         "last_observables": {"bond_sum": obs.bond_sum, "M": obs.M, "sweeps_done": obs.sweeps_done},
         "paper_context": "GB200: 1802 upd/ns (1-bit Ising, 1/2 RNG per spin), 948 upd/ns (Blume-Capel, 1 RNG per spin) -- other hardware/contract",

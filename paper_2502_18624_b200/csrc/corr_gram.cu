@@ -79,10 +79,23 @@ __device__ __forceinline__ void umma_commit(uint64_t *bar)
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
+// Work split: the K dimension (the L columns of the spin matrix) is cut into chunks of kc bytes
+// so that the L x kc slab every tile of a launch reads stays resident in L2 (S(r) is linear in
+// G, so the chunks simply add up); one launch per chunk.  Inside a launch the tiles are ordered
+// column-tile-major and every CTA takes a contiguous run of them: consecutive tiles of a run
+// share jk, hence the same diagonal bins, which are flushed only when jk changes.
 struct GramParams {
     int L, rmax, n_ib, n_jk;          // row blocks, column tiles per row block
+    int k0, n_kb;                     // first K byte of this chunk, 128-byte K blocks per tile
     long long *out;                   // S(r), r = 1..rmax at out[r-1]
 };
+
+__device__ __forceinline__ void tile_range(const GramParams &p, int &lo, int &hi)
+{
+    const long long n = (long long)p.n_ib * p.n_jk;
+    lo = (int)(n * blockIdx.x / gridDim.x);
+    hi = (int)(n * (blockIdx.x + 1) / gridDim.x);
+}
 
 }  // namespace
 
@@ -100,7 +113,9 @@ __global__ void __launch_bounds__(192, 1) gram_kernel(const __grid_constant__ CU
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + 2);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n_tiles = p.n_ib * p.n_jk, n_kb = p.L / TKB;
+    const int n_kb = p.n_kb;
+    int t_lo, t_hi;
+    tile_range(p, t_lo, t_hi);
 
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
@@ -121,8 +136,8 @@ __global__ void __launch_bounds__(192, 1) gram_kernel(const __grid_constant__ CU
         // ===== TMA producer =====
         if (lane == 0) {
             int stage = 0; uint32_t phase = 0;
-            for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-                const int ib = t / p.n_jk, jk = t - ib * p.n_jk;
+            for (int t = t_lo; t < t_hi; ++t) {
+                const int jk = t / p.n_ib, ib = t - jk * p.n_ib;
                 const int I0 = ib * TM;
                 int J0 = I0 + jk * TN; if (J0 >= p.L) J0 -= p.L;
                 int J1 = J0 + TM; if (J1 >= p.L) J1 -= p.L;                 // second half of the B tile (wraps)
@@ -130,9 +145,9 @@ __global__ void __launch_bounds__(192, 1) gram_kernel(const __grid_constant__ CU
                     mbar_wait(&empty[stage], phase ^ 1);
                     mbar_expect_tx(&full[stage], STAGE_BYTES);
                     uint8_t *sa = smem + stage * STAGE_BYTES, *sb = sa + A_BYTES;
-                    tma_load_2d(sa, &tmap, &full[stage], kb * TKB, I0);
-                    tma_load_2d(sb, &tmap, &full[stage], kb * TKB, J0);
-                    tma_load_2d(sb + A_BYTES, &tmap, &full[stage], kb * TKB, J1);
+                    tma_load_2d(sa, &tmap, &full[stage], p.k0 + kb * TKB, I0);
+                    tma_load_2d(sb, &tmap, &full[stage], p.k0 + kb * TKB, J0);
+                    tma_load_2d(sb + A_BYTES, &tmap, &full[stage], p.k0 + kb * TKB, J1);
                     if (++stage == STAGES) { stage = 0; phase ^= 1; }
                 }
             }
@@ -142,7 +157,7 @@ __global__ void __launch_bounds__(192, 1) gram_kernel(const __grid_constant__ CU
         if (lane == 0) {
             int stage = 0; uint32_t phase = 0;
             int as = 0; uint32_t aphase = 0;
-            for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+            for (int t = t_lo; t < t_hi; ++t) {
                 mbar_wait(&tempty[as], aphase ^ 1);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const uint32_t d_tmem = tmem_base + (uint32_t)(as * TN);
@@ -166,8 +181,8 @@ __global__ void __launch_bounds__(192, 1) gram_kernel(const __grid_constant__ CU
         const int q = warp & 3, row = q * 32 + lane;                        // tile row i of this thread
         const int et = threadIdx.x - 64;                                    // 0..127 among the epilogue threads
         int as = 0; uint32_t aphase = 0;
-        for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-            const int ib = t / p.n_jk, jk = t - ib * p.n_jk;
+        for (int t = t_lo; t < t_hi; ++t) {
+            const int jk = t / p.n_ib;
             mbar_wait(&tfull[as], aphase);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * TN);
@@ -194,7 +209,9 @@ __global__ void __launch_bounds__(192, 1) gram_kernel(const __grid_constant__ CU
             __syncwarp();
             if (lane == 0) mbar_arrive(&tempty[as]);                        // this warp has drained its quarter
             if (++as == 2) { as = 0; aphase ^= 1; }
-            // flush the diagonal bins of this tile: r = jk * TN + (bin - (TM - 1))
+            // the next tile of the run has the same jk (same bins) unless the run crosses into the
+            // next column tile: flush the bins then, r = jk * TN + (bin - (TM - 1))
+            if (t + 1 < t_hi && (t + 1) / p.n_ib == jk) continue;
             asm volatile("bar.sync 1, 128;" ::: "memory");
             for (int b = et; b < NBINS; b += 128) {
                 const int r = jk * TN + b - (TM - 1);
@@ -293,6 +310,11 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
     GramParams p;
     p.L = L; p.rmax = (int)count; p.n_ib = L / TM;
     p.n_jk = (int)((count + TM + TN - 1) / TN);          // columns I0 .. I0 + 127 + rmax
+    // K chunk: keep the L x kc slab within about half of the 126 MB L2
+    int kc = (int)(((64ll << 20) / L) / TKB * TKB);
+    if (kc < 4 * TKB) kc = 4 * TKB;
+    if (kc > L) kc = L;
+    p.n_kb = kc / TKB;
     const int n_tiles = p.n_ib * p.n_jk;
     const int grid = n_tiles < n_sm ? n_tiles : n_sm;
     for (int axis = 0; axis < 2; ++axis) {              // 0: S_y from the planes, 1: S_x from the transposed planes
@@ -303,8 +325,13 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
         if (e != cudaSuccess) return e;
         expand_kernel<<<(unsigned)((pw + 255) / 256), 256, 0, h->stream>>>(sg, nz, h->gram, (int64_t)pw);
         p.out = out;
-        gram_kernel<<<grid, 192, SMEM_BYTES, h->stream>>>(tmap, p);
-        h->launches += 2;
+        h->launches++;
+        for (int k0 = 0; k0 < L; k0 += kc) {
+            p.k0 = k0;
+            p.n_kb = (L - k0 < kc ? L - k0 : kc) / TKB;
+            gram_kernel<<<grid, 192, SMEM_BYTES, h->stream>>>(tmap, p);
+            h->launches++;
+        }
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }

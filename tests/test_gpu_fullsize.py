@@ -182,7 +182,12 @@ def test_config4_ising_L2p16_correlation_protocol(eng):
             assert (r == pr).all() and (nsrc == (L // pstride) ** 2).all()
             assert int(sx[0]) + int(sy[0]) == o.bond_sum            # r[0] = 1, all sources
             if t in (1, 64):
-                fx, fy = sim.correlation(L // 2)
+                fx, fy = sim.correlation(L // 2)                    # automatic path: tensor cores at this size
+                if t == 1:
+                    sim.set_corr_path(1)                            # XOR + POPC kernels: identical integers
+                    bx, by = sim.correlation(L // 2)
+                    sim.set_corr_path(0)
+                    assert (bx == fx).all() and (by == fy).all()
                 dense = pstride == 1
                 assert (sx[dense] == fx[r[dense] - 1]).all() and (sy[dense] == fy[r[dense] - 1]).all()
                 lat = sim.read_lattice()

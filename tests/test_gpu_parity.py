@@ -318,6 +318,42 @@ def test_correlation_list_and_protocol(eng, model):
         assert (pr == orr).all() and (pn == on).all() and (px == ox).all() and (py == oy).all()
 
 
+@pytest.mark.parametrize("model,L", [(ISING, 512), (BC, 512), (ISING, 768), (BC, 1280), (ISING, 2048)])
+def test_correlation_tensor_core_path(eng, model, L):
+    """The int8 tcgen05 Gram kernel (path 2) against the oracle's plain sums and against the
+    XOR + POPC kernels (path 1): full band, a band that ends inside a tile, a single distance;
+    L = 768 and 1280 make the 256-row B tile wrap around the lattice edge."""
+    beta, D = (wl.BETA_C / 0.5, 0.0) if model == ISING else (1 / 1.4, 1.0)
+    with eng.IsingSim(model, L, beta, D, 5) as sim:
+        sim.sweep(4)
+        lat = sim.read_lattice()
+        ox, oy = oracle.correlation(lat, L // 2)
+        for rmax in (L // 2, L // 2 - 37, 129, 1):
+            sim.set_corr_path(2)
+            tx, ty = sim.correlation(rmax)
+            assert (tx == ox[:rmax]).all() and (ty == oy[:rmax]).all(), rmax
+            sim.set_corr_path(1)
+            bx, by = sim.correlation(rmax)
+            assert (bx == tx).all() and (by == ty).all(), rmax
+        sim.set_corr_path(0)
+        ax, ay = sim.correlation(L // 2)                     # automatic choice
+        assert (ax == ox).all() and (ay == oy).all()
+        # closed form at the largest accumulator magnitude: all +1 -> every Gram entry is L, S(r) = N
+        sim.write_lattice(np.ones((L, L), dtype=np.int8))
+        sim.set_corr_path(2)
+        tx, ty = sim.correlation(L // 2)
+        assert (tx == L * L).all() and (ty == L * L).all()
+    with eng.IsingSim(model, 192, beta, D, 5) as sim:        # L % 256 != 0: tensor path refuses, auto falls back
+        sim.set_corr_path(2)
+        with pytest.raises(eng.IsingError):
+            sim.correlation(96)
+        sim.set_corr_path(0)
+        lat = sim.read_lattice()
+        ax, ay = sim.correlation(96)
+        ox, oy = oracle.correlation(lat, 96)
+        assert (ax == ox).all() and (ay == oy).all()
+
+
 @pytest.mark.parametrize("model", [ISING, BC])
 @pytest.mark.parametrize("L", [64, 192, 320])
 def test_correlation_list_small_and_ragged_comb(eng, model, L):
