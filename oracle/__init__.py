@@ -188,5 +188,57 @@ def time_grid(tmax: int) -> np.ndarray:
     return out[:n].copy()
 
 
+# ------------------------------------------------------------ NEXT-2: 1-bit LUT kernel ---
+def lut_table(beta: float) -> np.ndarray:
+    out = np.zeros(16, dtype=np.uint64)
+    lib().orc_lut_table(C.c_double(beta), _p(out, C.c_uint64))
+    return out
+
+
+def lut_bits(table: np.ndarray, seed: int, w: int, t: int, tag: int, which: int) -> int:
+    table = np.ascontiguousarray(table, dtype=np.uint64)
+    lib().orc_lut_bits.restype = C.c_uint64
+    return int(lib().orc_lut_bits(_p(table, C.c_uint64), C.c_uint64(seed), C.c_uint64(w), C.c_uint32(t),
+                                  C.c_uint32(tag), C.c_int(which)))
+
+
+def lut_init(L: int, seed: int) -> np.ndarray:
+    s = np.zeros((L, L), dtype=np.int8)
+    lib().orc_lut_init(C.c_int64(L), C.c_uint64(seed), _p(s, C.c_int8))
+    return s
+
+
+def lut_init_patch(L, seed, x0, y0, w, h) -> np.ndarray:
+    s = np.zeros((h, w), dtype=np.int8)
+    lib().orc_lut_init_patch(C.c_int64(L), C.c_uint64(seed), C.c_int64(x0), C.c_int64(y0), C.c_int64(w),
+                             C.c_int64(h), _p(s, C.c_int8))
+    return s
+
+
+def lut_sweep(s: np.ndarray, beta, seed, t, tallies=None):
+    """One sweep number ``t`` of the 1-bit LUT kernel in place; returns the updated (B, M, Q)."""
+    assert s.dtype == np.int8 and s.flags.c_contiguous and s.shape[0] == s.shape[1]
+    tl = np.asarray(observables(s) if tallies is None else tallies, dtype=np.int64).copy()
+    lib().orc_lut_sweep(C.c_int64(s.shape[0]), C.c_double(beta), C.c_uint64(seed), C.c_uint32(t),
+                        _p(s, C.c_int8), _p(tl, C.c_int64))
+    return int(tl[0]), int(tl[1]), int(tl[2])
+
+
+def lut_sweep_patch(L, s: np.ndarray, beta, seed, t, x0, y0):
+    assert s.dtype == np.int8 and s.flags.c_contiguous
+    h, w = s.shape
+    lib().orc_lut_sweep_patch(C.c_int64(L), C.c_double(beta), C.c_uint64(seed), C.c_uint32(t),
+                              C.c_int64(x0), C.c_int64(y0), C.c_int64(w), C.c_int64(h), _p(s, C.c_int8))
+
+
+def lut_window_after(L, beta, seed, n_sweeps, x0, y0, w, h) -> np.ndarray:
+    m = 2 * n_sweeps
+    assert w + 2 * m <= L and h + 2 * m <= L, "light cone wraps onto itself"
+    s = lut_init_patch(L, seed, x0 - m, y0 - m, w + 2 * m, h + 2 * m)
+    for t in range(n_sweeps):
+        lut_sweep_patch(L, s, beta, seed, t, x0 - m, y0 - m)
+    return s[m:m + h, m:m + w].copy()
+
+
 def threads() -> int:
     return int(lib().orc_threads())

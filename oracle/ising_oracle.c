@@ -20,8 +20,11 @@
  * vectors, closed-form thresholds, tally == recompute invariant, exact
  * enumeration of 4x4 Ising / 3x3 + 4x4 Blume-Capel, Onsager energy and
  * magnetisation, crafted-lattice closed forms for observables, brute force and
- * sum identities for correlation, Schwinger-Dyson -> 1.  No function is
- * "parity unpinned".
+ * sum identities for correlation, Schwinger-Dyson -> 1.  Section O7 (the
+ * paper's 1-bit look-up-table kernel, tests/test_oracle_lut.py): table
+ * marginals / independence / closed forms, getMaxLE against a library
+ * search, per-word sweep == independently written per-site sweep, tally ==
+ * recompute, 4x4 exact enumeration, Onsager.  No function is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -370,6 +373,176 @@ void orc_run(int model, int64_t L, double beta, double D, uint64_t seed,
 {
     for (int64_t i = 0; i < n; ++i) {
         orc_sweep(model, L, beta, D, seed, t0 + (uint32_t)i, s, tallies);
+        if (trace) { trace[3 * i] = tallies[0]; trace[3 * i + 1] = tallies[1]; trace[3 * i + 2] = tallies[2]; }
+    }
+}
+
+/* ================================================================== O7 === */
+/* NEXT-2: the paper's own Ising kernel: one bit per spin, and
+ * non-uniform random BITS from a look-up table instead of one uniform number
+ * per spin.  Same acceptance probabilities as O4, a different trajectory
+ * contract (readings L1-L6 in DESIGN.md):
+ *
+ *   flip = (eq4 & exp8) | (eq3 & exp4) | (~eq4 & ~eq3)
+ *   exp4 = nonUniformRandBits();  exp8 = nonUniformRandBits() & exp4;
+ *
+ * where every bit of nonUniformRandBits() is 1 with probability p = e^{-4 beta},
+ * so a spin with 4 equal neighbours flips with probability p^2 = e^{-8 beta}.
+ * Four bits come from one 32-bit Philox number: getMaxLE(table, rnd) = the
+ * largest index i in 0..15 with table[i] <= rnd, table[i] =
+ * floor(2^32 * sum_{j<i} P(j)), P(j) = p^popc(j) (1-p)^(4-popc(j)).
+ *
+ * Keying (L3): the same-colour sites of a row are grouped in words of 64
+ * (compact index k = x >> 1, word m = k >> 6, bit j = k & 63; Wr = ceil(L/128)
+ * words per colour row, global word index w = y*Wr + m).  The 32 numbers of a
+ * word come from 8 Philox calls with counter (g_lo, g_hi, t, colour), g = 8 w + q:
+ * calls q = 0..3 feed exp4, q = 4..7 feed exp8; call q's output word u gives the
+ * nibble 4 (q & 3) + u of its 64-bit word, i.e. bits 16 (q & 3) + 4 u + (0..3).   */
+
+/* L2: the table in double, sums taken in index order; entries in [0, 2^32]. */
+void orc_lut_table(double beta, uint64_t table[16])
+{
+    const double p = exp(-(4.0 * beta)), q = 1.0 - p;
+    double pw[5], qw[5];
+    pw[0] = 1.0; qw[0] = 1.0;
+    for (int a = 1; a <= 4; ++a) { pw[a] = pw[a - 1] * p; qw[a] = qw[a - 1] * q; }
+    double cum = 0.0;
+    for (int i = 0; i < 16; ++i) {
+        double v = floor(ldexp(cum, 32));
+        if (v > 4294967296.0) v = 4294967296.0;
+        table[i] = (uint64_t)v;
+        const int ones = __builtin_popcount((unsigned)i);
+        cum += pw[ones] * qw[4 - ones];
+    }
+}
+
+static inline unsigned get_max_le(const uint64_t table[16], uint32_t rnd)
+{
+    unsigned idx = 0;
+    for (unsigned i = 0; i < 16; ++i)
+        if (table[i] <= (uint64_t)rnd) idx = i;      /* table is non-decreasing, table[0] = 0 */
+    return idx;
+}
+
+static inline int64_t lut_words_per_row(int64_t L) { return (L / 2 + 63) / 64; }
+
+/* The 64 random bits of word w: which = 0 -> exp4 source, 1 -> exp8 source.  */
+uint64_t orc_lut_bits(const uint64_t table[16], uint64_t seed, uint64_t w, uint32_t t, uint32_t tag, int which)
+{
+    const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    uint64_t ret = 0;
+    for (int k = 0; k < 64; k += 4) {                /* the paper's loop */
+        const int nib = k / 4, q = which * 4 + nib / 4, u = nib % 4;
+        const uint64_t g = 8 * w + (uint64_t)q;
+        const uint32_t ctr[4] = { (uint32_t)g, (uint32_t)(g >> 32), t, tag };
+        uint32_t out[4];
+        orc_philox4x32_10(ctr, key, out);
+        ret |= (uint64_t)get_max_le(table, out[u]) << k;
+    }
+    return ret;
+}
+
+/* L5: initial spins, one bit each: word w of colour c = (x | y << 32) of Philox(ctr = (w, t = 0, tag = 2 + c)). */
+void orc_lut_init_patch(int64_t L, uint64_t seed, int64_t x0, int64_t y0, int64_t w, int64_t h, int8_t *s)
+{
+    const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    const int64_t Wr = lut_words_per_row(L);
+    for (int64_t j = 0; j < h; ++j)
+        for (int64_t i = 0; i < w; ++i) {
+            const int64_t x = ((x0 + i) % L + L) % L, y = ((y0 + j) % L + L) % L;
+            const uint32_t c = (uint32_t)((x + y) & 1);
+            const int64_t k = x >> 1;
+            const uint64_t wd = (uint64_t)(y * Wr + (k >> 6));
+            const uint32_t ctr[4] = { (uint32_t)wd, (uint32_t)(wd >> 32), 0u, 2u + c };
+            uint32_t out[4];
+            orc_philox4x32_10(ctr, key, out);
+            const uint64_t bits = (uint64_t)out[0] | ((uint64_t)out[1] << 32);
+            s[j * w + i] = ((bits >> (k & 63)) & 1u) ? 1 : -1;
+        }
+}
+
+void orc_lut_init(int64_t L, uint64_t seed, int8_t *s) { orc_lut_init_patch(L, seed, 0, 0, L, L, s); }
+
+/* L4: one sweep in the paper's order: colour 0 then colour 1; for every word of 64 same-colour
+ * sites the two random words are drawn, then each site applies the flip formula with its own
+ * bit.  tallies = {B, M, Q} updated incrementally (E = -B).                                   */
+void orc_lut_sweep(int64_t L, double beta, uint64_t seed, uint32_t t, int8_t *s, int64_t *tallies)
+{
+    uint64_t table[16];
+    orc_lut_table(beta, table);
+    const int64_t Wr = lut_words_per_row(L), half = L / 2;
+    int64_t B = tallies[0], M = tallies[1];
+    for (uint32_t c = 0; c < 2; ++c) {
+        int64_t dB = 0, dM = 0;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) reduction(+ : dB, dM) if (L >= 64)
+#endif
+        for (int64_t y = 0; y < L; ++y) {
+            const int64_t ym = (y + L - 1) % L, yp = (y + 1) % L, par = (y + c) & 1;
+            for (int64_t m = 0; m < Wr; ++m) {
+                const uint64_t w = (uint64_t)(y * Wr + m);
+                const uint64_t exp4 = orc_lut_bits(table, seed, w, t, c, 0);
+                const uint64_t exp8 = orc_lut_bits(table, seed, w, t, c, 1) & exp4;
+                for (int j = 0; j < 64; ++j) {
+                    const int64_t k = 64 * m + j;
+                    if (k >= half) break;
+                    const int64_t x = 2 * k + par, xm = (x + L - 1) % L, xp = (x + 1) % L;
+                    const int sp = s[y * L + x];
+                    const int h = s[ym * L + x] + s[yp * L + x] + s[y * L + xm] + s[y * L + xp];
+                    const int eq = (4 + sp * h) / 2;             /* neighbours equal to the spin, 0..4 */
+                    const int b4 = (int)((exp4 >> j) & 1u), b8 = (int)((exp8 >> j) & 1u);
+                    const int flip = (eq == 4 && b8) || (eq == 3 && b4) || (eq <= 2);
+                    if (flip) { dB -= 2 * sp * h; dM -= 2 * sp; s[y * L + x] = (int8_t)(-sp); }
+                }
+            }
+        }
+        B += dB; M += dM;
+    }
+    tallies[0] = B; tallies[1] = M;
+}
+
+/* Light-cone patch version, written per SITE (not per word): the bit of site (x, y) is looked
+ * up from scratch, so it also serves as an independent restatement of the keying.            */
+void orc_lut_sweep_patch(int64_t L, double beta, uint64_t seed, uint32_t t,
+                         int64_t x0, int64_t y0, int64_t w, int64_t h, int8_t *s)
+{
+    uint64_t table[16];
+    orc_lut_table(beta, table);
+    const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    const int64_t Wr = lut_words_per_row(L);
+    for (uint32_t c = 0; c < 2; ++c)
+        for (int64_t j = 0; j < h; ++j)
+            for (int64_t i = 0; i < w; ++i) {
+                const int64_t x = ((x0 + i) % L + L) % L, y = ((y0 + j) % L + L) % L;
+                if ((uint32_t)((x + y) & 1) != c) continue;
+                int hs = 0;
+                if (j > 0) hs += s[(j - 1) * w + i];
+                if (j < h - 1) hs += s[(j + 1) * w + i];
+                if (i > 0) hs += s[j * w + i - 1];
+                if (i < w - 1) hs += s[j * w + i + 1];
+                const int64_t k = x >> 1, bit = k & 63;
+                const uint64_t wd = (uint64_t)(y * Wr + (k >> 6));
+                int b[2];
+                for (int which = 0; which < 2; ++which) {
+                    const uint64_t g = 8 * wd + (uint64_t)(which * 4 + bit / 16);
+                    const uint32_t ctr[4] = { (uint32_t)g, (uint32_t)(g >> 32), t, c };
+                    uint32_t out[4];
+                    orc_philox4x32_10(ctr, key, out);
+                    b[which] = (int)((get_max_le(table, out[(bit / 4) % 4]) >> (bit % 4)) & 1u);
+                }
+                const int sp = s[j * w + i];
+                const int eq = (4 + sp * hs) / 2;
+                const int flip = (eq == 4 && b[0] && b[1]) || (eq == 3 && b[0]) || (eq <= 2);
+                if (flip) s[j * w + i] = (int8_t)(-sp);
+            }
+}
+
+/* n sweeps t0..t0+n-1 of the LUT kernel with the (B, M, Q) trace after each (test helper). */
+void orc_lut_run(int64_t L, double beta, uint64_t seed, uint32_t t0, int64_t n, int8_t *s,
+                 int64_t *tallies, int64_t *trace)
+{
+    for (int64_t i = 0; i < n; ++i) {
+        orc_lut_sweep(L, beta, seed, t0 + (uint32_t)i, s, tallies);
         if (trace) { trace[3 * i] = tallies[0]; trace[3 * i + 1] = tallies[1]; trace[3 * i + 2] = tallies[2]; }
     }
 }
