@@ -37,7 +37,8 @@ extern "C" {
 
 typedef struct ising_sim ising_t; /* opaque */
 
-enum { ISING_MODEL_ISING = 0, ISING_MODEL_BLUME_CAPEL = 1 };
+enum { ISING_MODEL_ISING = 0, ISING_MODEL_BLUME_CAPEL = 1,
+       ISING_MODEL_ISING_LUT = 2 /* the paper's own kernel: 1 bit per spin, look-up-table random bits */ };
 enum { ISING_OK = 0, ISING_EINVAL = -1, ISING_ENOMEM = -2, ISING_ECUDA = -3 };
 
 /* Integer observables are the bit-exact contract; the doubles are formed on

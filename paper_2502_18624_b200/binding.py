@@ -8,7 +8,7 @@ from dataclasses import dataclass
 
 import numpy as np
 
-ISING, BLUME_CAPEL = 0, 1
+ISING, BLUME_CAPEL, ISING_LUT = 0, 1, 2
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libising_b200.so")
 _lib = None
@@ -138,7 +138,7 @@ class IsingSim:
         self.model, self.L, self.beta, self.D, self.seed = model, L, float(beta), float(D), seed
         nbytes = workspace_bytes(model, L)
         if nbytes == 0:
-            raise IsingError(-1, "invalid (model, L): L must be a multiple of 64, >= 64")
+            raise IsingError(-1, "invalid (model, L): L must be a multiple of 64, >= 64 (256 for the LUT model)")
         self._h = C.c_void_p()
         with torch.cuda.device(self.device):
             self._stream = torch.cuda.current_stream(self.device)
@@ -226,7 +226,7 @@ class IsingSim:
         _check(self._lib.ising_write_lattice(self._h, y0, spins.shape[0], spins.ctypes.data))
 
     def read_packed(self, colour: int, word0: int = 0, nwords: int | None = None, out=None):
-        total = self.L * (self.L // 32)
+        total = self.L * (self.L // (128 if self.model == ISING_LUT else 32))
         nwords = total - word0 if nwords is None else nwords
         if out is None:
             out = np.empty(nwords, dtype=np.uint64)

@@ -29,6 +29,7 @@ extern "C" const char *ising_last_error(void) { return g_err.c_str(); }
 
 static bool valid_model_L(int model, int64_t L)
 {
+    if (model == ISING_MODEL_ISING_LUT) return L >= 256 && (L % 256) == 0 && L <= (1ll << 20);   // 128-bit vector = 128 sites
     return (model == ISING_MODEL_ISING || model == ISING_MODEL_BLUME_CAPEL) && L >= 64 && (L % 64) == 0 &&
            L <= (1ll << 20);
 }
@@ -36,6 +37,7 @@ static bool valid_model_L(int model, int64_t L)
 extern "C" size_t ising_workspace_bytes(int model, int64_t L)
 {
     if (!valid_model_L(model, L)) return 0;
+    if (model == ISING_MODEL_ISING_LUT) return (size_t)L * (size_t)L / 8 + kScratchBytes;   // 1 bit per spin
     return (size_t)L * (size_t)L / 2 + kScratchBytes;
 }
 
@@ -48,8 +50,29 @@ static uint64_t metropolis_threshold(double beta, double dE)
     return (uint64_t)floor(ldexp(p, 32));
 }
 
+// NEXT-2 (reading L2): table[i] = floor(2^32 sum_{j<i} P(j)),
+// P(j) = p^popc(j) (1-p)^(4-popc(j)), p = exp(-4 beta), sums in index order in double.
+static void build_lut_table(ising_sim *h)
+{
+    const double p = exp(-(4.0 * h->beta)), q = 1.0 - p;
+    double pw[5] = {1, 0, 0, 0, 0}, qw[5] = {1, 0, 0, 0, 0};
+    for (int k = 1; k <= 4; ++k) { pw[k] = pw[k - 1] * p; qw[k] = qw[k - 1] * q; }
+    double cum = 0.0;
+    h->n_T = 16;
+    for (int i = 0; i < 16; ++i) {
+        double v = floor(ldexp(cum, 32));
+        if (v > 4294967296.0) v = 4294967296.0;
+        h->T[i] = (uint64_t)v;
+        int ones = 0;
+        for (int b = 0; b < 4; ++b) ones += (i >> b) & 1;
+        volatile double term = pw[ones] * qw[4 - ones];      // rounded product, then the sum (no FMA)
+        cum += term;
+    }
+}
+
 static void build_thresholds(ising_sim *h)
 {
+    if (h->model == ISING_MODEL_ISING_LUT) { build_lut_table(h); return; }
     if (h->model == ISING_MODEL_ISING) {
         // entry i: dE = 4 i - 8, i.e. the spin agrees with i of... dE = 2 s h in {-8,-4,0,4,8}
         h->n_T = 5;
@@ -100,7 +123,7 @@ extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_
 
     ising_sim *h = new (std::nothrow) ising_sim();
     if (!h) return set_error(ISING_ENOMEM, "ising_create: host allocation failed");
-    h->model = model; h->L = L; h->beta = beta; h->D = (model == ISING_MODEL_ISING) ? 0.0 : D; h->seed = seed;
+    h->model = model; h->L = L; h->beta = beta; h->D = (model == ISING_MODEL_BLUME_CAPEL) ? D : 0.0; h->seed = seed;
     h->stream = (cudaStream_t)cuda_stream;
     char *base = (char *)dev_buf;
     if (!base) {
@@ -113,7 +136,7 @@ extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_
         }
         base = (char *)h->owned;
     }
-    const size_t colour_bytes = (size_t)L * (size_t)L / 4;
+    const size_t colour_bytes = (model == ISING_MODEL_ISING_LUT) ? (size_t)L * (size_t)L / 16 : (size_t)L * (size_t)L / 4;
     h->lat[0] = (uint64_t *)base;
     h->lat[1] = (uint64_t *)(base + colour_bytes);
     h->d_acc = (long long *)(base + 2 * colour_bytes);                 // 64 int64 = 512 B (+ 4 KiB sink area unused)
@@ -146,7 +169,27 @@ extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_
         if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
         if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "upload of the Blume-Capel table"); }
     }
-    e = launch_init(h);
+    if (model == ISING_MODEL_ISING_LUT) {
+        // heap-ordered carry constants of the binary search: node n at level l splits at table index
+        // ((n - 2^l) << (4 - l)) | (1 << (3 - l));  rnd >= table[i]  <=>  rnd + (2^32 - table[i]) carries
+        uint32_t tree[16] = {};
+        for (int i = 1; i < 16; ++i)
+            if (h->T[i] == 0) {      // "rnd >= 0" has no 32-bit carry constant (2^32 is fine: constant 0, never a carry)
+                ising_destroy(h);
+                return set_error(ISING_EINVAL, "ising_create: beta too small for the look-up-table model "
+                                               "(a table entry above index 0 is 0; needs beta > about 0.001)");
+            }
+        for (int l = 0; l < 4; ++l)
+            for (int n = 1 << l; n < (2 << l); ++n) {
+                const int idx = ((n - (1 << l)) << (4 - l)) | (1 << (3 - l));
+                tree[n] = (uint32_t)((1ull << 32) - h->T[idx]);
+            }
+        memcpy(h->h_acc, tree, sizeof(tree));
+        e = cudaMemcpyAsync(h->d_bc_table, h->h_acc, sizeof(tree), cudaMemcpyHostToDevice, h->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+        if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "upload of the look-up table"); }
+    }
+    e = (model == ISING_MODEL_ISING_LUT) ? launch_lut_init(h) : launch_init(h);
     if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "init kernel"); }
     *out = h;
     return ISING_OK;
@@ -185,7 +228,8 @@ extern "C" int ising_sweep(ising_t *h, int64_t n)
     if (h->t + (uint64_t)n > 0xFFFFFFFFull) return set_error(ISING_EINVAL, "ising_sweep: sweep counter would exceed 2^32-1");
     for (int64_t i = 0; i < n; ++i) {
         for (int c = 0; c < 2; ++c) {
-            cudaError_t e = launch_update(h, c, (uint32_t)h->t);
+            cudaError_t e = (h->model == ISING_MODEL_ISING_LUT) ? launch_lut_update(h, c, (uint32_t)h->t)
+                                                                : launch_update(h, c, (uint32_t)h->t);
             if (e != cudaSuccess) return cuda_fail(e, "update kernel");
         }
         h->t++;
@@ -225,15 +269,16 @@ extern "C" int ising_set_variant(ising_t *h, int variant)
 extern "C" int ising_observables(ising_t *h, ising_obs_t *out)
 {
     if (!h || !out) return set_error(ISING_EINVAL, "ising_observables: NULL argument");
-    cudaError_t e = launch_observables(h);
+    const bool lut = h->model == ISING_MODEL_ISING_LUT;
+    cudaError_t e = lut ? launch_lut_observables(h) : launch_observables(h);
     if (e != cudaSuccess) return cuda_fail(e, "observables kernel");
     CUDA_TRY(cudaMemcpyAsync(h->h_acc, h->d_acc, 3 * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     ising_obs_t o;
-    o.bond_sum = h->h_acc[0]; o.M = h->h_acc[1]; o.Q = h->h_acc[2];
+    o.bond_sum = h->h_acc[0]; o.M = h->h_acc[1]; o.Q = lut ? h->L * h->L : h->h_acc[2];
     o.n_sites = h->L * h->L; o.sweeps_done = h->t;
     const double N = (double)h->L * (double)h->L;
-    o.E = (h->model == ISING_MODEL_ISING) ? -(double)o.bond_sum : -(double)o.bond_sum + h->D * (double)o.Q;
+    o.E = (h->model != ISING_MODEL_BLUME_CAPEL) ? -(double)o.bond_sum : -(double)o.bond_sum + h->D * (double)o.Q;
     o.e_per_site = o.E / N;
     o.m_per_site = (double)o.M / N;
     o.zero_density = (double)(o.n_sites - o.Q) / N;
@@ -244,7 +289,7 @@ extern "C" int ising_observables(ising_t *h, ising_obs_t *out)
 extern "C" int ising_schwinger_dyson(ising_t *h, int64_t hist[9], double *value)
 {
     if (!h || !hist || !value) return set_error(ISING_EINVAL, "ising_schwinger_dyson: NULL argument");
-    cudaError_t e = launch_sd_hist(h);
+    cudaError_t e = (h->model == ISING_MODEL_ISING_LUT) ? launch_lut_sd_hist(h) : launch_sd_hist(h);
     if (e != cudaSuccess) return cuda_fail(e, "Schwinger-Dyson kernel");
     CUDA_TRY(cudaMemcpyAsync(h->h_acc + 8, h->d_acc + 8, 9 * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
@@ -333,7 +378,7 @@ extern "C" int ising_write_lattice(ising_t *h, int64_t y0, int64_t ny, const int
 extern "C" int ising_read_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, uint64_t *host_out)
 {
     if (!h || !host_out) return set_error(ISING_EINVAL, "ising_read_packed: NULL argument");
-    if ((colour != 0 && colour != 1) || word0 < 0 || nwords < 0 || word0 + nwords > words_per_colour(h->L))
+    if ((colour != 0 && colour != 1) || word0 < 0 || nwords < 0 || word0 + nwords > colour_words(h))
         return set_error(ISING_EINVAL, "ising_read_packed: range outside the colour array");
     CUDA_TRY(cudaMemcpyAsync(host_out, h->lat[colour] + word0, (size_t)nwords * 8, cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
@@ -343,7 +388,7 @@ extern "C" int ising_read_packed(ising_t *h, int colour, int64_t word0, int64_t 
 extern "C" int ising_write_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, const uint64_t *host_in)
 {
     if (!h || !host_in) return set_error(ISING_EINVAL, "ising_write_packed: NULL argument");
-    if ((colour != 0 && colour != 1) || word0 < 0 || nwords < 0 || word0 + nwords > words_per_colour(h->L))
+    if ((colour != 0 && colour != 1) || word0 < 0 || nwords < 0 || word0 + nwords > colour_words(h))
         return set_error(ISING_EINVAL, "ising_write_packed: range outside the colour array");
     CUDA_TRY(cudaMemcpyAsync(h->lat[colour] + word0, host_in, (size_t)nwords * 8, cudaMemcpyHostToDevice, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
@@ -354,7 +399,7 @@ extern "C" int ising_write_packed(ising_t *h, int colour, int64_t word0, int64_t
 static int ensure_planes(ising_sim *h)
 {
     const size_t pw = (size_t)h->L * (size_t)(h->L / 64);
-    const size_t bytes = pw * 8 * (h->model == ISING_MODEL_ISING ? 2 : 4);
+    const size_t bytes = pw * 8 * (h->model != ISING_MODEL_BLUME_CAPEL ? 2 : 4);
     if (h->planes_bytes >= bytes) return ISING_OK;
     cudaError_t e = cudaMalloc((void **)&h->planes, bytes);
     if (e != cudaSuccess) { cudaGetLastError(); h->planes = nullptr; return set_error(ISING_ENOMEM, "bit planes: cudaMalloc failed"); }
@@ -365,7 +410,7 @@ static int ensure_planes(ising_sim *h)
 static int ensure_comb(ising_sim *h, int64_t stride)
 {
     const size_t bytes = (size_t)h->L * (size_t)comb_words_per_row(h->L, stride) * 8 *
-                         (h->model == ISING_MODEL_ISING ? 2 : 4);
+                         (h->model != ISING_MODEL_BLUME_CAPEL ? 2 : 4);
     if (h->comb_bytes >= bytes) return ISING_OK;
     if (h->comb) { cudaFree(h->comb); h->comb = nullptr; h->comb_bytes = 0; }
     cudaError_t e = cudaMalloc((void **)&h->comb, bytes);
@@ -409,7 +454,7 @@ static int run_corr(ising_sim *h, int64_t stride, int64_t count, const int64_t *
     CUDA_TRY(cudaMemcpyAsync(sx, d_sx, (size_t)count * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaMemcpyAsync(sy, d_sy, (size_t)count * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
-    if (h->model == ISING_MODEL_ISING) {   // popcount of unequal pairs -> pair sum
+    if (h->model != ISING_MODEL_BLUME_CAPEL) {   // popcount of unequal pairs -> pair sum
         const int64_t s = stride > 0 ? stride : 1;
         const int64_t n_src = (h->L / s) * (h->L / s);
         for (int64_t i = 0; i < count; ++i) { sx[i] = n_src - 2 * sx[i]; sy[i] = n_src - 2 * sy[i]; }
@@ -529,7 +574,7 @@ extern "C" int ising_correlation_protocol(ising_t *h, int64_t cap, int64_t *r, i
 // ----------------------------------------------------- measurement helpers ---
 extern "C" int ising_bench_philox_only(ising_t *h, int n)
 {
-    if (!h || n < 0) return set_error(ISING_EINVAL, "ising_bench_philox_only: bad argument");
+    if (!h || n < 0 || h->model == ISING_MODEL_ISING_LUT) return set_error(ISING_EINVAL, "ising_bench_philox_only: bad argument");
     for (int i = 0; i < n; ++i) {
         cudaError_t e = launch_philox_only(h, (uint32_t)i);
         if (e != cudaSuccess) return cuda_fail(e, "philox-only kernel");
@@ -539,7 +584,7 @@ extern "C" int ising_bench_philox_only(ising_t *h, int n)
 
 extern "C" int ising_bench_copy(ising_t *h, int n)
 {
-    if (!h || n < 0) return set_error(ISING_EINVAL, "ising_bench_copy: bad argument");
+    if (!h || n < 0 || h->model == ISING_MODEL_ISING_LUT) return set_error(ISING_EINVAL, "ising_bench_copy: bad argument");
     for (int i = 0; i < n; ++i) {
         cudaError_t e = launch_copy(h);
         if (e != cudaSuccess) return cuda_fail(e, "copy kernel");

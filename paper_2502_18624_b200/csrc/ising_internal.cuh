@@ -53,6 +53,11 @@ int cuda_fail(cudaError_t e, const char *what);
 
 static inline int64_t words_per_row(int64_t L) { return L / 32; }              // uint64 per colour row
 static inline int64_t words_per_colour(int64_t L) { return L * (L / 32); }
+// uint64 words of one colour array: 16 sites per word (4 bits each), or 64 for the 1-bit LUT model
+static inline int64_t colour_words(const ising_sim *h)
+{
+    return h->model == ISING_MODEL_ISING_LUT ? h->L * (h->L / 128) : h->L * (h->L / 32);
+}
 // 64-bit words per row of a plane down-sampled to the bits x % stride == 0 (zero padded)
 static inline int64_t comb_words_per_row(int64_t L, int64_t stride) { return (L / stride + 63) / 64; }
 
@@ -69,6 +74,10 @@ cudaError_t launch_corr(ising_sim *h, int64_t stride, int64_t count, const long 
 bool corr_gram_supported(const ising_sim *h, int64_t rmax);
 size_t corr_gram_bytes(const ising_sim *h);
 cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, long long *dev_sy);
+cudaError_t launch_lut_init(ising_sim *h);
+cudaError_t launch_lut_update(ising_sim *h, int colour, uint32_t t);
+cudaError_t launch_lut_observables(ising_sim *h);                   // -> d_acc[0..1] = B, M
+cudaError_t launch_lut_sd_hist(ising_sim *h);                       // -> d_acc[8..16]
 cudaError_t launch_philox_only(ising_sim *h, uint32_t t);
 cudaError_t launch_copy(ising_sim *h);
 cudaError_t launch_debug_philox(int64_t count, const uint32_t *d_ctr, const uint32_t *d_key,

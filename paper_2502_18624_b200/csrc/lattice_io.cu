@@ -18,6 +18,11 @@ __global__ void __launch_bounds__(256) unpack_kernel(const __grid_constant__ Unp
     int64_t x = (p.x0 + i) % p.L, y = (p.y0 + j) % p.L;     // x0, y0 already reduced to [0, L)
     int c = (int)((x + y) & 1);
     int64_t k = x >> 1;
+    if (p.model == ISING_MODEL_ISING_LUT) {                  // 1 bit per spin, 64 sites per word
+        uint64_t word = p.lat[c][y * (p.L / 128) + (k >> 6)];
+        p.out[idx] = (int8_t)(2 * (int)((word >> (k & 63)) & 1u) - 1);
+        return;
+    }
     uint64_t word = p.lat[c][y * (p.L / 32) + (k >> 4)];
     int nib = (int)((word >> (4 * (k & 15))) & 15u);
     p.out[idx] = (int8_t)(p.model == ISING_MODEL_ISING ? 2 * nib - 1 : nib - 1);
@@ -69,6 +74,28 @@ __global__ void __launch_bounds__(256) pack_kernel(const __grid_constant__ PackP
     if (!p.dry) p.lat[c][y * halves_per_row + hf] = w;
 }
 
+// 1-bit layout (ISING_MODEL_ISING_LUT): one thread per 32-bit half (32 same-colour sites)
+__global__ void __launch_bounds__(256) pack_lut_kernel(const __grid_constant__ PackParams p)
+{
+    const int64_t halves_per_row = p.L / 64;
+    int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= p.ny * halves_per_row * 2) return;
+    int c = (int)(idx & 1);
+    int64_t rest = idx >> 1;
+    int64_t row = rest / halves_per_row, hf = rest - row * halves_per_row;
+    int64_t y = p.y0 + row;
+    int par = (int)((y + c) & 1);
+    uint32_t w = 0;
+    bool bad = false;
+    for (int j = 0; j < 32; ++j) {
+        int v = p.in[row * p.L + 2 * (hf * 32 + j) + par];
+        bad |= (v != 1 && v != -1);
+        w |= (v > 0 ? 1u : 0u) << j;
+    }
+    if (bad) atomicOr(p.bad, 1);
+    if (!p.dry) p.lat[c][y * halves_per_row + hf] = w;
+}
+
 // write = 0: validate only (cudaErrorInvalidValue if a value is outside the model's set;
 // synchronises).  write = 1: pack and store, no validation result.
 cudaError_t launch_pack(ising_sim *h, int64_t y0, int64_t ny, const int8_t *dev_in, int *dev_bad, int write)
@@ -77,13 +104,15 @@ cudaError_t launch_pack(ising_sim *h, int64_t y0, int64_t ny, const int8_t *dev_
     p.lat[0] = reinterpret_cast<uint32_t *>(h->lat[0]);
     p.lat[1] = reinterpret_cast<uint32_t *>(h->lat[1]);
     p.L = h->L; p.y0 = y0; p.ny = ny; p.model = h->model; p.dry = !write; p.in = dev_in; p.bad = dev_bad;
-    int64_t n = ny * (h->L / 16) * 2;
+    const bool lut = h->model == ISING_MODEL_ISING_LUT;
+    int64_t n = ny * (lut ? h->L / 64 : h->L / 16) * 2;
     cudaError_t e;
     if (!write) {
         e = cudaMemsetAsync(dev_bad, 0, sizeof(int), h->stream);
         if (e != cudaSuccess) return e;
     }
-    pack_kernel<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(p);
+    if (lut) pack_lut_kernel<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(p);
+    else pack_kernel<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(p);
     h->launches++;
     e = cudaGetLastError();
     if (e != cudaSuccess || write) return e;
@@ -136,6 +165,14 @@ __global__ void __launch_bounds__(256) planes_kernel(const __grid_constant__ Pla
     if (idx >= p.L * Wq) return;
     int64_t y = idx / Wq, q = idx - y * Wq;
     uint64_t sg = 0, nz = 0;
+    if (p.model == ISING_MODEL_ISING_LUT) {                  // 1-bit layout: 32 sites of each colour per plane word
+        for (int c = 0; c < 2; ++c) {
+            const uint32_t *row32 = reinterpret_cast<const uint32_t *>(p.lat[c]) + y * Wq;
+            sg |= spread_even(row32[q]) << (int)((y + c) & 1);
+        }
+        p.sg[idx] = sg;
+        return;
+    }
     for (int c = 0; c < 2; ++c) {
         int par = (int)((y + c) & 1);
         const uint64_t *row = p.lat[c] + y * (p.L / 32);
@@ -172,7 +209,7 @@ __global__ void __launch_bounds__(64) transpose_kernel(const uint64_t *__restric
 cudaError_t launch_planes(ising_sim *h)
 {
     const int64_t L = h->L, Wq = L / 64, plane_words = L * Wq;
-    const int np = (h->model == ISING_MODEL_ISING) ? 1 : 2;
+    const int np = (h->model != ISING_MODEL_BLUME_CAPEL) ? 1 : 2;
     PlaneParams p;
     p.lat[0] = h->lat[0]; p.lat[1] = h->lat[1];
     p.L = L; p.model = h->model;

@@ -1,0 +1,272 @@
+// NEXT-2: the paper's own Ising kernel -- one bit per spin and non-uniform
+// random bits from a 16-entry look-up table (4 bits per Philox number, 1/2 number per spin).
+// Model ISING_MODEL_ISING_LUT; readings L1-L7 of DESIGN.md.  Layout: two colour arrays, each
+// L rows x (L/128) uint64 words, bit j of word m of row y = compact site k = 64 m + j
+// (x = 2k + ((y + colour) & 1)), 1 = spin +1.
+//
+// Update kernel: one thread owns one 128-bit column (128 same-colour sites) and walks R rows with
+// the opposite-colour rows y-1, y, y+1 in registers (same sliding window as update.cu).  Per
+// 32-bit word: eq3 / eq4 from a bit-sliced adder of the four "equal to the spin" words, two random
+// words from 4 Philox calls whose 16 numbers each go through a 4-level binary search of the table
+// (shared memory, heap order; IADD3 carry + IMAD.X per level), then the paper's flip formula.
+#include "ising_internal.cuh"
+
+struct LutParams {
+    const uint4 *opp;
+    uint4 *own;
+    int L, cols, R;              // cols = uint4 per colour row = L / 256
+    uint32_t colour, t;
+    const uint32_t *tree;        // 16 carry constants in heap order (device): tree[n] = 2^32 - threshold(node n)
+    RoundKeys rk;
+};
+
+// node n of the heap (1..15) splits at table index: level 0 -> 8; level 1 -> 4, 12; ...
+// host helper (api.cu) fills tree[n]; here only the search.
+__device__ __forceinline__ uint32_t lut_search(uint32_t rnd, uint32_t c_root, const uint32_t *tree)
+{
+    uint32_t node = 1;
+    // level 0: uniform threshold, no load
+    asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\tmadc.lo.u32 %0, %0, 2, 0;\n\t}" : "+r"(node) : "r"(rnd), "r"(c_root));
+#pragma unroll
+    for (int level = 1; level < 4; ++level) {
+        const uint32_t c = tree[node];
+        asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\tmadc.lo.u32 %0, %0, 2, 0;\n\t}" : "+r"(node) : "r"(rnd), "r"(c));
+    }
+    return node;                 // 16 + table index
+}
+
+// 32 random bits (8 nibbles) from two Philox calls: nibble u of call 0, then of call 1
+__device__ __forceinline__ uint32_t lut_bits32(uint32_t g_lo, const PhiloxRow &pr, const RoundKeys &rk,
+                                               uint32_t c_root, const uint32_t *tree)
+{
+    const uint4 a = philox_site4(g_lo, pr, rk), b = philox_site4(g_lo | 1u, pr, rk);
+    uint32_t w = 0;              // highest nibble first; the "+16" of every node is removed at the end
+    w = w * 16u + lut_search(b.w, c_root, tree); w = w * 16u + lut_search(b.z, c_root, tree);
+    w = w * 16u + lut_search(b.y, c_root, tree); w = w * 16u + lut_search(b.x, c_root, tree);
+    w = w * 16u + lut_search(a.w, c_root, tree); w = w * 16u + lut_search(a.z, c_root, tree);
+    w = w * 16u + lut_search(a.y, c_root, tree); w = w * 16u + lut_search(a.x, c_root, tree);
+    // sum_j 16 * 16^j = 0x11111110 + ... : every nibble got +16, i.e. +1 carried into the next nibble
+    return w - 0x11111110u;      // (the carry out of nibble 7 leaves the word)
+}
+
+__device__ __forceinline__ uint32_t lut_flip(uint32_t x, uint32_t up, uint32_t dn, uint32_t sm, uint32_t sd,
+                                             uint32_t e4, uint32_t e8)
+{
+    // 1 where the neighbour equals the spin; bit-sliced count of the four
+    const uint32_t a = ~(up ^ x), b = ~(dn ^ x), c = ~(sm ^ x), d = ~(sd ^ x);
+    const uint32_t s0 = a ^ b, c0 = a & b, s1 = c ^ d, c1 = c & d;
+    const uint32_t eq4 = c0 & c1;
+    const uint32_t eq3 = (c0 ^ c1) & (s0 ^ s1);
+    const uint32_t flip = (eq4 & e8 & e4) | (eq3 & e4) | ~(eq4 | eq3);
+    return x ^ flip;
+}
+
+template <int P>
+__device__ __forceinline__ void lut_side(const uint4 &sm, uint32_t edge, uint32_t sd[4])
+{
+    if (P == 0) {   // neighbour k-1: shift up by one bit, carry in the top bit of the previous word
+        sd[0] = __funnelshift_l(edge, sm.x, 1); sd[1] = __funnelshift_l(sm.x, sm.y, 1);
+        sd[2] = __funnelshift_l(sm.y, sm.z, 1); sd[3] = __funnelshift_l(sm.z, sm.w, 1);
+    } else {        // neighbour k+1
+        sd[0] = __funnelshift_r(sm.x, sm.y, 1); sd[1] = __funnelshift_r(sm.y, sm.z, 1);
+        sd[2] = __funnelshift_r(sm.z, sm.w, 1); sd[3] = __funnelshift_r(sm.w, edge, 1);
+    }
+}
+
+template <int P>
+__device__ __forceinline__ uint4 lut_row(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
+                                         uint32_t edge, uint64_t g0, const LutParams &p, uint32_t c_root,
+                                         const uint32_t *tree)
+{
+    uint32_t sd[4];
+    lut_side<P>(sm, edge, sd);
+    // g0 = 8 * (first 64-site word of this thread): words 2 col, 2 col + 1 -> g0, g0 + 8
+    const PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), p.t, p.colour, p.rk);
+    const uint32_t gl = (uint32_t)g0;         // multiple of 16
+    uint4 o;
+    {
+        const uint32_t e4 = lut_bits32(gl | 0u, pr, p.rk, c_root, tree), e8 = lut_bits32(gl | 4u, pr, p.rk, c_root, tree);
+        o.x = lut_flip(src.x, up.x, dn.x, sm.x, sd[0], e4, e8);
+    }
+    {
+        const uint32_t e4 = lut_bits32(gl | 2u, pr, p.rk, c_root, tree), e8 = lut_bits32(gl | 6u, pr, p.rk, c_root, tree);
+        o.y = lut_flip(src.y, up.y, dn.y, sm.y, sd[1], e4, e8);
+    }
+    {
+        const uint32_t e4 = lut_bits32(gl | 8u, pr, p.rk, c_root, tree), e8 = lut_bits32(gl | 12u, pr, p.rk, c_root, tree);
+        o.z = lut_flip(src.z, up.z, dn.z, sm.z, sd[2], e4, e8);
+    }
+    {
+        const uint32_t e4 = lut_bits32(gl | 10u, pr, p.rk, c_root, tree), e8 = lut_bits32(gl | 14u, pr, p.rk, c_root, tree);
+        o.w = lut_flip(src.w, up.w, dn.w, sm.w, sd[3], e4, e8);
+    }
+    return o;
+}
+
+template <int C>
+__global__ void __launch_bounds__(256) lut_update_kernel(const __grid_constant__ LutParams p)
+{
+    __shared__ uint32_t s_tree[16];
+    if (threadIdx.x < 16) s_tree[threadIdx.x] = p.tree[threadIdx.x];
+    __syncthreads();
+    const uint32_t c_root = s_tree[1];
+    const int cols = p.cols, L = p.L;
+    unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned chunk = tid / (unsigned)cols;
+    int col = (int)(tid - chunk * (unsigned)cols);
+    int y0 = (int)chunk * p.R;
+    if (y0 >= L) return;
+    int yend = min(L, y0 + p.R);
+
+    const size_t rs = (size_t)cols * 16;                               // bytes per colour row
+    const char *oppb = reinterpret_cast<const char *>(p.opp);
+    char *ownb = reinterpret_cast<char *>(p.own);
+    const size_t row0 = (size_t)y0 * rs, cb = (size_t)col * 16;
+    // carry half: parity 0 needs the top bit of the previous 32-bit word, parity 1 the low bit of the next
+    const int halves = cols * 4;
+    const size_t e_p0 = (size_t)((col == 0) ? halves - 1 : 4 * col - 1) * 4;
+    const size_t e_p1 = (size_t)((col == cols - 1) ? 0 : 4 * col + 4) * 4;
+    const size_t e_even = C == 0 ? e_p0 : e_p1, e_odd = C == 0 ? e_p1 : e_p0;   // y0 even: parity = C on even offsets
+    const char *o1 = oppb + row0 + rs + cb;
+    const char *ee = oppb + row0 + e_even;
+    const char *eo = oppb + row0 + rs + e_odd;
+    char *w0 = ownb + row0 + cb;
+
+    const int ym = (y0 == 0) ? L - 1 : y0 - 1;
+    uint4 up = *reinterpret_cast<const uint4 *>(oppb + (size_t)ym * rs + cb);
+    uint4 sm = *reinterpret_cast<const uint4 *>(oppb + row0 + cb);
+    uint4 src = *reinterpret_cast<const uint4 *>(w0);
+    uint32_t edge = *reinterpret_cast<const uint32_t *>(ee);
+    // g = 8 * (64-site word index): word = y * (2 cols) + 2 col
+    const uint64_t gs = (uint64_t)cols * 16;
+    uint64_t g0 = (uint64_t)y0 * gs + (uint64_t)col * 16;
+
+    for (int y = y0; y < yend; y += 2) {
+        const char *o2 = (y + 2 == L) ? oppb + cb : o1 + rs;
+        uint4 dn = *reinterpret_cast<const uint4 *>(o1);
+        uint4 nsrc = *reinterpret_cast<const uint4 *>(w0 + rs);
+        uint32_t nedge = *reinterpret_cast<const uint32_t *>(eo);
+        uint4 dn2 = *reinterpret_cast<const uint4 *>(o2);
+        uint4 o = lut_row<C>(src, up, sm, dn, edge, g0, p, c_root, s_tree);
+        *reinterpret_cast<uint4 *>(w0) = o;
+        g0 += gs;
+        uint4 nsrc2 = src;
+        uint32_t nedge2 = 0;
+        ee += 2 * rs;
+        if (y + 2 < yend) {
+            nsrc2 = *reinterpret_cast<const uint4 *>(w0 + 2 * rs);
+            nedge2 = *reinterpret_cast<const uint32_t *>(ee);
+        }
+        o = lut_row<1 - C>(nsrc, sm, dn, dn2, nedge, g0, p, c_root, s_tree);
+        *reinterpret_cast<uint4 *>(w0 + rs) = o;
+        g0 += gs;
+        up = dn; sm = dn2; src = nsrc2; edge = nedge2;
+        o1 += 2 * rs; eo += 2 * rs; w0 += 2 * rs;
+    }
+}
+
+cudaError_t launch_lut_update(ising_sim *h, int colour, uint32_t t)
+{
+    LutParams p;
+    const int64_t L = h->L;
+    p.opp = reinterpret_cast<const uint4 *>(h->lat[1 - colour]);
+    p.own = reinterpret_cast<uint4 *>(h->lat[colour]);
+    p.L = (int)L; p.cols = (int)(L / 256); p.R = h->rows_per_thread;
+    p.colour = (uint32_t)colour; p.t = t;
+    p.tree = h->d_bc_table;
+    p.rk = h->rk;
+    int64_t chunks = (L + p.R - 1) / p.R;
+    int64_t threads = chunks * p.cols;
+    int block = h->block_threads;
+    unsigned grid = (unsigned)((threads + block - 1) / block);
+    if (colour == 0) lut_update_kernel<0><<<grid, block, 0, h->stream>>>(p);
+    else lut_update_kernel<1><<<grid, block, 0, h->stream>>>(p);
+    h->launches++;
+    return cudaGetLastError();
+}
+
+// L5: word w of colour c = (x | y << 32) of Philox(ctr = (w_lo, w_hi, 0, 2 + c))
+__global__ void __launch_bounds__(256) lut_init_kernel(uint64_t *lat0, uint64_t *lat1, int64_t words, RoundKeys rk)
+{
+    const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= words) return;
+    for (int c = 0; c < 2; ++c) {
+        const uint4 r = philox4x32_10(make_uint4((uint32_t)w, (uint32_t)((uint64_t)w >> 32), 0u, 2u + c), rk);
+        (c ? lat1 : lat0)[w] = (uint64_t)r.x | ((uint64_t)r.y << 32);
+    }
+}
+
+cudaError_t launch_lut_init(ising_sim *h)
+{
+    const int64_t words = h->L * (h->L / 128);
+    lut_init_kernel<<<(unsigned)((words + 255) / 256), 256, 0, h->stream>>>(h->lat[0], h->lat[1], words, h->rk);
+    h->launches++;
+    return cudaGetLastError();
+}
+
+// ----------------------------------------------------------- observables ---
+// One thread per 32-bit word of the CENTRE colour array: d = unequal neighbours per site from
+// four XORs.  MODE 0 (centre = black only): B = sum (4 - 2 d) over black sites (each bond once),
+// M from the black word and the white word of the same position.  MODE 1 (run for both
+// colours): histogram of s*h = 4 - 2 d, bit-sliced count of the four difference words.
+template <int MODE>
+__global__ void __launch_bounds__(256) lut_observe_kernel(const uint32_t *__restrict__ ctr, const uint32_t *__restrict__ nbr,
+                                                          int centre, int L, long long *acc)
+{
+    const int W = L / 64;                                    // 32-bit words per colour row
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    long long v[5] = {0, 0, 0, 0, 0};
+    if (idx < (int64_t)L * W) {
+        const int y = (int)(idx / W), q = (int)(idx - (int64_t)y * W);
+        const int ym = (y == 0) ? L - 1 : y - 1, yp = (y + 1 == L) ? 0 : y + 1;
+        const uint32_t x = ctr[idx], up = nbr[(int64_t)ym * W + q], dn = nbr[(int64_t)yp * W + q], sm = nbr[idx];
+        uint32_t sd;
+        if (((y + centre) & 1) == 0) sd = (sm << 1) | (nbr[(int64_t)y * W + (q == 0 ? W - 1 : q - 1)] >> 31);
+        else sd = (sm >> 1) | (nbr[(int64_t)y * W + (q == W - 1 ? 0 : q + 1)] << 31);
+        const uint32_t a = up ^ x, b = dn ^ x, c = sm ^ x, d = sd ^ x;   // 1 where the neighbour differs
+        if (MODE == 0) {
+            v[0] = 128 - 2 * (__popc(a) + __popc(b) + __popc(c) + __popc(d));
+            v[1] = 2 * (__popc(x) + __popc(sm)) - 64;
+        } else {
+            const uint32_t s0 = a ^ b, c0 = a & b, s1 = c ^ d, c1 = c & d;
+            const uint32_t b0 = s0 ^ s1, t = s0 & s1, b1 = c0 ^ c1 ^ t, b2 = c0 & c1;   // d = b0 + 2 b1 + 4 b2
+            v[0] = __popc(~b0 & ~b1 & ~b2); v[1] = __popc(b0 & ~b1); v[2] = __popc(~b0 & b1);
+            v[3] = __popc(b0 & b1); v[4] = __popc(b2);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        long long s = v[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+        if ((threadIdx.x & 31) == 0 && s) {
+            // MODE 0: acc[0] = B, acc[1] = M.  MODE 1: d = k  <->  s*h = 4 - 2k  <->  hist index 8 - 2k (acc + 8)
+            long long *dst = (MODE == 0) ? &acc[k] : &acc[8 + 8 - 2 * k];
+            if (MODE == 1 || k < 2) atomicAdd(reinterpret_cast<unsigned long long *>(dst), (unsigned long long)s);
+        }
+    }
+}
+
+cudaError_t launch_lut_observables(ising_sim *h)
+{
+    cudaError_t e = cudaMemsetAsync(h->d_acc, 0, 8 * sizeof(long long), h->stream);
+    if (e != cudaSuccess) return e;
+    const int64_t n = h->L * (h->L / 64);
+    lut_observe_kernel<0><<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(
+        reinterpret_cast<const uint32_t *>(h->lat[0]), reinterpret_cast<const uint32_t *>(h->lat[1]), 0, (int)h->L, h->d_acc);
+    h->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_lut_sd_hist(ising_sim *h)
+{
+    cudaError_t e = cudaMemsetAsync(h->d_acc + 8, 0, 9 * sizeof(long long), h->stream);
+    if (e != cudaSuccess) return e;
+    const int64_t n = h->L * (h->L / 64);
+    for (int c = 0; c < 2; ++c) {
+        lut_observe_kernel<1><<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(
+            reinterpret_cast<const uint32_t *>(h->lat[c]), reinterpret_cast<const uint32_t *>(h->lat[1 - c]), c, (int)h->L, h->d_acc);
+        h->launches++;
+    }
+    return cudaGetLastError();
+}
