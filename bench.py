@@ -56,7 +56,8 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--L", type=int, default=0, help="override the lattice size (default: configs[2], 2^18)")
-    ap.add_argument("--model", default="ising", choices=["ising", "bc"])
+    ap.add_argument("--model", default="ising", choices=["ising", "bc", "lut"],
+                    help="ising / bc: the north_star kernels (configs[2] / [3]); lut: NEXT-2, the paper's 1-bit look-up-table kernel on configs[2]'s parameters")
     ap.add_argument("--sweeps-per-step", type=int, default=10)
     ap.add_argument("--workload", default="sweep", choices=["sweep", "corr"],
                     help="sweep: S sweeps + observables (configs[2]/[3]); corr: configs[4], S sweeps + the paper's "
@@ -71,7 +72,7 @@ def parse_args():
 
 
 def pick_workload(args):
-    base = wl.config(2) if args.model == "ising" else wl.config(3)
+    base = wl.config(3) if args.model == "bc" else wl.config(2)
     if getattr(args, "workload", "sweep") == "corr":
         base = wl.config(4)
     L = args.L or base.L
@@ -130,12 +131,18 @@ def time_oracle(model: int, beta: float, D: float, seed: int, seconds: float, L:
     sample of the workload: same model / beta / seed, lattice cut to L x L, as many
     full sweeps as fit in `seconds` (at least 2).  Returns (updates/ns, cores, text)."""
     import oracle
-    s = oracle.init(model, L, seed)
+    if model == wl.ISING_LUT:
+        init = lambda: oracle.lut_init(L, seed)
+        sweep = lambda s, t, tl: oracle.lut_sweep(s, beta, seed, t, tl)
+    else:
+        init = lambda: oracle.init(model, L, seed)
+        sweep = lambda s, t, tl: oracle.sweep(model, s, beta, D, seed, t, tl)
+    s = init()
     tl = oracle.observables(s)
-    tl = oracle.sweep(model, s, beta, D, seed, 0, tl)          # untimed first touch
+    tl = sweep(s, 0, tl)                                       # untimed first touch
     n, t0 = 0, time.perf_counter()
     while True:
-        tl = oracle.sweep(model, s, beta, D, seed, 1 + n, tl)
+        tl = sweep(s, 1 + n, tl)
         n += 1
         dt = time.perf_counter() - t0
         if (dt >= seconds and n >= 2) or n >= 100000:
@@ -150,7 +157,7 @@ def run_reference(args):
     if rank != 0:
         return
     base, L, name = pick_workload(args)
-    model = wl.ISING if args.model == "ising" else wl.BLUME_CAPEL
+    model = {"ising": wl.ISING, "bc": wl.BLUME_CAPEL, "lut": wl.ISING_LUT}[args.model]
     per_step = max(1.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
     vals, info, cores = [], "", 0
     for i in range(args.warmup + args.steps):
@@ -211,13 +218,14 @@ def mem_available_bytes() -> int:
 def run_e2e(eng, torch, model, L, beta, D, seed, S, steps, device):
     """End to end through the C ABI with HOST buffers: per step upload both packed
     colour arrays from pinned host memory, run S sweeps, read the observables."""
-    colour_bytes = L * L // 4
+    per_colour = 16 if model == wl.ISING_LUT else 4            # sites per byte... L*L / per_colour bytes per colour array
+    colour_bytes = L * L // per_colour
     need = 2 * colour_bytes
     note = ""
     if mem_available_bytes() < need + (8 << 30):
-        while L > 4096 and mem_available_bytes() < 2 * (L * L // 4) + (8 << 30):
+        while L > 4096 and mem_available_bytes() < 2 * (L * L // per_colour) + (8 << 30):
             L //= 2
-        colour_bytes = L * L // 4
+        colour_bytes = L * L // per_colour
         note = f"host memory too small for the 2^18 lattice; e2e measured at L={L}"
     words = colour_bytes // 8
     host = [torch.empty(words, dtype=torch.int64).pin_memory() for _ in range(2)]
@@ -285,7 +293,7 @@ def run_ours(args):
     torch.cuda.set_device(device)
 
     base, L, name = pick_workload(args)
-    model = wl.ISING if args.model == "ising" else wl.BLUME_CAPEL
+    model = {"ising": wl.ISING, "bc": wl.BLUME_CAPEL, "lut": wl.ISING_LUT}[args.model]
     S, K, W = args.sweeps_per_step, args.steps, max(args.warmup, 0)
     sim = eng.IsingSim(model, L, base.beta, base.D, replica_seed(base.seed, rank), device=device)
     if args.rows_per_thread or args.block:
@@ -330,11 +338,16 @@ def run_ours(args):
     # roofs, measured in the same process right after the timed region (rank 0 only matters)
     n_roof = 2 * S
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
-    sim.bench_philox_only(2); sim.bench_copy(2); torch.cuda.synchronize(device)
-    ev[0].record(); sim.bench_philox_only(n_roof); ev[1].record(); sim.bench_copy(n_roof); ev[2].record()
-    torch.cuda.synchronize(device)
-    philox_ms = ev[0].elapsed_time(ev[1]) / n_roof
-    copy_ms = ev[1].elapsed_time(ev[2]) / n_roof
+    lut = model == wl.ISING_LUT
+    philox_ms = copy_ms = None
+    if not lut:                                            # the roof helpers work on the 4-bit layout
+        sim.bench_philox_only(2); sim.bench_copy(2); torch.cuda.synchronize(device)
+        ev[0].record(); sim.bench_philox_only(n_roof); ev[1].record(); sim.bench_copy(n_roof); ev[2].record()
+        torch.cuda.synchronize(device)
+        philox_ms = ev[0].elapsed_time(ev[1]) / n_roof
+        copy_ms = ev[1].elapsed_time(ev[2]) / n_roof
+    bytes_per_site = 0.375 if lut else BYTES_PER_SITE_LAUNCH   # 3 x 1 bit or 3 x 4 bits per updated site
+    slots_per_site = PHILOX_SLOTS_PER_SITE / 2 if lut else PHILOX_SLOTS_PER_SITE   # LUT: half a number per site
     tensor_roof = None
     if args.workload == "corr" and rank == 0:
         # full-range correlation (A9) on the tensor cores: whole ising_correlation(L/2) call, i.e.
@@ -360,22 +373,22 @@ def run_ours(args):
     sites_per_launch = L * L // 2
     kern_ms = sweep_ms / (2 * S * K)
     peak, peak_src, peaks = measured_peaks()
-    achieved = BYTES_PER_SITE_LAUNCH * sites_per_launch / (kern_ms * 1e-3) / 1e9
+    achieved = bytes_per_site * sites_per_launch / (kern_ms * 1e-3) / 1e9
     traffic = ncu_traffic(args.model, L)
     # ALU roofline: one Philox4x32-10 call = 18 IMAD.WIDE + 19 LOP3 for 4 sites =
     # 9.25 dispatch slots per site; a slot is 2 clocks of a 16-lane pipe (0.5 warp-instructions per
     # sub-partition per clock, a wide multiply also taking one); 4 sub-partitions per SM.
     sm_ghz = float(peaks.get("sm_max_mhz", 1965.0)) / 1e3
     n_sm = torch.cuda.get_device_properties(device).multi_processor_count
-    alu_peak = n_sm * 4 * sm_ghz * 32 * 0.5 / PHILOX_SLOTS_PER_SITE
+    alu_peak = n_sm * 4 * sm_ghz * 32 * 0.5 / slots_per_site
     kern_upd = sites_per_launch / (kern_ms * 1e6)
     alu_roof = {"bound": "alu", "kernel": "update_kernel (one colour phase)", "achieved": kern_upd, "peak": alu_peak,
                 "unit": "updates/ns", "frac": kern_upd / alu_peak, "traffic": traffic,
                 "peak_source": f"derived: {n_sm} SMs x 4 sub-partitions x {sm_ghz} GHz x 32 lanes x 0.5 slots/clk / "
-                               f"{PHILOX_SLOTS_PER_SITE} slots per site (Philox4x32-10 alone)",
+                               f"{slots_per_site} slots per site (Philox4x32-10 alone)",
                 "avg_launch_ms": kern_ms,
-                "philox_only_kernel_updates_per_ns": sites_per_launch / (philox_ms * 1e6),
-                "frac_of_philox_only_kernel": philox_ms / kern_ms,
+                "philox_only_kernel_updates_per_ns": sites_per_launch / (philox_ms * 1e6) if philox_ms else None,
+                "frac_of_philox_only_kernel": philox_ms / kern_ms if philox_ms else None,
                 "pipe_rates_warp_instr_per_subpartition_clk": pipes}
     value = whole_job_updates_per_ns(world, L, S, K, total_ms)
     line = {
@@ -388,16 +401,16 @@ def run_ours(args):
                    "step": "S sweeps + observables" if args.workload == "sweep" else "S sweeps + correlation protocol + observables",
                    "launch": {"rows_per_thread": args.rows_per_thread or "default", "block": args.block or "default",
                               "variant": args.variant},
-                   "lattice_bytes": L * L // 2, "l2": "inputs larger than L2 (no flush needed)" if L * L // 2 > (256 << 20)
+                   "lattice_bytes": L * L // (8 if model == wl.ISING_LUT else 2), "l2": "inputs larger than L2 (no flush needed)" if L * L // 2 > (256 << 20)
                    else "lattice fits L2: DRAM figures not meaningful", "parallelism": f"replicas x{world}"},
         "measurement_ms_per_step": (total_ms - sweep_ms) / K,
         "sweep_only_updates_per_ns": world * L * L * S * K / (sweep_ms * 1e6),
         "roofline": alu_roof,
         "roofline_hbm": {"bound": "hbm", "kernel": "update_kernel (one colour phase)", "achieved": achieved,
                          "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
-                         "peak_source": peak_src, "algorithmic_bytes_per_launch": BYTES_PER_SITE_LAUNCH * sites_per_launch,
+                         "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_per_site * sites_per_launch,
                          "avg_launch_ms": kern_ms,
-                         "copy_kernel_gbs": BYTES_PER_SITE_LAUNCH * sites_per_launch / (copy_ms * 1e-3) / 1e9},
+                         "copy_kernel_gbs": bytes_per_site * sites_per_launch / (copy_ms * 1e-3) / 1e9 if copy_ms else None},
         "roofline_tensor": tensor_roof,
         "clocks": clocks, "gpu_launches": launches,
         "last_observables": {"bond_sum": obs.bond_sum, "M": obs.M, "sweeps_done": obs.sweeps_done},

@@ -106,6 +106,10 @@ static void default_launch(ising_sim *h)
 {
     h->rows_per_thread = (h->L >= 4096) ? 32 : (h->L >= 512 ? 8 : 2);
     h->block_threads = 128;
+    if (h->model == ISING_MODEL_ISING_LUT) {     // 32 KB bucket table per block: fewer, larger blocks (measured)
+        h->rows_per_thread = (h->L >= 8192) ? 64 : (h->L >= 512 ? 8 : 2);
+        h->block_threads = 256;
+    }
 }
 
 // ---------------------------------------------------------------- create ---
@@ -188,6 +192,24 @@ extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_
         e = cudaMemcpyAsync(h->d_bc_table, h->h_acc, sizeof(tree), cudaMemcpyHostToDevice, h->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
         if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "upload of the look-up table"); }
+        // bucket table of the default kernel variant: entry b covers rnd in [b 2^20, (b+1) 2^20):
+        // {C, meta} with getMaxLE(rnd) = meta + carry(rnd + C) when the bucket holds at most one threshold,
+        // meta = 256 (recompute by binary search) when it holds more
+        std::vector<uint32_t> bk(2 * 4096);
+        for (uint64_t b = 0; b < 4096; ++b) {
+            const uint64_t lo = b << 20, hi = lo + (1ull << 20) - 1;
+            int base = 0, inside = 0;
+            for (int i = 1; i < 16; ++i) {
+                if (h->T[i] <= lo) base = i;
+                else if (h->T[i] <= hi) ++inside;
+            }
+            if (inside == 0) { bk[2 * b] = 0u; bk[2 * b + 1] = (uint32_t)base; }
+            else if (inside == 1) { bk[2 * b] = (uint32_t)((1ull << 32) - h->T[base + 1]); bk[2 * b + 1] = (uint32_t)base; }
+            else { bk[2 * b] = 0u; bk[2 * b + 1] = 256u; }
+        }
+        e = cudaMalloc(&h->lut_buckets, bk.size() * sizeof(uint32_t));
+        if (e == cudaSuccess) e = cudaMemcpy(h->lut_buckets, bk.data(), bk.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "upload of the bucket table"); }
     }
     e = (model == ISING_MODEL_ISING_LUT) ? launch_lut_init(h) : launch_init(h);
     if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "init kernel"); }
@@ -203,6 +225,7 @@ extern "C" int ising_destroy(ising_t *h)
     if (h->planes) cudaFree(h->planes);
     if (h->comb) cudaFree(h->comb);
     if (h->gram) cudaFree(h->gram);
+    if (h->lut_buckets) cudaFree(h->lut_buckets);
     if (h->d_corr) cudaFree(h->d_corr);
     if (h->d_rlist) cudaFree(h->d_rlist);
     if (h->h_acc) cudaFreeHost(h->h_acc);

@@ -35,6 +35,7 @@ struct ising_sim {
     void *io_stage = nullptr; size_t io_stage_bytes = 0;
     uint64_t *planes = nullptr; size_t planes_bytes = 0;      // bit planes for the correlation
     uint64_t *comb = nullptr; size_t comb_bytes = 0;          // planes down-sampled to the source comb (stride >= 2)
+    void *lut_buckets = nullptr;                              // LUT model: 4096 x {C, meta} bucket table (cudaMalloc)
     int8_t *gram = nullptr; size_t gram_bytes = 0;            // L x L int8 spin matrix for the tensor-core correlation
     int corr_path = 0;                                        // 0 auto, 1 bit planes (XOR + POPC), 2 tensor cores
     long long *d_corr = nullptr; size_t d_corr_bytes = 0;

@@ -17,6 +17,7 @@ struct LutParams {
     int L, cols, R;              // cols = uint4 per colour row = L / 256
     uint32_t colour, t;
     const uint32_t *tree;        // 16 carry constants in heap order (device): tree[n] = 2^32 - threshold(node n)
+    const uint2 *buckets;        // 4096 entries indexed by the top 12 bits of the number (device), see lut_bits32
     RoundKeys rk;
 };
 
@@ -35,11 +36,35 @@ __device__ __forceinline__ uint32_t lut_search(uint32_t rnd, uint32_t c_root, co
     return node;                 // 16 + table index
 }
 
-// 32 random bits (8 nibbles) from two Philox calls: nibble u of call 0, then of call 1
+// 32 random bits (8 nibbles) from two Philox calls: nibble u of call 0, then of call 1.
+// V = 1: every number goes through the 4-level binary search.
+// V = 0 (default): bucket table.  The top 12 bits of the number select an entry {C, meta}: the
+// bucket [b 2^20, (b+1) 2^20) holds at most one table threshold t in all but a few buckets, so
+// getMaxLE = idx_base + [rnd >= t] = meta + carry(rnd + C), C = 2^32 - t (0 if the bucket has no
+// threshold): one shift, one LDS.64, one IADD3 and two IMADs per number.  Buckets with two or more
+// thresholds carry meta = 256 (+ anything): the sum of the eight metas then reaches 256 and the
+// word is recomputed by the binary search (rare: none at T >= 0.6 Tc, ~0.1 % of numbers at 0.5 Tc).
+#define LUT_BUCKET_BITS 12
+__device__ __forceinline__ void lut_bucket_step(uint32_t &w, uint32_t &f, uint32_t rnd, const unsigned char *buckets)
+{
+    const uint2 e = *reinterpret_cast<const uint2 *>(buckets + (rnd >> (32 - LUT_BUCKET_BITS)) * 8u);
+    asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\tmadc.lo.u32 %0, %0, 16, %3;\n\t}" : "+r"(w) : "r"(rnd), "r"(e.x), "r"(e.y));
+    asm("mad.lo.u32 %0, %1, 1, %0;" : "+r"(f) : "r"(e.y));
+}
+
+template <int V>
 __device__ __forceinline__ uint32_t lut_bits32(uint32_t g_lo, const PhiloxRow &pr, const RoundKeys &rk,
-                                               uint32_t c_root, const uint32_t *tree)
+                                               uint32_t c_root, const uint32_t *tree, const unsigned char *buckets)
 {
     const uint4 a = philox_site4(g_lo, pr, rk), b = philox_site4(g_lo | 1u, pr, rk);
+    if (V == 0) {
+        uint32_t w = 0, f = 0;   // highest nibble first
+        lut_bucket_step(w, f, b.w, buckets); lut_bucket_step(w, f, b.z, buckets);
+        lut_bucket_step(w, f, b.y, buckets); lut_bucket_step(w, f, b.x, buckets);
+        lut_bucket_step(w, f, a.w, buckets); lut_bucket_step(w, f, a.z, buckets);
+        lut_bucket_step(w, f, a.y, buckets); lut_bucket_step(w, f, a.x, buckets);
+        if (f < 256u) return w;
+    }
     uint32_t w = 0;              // highest nibble first; the "+16" of every node is removed at the end
     w = w * 16u + lut_search(b.w, c_root, tree); w = w * 16u + lut_search(b.z, c_root, tree);
     w = w * 16u + lut_search(b.y, c_root, tree); w = w * 16u + lut_search(b.x, c_root, tree);
@@ -73,10 +98,10 @@ __device__ __forceinline__ void lut_side(const uint4 &sm, uint32_t edge, uint32_
     }
 }
 
-template <int P>
+template <int P, int V>
 __device__ __forceinline__ uint4 lut_row(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
                                          uint32_t edge, uint64_t g0, const LutParams &p, uint32_t c_root,
-                                         const uint32_t *tree)
+                                         const uint32_t *tree, const unsigned char *bk)
 {
     uint32_t sd[4];
     lut_side<P>(sm, edge, sd);
@@ -85,29 +110,35 @@ __device__ __forceinline__ uint4 lut_row(const uint4 &src, const uint4 &up, cons
     const uint32_t gl = (uint32_t)g0;         // multiple of 16
     uint4 o;
     {
-        const uint32_t e4 = lut_bits32(gl | 0u, pr, p.rk, c_root, tree), e8 = lut_bits32(gl | 4u, pr, p.rk, c_root, tree);
+        const uint32_t e4 = lut_bits32<V>(gl | 0u, pr, p.rk, c_root, tree, bk), e8 = lut_bits32<V>(gl | 4u, pr, p.rk, c_root, tree, bk);
         o.x = lut_flip(src.x, up.x, dn.x, sm.x, sd[0], e4, e8);
     }
     {
-        const uint32_t e4 = lut_bits32(gl | 2u, pr, p.rk, c_root, tree), e8 = lut_bits32(gl | 6u, pr, p.rk, c_root, tree);
+        const uint32_t e4 = lut_bits32<V>(gl | 2u, pr, p.rk, c_root, tree, bk), e8 = lut_bits32<V>(gl | 6u, pr, p.rk, c_root, tree, bk);
         o.y = lut_flip(src.y, up.y, dn.y, sm.y, sd[1], e4, e8);
     }
     {
-        const uint32_t e4 = lut_bits32(gl | 8u, pr, p.rk, c_root, tree), e8 = lut_bits32(gl | 12u, pr, p.rk, c_root, tree);
+        const uint32_t e4 = lut_bits32<V>(gl | 8u, pr, p.rk, c_root, tree, bk), e8 = lut_bits32<V>(gl | 12u, pr, p.rk, c_root, tree, bk);
         o.z = lut_flip(src.z, up.z, dn.z, sm.z, sd[2], e4, e8);
     }
     {
-        const uint32_t e4 = lut_bits32(gl | 10u, pr, p.rk, c_root, tree), e8 = lut_bits32(gl | 14u, pr, p.rk, c_root, tree);
+        const uint32_t e4 = lut_bits32<V>(gl | 10u, pr, p.rk, c_root, tree, bk), e8 = lut_bits32<V>(gl | 14u, pr, p.rk, c_root, tree, bk);
         o.w = lut_flip(src.w, up.w, dn.w, sm.w, sd[3], e4, e8);
     }
     return o;
 }
 
-template <int C>
+template <int C, int V>
 __global__ void __launch_bounds__(256) lut_update_kernel(const __grid_constant__ LutParams p)
 {
     __shared__ uint32_t s_tree[16];
+    extern __shared__ __align__(16) unsigned char s_buckets[];          // V = 0: 4096 x 8 bytes
     if (threadIdx.x < 16) s_tree[threadIdx.x] = p.tree[threadIdx.x];
+    if (V == 0) {
+        const uint4 *src4 = reinterpret_cast<const uint4 *>(p.buckets);
+        uint4 *dst4 = reinterpret_cast<uint4 *>(s_buckets);
+        for (int i = threadIdx.x; i < (8 << LUT_BUCKET_BITS) / 16; i += blockDim.x) dst4[i] = src4[i];
+    }
     __syncthreads();
     const uint32_t c_root = s_tree[1];
     const int cols = p.cols, L = p.L;
@@ -147,7 +178,7 @@ __global__ void __launch_bounds__(256) lut_update_kernel(const __grid_constant__
         uint4 nsrc = *reinterpret_cast<const uint4 *>(w0 + rs);
         uint32_t nedge = *reinterpret_cast<const uint32_t *>(eo);
         uint4 dn2 = *reinterpret_cast<const uint4 *>(o2);
-        uint4 o = lut_row<C>(src, up, sm, dn, edge, g0, p, c_root, s_tree);
+        uint4 o = lut_row<C, V>(src, up, sm, dn, edge, g0, p, c_root, s_tree, s_buckets);
         *reinterpret_cast<uint4 *>(w0) = o;
         g0 += gs;
         uint4 nsrc2 = src;
@@ -157,7 +188,7 @@ __global__ void __launch_bounds__(256) lut_update_kernel(const __grid_constant__
             nsrc2 = *reinterpret_cast<const uint4 *>(w0 + 2 * rs);
             nedge2 = *reinterpret_cast<const uint32_t *>(ee);
         }
-        o = lut_row<1 - C>(nsrc, sm, dn, dn2, nedge, g0, p, c_root, s_tree);
+        o = lut_row<1 - C, V>(nsrc, sm, dn, dn2, nedge, g0, p, c_root, s_tree, s_buckets);
         *reinterpret_cast<uint4 *>(w0 + rs) = o;
         g0 += gs;
         up = dn; sm = dn2; src = nsrc2; edge = nedge2;
@@ -179,8 +210,21 @@ cudaError_t launch_lut_update(ising_sim *h, int colour, uint32_t t)
     int64_t threads = chunks * p.cols;
     int block = h->block_threads;
     unsigned grid = (unsigned)((threads + block - 1) / block);
-    if (colour == 0) lut_update_kernel<0><<<grid, block, 0, h->stream>>>(p);
-    else lut_update_kernel<1><<<grid, block, 0, h->stream>>>(p);
+    p.buckets = reinterpret_cast<const uint2 *>(h->lut_buckets);
+    const size_t smem = 8 << LUT_BUCKET_BITS;
+    if (h->variant == 0) {
+        static bool attr = false;
+        if (!attr) {
+            cudaFuncSetAttribute(lut_update_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaFuncSetAttribute(lut_update_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            attr = true;
+        }
+        if (colour == 0) lut_update_kernel<0, 0><<<grid, block, smem, h->stream>>>(p);
+        else lut_update_kernel<1, 0><<<grid, block, smem, h->stream>>>(p);
+    } else {
+        if (colour == 0) lut_update_kernel<0, 1><<<grid, block, 0, h->stream>>>(p);
+        else lut_update_kernel<1, 1><<<grid, block, 0, h->stream>>>(p);
+    }
     h->launches++;
     return cudaGetLastError();
 }

@@ -63,6 +63,21 @@ def test_lattice_and_observables_every_sweep(eng, L, beta, seed, n):
         assert (lx == olx).all() and (ly == oly).all()
 
 
+@pytest.mark.parametrize("beta", [wl.BETA_C / 0.9, wl.BETA_C / 0.5, 1.2, 2.5, 0.01])
+def test_bucket_table_and_binary_search_variants_agree(eng, beta):
+    """Variant 0 (bucket table + rare binary-search fallback; low temperatures have buckets with several
+    thresholds) and variant 1 (binary search only) against the oracle."""
+    L, seed, n = 512, 13, 5
+    s = oracle.lut_init(L, seed)
+    for t in range(n):
+        oracle.lut_sweep(s, beta, seed, t)
+    for variant in (0, 1):
+        with eng.IsingSim(LUT, L, beta, 0.0, seed) as sim:
+            sim.set_variant(variant)
+            sim.sweep(n)
+            assert (sim.read_lattice() == s).all(), variant
+
+
 def test_launch_geometry_and_io_roundtrip(eng):
     L, beta, seed = 512, wl.BETA_C / 0.9, 5
     ref = None
