@@ -45,6 +45,9 @@ __device__ __forceinline__ uint32_t lut_search(uint32_t rnd, uint32_t c_root, co
 // thresholds carry meta = 256 (+ anything): the sum of the eight metas then reaches 256 and the
 // word is recomputed by the binary search (rare: none at T >= 0.6 Tc, ~0.1 % of numbers at 0.5 Tc).
 #define LUT_BUCKET_BITS 12
+#ifndef LUT_MIN_BLOCKS
+#define LUT_MIN_BLOCKS 2
+#endif
 __device__ __forceinline__ void lut_bucket_step(uint32_t &w, uint32_t &f, uint32_t rnd, const unsigned char *buckets)
 {
     const uint2 e = *reinterpret_cast<const uint2 *>(buckets + (rnd >> (32 - LUT_BUCKET_BITS)) * 8u);
@@ -129,7 +132,7 @@ __device__ __forceinline__ uint4 lut_row(const uint4 &src, const uint4 &up, cons
 }
 
 template <int C, int V>
-__global__ void __launch_bounds__(256) lut_update_kernel(const __grid_constant__ LutParams p)
+__global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const __grid_constant__ LutParams p)
 {
     __shared__ uint32_t s_tree[16];
     extern __shared__ __align__(16) unsigned char s_buckets[];          // V = 0: 4096 x 8 bytes
@@ -258,9 +261,10 @@ __global__ void __launch_bounds__(256) lut_observe_kernel(const uint32_t *__rest
                                                           int centre, int L, long long *acc)
 {
     const int W = L / 64;                                    // 32-bit words per colour row
-    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t n = (int64_t)L * W, stride = (int64_t)gridDim.x * blockDim.x;
     long long v[5] = {0, 0, 0, 0, 0};
-    if (idx < (int64_t)L * W) {
+    // grid-stride loop: a few thousand threads keep private sums, so the atomics at the end are few
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += stride) {
         const int y = (int)(idx / W), q = (int)(idx - (int64_t)y * W);
         const int ym = (y == 0) ? L - 1 : y - 1, yp = (y + 1 == L) ? 0 : y + 1;
         const uint32_t x = ctr[idx], up = nbr[(int64_t)ym * W + q], dn = nbr[(int64_t)yp * W + q], sm = nbr[idx];
@@ -269,13 +273,13 @@ __global__ void __launch_bounds__(256) lut_observe_kernel(const uint32_t *__rest
         else sd = (sm >> 1) | (nbr[(int64_t)y * W + (q == W - 1 ? 0 : q + 1)] << 31);
         const uint32_t a = up ^ x, b = dn ^ x, c = sm ^ x, d = sd ^ x;   // 1 where the neighbour differs
         if (MODE == 0) {
-            v[0] = 128 - 2 * (__popc(a) + __popc(b) + __popc(c) + __popc(d));
-            v[1] = 2 * (__popc(x) + __popc(sm)) - 64;
+            v[0] += 128 - 2 * (__popc(a) + __popc(b) + __popc(c) + __popc(d));
+            v[1] += 2 * (__popc(x) + __popc(sm)) - 64;
         } else {
             const uint32_t s0 = a ^ b, c0 = a & b, s1 = c ^ d, c1 = c & d;
             const uint32_t b0 = s0 ^ s1, t = s0 & s1, b1 = c0 ^ c1 ^ t, b2 = c0 & c1;   // d = b0 + 2 b1 + 4 b2
-            v[0] = __popc(~b0 & ~b1 & ~b2); v[1] = __popc(b0 & ~b1); v[2] = __popc(~b0 & b1);
-            v[3] = __popc(b0 & b1); v[4] = __popc(b2);
+            v[0] += __popc(~b0 & ~b1 & ~b2); v[1] += __popc(b0 & ~b1); v[2] += __popc(~b0 & b1);
+            v[3] += __popc(b0 & b1); v[4] += __popc(b2);
         }
     }
 #pragma unroll
@@ -296,7 +300,8 @@ cudaError_t launch_lut_observables(ising_sim *h)
     cudaError_t e = cudaMemsetAsync(h->d_acc, 0, 8 * sizeof(long long), h->stream);
     if (e != cudaSuccess) return e;
     const int64_t n = h->L * (h->L / 64);
-    lut_observe_kernel<0><<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(
+    const unsigned grid_obs = (unsigned)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16);
+    lut_observe_kernel<0><<<grid_obs, 256, 0, h->stream>>>(
         reinterpret_cast<const uint32_t *>(h->lat[0]), reinterpret_cast<const uint32_t *>(h->lat[1]), 0, (int)h->L, h->d_acc);
     h->launches++;
     return cudaGetLastError();
@@ -308,7 +313,7 @@ cudaError_t launch_lut_sd_hist(ising_sim *h)
     if (e != cudaSuccess) return e;
     const int64_t n = h->L * (h->L / 64);
     for (int c = 0; c < 2; ++c) {
-        lut_observe_kernel<1><<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(
+        lut_observe_kernel<1><<<(unsigned)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16), 256, 0, h->stream>>>(
             reinterpret_cast<const uint32_t *>(h->lat[c]), reinterpret_cast<const uint32_t *>(h->lat[1 - c]), c, (int)h->L, h->d_acc);
         h->launches++;
     }
