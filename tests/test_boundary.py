@@ -37,7 +37,8 @@ def test_workspace_bytes_and_validation(lib):
     assert lib.ising_workspace_bytes(1, 1 << 18) == (1 << 36) // 2 + 4096
     for bad_L in (0, 32, 100, 65, -64, (1 << 20) + 64):
         assert lib.ising_workspace_bytes(0, bad_L) == 0
-    assert lib.ising_workspace_bytes(2, 256) == 0
+    assert lib.ising_workspace_bytes(2, 256) == 256 * 256 // 8 + 4096      # LUT model: one bit per spin
+    assert lib.ising_workspace_bytes(2, 192) == 0 and lib.ising_workspace_bytes(3, 256) == 0
 
 
 def test_null_handle_errors(lib):
