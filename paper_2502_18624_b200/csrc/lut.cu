@@ -55,9 +55,11 @@ __device__ __forceinline__ void lut_bucket_step(uint32_t &w, uint32_t &f, uint32
     asm("mad.lo.u32 %0, %1, 1, %0;" : "+r"(f) : "r"(e.y));
 }
 
+// bad: OR of the meta sums of the fast path (>= 256 iff some number fell into a multi-threshold bucket)
 template <int V>
 __device__ __forceinline__ uint32_t lut_bits32(uint32_t g_lo, const PhiloxRow &pr, const RoundKeys &rk,
-                                               uint32_t c_root, const uint32_t *tree, const unsigned char *buckets)
+                                               uint32_t c_root, const uint32_t *tree, const unsigned char *buckets,
+                                               uint32_t &bad)
 {
     const uint4 a = philox_site4(g_lo, pr, rk), b = philox_site4(g_lo | 1u, pr, rk);
     if (V == 0) {
@@ -66,7 +68,8 @@ __device__ __forceinline__ uint32_t lut_bits32(uint32_t g_lo, const PhiloxRow &p
         lut_bucket_step(w, f, b.y, buckets); lut_bucket_step(w, f, b.x, buckets);
         lut_bucket_step(w, f, a.w, buckets); lut_bucket_step(w, f, a.z, buckets);
         lut_bucket_step(w, f, a.y, buckets); lut_bucket_step(w, f, a.x, buckets);
-        if (f < 256u) return w;
+        bad |= f;
+        return w;
     }
     uint32_t w = 0;              // highest nibble first; the "+16" of every node is removed at the end
     w = w * 16u + lut_search(b.w, c_root, tree); w = w * 16u + lut_search(b.z, c_root, tree);
@@ -101,6 +104,11 @@ __device__ __forceinline__ void lut_side(const uint4 &sm, uint32_t edge, uint32_
     }
 }
 
+template <int P>
+__device__ __noinline__ uint4 lut_row_slow(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
+                                           uint32_t edge, uint64_t g0, const LutParams &p, uint32_t c_root,
+                                           const uint32_t *tree);
+
 template <int P, int V>
 __device__ __forceinline__ uint4 lut_row(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
                                          uint32_t edge, uint64_t g0, const LutParams &p, uint32_t c_root,
@@ -111,24 +119,36 @@ __device__ __forceinline__ uint4 lut_row(const uint4 &src, const uint4 &up, cons
     // g0 = 8 * (first 64-site word of this thread): words 2 col, 2 col + 1 -> g0, g0 + 8
     const PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), p.t, p.colour, p.rk);
     const uint32_t gl = (uint32_t)g0;         // multiple of 16
+    uint32_t bad = 0;
     uint4 o;
     {
-        const uint32_t e4 = lut_bits32<V>(gl | 0u, pr, p.rk, c_root, tree, bk), e8 = lut_bits32<V>(gl | 4u, pr, p.rk, c_root, tree, bk);
+        const uint32_t e4 = lut_bits32<V>(gl | 0u, pr, p.rk, c_root, tree, bk, bad), e8 = lut_bits32<V>(gl | 4u, pr, p.rk, c_root, tree, bk, bad);
         o.x = lut_flip(src.x, up.x, dn.x, sm.x, sd[0], e4, e8);
     }
     {
-        const uint32_t e4 = lut_bits32<V>(gl | 2u, pr, p.rk, c_root, tree, bk), e8 = lut_bits32<V>(gl | 6u, pr, p.rk, c_root, tree, bk);
+        const uint32_t e4 = lut_bits32<V>(gl | 2u, pr, p.rk, c_root, tree, bk, bad), e8 = lut_bits32<V>(gl | 6u, pr, p.rk, c_root, tree, bk, bad);
         o.y = lut_flip(src.y, up.y, dn.y, sm.y, sd[1], e4, e8);
     }
     {
-        const uint32_t e4 = lut_bits32<V>(gl | 8u, pr, p.rk, c_root, tree, bk), e8 = lut_bits32<V>(gl | 12u, pr, p.rk, c_root, tree, bk);
+        const uint32_t e4 = lut_bits32<V>(gl | 8u, pr, p.rk, c_root, tree, bk, bad), e8 = lut_bits32<V>(gl | 12u, pr, p.rk, c_root, tree, bk, bad);
         o.z = lut_flip(src.z, up.z, dn.z, sm.z, sd[2], e4, e8);
     }
     {
-        const uint32_t e4 = lut_bits32<V>(gl | 10u, pr, p.rk, c_root, tree, bk), e8 = lut_bits32<V>(gl | 14u, pr, p.rk, c_root, tree, bk);
+        const uint32_t e4 = lut_bits32<V>(gl | 10u, pr, p.rk, c_root, tree, bk, bad), e8 = lut_bits32<V>(gl | 14u, pr, p.rk, c_root, tree, bk, bad);
         o.w = lut_flip(src.w, up.w, dn.w, sm.w, sd[3], e4, e8);
     }
+    // one test per row keeps the 16 Philox calls and 128 bucket steps in one basic block; a number in
+    // a multi-threshold bucket (rare, see lut_bits32) redoes the row with the binary search
+    if (V == 0 && bad >= 256u) return lut_row_slow<P>(src, up, sm, dn, edge, g0, p, c_root, tree);
     return o;
+}
+
+template <int P>
+__device__ __noinline__ uint4 lut_row_slow(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
+                                           uint32_t edge, uint64_t g0, const LutParams &p, uint32_t c_root,
+                                           const uint32_t *tree)
+{
+    return lut_row<P, 1>(src, up, sm, dn, edge, g0, p, c_root, tree, nullptr);
 }
 
 template <int C, int V>
