@@ -290,12 +290,9 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
     const int np = ising ? 1 : 2;
     EncodeTiledFn enc = encode_tiled();
     if (!enc) return cudaErrorNotSupported;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    // per call: the attribute is per device, and a process may drive several devices
+    cudaError_t ea = cudaFuncSetAttribute(gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (ea != cudaSuccess) return ea;
     CUtensorMap tmap;
     const cuuint64_t gdim[2] = {(cuuint64_t)L, (cuuint64_t)L};
     const cuuint64_t gstride[1] = {(cuuint64_t)L};

@@ -236,12 +236,11 @@ cudaError_t launch_lut_update(ising_sim *h, int colour, uint32_t t)
     p.buckets = reinterpret_cast<const uint2 *>(h->lut_buckets);
     const size_t smem = 8 << LUT_BUCKET_BITS;
     if (h->variant == 0) {
-        static bool attr = false;
-        if (!attr) {
-            cudaFuncSetAttribute(lut_update_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            cudaFuncSetAttribute(lut_update_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            attr = true;
-        }
+        // per launch: the attribute is per device, and a process may drive several devices
+        cudaError_t ea = cudaFuncSetAttribute(lut_update_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (ea == cudaSuccess)
+            ea = cudaFuncSetAttribute(lut_update_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (ea != cudaSuccess) return ea;
         if (colour == 0) lut_update_kernel<0, 0><<<grid, block, smem, h->stream>>>(p);
         else lut_update_kernel<1, 0><<<grid, block, smem, h->stream>>>(p);
     } else {

@@ -381,6 +381,17 @@ def test_protocol_distance_lists_match_oracle(eng):
             assert (pn == np.where(ost == 1, L * L, (L // 16) ** 2)).all()
 
 
+def test_pipe_probe_rates_are_sane(eng):
+    """ising_bench_pipes (measurement helper behind the ALU roofline): rates are positive, no pipe
+    issues more than one warp-instruction per sub-partition per clock, the 16-lane pipes sit near
+    0.5 and a wide multiply is slower than a 32-bit one."""
+    r = eng.bench_pipes()
+    assert set(r) == set(eng.PIPE_PROBES)
+    assert all(0.05 < v < 1.1 for v in r.values()), r
+    assert 0.35 < r["LOP3"] < 0.6 and 0.35 < r["IMAD"] < 0.6
+    assert r["IMAD.WIDE"] < 0.8 * r["IMAD"]
+
+
 # --------------------------------------------------------- Schwinger-Dyson ---
 @pytest.mark.parametrize("model", [ISING, BC])
 def test_schwinger_dyson_histogram(eng, model):
