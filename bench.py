@@ -65,6 +65,7 @@ def parse_args():
     ap.add_argument("--rows-per-thread", type=int, default=0, help="update-kernel launch geometry (0 = library default)")
     ap.add_argument("--block", type=int, default=0, help="update-kernel threads per block (0 = library default)")
     ap.add_argument("--variant", type=int, default=0, help="update-kernel variant (0 = default carry form)")
+    ap.add_argument("--tally", action="store_true", help="A7: keep E, M by the fused tally of the update kernels instead of the observables pass")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
@@ -300,6 +301,8 @@ def run_ours(args):
         sim.set_launch(args.rows_per_thread, args.block)
     if args.variant:
         sim.set_variant(args.variant)
+    if args.tally:
+        sim.set_tally(True)
 
     def barrier():
         if dist is not None:
@@ -314,7 +317,7 @@ def run_ours(args):
             ev[1].record()
         if args.workload == "corr":
             sim.correlation_protocol()             # r <= 32 all sources + stride-16 sources up to L/2
-        return sim.observables()
+        return sim.tally() if args.tally else sim.observables()
 
     for _ in range(W):
         step()
@@ -400,7 +403,7 @@ def run_ours(args):
                    "seed": base.seed, "sweeps_per_step": S, "observables_every": S,
                    "step": "S sweeps + observables" if args.workload == "sweep" else "S sweeps + correlation protocol + observables",
                    "launch": {"rows_per_thread": args.rows_per_thread or "default", "block": args.block or "default",
-                              "variant": args.variant},
+                              "variant": args.variant, "fused_tally": bool(args.tally)},
                    "lattice_bytes": L * L // (8 if model == wl.ISING_LUT else 2), "l2": "inputs larger than L2 (no flush needed)" if L * L // 2 > (256 << 20)
                    else "lattice fits L2: DRAM figures not meaningful", "parallelism": f"replicas x{world}"},
         "measurement_ms_per_step": (total_ms - sweep_ms) / K,

@@ -83,6 +83,16 @@ int ising_sweep(ising_t *h, int64_t n);
  * arrays.  Synchronises.                                                    */
 int ising_observables(ising_t *h, ising_obs_t *out);
 
+/* Fused tally (optional, A7 of SURVEY.md Sec. 8(a)): on != 0 makes the update kernels keep
+ * running B, M, Q on the device -- the changes caused by every accepted move are added block
+ * by block -- starting from a full recompute made by this call (and again after every lattice
+ * write).  ising_tally returns the running values in the same struct as ising_observables
+ * (they must always agree: north_star's "incremental dE tally equals a full recompute of H")
+ * without a pass over the lattice.  Costs about 10 % of the update rate while on.
+ * ising_tally synchronises.                                                          */
+int ising_set_tally(ising_t *h, int on);
+int ising_tally(ising_t *h, ising_obs_t *out);
+
 /* Full-source pair sums: sx[r-1] = sum_{x,y} s(x,y) s(x+r,y),
  * sy[r-1] = sum_{x,y} s(x,y) s(x,y+r), periodic, r = 1..rmax, 1 <= rmax <= L/2.
  * Host arrays of length rmax.  Synchronises.                                */

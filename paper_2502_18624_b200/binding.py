@@ -17,7 +17,7 @@ EXPORTS = [
     "ising_workspace_bytes", "ising_create", "ising_sweep", "ising_observables", "ising_correlation",
     "ising_correlation_protocol", "ising_correlation_list", "ising_schwinger_dyson", "ising_read_lattice",
     "ising_read_window", "ising_write_lattice", "ising_read_packed", "ising_write_packed",
-    "ising_set_sweeps_done", "ising_thresholds", "ising_set_launch", "ising_set_variant", "ising_bench_pipes", "ising_set_corr_path",
+    "ising_set_sweeps_done", "ising_thresholds", "ising_set_launch", "ising_set_variant", "ising_bench_pipes", "ising_set_corr_path", "ising_set_tally", "ising_tally",
     "ising_launch_count", "ising_sync", "ising_destroy", "ising_last_error", "ising_bench_philox_only",
     "ising_bench_copy", "ising_debug_philox",
 ]
@@ -179,6 +179,16 @@ class IsingSim:
     def observables(self) -> Observables:
         o = _Obs()
         _check(self._lib.ising_observables(self._h, C.byref(o)))
+        return Observables(*(getattr(o, f[0]) for f in _Obs._fields_))
+
+    def set_tally(self, on: bool = True):
+        self._lib.ising_set_tally.argtypes = [C.c_void_p, C.c_int]
+        _check(self._lib.ising_set_tally(self._h, int(on)))
+
+    def tally(self) -> Observables:
+        o = _Obs()
+        self._lib.ising_tally.argtypes = [C.c_void_p, C.c_void_p]
+        _check(self._lib.ising_tally(self._h, C.byref(o)))
         return Observables(*(getattr(o, f[0]) for f in _Obs._fields_))
 
     def correlation(self, rmax: int):

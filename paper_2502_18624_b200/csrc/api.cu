@@ -309,6 +309,45 @@ extern "C" int ising_observables(ising_t *h, ising_obs_t *out)
     return ISING_OK;
 }
 
+// A7: fused tally.  d_acc[40..42] hold running B, M, Q; the update kernels add the changes.
+static int tally_resync(ising_sim *h)
+{
+    const bool lut = h->model == ISING_MODEL_ISING_LUT;
+    cudaError_t e = lut ? launch_lut_observables(h) : launch_observables(h);
+    if (e != cudaSuccess) return cuda_fail(e, "observables kernel");
+    CUDA_TRY(cudaMemcpyAsync(h->d_acc + 40, h->d_acc, 3 * sizeof(long long), cudaMemcpyDeviceToDevice, h->stream));
+    return ISING_OK;
+}
+
+extern "C" int ising_set_tally(ising_t *h, int on)
+{
+    if (!h) return set_error(ISING_EINVAL, "ising_set_tally: NULL handle");
+    h->tally_on = on != 0;
+    return h->tally_on ? tally_resync(h) : ISING_OK;
+}
+
+static void fill_obs(const ising_sim *h, const long long *bmq, ising_obs_t *o)
+{
+    const bool lut = h->model == ISING_MODEL_ISING_LUT;
+    o->bond_sum = bmq[0]; o->M = bmq[1]; o->Q = (lut || h->model == ISING_MODEL_ISING) ? h->L * h->L : bmq[2];
+    o->n_sites = h->L * h->L; o->sweeps_done = h->t;
+    const double N = (double)h->L * (double)h->L;
+    o->E = (h->model != ISING_MODEL_BLUME_CAPEL) ? -(double)o->bond_sum : -(double)o->bond_sum + h->D * (double)o->Q;
+    o->e_per_site = o->E / N;
+    o->m_per_site = (double)o->M / N;
+    o->zero_density = (double)(o->n_sites - o->Q) / N;
+}
+
+extern "C" int ising_tally(ising_t *h, ising_obs_t *out)
+{
+    if (!h || !out) return set_error(ISING_EINVAL, "ising_tally: NULL argument");
+    if (!h->tally_on) return set_error(ISING_EINVAL, "ising_tally: the tally is off (ising_set_tally)");
+    CUDA_TRY(cudaMemcpyAsync(h->h_acc + 40, h->d_acc + 40, 3 * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    fill_obs(h, h->h_acc + 40, out);
+    return ISING_OK;
+}
+
 extern "C" int ising_schwinger_dyson(ising_t *h, int64_t hist[9], double *value)
 {
     if (!h || !hist || !value) return set_error(ISING_EINVAL, "ising_schwinger_dyson: NULL argument");
@@ -395,7 +434,7 @@ extern "C" int ising_write_lattice(ising_t *h, int64_t y0, int64_t ny, const int
             if (e != cudaSuccess) return cuda_fail(e, "pack kernel");
             if (pass == 1) CUDA_TRY(cudaStreamSynchronize(h->stream));   // staging buffer is reused
         }
-    return ISING_OK;
+    return h->tally_on ? tally_resync(h) : ISING_OK;
 }
 
 extern "C" int ising_read_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, uint64_t *host_out)
@@ -415,7 +454,7 @@ extern "C" int ising_write_packed(ising_t *h, int colour, int64_t word0, int64_t
         return set_error(ISING_EINVAL, "ising_write_packed: range outside the colour array");
     CUDA_TRY(cudaMemcpyAsync(h->lat[colour] + word0, host_in, (size_t)nwords * 8, cudaMemcpyHostToDevice, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
-    return ISING_OK;
+    return h->tally_on ? tally_resync(h) : ISING_OK;
 }
 
 // ----------------------------------------------------------- correlation ---

@@ -37,6 +37,7 @@ struct ising_sim {
     uint64_t *comb = nullptr; size_t comb_bytes = 0;          // planes down-sampled to the source comb (stride >= 2)
     void *lut_buckets = nullptr;                              // LUT model: 4096 x {C, meta} bucket table (cudaMalloc)
     int8_t *gram = nullptr; size_t gram_bytes = 0;            // L x L int8 spin matrix for the tensor-core correlation
+    bool tally_on = false;                                    // A7: update kernels keep running B, M, Q at d_acc[40..42]
     int corr_path = 0;                                        // 0 auto, 1 bit planes (XOR + POPC), 2 tensor cores
     long long *d_corr = nullptr; size_t d_corr_bytes = 0;
     long long *d_rlist = nullptr; size_t d_rlist_bytes = 0;

@@ -18,6 +18,7 @@ struct LutParams {
     uint32_t colour, t;
     const uint32_t *tree;        // 16 carry constants in heap order (device): tree[n] = 2^32 - threshold(node n)
     const uint2 *buckets;        // 4096 entries indexed by the top 12 bits of the number (device), see lut_bits32
+    long long *tally;            // A7: running B, M (device), updated when the kernel is built with TALLY
     RoundKeys rk;
 };
 
@@ -151,9 +152,32 @@ __device__ __noinline__ uint4 lut_row_slow(const uint4 &src, const uint4 &up, co
     return lut_row<P, 1>(src, up, sm, dn, edge, g0, p, c_root, tree, nullptr);
 }
 
-template <int C, int V>
+// A7 (optional): change of B and M caused by one updated row, from old / new words and the neighbours.
+// A flipped site with d unequal neighbours changes B by 4 d - 8 and M by -2 sigma; d is counted bit-sliced.
+template <int P>
+__device__ __forceinline__ void lut_tally_row(const uint4 &x4, const uint4 &y4, const uint4 &up, const uint4 &sm, const uint4 &dn,
+                                              uint32_t edge, int &dB, int &dM)
+{
+    uint32_t sd[4];
+    lut_side<P>(sm, edge, sd);
+    const uint32_t xs[4] = {x4.x, x4.y, x4.z, x4.w}, ys[4] = {y4.x, y4.y, y4.z, y4.w};
+    const uint32_t us[4] = {up.x, up.y, up.z, up.w}, ds[4] = {dn.x, dn.y, dn.z, dn.w}, ms[4] = {sm.x, sm.y, sm.z, sm.w};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const uint32_t x = xs[k], F = x ^ ys[k];
+        const uint32_t a = us[k] ^ x, b = ds[k] ^ x, c = ms[k] ^ x, d = sd[k] ^ x;     // 1 where the neighbour differs
+        const uint32_t s0 = a ^ b, c0 = a & b, s1 = c ^ d, c1 = c & d;
+        const uint32_t b0 = s0 ^ s1, t = s0 & s1, b1 = c0 ^ c1 ^ t, b2 = c0 & c1;       // d = b0 + 2 b1 + 4 b2
+        const int cnt = __popc(F), cnt_up = __popc(F & x);
+        dB += 4 * (__popc(F & b0) + 2 * __popc(F & b1) + 4 * __popc(F & b2)) - 8 * cnt;
+        dM += 2 * cnt - 4 * cnt_up;
+    }
+}
+
+template <int C, int V, int TALLY>
 __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const __grid_constant__ LutParams p)
 {
+    int dB = 0, dM = 0;
     __shared__ uint32_t s_tree[16];
     extern __shared__ __align__(16) unsigned char s_buckets[];          // V = 0: 4096 x 8 bytes
     if (threadIdx.x < 16) s_tree[threadIdx.x] = p.tree[threadIdx.x];
@@ -202,6 +226,7 @@ __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const _
         uint32_t nedge = *reinterpret_cast<const uint32_t *>(eo);
         uint4 dn2 = *reinterpret_cast<const uint4 *>(o2);
         uint4 o = lut_row<C, V>(src, up, sm, dn, edge, g0, p, c_root, s_tree, s_buckets);
+        if (TALLY) lut_tally_row<C>(src, o, up, sm, dn, edge, dB, dM);
         *reinterpret_cast<uint4 *>(w0) = o;
         g0 += gs;
         uint4 nsrc2 = src;
@@ -212,10 +237,21 @@ __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const _
             nedge2 = *reinterpret_cast<const uint32_t *>(ee);
         }
         o = lut_row<1 - C, V>(nsrc, sm, dn, dn2, nedge, g0, p, c_root, s_tree, s_buckets);
+        if (TALLY) lut_tally_row<1 - C>(nsrc, o, sm, dn, dn2, nedge, dB, dM);
         *reinterpret_cast<uint4 *>(w0 + rs) = o;
         g0 += gs;
         up = dn; sm = dn2; src = nsrc2; edge = nedge2;
         o1 += 2 * rs; eo += 2 * rs; w0 += 2 * rs;
+    }
+    if (TALLY) {
+        const unsigned m = __activemask();
+        const int v[2] = {dB, dM};
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            const int sum = __reduce_add_sync(m, v[k]);
+            if ((int)(threadIdx.x & 31) == __ffs(m) - 1 && sum)
+                atomicAdd(reinterpret_cast<unsigned long long *>(&p.tally[k]), (unsigned long long)(long long)sum);
+        }
     }
 }
 
@@ -235,18 +271,22 @@ cudaError_t launch_lut_update(ising_sim *h, int colour, uint32_t t)
     unsigned grid = (unsigned)((threads + block - 1) / block);
     p.buckets = reinterpret_cast<const uint2 *>(h->lut_buckets);
     const size_t smem = 8 << LUT_BUCKET_BITS;
+    p.tally = h->d_acc + 40;
+#define LUT_LAUNCH(C, V, T, SM) lut_update_kernel<C, V, T><<<grid, block, SM, h->stream>>>(p)
     if (h->variant == 0) {
         // per launch: the attribute is per device, and a process may drive several devices
-        cudaError_t ea = cudaFuncSetAttribute(lut_update_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (ea == cudaSuccess)
-            ea = cudaFuncSetAttribute(lut_update_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t ea = cudaFuncSetAttribute(lut_update_kernel<0, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(lut_update_kernel<1, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(lut_update_kernel<0, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(lut_update_kernel<1, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (ea != cudaSuccess) return ea;
-        if (colour == 0) lut_update_kernel<0, 0><<<grid, block, smem, h->stream>>>(p);
-        else lut_update_kernel<1, 0><<<grid, block, smem, h->stream>>>(p);
+        if (h->tally_on) { if (colour == 0) LUT_LAUNCH(0, 0, 1, smem); else LUT_LAUNCH(1, 0, 1, smem); }
+        else { if (colour == 0) LUT_LAUNCH(0, 0, 0, smem); else LUT_LAUNCH(1, 0, 0, smem); }
     } else {
-        if (colour == 0) lut_update_kernel<0, 1><<<grid, block, 0, h->stream>>>(p);
-        else lut_update_kernel<1, 1><<<grid, block, 0, h->stream>>>(p);
+        if (h->tally_on) { if (colour == 0) LUT_LAUNCH(0, 1, 1, 0); else LUT_LAUNCH(1, 1, 1, 0); }
+        else { if (colour == 0) LUT_LAUNCH(0, 1, 0, 0); else LUT_LAUNCH(1, 1, 0, 0); }
     }
+#undef LUT_LAUNCH
     h->launches++;
     return cudaGetLastError();
 }

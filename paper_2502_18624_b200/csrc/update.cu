@@ -25,6 +25,7 @@ struct UpdParams {
     uint32_t C4, C8;            // carry form: [r >= T] = carry out of r + (2^32 - T); 0 when T is 0 or 2^32
     uint32_t Kc;                // (8 - number of thresholds that are 0) in every nibble
     const uint32_t *bc_table;   // Blume-Capel table (device)
+    long long *tally;           // A7: running B, M, Q (device), updated when the kernel is built with TALLY
     RoundKeys rk;
 };
 
@@ -271,10 +272,56 @@ __device__ __forceinline__ uint4 bc_row_carry(const uint4 &src, const uint4 &up,
     return o;
 }
 
+// ------------------------------------------------------------ fused tally ---
+// A7 (optional, ising_set_tally): changes of B, M, Q caused by one updated row, from the old
+// word x, the new word y and the neighbour words -- independent of the kernel variant.
+// Ising: a flipped site with d unequal neighbours changes B by 4 d - 8 and M by -2 sigma.
+// Blume-Capel: dB = (s' - s) h, dM = s' - s, dQ = s'^2 - s^2.
+__device__ __forceinline__ uint32_t nibble_sum32(uint32_t v)
+{
+    uint32_t t = (v & 0x0F0F0F0Fu) + ((v >> 4) & 0x0F0F0F0Fu);
+    return (t * 0x01010101u) >> 24;
+}
+
+template <int MODEL>
+__device__ __forceinline__ void tally_half(uint32_t x, uint32_t y, uint32_t up, uint32_t dn, uint32_t sm, uint32_t sd,
+                                           int &dB, int &dM, int &dQ)
+{
+    if (MODEL == ISING_MODEL_ISING) {
+        const uint32_t F = x ^ y;                                  // 1 in the nibbles that flipped
+        const uint32_t n = up + dn + sm + sd;
+        const uint32_t d = (n ^ (x * 7u)) - x * 3u;                // unequal neighbours before the flip
+        const int cnt = __popc(F), cnt_up = __popc(F & x);
+        dB += 4 * (int)nibble_sum32(d & (F * 15u)) - 8 * cnt;
+        dM += 2 * cnt - 4 * cnt_up;
+    } else {
+        const uint32_t S = up + dn + sm + sd;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int s0 = (int)((x >> (4 * j)) & 15u) - 1, s1 = (int)((y >> (4 * j)) & 15u) - 1;
+            const int h = (int)((S >> (4 * j)) & 15u) - 4;
+            dB += (s1 - s0) * h; dM += s1 - s0; dQ += s1 * s1 - s0 * s0;
+        }
+    }
+}
+
+template <int MODEL, int P>
+__device__ __forceinline__ void tally_row(const uint4 &x, const uint4 &y, const uint4 &up, const uint4 &sm, const uint4 &dn,
+                                          uint32_t edge, int &dB, int &dM, int &dQ)
+{
+    uint32_t sd[4];
+    side_words<P>(sm, edge, sd);
+    tally_half<MODEL>(x.x, y.x, up.x, dn.x, sm.x, sd[0], dB, dM, dQ);
+    tally_half<MODEL>(x.y, y.y, up.y, dn.y, sm.y, sd[1], dB, dM, dQ);
+    tally_half<MODEL>(x.z, y.z, up.z, dn.z, sm.z, sd[2], dB, dM, dQ);
+    tally_half<MODEL>(x.w, y.w, up.w, dn.w, sm.w, sd[3], dB, dM, dQ);
+}
+
 // ----------------------------------------------------------------- kernel ---
-template <int MODEL, int C, int V>
+template <int MODEL, int C, int V, int TALLY>
 __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ UpdParams p)
 {
+    int dB = 0, dM = 0, dQ = 0;                            // TALLY: this thread's share of the changes
     __shared__ __align__(16) uint32_t s_tab[80 + 132];   // both table forms (api.cu)
     uint64_t always = 0;
     if (MODEL == ISING_MODEL_BLUME_CAPEL) {
@@ -322,6 +369,7 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
         if (MODEL == ISING_MODEL_ISING) o = ising_row<C, V>(src, up, sm, dn, edge, g0, p.colour, p);
         else if (V == 0) o = bc_row_carry<C>(src, up, sm, dn, edge, g0, p.colour, p, ctab);
         else o = bc_row<C>(src, up, sm, dn, edge, g0, p.colour, p, s_tab, always);
+        if (TALLY) tally_row<MODEL, C>(src, o, up, sm, dn, edge, dB, dM, dQ);
         *reinterpret_cast<uint4 *>(w0) = o;
         g0 += gs;
         // ---- odd offset: parity 1 - C.  Prefetch the next even row first.
@@ -335,10 +383,21 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
         if (MODEL == ISING_MODEL_ISING) o = ising_row<1 - C, V>(nsrc, sm, dn, dn2, nedge, g0, p.colour, p);
         else if (V == 0) o = bc_row_carry<1 - C>(nsrc, sm, dn, dn2, nedge, g0, p.colour, p, ctab);
         else o = bc_row<1 - C>(nsrc, sm, dn, dn2, nedge, g0, p.colour, p, s_tab, always);
+        if (TALLY) tally_row<MODEL, 1 - C>(nsrc, o, sm, dn, dn2, nedge, dB, dM, dQ);
         *reinterpret_cast<uint4 *>(w0 + rs) = o;
         g0 += gs;
         up = dn; sm = dn2; src = nsrc2; edge = nedge2;
         o1 += 2 * rs; eo += 2 * rs; w0 += 2 * rs;
+    }
+    if (TALLY) {            // warp sums fit 32 bits (<= 32 lanes x R rows x 32 sites x 8); threads past the lattice have returned
+        const unsigned m = __activemask();
+        const int v[3] = {dB, dM, dQ};
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const int sum = __reduce_add_sync(m, v[k]);
+            if ((int)(threadIdx.x & 31) == __ffs(m) - 1 && sum)
+                atomicAdd(reinterpret_cast<unsigned long long *>(&p.tally[k]), (unsigned long long)(long long)sum);
+        }
     }
 }
 
@@ -363,25 +422,19 @@ cudaError_t launch_update(ising_sim *h, int colour, uint32_t t)
     int64_t threads = chunks * p.cols;
     int block = h->block_threads;
     unsigned grid = (unsigned)((threads + block - 1) / block);
-    if (h->model == ISING_MODEL_ISING) {
-        if (h->variant == 0) {
-            if (colour == 0) update_kernel<ISING_MODEL_ISING, 0, 0><<<grid, block, 0, h->stream>>>(p);
-            else update_kernel<ISING_MODEL_ISING, 1, 0><<<grid, block, 0, h->stream>>>(p);
-        } else {
-            if (colour == 0) update_kernel<ISING_MODEL_ISING, 0, 1><<<grid, block, 0, h->stream>>>(p);
-            else update_kernel<ISING_MODEL_ISING, 1, 1><<<grid, block, 0, h->stream>>>(p);
-        }
-    } else {
-        bool never = false;                       // a threshold that is exactly 0
+    p.tally = h->d_acc + 40;
+    bool never = false;                           // Blume-Capel: a threshold that is exactly 0 -> compare/select form
+    if (h->model == ISING_MODEL_BLUME_CAPEL)
         for (int i = 0; i < h->n_T; ++i) never = never || h->T[i] == 0;
-        if (h->variant == 0 && !never) {
-            if (colour == 0) update_kernel<ISING_MODEL_BLUME_CAPEL, 0, 0><<<grid, block, 0, h->stream>>>(p);
-            else update_kernel<ISING_MODEL_BLUME_CAPEL, 1, 0><<<grid, block, 0, h->stream>>>(p);
-        } else {
-            if (colour == 0) update_kernel<ISING_MODEL_BLUME_CAPEL, 0, 1><<<grid, block, 0, h->stream>>>(p);
-            else update_kernel<ISING_MODEL_BLUME_CAPEL, 1, 1><<<grid, block, 0, h->stream>>>(p);
-        }
-    }
+    const int v = (h->variant == 0 && !never) ? 0 : 1;
+#define LAUNCH_UPD(MODEL, C, V, T) update_kernel<MODEL, C, V, T><<<grid, block, 0, h->stream>>>(p)
+#define PICK_T(MODEL, C, V) do { if (h->tally_on) LAUNCH_UPD(MODEL, C, V, 1); else LAUNCH_UPD(MODEL, C, V, 0); } while (0)
+#define PICK_V(MODEL, C) do { if (v == 0) PICK_T(MODEL, C, 0); else PICK_T(MODEL, C, 1); } while (0)
+    if (h->model == ISING_MODEL_ISING) { if (colour == 0) PICK_V(ISING_MODEL_ISING, 0); else PICK_V(ISING_MODEL_ISING, 1); }
+    else { if (colour == 0) PICK_V(ISING_MODEL_BLUME_CAPEL, 0); else PICK_V(ISING_MODEL_BLUME_CAPEL, 1); }
+#undef PICK_V
+#undef PICK_T
+#undef LAUNCH_UPD
     h->launches++;
     return cudaGetLastError();
 }

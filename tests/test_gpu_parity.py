@@ -381,6 +381,42 @@ def test_protocol_distance_lists_match_oracle(eng):
             assert (pn == np.where(ost == 1, L * L, (L // 16) ** 2)).all()
 
 
+@pytest.mark.parametrize("model,L,beta,D", [(ISING, 256, wl.BETA_C, 0.0), (ISING, 1088, wl.BETA_C / 0.5, 0.0), (BC, 320, 1 / 1.4, 1.0),
+                                            (BC, 192, 12.0, 0.5), (wl.ISING_LUT, 512, wl.BETA_C / 0.9, 0.0)])
+def test_fused_tally_equals_recompute_and_oracle(eng, model, L, beta, D):
+    """A7 / north_star: the incremental tally kept by the update kernels equals a full recompute of
+    B, M, Q after every sweep, and the oracle's own incremental tally."""
+    seed = 17
+    if model == wl.ISING_LUT:
+        s = oracle.lut_init(L, seed)
+        osweep = lambda t, tl: oracle.lut_sweep(s, beta, seed, t, tl)
+    else:
+        s = oracle.init(model, L, seed)
+        osweep = lambda t, tl: oracle.sweep(model, s, beta, D, seed, t, tl)
+    tl = oracle.observables(s)
+    with eng.IsingSim(model, L, beta, D, seed) as sim:
+        with pytest.raises(eng.IsingError):
+            sim.tally()                                      # off by default
+        sim.set_tally(True)
+        a = sim.tally()
+        assert (a.bond_sum, a.M, a.Q) == tl
+        for t in range(6):
+            sim.sweep(1)
+            tl = osweep(t, tl)
+            a, b = sim.tally(), sim.observables()
+            assert (a.bond_sum, a.M, a.Q) == tl == (b.bond_sum, b.M, b.Q), t
+            assert a.E == b.E and a.m_per_site == b.m_per_site and a.sweeps_done == t + 1
+        assert (sim.read_lattice() == s).all()               # the tally kernels give the same trajectory
+        ones = np.ones((L, L), dtype=np.int8)
+        sim.write_lattice(ones)                              # a lattice write re-synchronises the tally
+        a = sim.tally()
+        assert (a.bond_sum, a.M) == (2 * L * L, L * L)
+        sim.set_tally(False)
+        sim.sweep(1)
+        with pytest.raises(eng.IsingError):
+            sim.tally()
+
+
 def test_pipe_probe_rates_are_sane(eng):
     """ising_bench_pipes (measurement helper behind the ALU roofline): rates are positive, no pipe
     issues more than one warp-instruction per sub-partition per clock, the 16-lane pipes sit near
