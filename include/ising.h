@@ -136,6 +136,15 @@ int ising_write_lattice(ising_t *h, int64_t y0, int64_t ny, const int8_t *host_i
  * c (row-major L x L/32).  For checkpoints and the end-to-end benchmark.    */
 int ising_read_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, uint64_t *host_out);
 int ising_write_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, const uint64_t *host_in);
+/* Schedule interleave (A11 of SURVEY.md Sec. 8(a)).  ising_time_grid: the paper's measurement
+ * times t = floor(2^(x/8) + 0.5), x = 1, 2, ..., de-duplicated, t <= tmax, into the
+ * host array out (capacity cap); *count = number of times (also when cap is too small, with
+ * ISING_EINVAL).  ising_run_schedule: sweeps to each time of the ascending host array times
+ * (all >= sweeps_done) and records the integer observables there in out[i] (by the fused tally
+ * if it is on, else by the observables pass).  Synchronises at every measurement.        */
+int ising_time_grid(uint64_t tmax, uint64_t *out, int64_t cap, int64_t *count);
+int ising_run_schedule(ising_t *h, int64_t n_times, const uint64_t *times, ising_obs_t *out);
+
 /* Set the sweep counter t (exact resume: state = lattice + t).               */
 int ising_set_sweeps_done(ising_t *h, uint64_t t);
 

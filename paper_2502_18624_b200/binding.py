@@ -17,7 +17,7 @@ EXPORTS = [
     "ising_workspace_bytes", "ising_create", "ising_sweep", "ising_observables", "ising_correlation",
     "ising_correlation_protocol", "ising_correlation_list", "ising_schwinger_dyson", "ising_read_lattice",
     "ising_read_window", "ising_write_lattice", "ising_read_packed", "ising_write_packed",
-    "ising_set_sweeps_done", "ising_thresholds", "ising_set_launch", "ising_set_variant", "ising_bench_pipes", "ising_set_corr_path", "ising_set_tally", "ising_tally",
+    "ising_set_sweeps_done", "ising_thresholds", "ising_set_launch", "ising_set_variant", "ising_bench_pipes", "ising_set_corr_path", "ising_set_tally", "ising_tally", "ising_time_grid", "ising_run_schedule",
     "ising_launch_count", "ising_sync", "ising_destroy", "ising_last_error", "ising_bench_philox_only",
     "ising_bench_copy", "ising_debug_philox",
 ]
@@ -115,6 +115,17 @@ def bench_pipes(sm_mhz: float = 0.0) -> dict:
     return {k: float(v) for k, v in zip(PIPE_PROBES, rates)}
 
 
+def time_grid(tmax: int) -> np.ndarray:
+    """The paper's measurement times up to tmax."""
+    lib = load_library()
+    lib.ising_time_grid.argtypes = [C.c_uint64, C.c_void_p, C.c_int64, C.c_void_p]
+    n = C.c_int64(0)
+    lib.ising_time_grid(int(tmax), None, 0, C.addressof(n))
+    out = np.zeros(n.value, dtype=np.uint64)
+    _check(lib.ising_time_grid(int(tmax), out.ctypes.data, len(out), C.addressof(n)))
+    return out
+
+
 def debug_philox(ctr: np.ndarray, key: np.ndarray, with_curand: bool = False) -> np.ndarray:
     ctr = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
     key = np.ascontiguousarray(key, dtype=np.uint32).reshape(-1, 2)
@@ -190,6 +201,14 @@ class IsingSim:
         self._lib.ising_tally.argtypes = [C.c_void_p, C.c_void_p]
         _check(self._lib.ising_tally(self._h, C.byref(o)))
         return Observables(*(getattr(o, f[0]) for f in _Obs._fields_))
+
+    def run_schedule(self, times):
+        """Sweep to every time of the ascending list and record the observables there (one native call)."""
+        times = np.ascontiguousarray(times, dtype=np.uint64)
+        arr = (_Obs * len(times))()
+        self._lib.ising_run_schedule.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+        _check(self._lib.ising_run_schedule(self._h, len(times), times.ctypes.data, C.addressof(arr)))
+        return [Observables(*(getattr(o, f[0]) for f in _Obs._fields_)) for o in arr]
 
     def correlation(self, rmax: int):
         sx = np.zeros(rmax, dtype=np.int64)

@@ -260,6 +260,44 @@ extern "C" int ising_sweep(ising_t *h, int64_t n)
     return ISING_OK;
 }
 
+// A11: measurement times of the paper, t = floor(2^(x/8) + 0.5), x = 1, 2, ..., de-duplicated
+extern "C" int ising_time_grid(uint64_t tmax, uint64_t *out, int64_t cap, int64_t *count)
+{
+    if (!count) return set_error(ISING_EINVAL, "ising_time_grid: count is NULL");
+    int64_t n = 0;
+    uint64_t last = 0;
+    for (int x = 1; x < 8 * 64; ++x) {
+        const double v = floor(exp2((double)x / 8.0) + 0.5);
+        if (v > (double)tmax) break;
+        const uint64_t t = (uint64_t)v;
+        if (t == last) continue;
+        if (out && n < cap) out[n] = t;
+        ++n; last = t;
+    }
+    *count = n;
+    if (!out || cap < n) return set_error(ISING_EINVAL, "ising_time_grid: cap too small");
+    return ISING_OK;
+}
+
+// A11: sweep to every time of an ascending schedule and record B, M, Q there (fused tally if it is on,
+// else the observables pass).  One call for "E and M every k sweeps" (BASELINE.json configs 1-3).
+extern "C" int ising_run_schedule(ising_t *h, int64_t n_times, const uint64_t *times, ising_obs_t *out)
+{
+    if (!h || !times || !out || n_times < 0) return set_error(ISING_EINVAL, "ising_run_schedule: bad argument");
+    uint64_t prev = h->t;
+    for (int64_t i = 0; i < n_times; ++i) {
+        if (times[i] < prev) return set_error(ISING_EINVAL, "ising_run_schedule: times must be ascending and >= sweeps_done");
+        prev = times[i];
+    }
+    for (int64_t i = 0; i < n_times; ++i) {
+        int rc = ising_sweep(h, (int64_t)(times[i] - h->t));
+        if (rc) return rc;
+        rc = h->tally_on ? ising_tally(h, &out[i]) : ising_observables(h, &out[i]);
+        if (rc) return rc;
+    }
+    return ISING_OK;
+}
+
 extern "C" int ising_set_sweeps_done(ising_t *h, uint64_t t)
 {
     if (!h) return set_error(ISING_EINVAL, "ising_set_sweeps_done: NULL handle");

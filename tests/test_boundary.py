@@ -71,3 +71,18 @@ def test_product_does_not_import_oracle():
                 assert "import oracle" not in txt and "from oracle" not in txt and "ising_oracle" not in txt, f
     orc = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "ising_oracle.c")).read()
     assert "import paper_2502_18624_b200" not in orc and "ising.h" not in orc
+
+
+def test_time_grid_host_logic_matches_oracle(lib):
+    """A11 host logic through the C ABI (no GPU needed): the paper's measurement times."""
+    import ctypes as C
+    import numpy as np
+    import oracle
+    lib.ising_time_grid.argtypes = [C.c_uint64, C.c_void_p, C.c_int64, C.c_void_p]
+    for tmax in (1, 12, 2000, 524288):
+        n = C.c_int64(0)
+        assert lib.ising_time_grid(tmax, None, 0, C.addressof(n)) != 0          # cap too small, count still written
+        out = np.zeros(n.value, dtype=np.uint64)
+        assert lib.ising_time_grid(tmax, out.ctypes.data, len(out), C.addressof(n)) == 0
+        assert (out == oracle.time_grid(tmax)).all()
+    assert n.value > 100 and out[-1] == 524288

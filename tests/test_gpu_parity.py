@@ -417,6 +417,30 @@ def test_fused_tally_equals_recompute_and_oracle(eng, model, L, beta, D):
             sim.tally()
 
 
+def test_run_schedule_matches_stepwise_run(eng):
+    """A11: one native call over the paper's time grid gives the same observables as sweeping step by step
+    (and as the oracle), with and without the fused tally."""
+    L, beta, seed = 256, wl.BETA_C / 0.5, 4
+    times = eng.time_grid(40)
+    assert (times == oracle.time_grid(40)).all()
+    s = oracle.init(ISING, L, seed)
+    tl = oracle.observables(s)
+    want, t = [], 0
+    for tt in times:
+        while t < tt:
+            tl = oracle.sweep(ISING, s, beta, 0.0, seed, t, tl)
+            t += 1
+        want.append(tl)
+    for tally in (False, True):
+        with eng.IsingSim(ISING, L, beta, 0.0, seed) as sim:
+            sim.set_tally(tally)
+            got = sim.run_schedule(times)
+            assert [(o.bond_sum, o.M, o.Q) for o in got] == want
+            assert [o.sweeps_done for o in got] == [int(x) for x in times]
+            with pytest.raises(eng.IsingError):
+                sim.run_schedule([3])                        # earlier than sweeps_done
+
+
 def test_pipe_probe_rates_are_sane(eng):
     """ising_bench_pipes (measurement helper behind the ALU roofline): rates are positive, no pipe
     issues more than one warp-instruction per sub-partition per clock, the 16-lane pipes sit near
