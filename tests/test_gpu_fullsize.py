@@ -90,6 +90,12 @@ def test_config2_ising_L2p18_windows_and_observables(eng):
         assert o.M == M
         sx, sy = sim.correlation_list(1, [1, 2])                   # independent kernels (bit planes)
         assert int(sx[0]) + int(sy[0]) == o.bond_sum               # S_x(1) + S_y(1) = B
+        sim.set_corr_path(2)                                       # tensor cores at L = 2^18 (69 GB int8 matrix)
+        tx, ty = sim.correlation(1024)
+        sim.set_corr_path(1)                                       # XOR + POPC kernels
+        bx, by = sim.correlation(1024)
+        assert (tx == bx).all() and (ty == by).all()
+        assert int(tx[0]) + int(ty[0]) == o.bond_sum and (int(tx[1]), int(ty[1])) == (int(sx[1]), int(sy[1]))
         assert o.E == -float(o.bond_sum) and o.e_per_site == o.E / float(L * L)
         assert o.m_per_site == float(o.M) / float(L * L)
 
