@@ -50,6 +50,13 @@ def test_null_handle_errors(lib):
     assert lib.ising_create(0, 100, 0.4, 0.0, 1, None, 0, None, C.byref(out)) == -1      # bad L, before any CUDA call
     assert lib.ising_create(0, 64, -1.0, 0.0, 1, None, 0, None, C.byref(out)) == -1
     assert lib.ising_create(0, 64, 0.4, 0.0, 1, None, 0, None, None) == -1
+    assert lib.ising_create(2, 192, 0.4, 0.0, 1, None, 0, None, C.byref(out)) == -1      # LUT model: L % 256
+    for fn, args in [(lib.ising_set_tally, (None, 1)), (lib.ising_tally, (None, None)), (lib.ising_set_corr_path, (None, 1)),
+                     (lib.ising_run_schedule, (None, 0, None, None)), (lib.ising_correlation, (None, 1, None, None)),
+                     (lib.ising_set_variant, (None, 0)), (lib.ising_set_launch, (None, 0, 0)),
+                     (lib.ising_time_grid, (10, None, 0, None))]:
+        assert fn(*args) == -1, fn.__name__
+        assert len(lib.ising_last_error()) > 0
 
 
 def test_no_cpu_fallback():
