@@ -410,7 +410,8 @@ def run_ours(args):
         "sweep_only_updates_per_ns": world * L * L * S * K / (sweep_ms * 1e6),
         "roofline": alu_roof,
         "roofline_hbm": {"bound": "hbm", "kernel": "update_kernel (one colour phase)", "achieved": achieved,
-                         "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+                         "peak": peak, "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8000_gbs": achieved / 8000.0,
+                         "traffic": traffic,
                          "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_per_site * sites_per_launch,
                          "avg_launch_ms": kern_ms,
                          "copy_kernel_gbs": bytes_per_site * sites_per_launch / (copy_ms * 1e-3) / 1e9 if copy_ms else None},
