@@ -597,16 +597,16 @@ extern "C" int ising_correlation(ising_t *h, int64_t rmax, int64_t *sx, int64_t 
     cudaError_t e = launch_planes(h);
     if (e != cudaSuccess) return cuda_fail(e, "bit-plane kernels");
     // tensor cores pay off once the band is wide; narrow bands stay on the bit planes
-    const bool tensor = h->corr_path == 2 || (h->corr_path == 0 && rmax >= 512);
+    const bool tensor = h->corr_path >= 2 || (h->corr_path == 0 && rmax >= 512);
     if (tensor && corr_gram_supported(h, rmax)) return run_corr_gram(h, rmax, sx, sy);
-    if (h->corr_path == 2) return set_error(ISING_EINVAL, "ising_correlation: tensor-core path needs L % 256 == 0 and L >= 512");
+    if (h->corr_path >= 2) return set_error(ISING_EINVAL, "ising_correlation: tensor-core path needs L % 256 == 0 and L >= 512");
     return run_corr(h, 0, rmax, nullptr, sx, sy);
 }
 
 extern "C" int ising_set_corr_path(ising_t *h, int path)
 {
     if (!h) return set_error(ISING_EINVAL, "ising_set_corr_path: NULL handle");
-    if (path < 0 || path > 2) return set_error(ISING_EINVAL, "ising_set_corr_path: path must be 0 (auto), 1 (bit planes) or 2 (tensor cores)");
+    if (path < 0 || path > 3) return set_error(ISING_EINVAL, "ising_set_corr_path: path must be 0 (auto), 1 (bit planes), 2 (tensor cores) or 3 (tensor cores, CTA pairs)");
     h->corr_path = path;
     return ISING_OK;
 }

@@ -228,6 +228,184 @@ __global__ void __launch_bounds__(192, 1) gram_kernel(const __grid_constant__ CU
     if (warp == 2) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
 }
 
+// ------------------------------------------------ CTA-pair variant (opt-in) ---
+// cta_group::2: two CTAs of a cluster (one TPC) share one 256 x 256 tile.  Each CTA loads its own
+// 128 rows of A and 128 of the 256 B rows (32 KB per stage instead of 48 KB: a third less L2 -> SM
+// traffic, 6 stages), the leader CTA issues tcgen05.mma.cta_group::2 (M = 256), and each CTA's
+// TMEM receives the accumulator rows of its own A half, which its epilogue warps bin as before.
+namespace {
+constexpr int STAGES2 = 6, HALF_BYTES = TM * TKB, STAGE2_BYTES = 2 * HALF_BYTES;
+constexpr int SMEM2_BYTES = STAGES2 * STAGE2_BYTES + 1024 + 2048;
+constexpr uint32_t kInstrDesc2 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(256 >> 3) << 17) | ((uint32_t)(256 >> 4) << 24);
+
+__device__ __forceinline__ uint32_t cluster_rank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_remote(uint64_t *bar, uint32_t cta)
+{
+    asm volatile("{\n\t.reg .b32 ra;\n\tmapa.shared::cluster.u32 ra, %0, %1;\n\tmbarrier.arrive.shared::cluster.b64 _, [ra];\n\t}"
+                 ::"r"(smem_u32(bar)), "r"(cta) : "memory");
+}
+// 2-SM TMA load: the transaction bytes are counted on the LEADER CTA's barrier (peer bit cleared)
+__device__ __forceinline__ void tma_load_2d_2sm(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar) & 0xFEFFFFFFu), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void umma_i8_2sm(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::i8 [%0], %1, %2, %3, {%5, %5, %5, %5, %5, %5, %5, %5}, p;\n\t}"
+        ::"r"(tmem_d), "l"(da), "l"(db), "r"(kInstrDesc2), "r"(accumulate), "r"(0u) : "memory");
+}
+__device__ __forceinline__ void umma_commit_2sm(uint64_t *bar)      // arrives on the barrier at this offset in BOTH CTAs
+{
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(smem_u32(bar)), "h"((uint16_t)3) : "memory");
+}
+}  // namespace
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1)
+gram2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ GramParams p)
+{
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    uint8_t *tail = smem + STAGES2 * STAGE2_BYTES;
+    int *bins = reinterpret_cast<int *>(tail);
+    uint64_t *full = reinterpret_cast<uint64_t *>(tail + 1536);             // [STAGES2]  (used on the leader)
+    uint64_t *empty = full + STAGES2;                                       // [STAGES2]  (both CTAs)
+    uint64_t *tfull = empty + STAGES2;                                      // [2]        (both CTAs)
+    uint64_t *tempty = tfull + 2;                                           // [2]        (used on the leader)
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + 2);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_rank();
+    const bool leader = rank == 0;
+    const int n_kb = p.n_kb;
+    // tiles of 256 rows: p.n_ib row blocks; a contiguous run per CLUSTER, column-tile-major
+    const long long n_tiles = (long long)p.n_ib * p.n_jk;
+    const int n_cl = gridDim.x >> 1, cl = blockIdx.x >> 1;
+    const int t_lo = (int)(n_tiles * cl / n_cl), t_hi = (int)(n_tiles * (cl + 1) / n_cl);
+
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < STAGES2; ++s) { mbar_init(&full[s], 2); mbar_init(&empty[s], 1); }
+        for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], 8); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int i = threadIdx.x; i < NBINS; i += blockDim.x) bins[i] = 0;
+    cluster_sync_all();                                                      // barriers of both CTAs exist
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    cluster_sync_all();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (warp == 0) {
+        // ===== TMA producer (both CTAs): own A half, own half of the B rows =====
+        if (lane == 0) {
+            int stage = 0; uint32_t phase = 0;
+            for (int t = t_lo; t < t_hi; ++t) {
+                const int jk = t / p.n_ib, ib = t - jk * p.n_ib;
+                const int I0 = ib * 256 + (int)rank * TM;
+                int J0 = ib * 256 + jk * TN; if (J0 >= p.L) J0 -= p.L;      // multiple of 256: the tile never wraps
+                J0 += (int)rank * TM;
+                for (int kb = 0; kb < n_kb; ++kb) {
+                    mbar_wait(&empty[stage], phase ^ 1);
+                    if (leader) mbar_expect_tx(&full[stage], 2 * STAGE2_BYTES);   // bytes of both CTAs land on this barrier
+                    uint8_t *sa = smem + stage * STAGE2_BYTES, *sb = sa + HALF_BYTES;
+                    tma_load_2d_2sm(sa, &tmap, &full[stage], p.k0 + kb * TKB, I0);
+                    tma_load_2d_2sm(sb, &tmap, &full[stage], p.k0 + kb * TKB, J0);
+                    if (!leader) mbar_arrive_remote(&full[stage], 0);
+                    if (++stage == STAGES2) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer: leader CTA only =====
+        if (leader && lane == 0) {
+            int stage = 0; uint32_t phase = 0;
+            int as = 0; uint32_t aphase = 0;
+            for (int t = t_lo; t < t_hi; ++t) {
+                mbar_wait(&tempty[as], aphase ^ 1);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t d_tmem = tmem_base + (uint32_t)(as * TN);
+                for (int kb = 0; kb < n_kb; ++kb) {
+                    mbar_wait(&full[stage], phase);
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    const uint32_t sa = smem_u32(smem + stage * STAGE2_BYTES), sb = sa + HALF_BYTES;
+                    const uint64_t da = umma_desc(sa), db = umma_desc(sb);
+#pragma unroll
+                    for (int k = 0; k < TKB / 32; ++k)
+                        umma_i8_2sm(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), (kb | k) ? 1u : 0u);
+                    umma_commit_2sm(&empty[stage]);
+                    if (++stage == STAGES2) { stage = 0; phase ^= 1; }
+                }
+                umma_commit_2sm(&tfull[as]);
+                if (++as == 2) { as = 0; aphase ^= 1; }
+            }
+        }
+    } else {
+        // ===== epilogue (both CTAs): rows I0 + 128 rank + i of the pair tile =====
+        const int q = warp & 3, row = q * 32 + lane;
+        const int et = threadIdx.x - 64;
+        int as = 0; uint32_t aphase = 0;
+        for (int t = t_lo; t < t_hi; ++t) {
+            const int jk = t / p.n_ib;
+            mbar_wait(&tfull[as], aphase);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * TN);
+#pragma unroll 1
+            for (int c = 0; c < TN / 32; ++c) {
+                uint32_t v[32];
+                asm volatile(
+                    "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                    "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+                    "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+                    : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                      "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+                      "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+                      "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+                    : "r"(taddr + (uint32_t)(c * 32)));
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                const uint32_t b0 = smem_u32(bins) + 4u * (uint32_t)((TM - 1) + 32 * c - row);
+#pragma unroll
+                for (int k = 0; k < 32; ++k)
+                    asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(b0 + 4u * k), "r"(v[k]) : "memory");
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) { if (leader) mbar_arrive(&tempty[as]); else mbar_arrive_remote(&tempty[as], 0); }
+            if (++as == 2) { as = 0; aphase ^= 1; }
+            if (t + 1 < t_hi && (t + 1) / p.n_ib == jk) continue;
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            for (int b = et; b < NBINS; b += 128) {
+                const int r = jk * TN - (int)rank * TM + b - (TM - 1);
+                const int v = bins[b];
+                bins[b] = 0;
+                if (r >= 1 && r <= p.rmax && v != 0)
+                    atomicAdd(reinterpret_cast<unsigned long long *>(&p.out[r - 1]), (unsigned long long)(long long)v);
+            }
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    cluster_sync_all();                                                      // the peer may still be read by MMAs / arrive remotely
+    if (warp == 2) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+}
+
 // ------------------------------------------------- planes -> int8 matrix ---
 // out[y][64 q + i] = nz bit ? (sg bit ? +1 : -1) : 0   (Ising: nz == nullptr, every site non-zero)
 __global__ void __launch_bounds__(256) expand_kernel(const uint64_t *__restrict__ sg, const uint64_t *__restrict__ nz,
@@ -312,8 +490,16 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
     if (kc < 4 * TKB) kc = 4 * TKB;
     if (kc > L) kc = L;
     p.n_kb = kc / TKB;
+    const bool pair = h->corr_path == 3;              // opt-in: cta_group::2 kernel, 256-row tiles
+    if (pair) {
+        ea = cudaFuncSetAttribute(gram2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM2_BYTES);
+        if (ea != cudaSuccess) return ea;
+        p.n_ib = L / 256;
+        p.n_jk = (int)((count + 256 + TN - 1) / TN);      // columns I0 .. I0 + 255 + rmax
+    }
     const int n_tiles = p.n_ib * p.n_jk;
-    const int grid = n_tiles < n_sm ? n_tiles : n_sm;
+    int grid = n_tiles < n_sm ? n_tiles : n_sm;
+    if (pair) { grid = 2 * (n_tiles < n_sm / 2 ? n_tiles : n_sm / 2); }
     for (int axis = 0; axis < 2; ++axis) {              // 0: S_y from the planes, 1: S_x from the transposed planes
         const uint64_t *sg = h->planes + (axis ? np * pw : 0);
         const uint64_t *nz = ising ? nullptr : sg + pw;
@@ -326,7 +512,8 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
         for (int k0 = 0; k0 < L; k0 += kc) {
             p.k0 = k0;
             p.n_kb = (L - k0 < kc ? L - k0 : kc) / TKB;
-            gram_kernel<<<grid, 192, SMEM_BYTES, h->stream>>>(tmap, p);
+            if (pair) gram2_kernel<<<grid, 192, SMEM2_BYTES, h->stream>>>(tmap, p);
+            else gram_kernel<<<grid, 192, SMEM_BYTES, h->stream>>>(tmap, p);
             h->launches++;
         }
         e = cudaGetLastError();
