@@ -485,12 +485,13 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
     GramParams p;
     p.L = L; p.rmax = (int)count; p.n_ib = L / TM;
     p.n_jk = (int)((count + TM + TN - 1) / TN);          // columns I0 .. I0 + 127 + rmax
-    // K chunk: keep the L x kc slab within about half of the 126 MB L2
+    // K chunk: keep the L x kc slab within about half of the 126 MB L2 (measured at L = 2^16: 1024 bytes
+    // is the optimum for both kernels; 512 pays more epilogues, 2048 falls out of L2)
     int kc = (int)(((64ll << 20) / L) / TKB * TKB);
     if (kc < 4 * TKB) kc = 4 * TKB;
     if (kc > L) kc = L;
     p.n_kb = kc / TKB;
-    const bool pair = h->corr_path == 3;              // opt-in: cta_group::2 kernel, 256-row tiles
+    const bool pair = h->corr_path != 2;              // default: cta_group::2 kernel, 256-row tiles; path 2 = single-CTA kernel
     if (pair) {
         ea = cudaFuncSetAttribute(gram2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM2_BYTES);
         if (ea != cudaSuccess) return ea;

@@ -329,7 +329,10 @@ def test_correlation_tensor_core_path(eng, model, L):
         lat = sim.read_lattice()
         ox, oy = oracle.correlation(lat, L // 2)
         for rmax in (L // 2, L // 2 - 37, 129, 1):
-            sim.set_corr_path(2)
+            sim.set_corr_path(3)                             # CTA-pair kernel (cta_group::2), the automatic choice
+            px, py = sim.correlation(rmax)
+            assert (px == ox[:rmax]).all() and (py == oy[:rmax]).all(), rmax
+            sim.set_corr_path(2)                             # single-CTA kernel
             tx, ty = sim.correlation(rmax)
             assert (tx == ox[:rmax]).all() and (ty == oy[:rmax]).all(), rmax
             sim.set_corr_path(1)
