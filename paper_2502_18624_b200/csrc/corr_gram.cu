@@ -11,6 +11,8 @@
 // element added to the shared-memory bin of its diagonal j - i, bins flushed to the int64
 // result with one atomic per distance per tile).  Tile (I0, J0 = I0 + 256 k) holds the ordered
 // pairs (y = I0 + i, y + r = J0 + j): r = J0 - I0 + j - i, kept when 1 <= r <= rmax.
+// The default is the CTA-pair variant further down (gram2_kernel: cta_group::2, 256 x 256 tiles);
+// this single-CTA kernel stays selectable (ising_set_corr_path(h, 2)) and is tested against it.
 #include "ising_internal.cuh"
 
 #include <cuda.h>
