@@ -205,3 +205,24 @@ def test_config4_ising_L2p16_correlation_protocol(eng):
                 assert (sx[sel] == bx).all() and (sy[sel] == by).all()
                 del lat
         assert done == 64
+
+
+# ------------------------------------------------------------ maximum sizes ---
+@pytest.mark.parametrize("model,L,beta,D", [(wl.ISING_LUT, 1 << 20, wl.BETA_C / 0.9, 0.0),
+                                            (ISING, 1 << 19, wl.BETA_C / 0.9, 0.0), (BC, 1 << 19, 1 / 1.4, 1.0)])
+def test_maximum_lattice_sizes(eng, model, L, beta, D):
+    """The largest lattices one B200 holds -- the paper's single-GPU maxima: 2^40 spins at
+    one bit (137 GB) and 2^38 at four bits (137 GB).  Light-cone windows on the wraps and in the last rows
+    (64-bit offsets), Q and n_sites at 2^40."""
+    n = 3
+    with eng.IsingSim(model, L, beta, D, 1) as sim:
+        sim.sweep(n)
+        for (x0, y0) in [(-W // 2, -W // 2), (L - W // 2, L // 3 + 5), (L // 5 + 3, L - W // 2), (L // 2 + 7, L - 40)]:
+            if model == wl.ISING_LUT:
+                want = oracle.lut_window_after(L, beta, 1, n, x0, y0, W, W)
+            else:
+                want = oracle.window_after(model, L, beta, D, 1, n, x0, y0, W, W)
+            assert (sim.read_window(x0, y0, W, W) == want).all(), (x0, y0)
+        o = sim.observables()
+        assert o.n_sites == L * L and o.sweeps_done == n and abs(o.M) < L * L // 1000
+        assert o.Q == L * L if model != BC else 0 < o.Q < L * L
