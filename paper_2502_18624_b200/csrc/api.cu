@@ -102,14 +102,20 @@ static void build_round_keys(ising_sim *h)
     }
 }
 
+// Rows per thread: as many as 32 (64 for the LUT model) to amortise the two halo rows of the sliding
+// window, but never so many that the grid drops below ~1024 threads per SM: mid-size lattices
+// (L = 4096: 64 columns) would otherwise run on a fraction of the 148 SMs.
 static void default_launch(ising_sim *h)
 {
-    h->rows_per_thread = (h->L >= 4096) ? 32 : (h->L >= 512 ? 8 : 2);
-    h->block_threads = 128;
-    if (h->model == ISING_MODEL_ISING_LUT) {     // 32 KB bucket table per block: fewer, larger blocks (measured)
-        h->rows_per_thread = (h->L >= 8192) ? 64 : (h->L >= 512 ? 8 : 2);
-        h->block_threads = 256;
-    }
+    const bool lut = h->model == ISING_MODEL_ISING_LUT;
+    const int64_t cols = lut ? h->L / 256 : h->L / 64;
+    const int64_t target = 148 * 1024;
+    int64_t r = 2 * ((h->L * cols) / (2 * target));
+    const int64_t rmax = lut ? 64 : 32;
+    if (r > rmax) r = rmax;
+    if (r < 2) r = 2;
+    h->rows_per_thread = (int)r;
+    h->block_threads = lut ? 256 : 128;           // LUT: 32 KB bucket table per block, fewer and larger blocks
 }
 
 // ---------------------------------------------------------------- create ---
