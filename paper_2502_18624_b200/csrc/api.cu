@@ -27,6 +27,8 @@ int cuda_fail(cudaError_t e, const char *what)
 
 extern "C" const char *ising_last_error(void) { return g_err.c_str(); }
 
+static void drop_graph(ising_sim *h);
+
 static bool valid_model_L(int model, int64_t L)
 {
     if (model == ISING_MODEL_ISING_LUT) return L >= 256 && (L % 256) == 0 && L <= (1ll << 20);   // 128-bit vector = 128 sites
@@ -154,6 +156,10 @@ extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_
     build_thresholds(h);
     build_round_keys(h);
     default_launch(h);
+    {
+        cudaError_t ez = cudaMemsetAsync(h->d_acc, 0, 1024, h->stream);   // accumulators, tally, t_base words
+        if (ez != cudaSuccess) { ising_destroy(h); return cuda_fail(ez, "cudaMemsetAsync(scratch)"); }
+    }
     cudaError_t e = cudaMallocHost(&h->h_acc, 256 * sizeof(long long));
     if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "cudaMallocHost"); }
     if (model == ISING_MODEL_BLUME_CAPEL) {
@@ -231,6 +237,7 @@ extern "C" int ising_destroy(ising_t *h)
     if (h->planes) cudaFree(h->planes);
     if (h->comb) cudaFree(h->comb);
     if (h->gram) cudaFree(h->gram);
+    drop_graph(h);
     if (h->lut_buckets) cudaFree(h->lut_buckets);
     if (h->d_corr) cudaFree(h->d_corr);
     if (h->d_rlist) cudaFree(h->d_rlist);
@@ -250,15 +257,82 @@ extern "C" int ising_sync(ising_t *h)
 extern "C" int64_t ising_launch_count(const ising_t *h) { return h ? h->launches : 0; }
 
 // ----------------------------------------------------------------- sweep ---
+// Launch-bound lattices (a colour phase of a few microseconds): sweeps are replayed from a CUDA graph
+// of kGraphSweeps sweeps whose kernels carry t = 0..K-1; the base sweep number is a device word that
+// a one-thread kernel sets before every replay.  Same kernels, same numbers, fewer launch gaps.
+static const int kGraphSweeps = 16;
+
+__global__ void set_t_base_kernel(uint32_t *t_base, uint32_t value) { *t_base = value; }
+
+static cudaError_t launch_colour(ising_sim *h, int c, uint32_t t)
+{
+    return (h->model == ISING_MODEL_ISING_LUT) ? launch_lut_update(h, c, t) : launch_update(h, c, t);
+}
+
+static void drop_graph(ising_sim *h)
+{
+    if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
+}
+
+static bool graph_worthwhile(const ising_sim *h, int64_t n)
+{
+    const int64_t sites = h->L * h->L;
+    return n >= 2 * kGraphSweeps && sites <= (1ll << 22);      // L <= 2048: a colour phase is launch-bound
+}
+
+static int ensure_graph(ising_sim *h)
+{
+    const int key[4] = {h->rows_per_thread, h->block_threads, h->variant, h->tally_on ? 1 : 0};
+    if (h->graph_exec && memcmp(key, h->graph_key, sizeof(key)) == 0) return ISING_OK;
+    drop_graph(h);
+    // captured on a private stream (the caller's may be the legacy default stream, which cannot be
+    // captured); the instantiated graph is then launched on the caller's stream
+    cudaGraph_t graph = nullptr;
+    cudaStream_t cap = nullptr, user = h->stream;
+    CUDA_TRY(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) { cudaStreamDestroy(cap); return cuda_fail(e, "cudaStreamBeginCapture"); }
+    h->graph_capture = true;
+    h->stream = cap;
+    const int64_t launches_before = h->launches;
+    for (int j = 0; j < kGraphSweeps && e == cudaSuccess; ++j)
+        for (int c = 0; c < 2 && e == cudaSuccess; ++c) e = launch_colour(h, c, (uint32_t)j);
+    h->stream = user;
+    h->graph_capture = false;
+    h->launches = launches_before;                              // counted when the graph is replayed
+    cudaError_t e2 = cudaStreamEndCapture(cap, &graph);
+    cudaStreamDestroy(cap);
+    if (e != cudaSuccess || e2 != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        return cuda_fail(e != cudaSuccess ? e : e2, "CUDA graph capture of the sweep loop");
+    }
+    e = cudaGraphInstantiate(&h->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) { h->graph_exec = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
+    memcpy(h->graph_key, key, sizeof(key));
+    return ISING_OK;
+}
+
 extern "C" int ising_sweep(ising_t *h, int64_t n)
 {
     if (!h) return set_error(ISING_EINVAL, "ising_sweep: NULL handle");
     if (n < 0) return set_error(ISING_EINVAL, "ising_sweep: n < 0");
     if (h->t + (uint64_t)n > 0xFFFFFFFFull) return set_error(ISING_EINVAL, "ising_sweep: sweep counter would exceed 2^32-1");
+    if (graph_worthwhile(h, n)) {
+        int rc = ensure_graph(h);
+        if (rc) return rc;
+        uint32_t *t_base = reinterpret_cast<uint32_t *>(h->d_acc + 48) + 1;
+        while (n >= kGraphSweeps) {
+            set_t_base_kernel<<<1, 1, 0, h->stream>>>(t_base, (uint32_t)h->t);
+            CUDA_TRY(cudaGraphLaunch(h->graph_exec, h->stream));
+            h->launches += 1 + 2 * kGraphSweeps;
+            h->t += kGraphSweeps;
+            n -= kGraphSweeps;
+        }
+    }
     for (int64_t i = 0; i < n; ++i) {
         for (int c = 0; c < 2; ++c) {
-            cudaError_t e = (h->model == ISING_MODEL_ISING_LUT) ? launch_lut_update(h, c, (uint32_t)h->t)
-                                                                : launch_update(h, c, (uint32_t)h->t);
+            cudaError_t e = launch_colour(h, c, (uint32_t)h->t);
             if (e != cudaSuccess) return cuda_fail(e, "update kernel");
         }
         h->t++;

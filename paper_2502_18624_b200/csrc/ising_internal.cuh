@@ -37,6 +37,11 @@ struct ising_sim {
     uint64_t *comb = nullptr; size_t comb_bytes = 0;          // planes down-sampled to the source comb (stride >= 2)
     void *lut_buckets = nullptr;                              // LUT model: 4096 x {C, meta} bucket table (cudaMalloc)
     int8_t *gram = nullptr; size_t gram_bytes = 0;            // L x L int8 spin matrix for the tensor-core correlation
+    // CUDA graph of K sweeps for launch-bound (small) lattices: kernels baked with t = 0..K-1, the base
+    // sweep number lives in device memory (d_acc[48] as two uint32: [0] = 0 for plain launches, [1] = base)
+    bool graph_capture = false;
+    cudaGraphExec_t graph_exec = nullptr;
+    int graph_key[4] = {0, 0, 0, 0};                          // rows_per_thread, block_threads, variant, tally_on
     bool tally_on = false;                                    // A7: update kernels keep running B, M, Q at d_acc[40..42]
     int corr_path = 0;                                        // 0 auto, 1 bit planes (XOR + POPC), 2 tensor cores
     long long *d_corr = nullptr; size_t d_corr_bytes = 0;

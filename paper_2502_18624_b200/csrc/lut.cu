@@ -18,6 +18,7 @@ struct LutParams {
     uint32_t colour, t;
     const uint32_t *tree;        // 16 carry constants in heap order (device): tree[n] = 2^32 - threshold(node n)
     const uint2 *buckets;        // 4096 entries indexed by the top 12 bits of the number (device), see lut_bits32
+    const uint32_t *t_base;      // sweep number = t + *t_base (see update.cu)
     long long *tally;            // A7: running B, M (device), updated when the kernel is built with TALLY
     RoundKeys rk;
 };
@@ -107,18 +108,18 @@ __device__ __forceinline__ void lut_side(const uint4 &sm, uint32_t edge, uint32_
 
 template <int P>
 __device__ __noinline__ uint4 lut_row_slow(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
-                                           uint32_t edge, uint64_t g0, const LutParams &p, uint32_t c_root,
+                                           uint32_t edge, uint64_t g0, uint32_t t, const LutParams &p, uint32_t c_root,
                                            const uint32_t *tree);
 
 template <int P, int V>
 __device__ __forceinline__ uint4 lut_row(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
-                                         uint32_t edge, uint64_t g0, const LutParams &p, uint32_t c_root,
+                                         uint32_t edge, uint64_t g0, uint32_t t, const LutParams &p, uint32_t c_root,
                                          const uint32_t *tree, const unsigned char *bk)
 {
     uint32_t sd[4];
     lut_side<P>(sm, edge, sd);
     // g0 = 8 * (first 64-site word of this thread): words 2 col, 2 col + 1 -> g0, g0 + 8
-    const PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), p.t, p.colour, p.rk);
+    const PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), t, p.colour, p.rk);
     const uint32_t gl = (uint32_t)g0;         // multiple of 16
     uint32_t bad = 0;
     uint4 o;
@@ -140,16 +141,16 @@ __device__ __forceinline__ uint4 lut_row(const uint4 &src, const uint4 &up, cons
     }
     // one test per row keeps the 16 Philox calls and 128 bucket steps in one basic block; a number in
     // a multi-threshold bucket (rare, see lut_bits32) redoes the row with the binary search
-    if (V == 0 && bad >= 256u) return lut_row_slow<P>(src, up, sm, dn, edge, g0, p, c_root, tree);
+    if (V == 0 && bad >= 256u) return lut_row_slow<P>(src, up, sm, dn, edge, g0, t, p, c_root, tree);
     return o;
 }
 
 template <int P>
 __device__ __noinline__ uint4 lut_row_slow(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
-                                           uint32_t edge, uint64_t g0, const LutParams &p, uint32_t c_root,
+                                           uint32_t edge, uint64_t g0, uint32_t t, const LutParams &p, uint32_t c_root,
                                            const uint32_t *tree)
 {
-    return lut_row<P, 1>(src, up, sm, dn, edge, g0, p, c_root, tree, nullptr);
+    return lut_row<P, 1>(src, up, sm, dn, edge, g0, t, p, c_root, tree, nullptr);
 }
 
 // A7 (optional): change of B and M caused by one updated row, from old / new words and the neighbours.
@@ -178,6 +179,7 @@ template <int C, int V, int TALLY>
 __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const __grid_constant__ LutParams p)
 {
     int dB = 0, dM = 0;
+    const uint32_t t_eff = p.t + __ldg(p.t_base);
     __shared__ uint32_t s_tree[16];
     extern __shared__ __align__(16) unsigned char s_buckets[];          // V = 0: 4096 x 8 bytes
     if (threadIdx.x < 16) s_tree[threadIdx.x] = p.tree[threadIdx.x];
@@ -225,7 +227,7 @@ __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const _
         uint4 nsrc = *reinterpret_cast<const uint4 *>(w0 + rs);
         uint32_t nedge = *reinterpret_cast<const uint32_t *>(eo);
         uint4 dn2 = *reinterpret_cast<const uint4 *>(o2);
-        uint4 o = lut_row<C, V>(src, up, sm, dn, edge, g0, p, c_root, s_tree, s_buckets);
+        uint4 o = lut_row<C, V>(src, up, sm, dn, edge, g0, t_eff, p, c_root, s_tree, s_buckets);
         if (TALLY) lut_tally_row<C>(src, o, up, sm, dn, edge, dB, dM);
         *reinterpret_cast<uint4 *>(w0) = o;
         g0 += gs;
@@ -236,7 +238,7 @@ __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const _
             nsrc2 = *reinterpret_cast<const uint4 *>(w0 + 2 * rs);
             nedge2 = *reinterpret_cast<const uint32_t *>(ee);
         }
-        o = lut_row<1 - C, V>(nsrc, sm, dn, dn2, nedge, g0, p, c_root, s_tree, s_buckets);
+        o = lut_row<1 - C, V>(nsrc, sm, dn, dn2, nedge, g0, t_eff, p, c_root, s_tree, s_buckets);
         if (TALLY) lut_tally_row<1 - C>(nsrc, o, sm, dn, dn2, nedge, dB, dM);
         *reinterpret_cast<uint4 *>(w0 + rs) = o;
         g0 += gs;
@@ -272,6 +274,7 @@ cudaError_t launch_lut_update(ising_sim *h, int colour, uint32_t t)
     p.buckets = reinterpret_cast<const uint2 *>(h->lut_buckets);
     const size_t smem = 8 << LUT_BUCKET_BITS;
     p.tally = h->d_acc + 40;
+    p.t_base = reinterpret_cast<const uint32_t *>(h->d_acc + 48) + (h->graph_capture ? 1 : 0);
 #define LUT_LAUNCH(C, V, T, SM) lut_update_kernel<C, V, T><<<grid, block, SM, h->stream>>>(p)
     if (h->variant == 0) {
         // per launch: the attribute is per device, and a process may drive several devices

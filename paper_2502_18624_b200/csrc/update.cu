@@ -25,6 +25,7 @@ struct UpdParams {
     uint32_t C4, C8;            // carry form: [r >= T] = carry out of r + (2^32 - T); 0 when T is 0 or 2^32
     uint32_t Kc;                // (8 - number of thresholds that are 0) in every nibble
     const uint32_t *bc_table;   // Blume-Capel table (device)
+    const uint32_t *t_base;     // sweep number = t + *t_base: a CUDA graph bakes t = 0..K-1 and moves *t_base
     long long *tally;           // A7: running B, M, Q (device), updated when the kernel is built with TALLY
     RoundKeys rk;
 };
@@ -121,11 +122,11 @@ __device__ __forceinline__ uint32_t ising_half_carry(uint32_t x, uint32_t up, ui
 
 template <int P, int V>
 __device__ __forceinline__ uint4 ising_row(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
-                                           uint32_t edge, uint64_t g0, uint32_t tag, const UpdParams &p)
+                                           uint32_t edge, uint64_t g0, uint32_t t, uint32_t tag, const UpdParams &p)
 {
     uint32_t sd[4];
     side_words<P>(sm, edge, sd);
-    PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), p.t, tag, p.rk);
+    PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), t, tag, p.rk);
     uint32_t gl = (uint32_t)g0;     // g0 is a multiple of 8: gl | q == gl + q
     uint4 r0 = philox_site4(gl | 0, pr, p.rk), r1 = philox_site4(gl | 1, pr, p.rk);
     uint4 r2 = philox_site4(gl | 2, pr, p.rk), r3 = philox_site4(gl | 3, pr, p.rk);
@@ -171,12 +172,12 @@ __device__ __forceinline__ uint32_t bc_half(uint32_t x, uint32_t up, uint32_t dn
 
 template <int P>
 __device__ __forceinline__ uint4 bc_row(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
-                                        uint32_t edge, uint64_t g0, uint32_t tag, const UpdParams &p,
+                                        uint32_t edge, uint64_t g0, uint32_t t, uint32_t tag, const UpdParams &p,
                                         const uint32_t *tab, uint64_t always)
 {
     uint32_t sd[4];
     side_words<P>(sm, edge, sd);
-    PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), p.t, tag, p.rk);
+    PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), t, tag, p.rk);
     uint32_t gl = (uint32_t)g0;
     uint4 o;
     {
@@ -245,12 +246,12 @@ __device__ __forceinline__ uint32_t bc_half_carry(uint32_t x, uint32_t up, uint3
 
 template <int P>
 __device__ __forceinline__ uint4 bc_row_carry(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
-                                              uint32_t edge, uint64_t g0, uint32_t tag, const UpdParams &p,
+                                              uint32_t edge, uint64_t g0, uint32_t t, uint32_t tag, const UpdParams &p,
                                               const unsigned char *tab)
 {
     uint32_t sd[4];
     side_words<P>(sm, edge, sd);
-    PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), p.t, tag, p.rk);
+    PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), t, tag, p.rk);
     uint32_t gl = (uint32_t)g0;
     uint4 o;
     {
@@ -322,6 +323,7 @@ template <int MODEL, int C, int V, int TALLY>
 __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ UpdParams p)
 {
     int dB = 0, dM = 0, dQ = 0;                            // TALLY: this thread's share of the changes
+    const uint32_t t_eff = p.t + __ldg(p.t_base);
     __shared__ __align__(16) uint32_t s_tab[80 + 132];   // both table forms (api.cu)
     uint64_t always = 0;
     if (MODEL == ISING_MODEL_BLUME_CAPEL) {
@@ -366,9 +368,9 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
         uint32_t nedge = *reinterpret_cast<const uint32_t *>(eo);
         uint4 dn2 = *reinterpret_cast<const uint4 *>(o2);
         uint4 o;
-        if (MODEL == ISING_MODEL_ISING) o = ising_row<C, V>(src, up, sm, dn, edge, g0, p.colour, p);
-        else if (V == 0) o = bc_row_carry<C>(src, up, sm, dn, edge, g0, p.colour, p, ctab);
-        else o = bc_row<C>(src, up, sm, dn, edge, g0, p.colour, p, s_tab, always);
+        if (MODEL == ISING_MODEL_ISING) o = ising_row<C, V>(src, up, sm, dn, edge, g0, t_eff, p.colour, p);
+        else if (V == 0) o = bc_row_carry<C>(src, up, sm, dn, edge, g0, t_eff, p.colour, p, ctab);
+        else o = bc_row<C>(src, up, sm, dn, edge, g0, t_eff, p.colour, p, s_tab, always);
         if (TALLY) tally_row<MODEL, C>(src, o, up, sm, dn, edge, dB, dM, dQ);
         *reinterpret_cast<uint4 *>(w0) = o;
         g0 += gs;
@@ -380,9 +382,9 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
             nsrc2 = *reinterpret_cast<const uint4 *>(w0 + 2 * rs);
             nedge2 = *reinterpret_cast<const uint32_t *>(ee);
         }
-        if (MODEL == ISING_MODEL_ISING) o = ising_row<1 - C, V>(nsrc, sm, dn, dn2, nedge, g0, p.colour, p);
-        else if (V == 0) o = bc_row_carry<1 - C>(nsrc, sm, dn, dn2, nedge, g0, p.colour, p, ctab);
-        else o = bc_row<1 - C>(nsrc, sm, dn, dn2, nedge, g0, p.colour, p, s_tab, always);
+        if (MODEL == ISING_MODEL_ISING) o = ising_row<1 - C, V>(nsrc, sm, dn, dn2, nedge, g0, t_eff, p.colour, p);
+        else if (V == 0) o = bc_row_carry<1 - C>(nsrc, sm, dn, dn2, nedge, g0, t_eff, p.colour, p, ctab);
+        else o = bc_row<1 - C>(nsrc, sm, dn, dn2, nedge, g0, t_eff, p.colour, p, s_tab, always);
         if (TALLY) tally_row<MODEL, 1 - C>(nsrc, o, sm, dn, dn2, nedge, dB, dM, dQ);
         *reinterpret_cast<uint4 *>(w0 + rs) = o;
         g0 += gs;
@@ -423,6 +425,7 @@ cudaError_t launch_update(ising_sim *h, int colour, uint32_t t)
     int block = h->block_threads;
     unsigned grid = (unsigned)((threads + block - 1) / block);
     p.tally = h->d_acc + 40;
+    p.t_base = reinterpret_cast<const uint32_t *>(h->d_acc + 48) + (h->graph_capture ? 1 : 0);   // [0] stays 0, [1] = base of a graph replay
     bool never = false;                           // Blume-Capel: a threshold that is exactly 0 -> compare/select form
     if (h->model == ISING_MODEL_BLUME_CAPEL)
         for (int i = 0; i < h->n_T; ++i) never = never || h->T[i] == 0;

@@ -420,6 +420,35 @@ def test_fused_tally_equals_recompute_and_oracle(eng, model, L, beta, D):
             sim.tally()
 
 
+@pytest.mark.parametrize("model,L,beta,D", [(ISING, 256, wl.BETA_C, 0.0), (BC, 192, 1 / 1.4, 1.0), (wl.ISING_LUT, 512, wl.BETA_C / 0.9, 0.0)])
+def test_graph_replayed_sweeps_equal_plain_launches(eng, model, L, beta, D):
+    """Small lattices replay the sweep loop from a CUDA graph (16 sweeps per replay, base sweep number in
+    device memory): 75 sweeps in one call (4 replays + 11 plain sweeps) must equal the oracle's 75 sweeps and
+    a sweep-by-sweep run; changing the launch geometry or the tally in between rebuilds the graph."""
+    seed, n = 23, 75
+    if model == wl.ISING_LUT:
+        s = oracle.lut_init(L, seed)
+        for t in range(n + 40):
+            oracle.lut_sweep(s, beta, seed, t)
+    else:
+        s = oracle.init(model, L, seed)
+        for t in range(n + 40):
+            oracle.sweep(model, s, beta, D, seed, t)
+    with eng.IsingSim(model, L, beta, D, seed) as sim:
+        sim.sweep(n)                                         # graph path
+        sim.set_launch(4, 64)
+        sim.set_tally(True)
+        sim.sweep(40)                                        # rebuilt graph (2 replays + 8 plain), tally kernels
+        assert (sim.read_lattice() == s).all()
+        a, b = sim.tally(), sim.observables()
+        assert (a.bond_sum, a.M, a.Q) == (b.bond_sum, b.M, b.Q) == oracle.observables(s)
+        assert b.sweeps_done == n + 40
+    with eng.IsingSim(model, L, beta, D, seed) as sim:
+        for _ in range(n + 40):
+            sim.sweep(1)                                     # plain launches only
+        assert (sim.read_lattice() == s).all()
+
+
 def test_run_schedule_matches_stepwise_run(eng):
     """A11: one native call over the paper's time grid gives the same observables as sweeping step by step
     (and as the oracle), with and without the fused tally."""
