@@ -65,6 +65,7 @@ def parse_args():
     ap.add_argument("--rows-per-thread", type=int, default=0, help="update-kernel launch geometry (0 = library default)")
     ap.add_argument("--block", type=int, default=0, help="update-kernel threads per block (0 = library default)")
     ap.add_argument("--variant", type=int, default=0, help="update-kernel variant (0 = default carry form)")
+    ap.add_argument("--corr-path", type=int, default=0, help="ising_set_corr_path: 0 auto (tensor cores, CTA pairs), 1 bit planes, 2 tensor cores one CTA per tile, 3 CTA pairs")
     ap.add_argument("--tally", action="store_true", help="A7: keep E, M by the fused tally of the update kernels instead of the observables pass")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -303,6 +304,8 @@ def run_ours(args):
         sim.set_variant(args.variant)
     if args.tally:
         sim.set_tally(True)
+    if args.corr_path:
+        sim.set_corr_path(args.corr_path)
 
     def barrier():
         if dist is not None:
@@ -404,7 +407,7 @@ def run_ours(args):
                    "seed": base.seed, "sweeps_per_step": S, "observables_every": S,
                    "step": "S sweeps + observables" if args.workload == "sweep" else "S sweeps + correlation protocol + observables",
                    "launch": {"rows_per_thread": args.rows_per_thread or "default", "block": args.block or "default",
-                              "variant": args.variant, "fused_tally": bool(args.tally)},
+                              "variant": args.variant, "fused_tally": bool(args.tally), "corr_path": args.corr_path},
                    "lattice_bytes": L * L // (8 if model == wl.ISING_LUT else 2), "l2": "inputs larger than L2 (no flush needed)" if L * L // 2 > (256 << 20)
                    else "lattice fits L2: DRAM figures not meaningful", "parallelism": f"replicas x{world}"},
         "measurement_ms_per_step": (total_ms - sweep_ms) / K,
