@@ -324,6 +324,7 @@ extern "C" int ising_sweep(ising_t *h, int64_t n)
         uint32_t *t_base = reinterpret_cast<uint32_t *>(h->d_acc + 48) + 1;
         while (n >= kGraphSweeps) {
             set_t_base_kernel<<<1, 1, 0, h->stream>>>(t_base, (uint32_t)h->t);
+            CUDA_TRY(cudaGetLastError());
             CUDA_TRY(cudaGraphLaunch(h->graph_exec, h->stream));
             h->launches += 1 + 2 * kGraphSweeps;
             h->t += kGraphSweeps;
