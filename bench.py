@@ -403,7 +403,7 @@ def run_ours(args):
         "warmup": W, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "u32 (Philox4x32-10, SWAR on 4-bit spins, integer compare)",
         "data": "synthetic (seeded random-start quench, the paper's own workload)",
-        "config": {"workload": name, "model": args.model, "L": L, "beta": base.beta, "D": base.D,
+        "config": {"workload": name, "hamiltonian": args.model, "L": L, "beta": base.beta, "D": base.D,
                    "seed": base.seed, "sweeps_per_step": S, "observables_every": S,
                    "step": "S sweeps + observables" if args.workload == "sweep" else "S sweeps + correlation protocol + observables",
                    "launch": {"rows_per_thread": args.rows_per_thread or "default", "block": args.block or "default",
