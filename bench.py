@@ -46,7 +46,10 @@ import workloads as wl  # noqa: E402
 
 BYTES_PER_SITE_LAUNCH = 1.5    # per UPDATED site: own nibble read + written, opposite nibble read once (3 x 4 bit)
 PHILOX_SLOTS_PER_SITE = 9.25   # (18 IMAD.WIDE + 19 LOP3) / 4 sites, rounds 1-2 partly hoisted
-PAPER_UPDATES_PER_NS = None    # no published number for THIS kernel contract / hardware
+# BASELINE.md Sec. 1 (the paper's single-GPU maxima, GB200, other machine: context): the 1-bit LUT Ising kernel
+# at L = 2^20 and the 4-bit Blume-Capel kernel at L = 2^19.  No published number exists for the north_star
+# contract (4-bit Ising, one number per spin), so the default workload reports vs_baseline = null.
+PAPER_UPDATES_PER_NS = {("lut", 1 << 20): 1802.0, ("bc", 1 << 19): 948.0}
 
 
 def parse_args():
@@ -79,6 +82,10 @@ def pick_workload(args):
         base = wl.config(4)
     L = args.L or base.L
     name = base.name if L == base.L else f"{base.name.split('_L')[0]}_L{L}_override"
+    if args.model == "lut":          # NEXT-2: the paper's 1-bit kernel on config 2's temperature and seed
+        name = f"ising_1bit_lut_L{L}_0.9Tc" + ("_paper_single_gpu_max" if L == (1 << 20) else "")
+    if args.model == "bc" and L == (1 << 19):
+        name = "bc_L524288_D1_paper_single_gpu_max"
     return base, L, name
 
 
@@ -401,7 +408,8 @@ def run_ours(args):
     line = {
         "metric": "spin updates/ns", "value": value, "unit": "updates/ns", "n_gpus": world, "steps": K,
         "warmup": W, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "u32 (Philox4x32-10, SWAR on 4-bit spins, integer compare)",
+        "vs_baseline": (value / PAPER_UPDATES_PER_NS[(args.model, L)]) if (args.model, L) in PAPER_UPDATES_PER_NS and args.workload == "sweep" else None,
+        "dtype": "u32 (Philox4x32-10, SWAR on 4-bit spins, integer compare)",
         "data": "synthetic (seeded random-start quench, the paper's own workload)",
         "config": {"workload": name, "hamiltonian": args.model, "L": L, "beta": base.beta, "D": base.D,
                    "seed": base.seed, "sweeps_per_step": S, "observables_every": S,
