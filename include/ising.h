@@ -61,7 +61,9 @@ size_t ising_workspace_bytes(int model, int64_t L);
 /* Create a simulation (PAPER.md:25 problem statement; Eq. 1 / Eq. 2).
  *   model       ISING_MODEL_*
  *   L           linear size, multiple of 64, >= 64 (one 128-bit vector = 32
- *               same-colour sites of a row)
+ *               same-colour sites of a row); ISING_MODEL_ISING_LUT stores one
+ *               bit per spin (128 sites per vector): multiple of 256, >= 256,
+ *               colour array = L rows x (L / 128) uint64 words, bit 1 = spin +1
  *   beta        1/(k_B T) >= 0, finite;  D = crystal field Delta of Eq. 2
  *               (finite; ignored for Ising);  seed = Philox key
  *   dev_buf     device memory of >= ising_workspace_bytes() bytes, 256-byte
@@ -76,7 +78,8 @@ int ising_create(int model, int64_t L, double beta, double D, uint64_t seed,
 
 /* n >= 0 full sweeps: colour 0 then colour 1 ("two update phases"),
  * one Philox number per site, accept iff r < T.  Asynchronous:
- * 2n kernel launches on the handle's stream, no host synchronisation.       */
+ * 2n kernel launches on the handle's stream, no host synchronisation; small
+ * lattices (L <= 2048) replay a CUDA graph of 16 sweeps when n >= 32.           */
 int ising_sweep(ising_t *h, int64_t n);
 
 /* Full recompute of B, M, Q by warp-shuffle / block reduction over both colour
@@ -158,7 +161,8 @@ int ising_thresholds(ising_t *h, uint64_t *out, int cap, int *count);
  * cf. PAPER.md:193): rows walked per thread and threads per block
  * (multiple of 32, <= 1024).  0 keeps the current value.                    */
 int ising_set_launch(ising_t *h, int rows_per_thread, int block_threads);
-/* Update kernel variant (0 = default; others are equivalent implementations
+/* Update kernel variant (0 = default: carry-chain compare, bucket table for the
+ * LUT model; 1 = compare/select, binary search; equivalent implementations
  * kept for parity / performance comparison).                                */
 int ising_set_variant(ising_t *h, int variant);
 
