@@ -437,7 +437,12 @@ def run_ours(args):
             line["e2e"] = run_e2e(eng, torch, model, L, base.beta, base.D, base.seed, S, min(K, 3), device)
         if not args.no_cpu and world == 1:
             v, cores, info = time_oracle(model, base.beta, base.D, base.seed, args.cpu_seconds)
-            line["cpu_baseline"] = {"value": v, "unit": "updates/ns", "cores": cores, "kind": "oracle", "sample": info}
+            import oracle
+            oracle.set_threads(1)                                   # also on one core
+            v1, _, info1 = time_oracle(model, base.beta, base.D, base.seed, min(4.0, args.cpu_seconds), L=1024)
+            oracle.set_threads(cores)
+            line["cpu_baseline"] = {"value": v, "unit": "updates/ns", "cores": cores, "kind": "oracle", "sample": info,
+                                    "one_core": {"value": v1, "unit": "updates/ns", "cores": 1, "sample": info1}}
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()

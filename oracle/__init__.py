@@ -240,5 +240,10 @@ def lut_window_after(L, beta, seed, n_sweeps, x0, y0, w, h) -> np.ndarray:
     return s[m:m + h, m:m + w].copy()
 
 
+def set_threads(n: int) -> None:
+    """OpenMP thread count of the sweeps (timing only)."""
+    lib().orc_set_threads(C.c_int(n))
+
+
 def threads() -> int:
     return int(lib().orc_threads())

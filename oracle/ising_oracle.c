@@ -357,6 +357,16 @@ int64_t orc_time_grid(uint64_t tmax, int64_t cap, uint64_t *out)
     return n;
 }
 
+/* Thread count of the OpenMP loops (timing only: bench.py reports the oracle on all cores and on one). */
+void orc_set_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 int orc_threads(void)
 {
 #ifdef _OPENMP
