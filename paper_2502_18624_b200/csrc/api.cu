@@ -687,7 +687,7 @@ extern "C" int ising_correlation(ising_t *h, int64_t rmax, int64_t *sx, int64_t 
 extern "C" int ising_set_corr_path(ising_t *h, int path)
 {
     if (!h) return set_error(ISING_EINVAL, "ising_set_corr_path: NULL handle");
-    if (path < 0 || path > 3) return set_error(ISING_EINVAL, "ising_set_corr_path: path must be 0 (auto), 1 (bit planes), 2 (tensor cores) or 3 (tensor cores, CTA pairs)");
+    if (path < 0 || path > 4) return set_error(ISING_EINVAL, "ising_set_corr_path: path must be 0 (auto), 1 (bit planes), 2 (tensor cores), 3 (CTA pairs) or 4 (CTA pairs, fp4)");
     h->corr_path = path;
     return ISING_OK;
 }

@@ -408,6 +408,169 @@ gram2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ G
     if (warp == 2) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
 }
 
+// ---------------------------------------------- fp4 variant (opt-in, path 4) ---
+// -1, 0, +1 are exact in e2m1, so the same Gram matrix can run at the fp4 rate: tcgen05.mma
+// kind::mxf4 (K = 64 per instruction, 128 smem bytes = 256 elements per stage), fp32 accumulators
+// (exact: |sum| <= elements per K chunk < 2^24), every block scale = 1.0.  TMEM: one 256-column
+// accumulator (columns 0..255) + the scale columns, so MMA and epilogue of consecutive tiles do not overlap.
+namespace {
+// block-scaled descriptor: a/b format E2M1 (1), scale format UE8M0 (bit 23), N >> 3 at bit 17, M >> 4 at bit 24
+constexpr uint32_t kInstrDescF4 = (1u << 7) | (1u << 10) | ((uint32_t)(256 >> 3) << 17) | (1u << 23) | ((uint32_t)(256 >> 4) << 24);
+__device__ __forceinline__ void umma_mxf4_2sm(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t accumulate, uint32_t tmem_sf)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::mxf4.block_scale.block32 [%0], %1, %2, %3, [%5], [%5], p;\n\t}"
+        ::"r"(tmem_d), "l"(da), "l"(db), "r"(kInstrDescF4), "r"(accumulate), "r"(tmem_sf) : "memory");
+}
+}  // namespace
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1)
+gram4_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ GramParams p)
+{
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    uint8_t *tail = smem + STAGES2 * STAGE2_BYTES;
+    int *bins = reinterpret_cast<int *>(tail);
+    uint64_t *full = reinterpret_cast<uint64_t *>(tail + 1536);             // [STAGES2]  (used on the leader)
+    uint64_t *empty = full + STAGES2;                                       // [STAGES2]  (both CTAs)
+    uint64_t *tfull = empty + STAGES2;                                      // [2]        (both CTAs)
+    uint64_t *tempty = tfull + 2;                                           // [2]        (used on the leader)
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + 2);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_rank();
+    const bool leader = rank == 0;
+    const int n_kb = p.n_kb;
+    // tiles of 256 rows: p.n_ib row blocks; a contiguous run per CLUSTER, column-tile-major
+    const long long n_tiles = (long long)p.n_ib * p.n_jk;
+    const int n_cl = gridDim.x >> 1, cl = blockIdx.x >> 1;
+    const int t_lo = (int)(n_tiles * cl / n_cl), t_hi = (int)(n_tiles * (cl + 1) / n_cl);
+
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < STAGES2; ++s) { mbar_init(&full[s], 2); mbar_init(&empty[s], 1); }
+        for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], 8); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int i = threadIdx.x; i < NBINS; i += blockDim.x) bins[i] = 0;
+    cluster_sync_all();                                                      // barriers of both CTAs exist
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    cluster_sync_all();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_base = *tmem_slot;
+    // scale factors: every block scale is 1.0 (ue8m0 byte 0x7F).  Columns 256..287 of all 128 lanes are
+    // filled with that byte, so whichever bytes the instruction picks as SFA / SFB read as 1.0.
+    if (warp >= 2) {
+        const uint32_t sf = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + 256u;
+        asm volatile(
+            "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+            "{%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, "
+            "%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1};"
+            ::"r"(sf), "r"(0x7F7F7F7Fu) : "memory");
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    cluster_sync_all();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+
+    if (warp == 0) {
+        // ===== TMA producer (both CTAs): own A half, own half of the B rows =====
+        if (lane == 0) {
+            int stage = 0; uint32_t phase = 0;
+            for (int t = t_lo; t < t_hi; ++t) {
+                const int jk = t / p.n_ib, ib = t - jk * p.n_ib;
+                const int I0 = ib * 256 + (int)rank * TM;
+                int J0 = ib * 256 + jk * TN; if (J0 >= p.L) J0 -= p.L;      // multiple of 256: the tile never wraps
+                J0 += (int)rank * TM;
+                for (int kb = 0; kb < n_kb; ++kb) {
+                    mbar_wait(&empty[stage], phase ^ 1);
+                    if (leader) mbar_expect_tx(&full[stage], 2 * STAGE2_BYTES);   // bytes of both CTAs land on this barrier
+                    uint8_t *sa = smem + stage * STAGE2_BYTES, *sb = sa + HALF_BYTES;
+                    tma_load_2d_2sm(sa, &tmap, &full[stage], p.k0 + kb * TKB, I0);
+                    tma_load_2d_2sm(sb, &tmap, &full[stage], p.k0 + kb * TKB, J0);
+                    if (!leader) mbar_arrive_remote(&full[stage], 0);
+                    if (++stage == STAGES2) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer: leader CTA only =====
+        if (leader && lane == 0) {
+            int stage = 0; uint32_t phase = 0;
+            const int as = 0; uint32_t aphase = 0;                       // one accumulator: columns 256.. hold the scales
+            for (int t = t_lo; t < t_hi; ++t) {
+                mbar_wait(&tempty[as], aphase ^ 1);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t d_tmem = tmem_base;
+                for (int kb = 0; kb < n_kb; ++kb) {
+                    mbar_wait(&full[stage], phase);
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    const uint32_t sa = smem_u32(smem + stage * STAGE2_BYTES), sb = sa + HALF_BYTES;
+                    const uint64_t da = umma_desc(sa), db = umma_desc(sb);
+#pragma unroll
+                    for (int k = 0; k < TKB / 32; ++k)
+                        umma_mxf4_2sm(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), (kb | k) ? 1u : 0u, tmem_base + 256u);
+                    umma_commit_2sm(&empty[stage]);
+                    if (++stage == STAGES2) { stage = 0; phase ^= 1; }
+                }
+                umma_commit_2sm(&tfull[as]);
+                aphase ^= 1;
+            }
+        }
+    } else {
+        // ===== epilogue (both CTAs): rows I0 + 128 rank + i of the pair tile =====
+        const int q = warp & 3, row = q * 32 + lane;
+        const int et = threadIdx.x - 64;
+        const int as = 0; uint32_t aphase = 0;
+        for (int t = t_lo; t < t_hi; ++t) {
+            const int jk = t / p.n_ib;
+            mbar_wait(&tfull[as], aphase);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16);
+#pragma unroll 1
+            for (int c = 0; c < TN / 32; ++c) {
+                uint32_t v[32];
+                asm volatile(
+                    "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                    "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+                    "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+                    : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                      "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+                      "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+                      "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+                    : "r"(taddr + (uint32_t)(c * 32)));
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                const uint32_t b0 = smem_u32(bins) + 4u * (uint32_t)((TM - 1) + 32 * c - row);
+#pragma unroll
+                for (int k = 0; k < 32; ++k)
+                    asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(b0 + 4u * k), "r"(__float2int_rn(__uint_as_float(v[k]))) : "memory");   // fp32 accumulators hold exact integers
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) { if (leader) mbar_arrive(&tempty[as]); else mbar_arrive_remote(&tempty[as], 0); }
+            aphase ^= 1;
+            if (t + 1 < t_hi && (t + 1) / p.n_ib == jk) continue;
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            for (int b = et; b < NBINS; b += 128) {
+                const int r = jk * TN - (int)rank * TM + b - (TM - 1);
+                const int v = bins[b];
+                bins[b] = 0;
+                if (r >= 1 && r <= p.rmax && v != 0)
+                    atomicAdd(reinterpret_cast<unsigned long long *>(&p.out[r - 1]), (unsigned long long)(long long)v);
+            }
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    cluster_sync_all();                                                      // the peer may still be read by MMAs / arrive remotely
+    if (warp == 2) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+}
+
 // ------------------------------------------------- planes -> int8 matrix ---
 // out[y][64 q + i] = nz bit ? (sg bit ? +1 : -1) : 0   (Ising: nz == nullptr, every site non-zero)
 __global__ void __launch_bounds__(256) expand_kernel(const uint64_t *__restrict__ sg, const uint64_t *__restrict__ nz,
@@ -428,6 +591,32 @@ __global__ void __launch_bounds__(256) expand_kernel(const uint64_t *__restrict_
                 const int bit = 16 * c + 4 * k + b;
                 const uint32_t val = ((z >> bit) & 1ull) ? (((s >> bit) & 1ull) ? 0x01u : 0xFFu) : 0u;
                 word |= val << (8 * b);
+            }
+            v[k] = word;
+        }
+        o[c] = make_uint4(v[0], v[1], v[2], v[3]);
+    }
+}
+
+// out[y][32 q + i/2] nibble (i & 1) = e2m1 code of site x = 64 q + i: +1 -> 0x2, -1 -> 0xA, 0 -> 0x0
+__global__ void __launch_bounds__(256) expand_fp4_kernel(const uint64_t *__restrict__ sg, const uint64_t *__restrict__ nz,
+                                                         uint8_t *__restrict__ out, int64_t n_words)
+{
+    const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= n_words) return;
+    const uint64_t s = sg[w], z = nz ? nz[w] : ~0ull;
+    uint4 *o = reinterpret_cast<uint4 *>(out + w * 32);
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+        uint32_t v[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            uint32_t word = 0;
+#pragma unroll
+            for (int b = 0; b < 8; ++b) {
+                const int bit = 32 * c + 8 * k + b;
+                const uint32_t val = ((z >> bit) & 1ull) ? (((s >> bit) & 1ull) ? 0x2u : 0xAu) : 0u;
+                word |= val << (4 * b);
             }
             v[k] = word;
         }
@@ -474,8 +663,9 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
     cudaError_t ea = cudaFuncSetAttribute(gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (ea != cudaSuccess) return ea;
     CUtensorMap tmap;
-    const cuuint64_t gdim[2] = {(cuuint64_t)L, (cuuint64_t)L};
-    const cuuint64_t gstride[1] = {(cuuint64_t)L};
+    const int row_bytes = (h->corr_path == 4) ? L / 2 : L;      // fp4: two elements per byte
+    const cuuint64_t gdim[2] = {(cuuint64_t)row_bytes, (cuuint64_t)L};
+    const cuuint64_t gstride[1] = {(cuuint64_t)row_bytes};
     const cuuint32_t box[2] = {(cuuint32_t)TKB, (cuuint32_t)TM};
     const cuuint32_t estr[2] = {1, 1};
     if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, h->gram, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -491,11 +681,13 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
     // is the optimum for both kernels; 512 pays more epilogues, 2048 falls out of L2)
     int kc = (int)(((64ll << 20) / L) / TKB * TKB);
     if (kc < 4 * TKB) kc = 4 * TKB;
-    if (kc > L) kc = L;
+    if (kc > row_bytes) kc = row_bytes;
     p.n_kb = kc / TKB;
+    const bool fp4 = h->corr_path == 4;               // opt-in: kind::mxf4 on a packed e2m1 matrix (L/2 bytes per row)
     const bool pair = h->corr_path != 2;              // default: cta_group::2 kernel, 256-row tiles; path 2 = single-CTA kernel
     if (pair) {
         ea = cudaFuncSetAttribute(gram2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM2_BYTES);
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(gram4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM2_BYTES);
         if (ea != cudaSuccess) return ea;
         p.n_ib = L / 256;
         p.n_jk = (int)((count + 256 + TN - 1) / TN);      // columns I0 .. I0 + 255 + rmax
@@ -509,13 +701,15 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
         long long *out = axis ? dev_sx : dev_sy;
         cudaError_t e = cudaMemsetAsync(out, 0, count * sizeof(long long), h->stream);
         if (e != cudaSuccess) return e;
-        expand_kernel<<<(unsigned)((pw + 255) / 256), 256, 0, h->stream>>>(sg, nz, h->gram, (int64_t)pw);
+        if (fp4) expand_fp4_kernel<<<(unsigned)((pw + 255) / 256), 256, 0, h->stream>>>(sg, nz, reinterpret_cast<uint8_t *>(h->gram), (int64_t)pw);
+        else expand_kernel<<<(unsigned)((pw + 255) / 256), 256, 0, h->stream>>>(sg, nz, h->gram, (int64_t)pw);
         p.out = out;
         h->launches++;
-        for (int k0 = 0; k0 < L; k0 += kc) {
+        for (int k0 = 0; k0 < row_bytes; k0 += kc) {
             p.k0 = k0;
-            p.n_kb = (L - k0 < kc ? L - k0 : kc) / TKB;
-            if (pair) gram2_kernel<<<grid, 192, SMEM2_BYTES, h->stream>>>(tmap, p);
+            p.n_kb = (row_bytes - k0 < kc ? row_bytes - k0 : kc) / TKB;
+            if (fp4) gram4_kernel<<<grid, 192, SMEM2_BYTES, h->stream>>>(tmap, p);
+            else if (pair) gram2_kernel<<<grid, 192, SMEM2_BYTES, h->stream>>>(tmap, p);
             else gram_kernel<<<grid, 192, SMEM_BYTES, h->stream>>>(tmap, p);
             h->launches++;
         }
