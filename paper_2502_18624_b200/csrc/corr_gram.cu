@@ -426,7 +426,7 @@ __device__ __forceinline__ void umma_mxf4_2sm(uint32_t tmem_d, uint64_t da, uint
 }
 }  // namespace
 
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1)
 gram4_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ GramParams p)
 {
     extern __shared__ uint8_t smem_raw[];
@@ -450,7 +450,7 @@ gram4_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ G
 
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < STAGES2; ++s) { mbar_init(&full[s], 2); mbar_init(&empty[s], 1); }
-        for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], 8); }
+        for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], 16); }   // 8 epilogue warps per CTA
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int i = threadIdx.x; i < NBINS; i += blockDim.x) bins[i] = 0;
@@ -465,7 +465,7 @@ gram4_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ G
     const uint32_t tmem_base = *tmem_slot;
     // scale factors: every block scale is 1.0 (ue8m0 byte 0x7F).  Columns 256..287 of all 128 lanes are
     // filled with that byte, so whichever bytes the instruction picks as SFA / SFB read as 1.0.
-    if (warp >= 2) {
+    if (warp >= 2 && warp < 6) {
         const uint32_t sf = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + 256u;
         asm volatile(
             "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
@@ -523,8 +523,8 @@ gram4_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ G
             }
         }
     } else {
-        // ===== epilogue (both CTAs): rows I0 + 128 rank + i of the pair tile =====
-        const int q = warp & 3, row = q * 32 + lane;
+        // ===== epilogue (both CTAs, 8 warps: two per TMEM lane quarter, each half of the columns) =====
+        const int q = warp & 3, row = q * 32 + lane, chalf = (warp - 2) >> 2;
         const int et = threadIdx.x - 64;
         const int as = 0; uint32_t aphase = 0;
         for (int t = t_lo; t < t_hi; ++t) {
@@ -533,7 +533,7 @@ gram4_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ G
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16);
 #pragma unroll 1
-            for (int c = 0; c < TN / 32; ++c) {
+            for (int c = chalf * (TN / 64); c < (chalf + 1) * (TN / 64); ++c) {
                 uint32_t v[32];
                 asm volatile(
                     "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
@@ -555,15 +555,15 @@ gram4_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ G
             if (lane == 0) { if (leader) mbar_arrive(&tempty[as]); else mbar_arrive_remote(&tempty[as], 0); }
             aphase ^= 1;
             if (t + 1 < t_hi && (t + 1) / p.n_ib == jk) continue;
-            asm volatile("bar.sync 1, 128;" ::: "memory");
-            for (int b = et; b < NBINS; b += 128) {
+            asm volatile("bar.sync 1, 256;" ::: "memory");
+            for (int b = et; b < NBINS; b += 256) {
                 const int r = jk * TN - (int)rank * TM + b - (TM - 1);
                 const int v = bins[b];
                 bins[b] = 0;
                 if (r >= 1 && r <= p.rmax && v != 0)
                     atomicAdd(reinterpret_cast<unsigned long long *>(&p.out[r - 1]), (unsigned long long)(long long)v);
             }
-            asm volatile("bar.sync 1, 128;" ::: "memory");
+            asm volatile("bar.sync 1, 256;" ::: "memory");
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -681,6 +681,10 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
     // is the optimum for both kernels; 512 pays more epilogues, 2048 falls out of L2)
     int kc = (int)(((64ll << 20) / L) / TKB * TKB);
     if (kc < 4 * TKB) kc = 4 * TKB;
+    if (h->corr_path == 4) {                          // fp4, one accumulator buffer: fewer, longer tiles pay (measured: 96 MB slab)
+        kc = (int)(((96ll << 20) / L) / TKB * TKB);
+        if (kc < 4 * TKB) kc = 4 * TKB;
+    }
     if (kc > row_bytes) kc = row_bytes;
     p.n_kb = kc / TKB;
     const bool fp4 = h->corr_path == 4;               // opt-in: kind::mxf4 on a packed e2m1 matrix (L/2 bytes per row)
@@ -708,7 +712,7 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
         for (int k0 = 0; k0 < row_bytes; k0 += kc) {
             p.k0 = k0;
             p.n_kb = (row_bytes - k0 < kc ? row_bytes - k0 : kc) / TKB;
-            if (fp4) gram4_kernel<<<grid, 192, SMEM2_BYTES, h->stream>>>(tmap, p);
+            if (fp4) gram4_kernel<<<grid, 320, SMEM2_BYTES, h->stream>>>(tmap, p);
             else if (pair) gram2_kernel<<<grid, 192, SMEM2_BYTES, h->stream>>>(tmap, p);
             else gram_kernel<<<grid, 192, SMEM_BYTES, h->stream>>>(tmap, p);
             h->launches++;

@@ -335,6 +335,9 @@ def test_correlation_tensor_core_path(eng, model, L):
             sim.set_corr_path(2)                             # single-CTA kernel
             tx, ty = sim.correlation(rmax)
             assert (tx == ox[:rmax]).all() and (ty == oy[:rmax]).all(), rmax
+            sim.set_corr_path(4)                             # fp4 (kind::mxf4, unit block scales), CTA pairs
+            fx, fy = sim.correlation(rmax)
+            assert (fx == ox[:rmax]).all() and (fy == oy[:rmax]).all(), rmax
             sim.set_corr_path(1)
             bx, by = sim.correlation(rmax)
             assert (bx == tx).all() and (by == ty).all(), rmax
@@ -343,9 +346,10 @@ def test_correlation_tensor_core_path(eng, model, L):
         assert (ax == ox).all() and (ay == oy).all()
         # closed form at the largest accumulator magnitude: all +1 -> every Gram entry is L, S(r) = N
         sim.write_lattice(np.ones((L, L), dtype=np.int8))
-        sim.set_corr_path(2)
-        tx, ty = sim.correlation(L // 2)
-        assert (tx == L * L).all() and (ty == L * L).all()
+        for path in (2, 3, 4):
+            sim.set_corr_path(path)
+            tx, ty = sim.correlation(L // 2)
+            assert (tx == L * L).all() and (ty == L * L).all(), path
     with eng.IsingSim(model, 192, beta, D, 5) as sim:        # L % 256 != 0: tensor path refuses, auto falls back
         sim.set_corr_path(2)
         with pytest.raises(eng.IsingError):
