@@ -371,15 +371,18 @@ def run_ours(args):
         ev2[0].record(); sim.correlation(L // 2); ev2[1].record()
         torch.cuda.synchronize(device)
         full_ms = ev2[0].elapsed_time(ev2[1])
-        n_jk = (L // 2 + 256 + 255) // 256                      # CTA-pair kernel: 256 x 256 tiles, columns I0 .. I0 + 255 + rmax
-        macs = 2.0 * (L // 256) * n_jk * 256 * 256 * L          # both axes, tiles actually multiplied
-        peak_t = 2.0 * float(measured_peaks()[2].get("bf16_tflops", 0.0)) or None
+        fp4 = args.corr_path in (0, 4)
+        tn = 224 if fp4 else 256                                # gram4_kernel: 256 x 224 tiles; gram2_kernel: 256 x 256
+        n_jk = (L // 2 + 256 + tn - 1) // tn                    # columns I0 .. I0 + 255 + rmax
+        macs = 2.0 * (L // 256) * n_jk * 256 * tn * L           # both axes, tiles actually multiplied
+        ratio, nominal = (4.0, 9000.0) if fp4 else (2.0, 4500.0)   # guide: dense fp4 / int8 : bf16
+        peak_t = ratio * float(measured_peaks()[2].get("bf16_tflops", 0.0)) or None
         tops = 2.0 * macs / (full_ms * 1e-3) / 1e12
-        tensor_roof = {"bound": "tensor", "kernel": "gram2_kernel (tcgen05 kind::i8, cta_group::2), whole ising_correlation(L/2) call",
-                       "achieved": tops, "peak": peak_t, "unit": "TOP/s (int8)",
-                       "frac": (tops / peak_t) if peak_t else None, "frac_of_nominal_4500": tops / 4500.0,
+        tensor_roof = {"bound": "tensor", "kernel": ("gram4_kernel (tcgen05 kind::mxf4, cta_group::2)" if fp4 else "gram2_kernel (tcgen05 kind::i8, cta_group::2)") + ", whole ising_correlation(L/2) call",
+                       "achieved": tops, "peak": peak_t, "unit": "TOP/s (fp4)" if fp4 else "TOP/s (int8)",
+                       "frac": (tops / peak_t) if peak_t else None, "frac_of_nominal": tops / nominal, "nominal_peak": nominal,
                        "traffic": None, "ms_per_call": full_ms,
-                       "peak_source": "2 x MEASURED_PEAKS.json bf16_tflops (nominal int8 : bf16 ratio)",
+                       "peak_source": f"{ratio:g} x MEASURED_PEAKS.json bf16_tflops (nominal ratio to bf16)",
                        "useful_pair_products": 2.0 * (L // 2) * L * L}
     sim.close()
     pipes = eng.bench_pipes(float(measured_peaks()[2].get("sm_max_mhz", 0.0))) if rank == 0 else {}

@@ -11,8 +11,9 @@
 // element added to the shared-memory bin of its diagonal j - i, bins flushed to the int64
 // result with one atomic per distance per tile).  Tile (I0, J0 = I0 + 256 k) holds the ordered
 // pairs (y = I0 + i, y + r = J0 + j): r = J0 - I0 + j - i, kept when 1 <= r <= rmax.
-// The default is the CTA-pair variant further down (gram2_kernel: cta_group::2, 256 x 256 tiles);
-// this single-CTA kernel stays selectable (ising_set_corr_path(h, 2)) and is tested against it.
+// The default is the fp4 CTA-pair variant further down (gram4_kernel: kind::mxf4, cta_group::2, 256 x 224
+// tiles); the int8 kernels stay selectable (ising_set_corr_path(h, 2): this single-CTA kernel, 3: gram2_kernel,
+// int8 CTA pairs) and are tested against it.
 #include "ising_internal.cuh"
 
 #include <cuda.h>
@@ -411,11 +412,16 @@ gram2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ G
 // ---------------------------------------------- fp4 variant (opt-in, path 4) ---
 // -1, 0, +1 are exact in e2m1, so the same Gram matrix can run at the fp4 rate: tcgen05.mma
 // kind::mxf4 (K = 64 per instruction, 128 smem bytes = 256 elements per stage), fp32 accumulators
-// (exact: |sum| <= elements per K chunk < 2^24), every block scale = 1.0.  TMEM: one 256-column
-// accumulator (columns 0..255) + the scale columns, so MMA and epilogue of consecutive tiles do not overlap.
+// (exact: |sum| <= elements per K chunk < 2^24), every block scale = 1.0.  TMEM must also hold the
+// scale columns, so the tile is 256 x 224: two 224-column accumulators (MMA and epilogue overlap) + 32
+// scale columns.  224 does not divide L: the matrix carries a replica of its first 256 rows behind
+// row L - 1, so a tile that starts below L never wraps.
 namespace {
 // block-scaled descriptor: a/b format E2M1 (1), scale format UE8M0 (bit 23), N >> 3 at bit 17, M >> 4 at bit 24
-constexpr uint32_t kInstrDescF4 = (1u << 7) | (1u << 10) | ((uint32_t)(256 >> 3) << 17) | (1u << 23) | ((uint32_t)(256 >> 4) << 24);
+constexpr int TN4 = 224;                                         // 2 x 224 accumulator columns + 32 scale columns <= 512
+constexpr int STAGE4_BYTES = HALF_BYTES + (TN4 / 2) * TKB, NBINS4 = TM + TN4 - 1;
+constexpr int SMEM4_BYTES = STAGES2 * STAGE4_BYTES + 1024 + 2048;
+constexpr uint32_t kInstrDescF4 = (1u << 7) | (1u << 10) | ((uint32_t)(TN4 >> 3) << 17) | (1u << 23) | ((uint32_t)(256 >> 4) << 24);
 __device__ __forceinline__ void umma_mxf4_2sm(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t accumulate, uint32_t tmem_sf)
 {
     asm volatile(
@@ -427,11 +433,12 @@ __device__ __forceinline__ void umma_mxf4_2sm(uint32_t tmem_d, uint64_t da, uint
 }  // namespace
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1)
-gram4_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ GramParams p)
+gram4_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_b,
+             const __grid_constant__ GramParams p)
 {
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-    uint8_t *tail = smem + STAGES2 * STAGE2_BYTES;
+    uint8_t *tail = smem + STAGES2 * STAGE4_BYTES;
     int *bins = reinterpret_cast<int *>(tail);
     uint64_t *full = reinterpret_cast<uint64_t *>(tail + 1536);             // [STAGES2]  (used on the leader)
     uint64_t *empty = full + STAGES2;                                       // [STAGES2]  (both CTAs)
@@ -453,7 +460,7 @@ gram4_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ G
         for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], 16); }   // 8 epilogue warps per CTA
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    for (int i = threadIdx.x; i < NBINS; i += blockDim.x) bins[i] = 0;
+    for (int i = threadIdx.x; i < NBINS4; i += blockDim.x) bins[i] = 0;
     cluster_sync_all();                                                      // barriers of both CTAs exist
     if (warp == 2) {
         asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
@@ -463,10 +470,10 @@ gram4_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ G
     cluster_sync_all();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem_base = *tmem_slot;
-    // scale factors: every block scale is 1.0 (ue8m0 byte 0x7F).  Columns 256..287 of all 128 lanes are
+    // scale factors: every block scale is 1.0 (ue8m0 byte 0x7F).  Columns 448..479 of all 128 lanes are
     // filled with that byte, so whichever bytes the instruction picks as SFA / SFB read as 1.0.
     if (warp >= 2 && warp < 6) {
-        const uint32_t sf = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + 256u;
+        const uint32_t sf = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(2 * TN4);
         asm volatile(
             "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
             "{%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, "
@@ -485,14 +492,14 @@ gram4_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ G
             for (int t = t_lo; t < t_hi; ++t) {
                 const int jk = t / p.n_ib, ib = t - jk * p.n_ib;
                 const int I0 = ib * 256 + (int)rank * TM;
-                int J0 = ib * 256 + jk * TN; if (J0 >= p.L) J0 -= p.L;      // multiple of 256: the tile never wraps
-                J0 += (int)rank * TM;
+                int J0 = ib * 256 + jk * TN4; if (J0 >= p.L) J0 -= p.L;     // rows J0 .. J0 + 223 may run past L - 1:
+                J0 += (int)rank * (TN4 / 2);                                //   the matrix carries a replica of its first 256 rows
                 for (int kb = 0; kb < n_kb; ++kb) {
                     mbar_wait(&empty[stage], phase ^ 1);
-                    if (leader) mbar_expect_tx(&full[stage], 2 * STAGE2_BYTES);   // bytes of both CTAs land on this barrier
-                    uint8_t *sa = smem + stage * STAGE2_BYTES, *sb = sa + HALF_BYTES;
+                    if (leader) mbar_expect_tx(&full[stage], 2 * STAGE4_BYTES);   // bytes of both CTAs land on this barrier
+                    uint8_t *sa = smem + stage * STAGE4_BYTES, *sb = sa + HALF_BYTES;
                     tma_load_2d_2sm(sa, &tmap, &full[stage], p.k0 + kb * TKB, I0);
-                    tma_load_2d_2sm(sb, &tmap, &full[stage], p.k0 + kb * TKB, J0);
+                    tma_load_2d_2sm(sb, &tmap_b, &full[stage], p.k0 + kb * TKB, J0);
                     if (!leader) mbar_arrive_remote(&full[stage], 0);
                     if (++stage == STAGES2) { stage = 0; phase ^= 1; }
                 }
@@ -502,38 +509,38 @@ gram4_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ G
         // ===== MMA issuer: leader CTA only =====
         if (leader && lane == 0) {
             int stage = 0; uint32_t phase = 0;
-            const int as = 0; uint32_t aphase = 0;                       // one accumulator: columns 256.. hold the scales
+            int as = 0; uint32_t aphase = 0;                             // two 224-column accumulators + the scale columns
             for (int t = t_lo; t < t_hi; ++t) {
                 mbar_wait(&tempty[as], aphase ^ 1);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const uint32_t d_tmem = tmem_base;
+                const uint32_t d_tmem = tmem_base + (uint32_t)(as * TN4);
                 for (int kb = 0; kb < n_kb; ++kb) {
                     mbar_wait(&full[stage], phase);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    const uint32_t sa = smem_u32(smem + stage * STAGE2_BYTES), sb = sa + HALF_BYTES;
+                    const uint32_t sa = smem_u32(smem + stage * STAGE4_BYTES), sb = sa + HALF_BYTES;
                     const uint64_t da = umma_desc(sa), db = umma_desc(sb);
 #pragma unroll
                     for (int k = 0; k < TKB / 32; ++k)
-                        umma_mxf4_2sm(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), (kb | k) ? 1u : 0u, tmem_base + 256u);
+                        umma_mxf4_2sm(d_tmem, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), (kb | k) ? 1u : 0u, tmem_base + (uint32_t)(2 * TN4));
                     umma_commit_2sm(&empty[stage]);
                     if (++stage == STAGES2) { stage = 0; phase ^= 1; }
                 }
                 umma_commit_2sm(&tfull[as]);
-                aphase ^= 1;
+                if (++as == 2) { as = 0; aphase ^= 1; }
             }
         }
     } else {
         // ===== epilogue (both CTAs, 8 warps: two per TMEM lane quarter, each half of the columns) =====
         const int q = warp & 3, row = q * 32 + lane, chalf = (warp - 2) >> 2;
         const int et = threadIdx.x - 64;
-        const int as = 0; uint32_t aphase = 0;
+        int as = 0; uint32_t aphase = 0;
         for (int t = t_lo; t < t_hi; ++t) {
             const int jk = t / p.n_ib;
             mbar_wait(&tfull[as], aphase);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16);
+            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * TN4);
 #pragma unroll 1
-            for (int c = chalf * (TN / 64); c < (chalf + 1) * (TN / 64); ++c) {
+            for (int c = chalf * 4; c < (chalf ? TN4 / 32 : 4); ++c) {       // 7 chunks of 32 columns: 4 + 3
                 uint32_t v[32];
                 asm volatile(
                     "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
@@ -553,11 +560,11 @@ gram4_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ G
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncwarp();
             if (lane == 0) { if (leader) mbar_arrive(&tempty[as]); else mbar_arrive_remote(&tempty[as], 0); }
-            aphase ^= 1;
+            if (++as == 2) { as = 0; aphase ^= 1; }
             if (t + 1 < t_hi && (t + 1) / p.n_ib == jk) continue;
             asm volatile("bar.sync 1, 256;" ::: "memory");
-            for (int b = et; b < NBINS; b += 256) {
-                const int r = jk * TN - (int)rank * TM + b - (TM - 1);
+            for (int b = et; b < NBINS4; b += 256) {
+                const int r = jk * TN4 - (int)rank * TM + b - (TM - 1);
                 const int v = bins[b];
                 bins[b] = 0;
                 if (r >= 1 && r <= p.rmax && v != 0)
@@ -600,12 +607,13 @@ __global__ void __launch_bounds__(256) expand_kernel(const uint64_t *__restrict_
 
 // out[y][32 q + i/2] nibble (i & 1) = e2m1 code of site x = 64 q + i: +1 -> 0x2, -1 -> 0xA, 0 -> 0x0
 __global__ void __launch_bounds__(256) expand_fp4_kernel(const uint64_t *__restrict__ sg, const uint64_t *__restrict__ nz,
-                                                         uint8_t *__restrict__ out, int64_t n_words)
+                                                         uint8_t *__restrict__ out, int64_t n_words, int64_t words_per_row)
 {
     const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (w >= n_words) return;
     const uint64_t s = sg[w], z = nz ? nz[w] : ~0ull;
     uint4 *o = reinterpret_cast<uint4 *>(out + w * 32);
+    uint4 *o_rep = (w < 256 * words_per_row) ? reinterpret_cast<uint4 *>(out + (n_words + w) * 32) : nullptr;   // rows 0..255 again behind row L - 1
 #pragma unroll
     for (int c = 0; c < 2; ++c) {
         uint32_t v[4];
@@ -621,6 +629,7 @@ __global__ void __launch_bounds__(256) expand_fp4_kernel(const uint64_t *__restr
             v[k] = word;
         }
         o[c] = make_uint4(v[0], v[1], v[2], v[3]);
+        if (o_rep) o_rep[c] = make_uint4(v[0], v[1], v[2], v[3]);
     }
 }
 
@@ -663,14 +672,22 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
     cudaError_t ea = cudaFuncSetAttribute(gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (ea != cudaSuccess) return ea;
     CUtensorMap tmap;
-    const int row_bytes = (h->corr_path == 4) ? L / 2 : L;      // fp4: two elements per byte
-    const cuuint64_t gdim[2] = {(cuuint64_t)row_bytes, (cuuint64_t)L};
+    const bool fp4_layout = h->corr_path == 0 || h->corr_path == 4;
+    const int row_bytes = fp4_layout ? L / 2 : L;               // fp4: two elements per byte
+    const cuuint64_t gdim[2] = {(cuuint64_t)row_bytes, (cuuint64_t)(fp4_layout ? L + 256 : L)};
     const cuuint64_t gstride[1] = {(cuuint64_t)row_bytes};
     const cuuint32_t box[2] = {(cuuint32_t)TKB, (cuuint32_t)TM};
     const cuuint32_t estr[2] = {1, 1};
     if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, h->gram, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return cudaErrorInvalidValue;
+    CUtensorMap tmap_b = tmap;                         // fp4 path: 112-row boxes for the B halves
+    if (fp4_layout) {
+        const cuuint32_t box_b[2] = {(cuuint32_t)TKB, (cuuint32_t)(TN4 / 2)};
+        if (enc(&tmap_b, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, h->gram, gdim, gstride, box_b, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return cudaErrorInvalidValue;
+    }
     int dev = 0, n_sm = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
@@ -681,20 +698,17 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
     // is the optimum for both kernels; 512 pays more epilogues, 2048 falls out of L2)
     int kc = (int)(((64ll << 20) / L) / TKB * TKB);
     if (kc < 4 * TKB) kc = 4 * TKB;
-    if (h->corr_path == 4) {                          // fp4, one accumulator buffer: fewer, longer tiles pay (measured: 96 MB slab)
-        kc = (int)(((96ll << 20) / L) / TKB * TKB);
-        if (kc < 4 * TKB) kc = 4 * TKB;
-    }
     if (kc > row_bytes) kc = row_bytes;
     p.n_kb = kc / TKB;
-    const bool fp4 = h->corr_path == 4;               // opt-in: kind::mxf4 on a packed e2m1 matrix (L/2 bytes per row)
+    const bool fp4 = h->corr_path == 0 || h->corr_path == 4;   // default: kind::mxf4 on a packed e2m1 matrix (L/2 bytes per row)
     const bool pair = h->corr_path != 2;              // default: cta_group::2 kernel, 256-row tiles; path 2 = single-CTA kernel
     if (pair) {
         ea = cudaFuncSetAttribute(gram2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM2_BYTES);
-        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(gram4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM2_BYTES);
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(gram4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM4_BYTES);
         if (ea != cudaSuccess) return ea;
         p.n_ib = L / 256;
         p.n_jk = (int)((count + 256 + TN - 1) / TN);      // columns I0 .. I0 + 255 + rmax
+        if (fp4) p.n_jk = (int)((count + 256 + TN4 - 1) / TN4);
     }
     const int n_tiles = p.n_ib * p.n_jk;
     int grid = n_tiles < n_sm ? n_tiles : n_sm;
@@ -705,14 +719,14 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
         long long *out = axis ? dev_sx : dev_sy;
         cudaError_t e = cudaMemsetAsync(out, 0, count * sizeof(long long), h->stream);
         if (e != cudaSuccess) return e;
-        if (fp4) expand_fp4_kernel<<<(unsigned)((pw + 255) / 256), 256, 0, h->stream>>>(sg, nz, reinterpret_cast<uint8_t *>(h->gram), (int64_t)pw);
+        if (fp4) expand_fp4_kernel<<<(unsigned)((pw + 255) / 256), 256, 0, h->stream>>>(sg, nz, reinterpret_cast<uint8_t *>(h->gram), (int64_t)pw, (int64_t)Wq);
         else expand_kernel<<<(unsigned)((pw + 255) / 256), 256, 0, h->stream>>>(sg, nz, h->gram, (int64_t)pw);
         p.out = out;
         h->launches++;
         for (int k0 = 0; k0 < row_bytes; k0 += kc) {
             p.k0 = k0;
             p.n_kb = (row_bytes - k0 < kc ? row_bytes - k0 : kc) / TKB;
-            if (fp4) gram4_kernel<<<grid, 320, SMEM2_BYTES, h->stream>>>(tmap, p);
+            if (fp4) gram4_kernel<<<grid, 320, SMEM4_BYTES, h->stream>>>(tmap, tmap_b, p);
             else if (pair) gram2_kernel<<<grid, 192, SMEM2_BYTES, h->stream>>>(tmap, p);
             else gram_kernel<<<grid, 192, SMEM_BYTES, h->stream>>>(tmap, p);
             h->launches++;
