@@ -90,8 +90,11 @@ def test_config2_ising_L2p18_windows_and_observables(eng):
         assert o.M == M
         sx, sy = sim.correlation_list(1, [1, 2])                   # independent kernels (bit planes)
         assert int(sx[0]) + int(sy[0]) == o.bond_sum               # S_x(1) + S_y(1) = B
-        sim.set_corr_path(2)                                       # tensor cores at L = 2^18 (69 GB int8 matrix)
+        sim.set_corr_path(4)                                       # tensor cores at L = 2^18 (34 GB e2m1 matrix)
         tx, ty = sim.correlation(1024)
+        sim.set_corr_path(3)                                       # int8 CTA pairs (69 GB int8 matrix)
+        ix, iy = sim.correlation(1024)
+        assert (tx == ix).all() and (ty == iy).all()
         sim.set_corr_path(1)                                       # XOR + POPC kernels
         bx, by = sim.correlation(1024)
         assert (tx == bx).all() and (ty == by).all()
