@@ -105,8 +105,8 @@ int ising_correlation(ising_t *h, int64_t rmax, int64_t *sx, int64_t *sy);
  * rmax >= 512 and L is a multiple of 256; bit planes otherwise), 1 = bit planes (XOR + POPC),
  * 2 = tensor cores, int8, one CTA per 128 x 256 tile, 3 = int8, CTA pairs (cta_group::2, 256 x 256
  * tiles), 4 = CTA pairs at the fp4 rate (e2m1 matrix, kind::mxf4 with unit block scales, 256 x 224
- * tiles, fp32 accumulation of exact integers).  Paths 2-4 need L % 256 == 0 and allocate L*L
- * bytes on first use.  The results are identical integers in every case.                    */
+ * tiles, fp32 accumulation of exact integers).  Paths 2-4 need L % 256 == 0 and allocate the
+ * spin matrix on first use (L*L bytes for int8, about L*L/2 for fp4).  The results are identical integers in every case.                    */
 int ising_set_corr_path(ising_t *h, int path);
 
 /* The paper's down-sampled protocol at t = sweeps_done:

@@ -647,6 +647,7 @@ static int ensure_gram(ising_sim *h)
 {
     const size_t bytes = corr_gram_bytes(h);
     if (h->gram_bytes >= bytes) return ISING_OK;
+    if (h->gram) { cudaFree(h->gram); h->gram = nullptr; h->gram_bytes = 0; }
     cudaError_t e = cudaMalloc((void **)&h->gram, bytes);
     if (e != cudaSuccess) { cudaGetLastError(); h->gram = nullptr; return set_error(ISING_ENOMEM, "int8 spin matrix: cudaMalloc failed"); }
     h->gram_bytes = bytes;

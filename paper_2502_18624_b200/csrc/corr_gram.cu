@@ -644,7 +644,12 @@ bool corr_gram_supported(const ising_sim *h, int64_t rmax)
     return (h->L % 256) == 0 && h->L >= 512 && rmax >= 1;
 }
 
-size_t corr_gram_bytes(const ising_sim *h) { return (size_t)h->L * (size_t)h->L; }
+// int8 paths: L x L bytes; fp4 path: (L + 256) rows of L / 2 bytes (replica of the first 256 rows)
+size_t corr_gram_bytes(const ising_sim *h)
+{
+    const bool fp4 = h->corr_path == 0 || h->corr_path == 4;
+    return fp4 ? (size_t)(h->L + 256) * (size_t)(h->L / 2) : (size_t)h->L * (size_t)h->L;
+}
 
 // S_y (planes sg/nz) and S_x (transposed planes) for r = 1..count via the int8 Gram kernel.
 // dev_sx / dev_sy receive the pair sums themselves (no popcount conversion needed).
