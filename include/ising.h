@@ -162,8 +162,9 @@ int ising_thresholds(ising_t *h, uint64_t *out, int cap, int *count);
  * cf. PAPER.md:193): rows walked per thread and threads per block
  * (multiple of 32, <= 1024).  0 keeps the current value.                    */
 int ising_set_launch(ising_t *h, int rows_per_thread, int block_threads);
-/* Update kernel variant (0 = default: carry-chain compare, bucket table for the
- * LUT model; 1 = compare/select, binary search; equivalent implementations
+/* Update kernel variant (0 = default: carry-chain compare; for the LUT model the
+ * bucket table at L >= 8192 and the binary search below; 1 = compare/select,
+ * binary search; 2 (LUT model only) = bucket table; equivalent implementations
  * kept for parity / performance comparison).                                */
 int ising_set_variant(ising_t *h, int variant);
 

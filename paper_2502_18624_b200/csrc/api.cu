@@ -402,7 +402,7 @@ extern "C" int ising_set_launch(ising_t *h, int rows_per_thread, int block_threa
 extern "C" int ising_set_variant(ising_t *h, int variant)
 {
     if (!h) return set_error(ISING_EINVAL, "ising_set_variant: NULL handle");
-    if (variant < 0 || variant > 1) return set_error(ISING_EINVAL, "ising_set_variant: unknown variant");
+    if (variant < 0 || variant > (h->model == ISING_MODEL_ISING_LUT ? 2 : 1)) return set_error(ISING_EINVAL, "ising_set_variant: unknown variant");
     h->variant = variant;
     return ISING_OK;
 }

@@ -276,7 +276,11 @@ cudaError_t launch_lut_update(ising_sim *h, int colour, uint32_t t)
     p.tally = h->d_acc + 40;
     p.t_base = reinterpret_cast<const uint32_t *>(h->d_acc + 48) + (h->graph_capture ? 1 : 0);
 #define LUT_LAUNCH(C, V, T, SM) lut_update_kernel<C, V, T><<<grid, block, SM, h->stream>>>(p)
-    if (h->variant == 0) {
+    // variant 0 = automatic: the bucket table pays once its 32 KB fill per block is amortised over several
+    // waves (L >= 8192); a single-wave launch starts faster with the table-free binary search.
+    // 1 = binary search, 2 = bucket table
+    const bool bucket = h->variant == 2 || (h->variant == 0 && h->L >= 8192);
+    if (bucket) {
         // per launch: the attribute is per device, and a process may drive several devices
         cudaError_t ea = cudaFuncSetAttribute(lut_update_kernel<0, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (ea == cudaSuccess) ea = cudaFuncSetAttribute(lut_update_kernel<1, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -44,6 +44,7 @@ def test_lattice_and_observables_every_sweep(eng, L, beta, seed, n):
     s = oracle.lut_init(L, seed)
     tl = oracle.observables(s)
     with eng.IsingSim(LUT, L, beta, 0.0, seed) as sim:
+        sim.set_variant(2)                                   # the bucket-table kernel (automatic from L = 8192)
         assert (sim.read_lattice() == s).all()
         for t in range(n):
             sim.sweep(1)
@@ -65,13 +66,13 @@ def test_lattice_and_observables_every_sweep(eng, L, beta, seed, n):
 
 @pytest.mark.parametrize("beta", [wl.BETA_C / 0.9, wl.BETA_C / 0.5, 1.2, 2.5, 0.01])
 def test_bucket_table_and_binary_search_variants_agree(eng, beta):
-    """Variant 0 (bucket table + rare binary-search fallback; low temperatures have buckets with several
-    thresholds) and variant 1 (binary search only) against the oracle."""
+    """Variant 2 (bucket table + rare binary-search fallback; low temperatures have buckets with several
+    thresholds), variant 1 (binary search only) and the automatic choice against the oracle."""
     L, seed, n = 512, 13, 5
     s = oracle.lut_init(L, seed)
     for t in range(n):
         oracle.lut_sweep(s, beta, seed, t)
-    for variant in (0, 1):
+    for variant in (2, 1, 0):
         with eng.IsingSim(LUT, L, beta, 0.0, seed) as sim:
             sim.set_variant(variant)
             sim.sweep(n)
