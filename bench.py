@@ -49,6 +49,8 @@ PHILOX_SLOTS_PER_SITE = 9.25   # (18 IMAD.WIDE + 19 LOP3) / 4 sites, rounds 1-2 
 # BASELINE.md Sec. 1 (the paper's single-GPU maxima, GB200, other machine: context): the 1-bit LUT Ising kernel
 # at L = 2^20 and the 4-bit Blume-Capel kernel at L = 2^19.  No published number exists for the north_star
 # contract (4-bit Ising, one number per spin), so the default workload reports vs_baseline = null.
+MODEL_IDS = {"ising": wl.ISING, "bc": wl.BLUME_CAPEL, "lut": wl.ISING_LUT, "bc2": wl.BLUME_CAPEL_2BIT}
+BITS_PER_SITE = {wl.ISING: 4, wl.BLUME_CAPEL: 4, wl.ISING_LUT: 1, wl.BLUME_CAPEL_2BIT: 2}
 PAPER_UPDATES_PER_NS = {("lut", 1 << 20): 1802.0, ("bc", 1 << 19): 948.0}
 
 
@@ -59,7 +61,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--L", type=int, default=0, help="override the lattice size (default: configs[2], 2^18)")
-    ap.add_argument("--model", default="ising", choices=["ising", "bc", "lut"],
+    ap.add_argument("--model", default="ising", choices=["ising", "bc", "lut", "bc2"],
                     help="ising / bc: the north_star kernels (configs[2] / [3]); lut: NEXT-2, the paper's 1-bit look-up-table kernel on configs[2]'s parameters")
     ap.add_argument("--sweeps-per-step", type=int, default=10)
     ap.add_argument("--workload", default="sweep", choices=["sweep", "corr"],
@@ -77,7 +79,7 @@ def parse_args():
 
 
 def pick_workload(args):
-    base = wl.config(3) if args.model == "bc" else wl.config(2)
+    base = wl.config(3) if args.model in ("bc", "bc2") else wl.config(2)
     if getattr(args, "workload", "sweep") == "corr":
         base = wl.config(4)
     L = args.L or base.L
@@ -86,6 +88,8 @@ def pick_workload(args):
         name = f"ising_1bit_lut_L{L}_0.9Tc" + ("_paper_single_gpu_max" if L == (1 << 20) else "")
     if args.model == "bc" and L == (1 << 19):
         name = "bc_L524288_D1_paper_single_gpu_max"
+    if args.model == "bc2":          # NEXT-3: the same Blume-Capel run stored at 2 bits per spin
+        name = f"bc_2bit_L{L}_D1"
     return base, L, name
 
 
@@ -166,7 +170,7 @@ def run_reference(args):
     if rank != 0:
         return
     base, L, name = pick_workload(args)
-    model = {"ising": wl.ISING, "bc": wl.BLUME_CAPEL, "lut": wl.ISING_LUT}[args.model]
+    model = MODEL_IDS[args.model]
     per_step = max(1.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
     vals, info, cores = [], "", 0
     for i in range(args.warmup + args.steps):
@@ -227,7 +231,7 @@ def mem_available_bytes() -> int:
 def run_e2e(eng, torch, model, L, beta, D, seed, S, steps, device):
     """End to end through the C ABI with HOST buffers: per step upload both packed
     colour arrays from pinned host memory, run S sweeps, read the observables."""
-    per_colour = 16 if model == wl.ISING_LUT else 4            # sites per byte... L*L / per_colour bytes per colour array
+    per_colour = 16 // BITS_PER_SITE[model]                    # L*L / per_colour bytes per colour array
     colour_bytes = L * L // per_colour
     need = 2 * colour_bytes
     note = ""
@@ -302,7 +306,7 @@ def run_ours(args):
     torch.cuda.set_device(device)
 
     base, L, name = pick_workload(args)
-    model = {"ising": wl.ISING, "bc": wl.BLUME_CAPEL, "lut": wl.ISING_LUT}[args.model]
+    model = MODEL_IDS[args.model]
     S, K, W = args.sweeps_per_step, args.steps, max(args.warmup, 0)
     sim = eng.IsingSim(model, L, base.beta, base.D, replica_seed(base.seed, rank), device=device)
     if args.rows_per_thread or args.block:
@@ -359,7 +363,7 @@ def run_ours(args):
         torch.cuda.synchronize(device)
         philox_ms = ev[0].elapsed_time(ev[1]) / n_roof
         copy_ms = ev[1].elapsed_time(ev[2]) / n_roof
-    bytes_per_site = 0.375 if lut else BYTES_PER_SITE_LAUNCH   # 3 x 1 bit or 3 x 4 bits per updated site
+    bytes_per_site = BYTES_PER_SITE_LAUNCH * BITS_PER_SITE[model] / 4   # 3 x (bits per site) per updated site
     slots_per_site = PHILOX_SLOTS_PER_SITE / 2 if lut else PHILOX_SLOTS_PER_SITE   # LUT: half a number per site
     tensor_roof = None
     if args.workload == "corr" and rank == 0:
@@ -419,7 +423,7 @@ def run_ours(args):
                    "step": "S sweeps + observables" if args.workload == "sweep" else "S sweeps + correlation protocol + observables",
                    "launch": {"rows_per_thread": args.rows_per_thread or "default", "block": args.block or "default",
                               "variant": args.variant, "fused_tally": bool(args.tally), "corr_path": args.corr_path},
-                   "lattice_bytes": L * L // (8 if model == wl.ISING_LUT else 2), "l2": "inputs larger than L2 (no flush needed)" if L * L // 2 > (256 << 20)
+                   "lattice_bytes": L * L * BITS_PER_SITE[model] // 8, "l2": "inputs larger than L2 (no flush needed)" if L * L // 2 > (256 << 20)
                    else "lattice fits L2: DRAM figures not meaningful", "parallelism": f"replicas x{world}"},
         "measurement_ms_per_step": (total_ms - sweep_ms) / K,
         "sweep_only_updates_per_ns": world * L * L * S * K / (sweep_ms * 1e6),

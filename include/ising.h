@@ -38,7 +38,9 @@ extern "C" {
 typedef struct ising_sim ising_t; /* opaque */
 
 enum { ISING_MODEL_ISING = 0, ISING_MODEL_BLUME_CAPEL = 1,
-       ISING_MODEL_ISING_LUT = 2 /* the paper's own kernel: 1 bit per spin, look-up-table random bits */ };
+       ISING_MODEL_ISING_LUT = 2, /* the paper's own kernel: 1 bit per spin, look-up-table random bits */
+       ISING_MODEL_BLUME_CAPEL_2BIT = 3 /* Blume-Capel stored at 2 bits per spin, expanded to nibbles in
+                                           registers: the same trajectory and results as ISING_MODEL_BLUME_CAPEL in half the memory */ };
 enum { ISING_OK = 0, ISING_EINVAL = -1, ISING_ENOMEM = -2, ISING_ECUDA = -3 };
 
 /* Integer observables are the bit-exact contract; the doubles are formed on
@@ -54,8 +56,8 @@ typedef struct {
 } ising_obs_t;
 
 /* Device bytes a caller-provided buffer must have for (model, L): the two
- * colour arrays (L*L/2 bytes) plus a small fixed scratch area.  0 if (model, L)
- * is invalid.                                                               */
+ * colour arrays (L*L/2 bytes at 4 bits per spin, L*L/4 at 2 bits, L*L/8 at 1 bit)
+ * plus a small fixed scratch area.  0 if (model, L) is invalid.             */
 size_t ising_workspace_bytes(int model, int64_t L);
 
 /* Create a simulation (PAPER.md:25 problem statement; Eq. 1 / Eq. 2).
@@ -63,7 +65,9 @@ size_t ising_workspace_bytes(int model, int64_t L);
  *   L           linear size, multiple of 64, >= 64 (one 128-bit vector = 32
  *               same-colour sites of a row); ISING_MODEL_ISING_LUT stores one
  *               bit per spin (128 sites per vector): multiple of 256, >= 256,
- *               colour array = L rows x (L / 128) uint64 words, bit 1 = spin +1
+ *               colour array = L rows x (L / 128) uint64 words, bit 1 = spin +1;
+               ISING_MODEL_BLUME_CAPEL_2BIT: L rows x (L / 64) uint64 words, site j
+               of a word at bits 2j..2j+1, code = spin + 1
  *   beta        1/(k_B T) >= 0, finite;  D = crystal field Delta of Eq. 2
  *               (finite; ignored for Ising);  seed = Philox key
  *   dev_buf     device memory of >= ising_workspace_bytes() bytes, 256-byte

@@ -8,7 +8,7 @@ from dataclasses import dataclass
 
 import numpy as np
 
-ISING, BLUME_CAPEL, ISING_LUT = 0, 1, 2
+ISING, BLUME_CAPEL, ISING_LUT, BLUME_CAPEL_2BIT = 0, 1, 2, 3
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libising_b200.so")
 _lib = None
@@ -255,7 +255,7 @@ class IsingSim:
         _check(self._lib.ising_write_lattice(self._h, y0, spins.shape[0], spins.ctypes.data))
 
     def read_packed(self, colour: int, word0: int = 0, nwords: int | None = None, out=None):
-        total = self.L * (self.L // (128 if self.model == ISING_LUT else 32))
+        total = self.L * (self.L // {ISING_LUT: 128, BLUME_CAPEL_2BIT: 64}.get(self.model, 32))
         nwords = total - word0 if nwords is None else nwords
         if out is None:
             out = np.empty(nwords, dtype=np.uint64)

@@ -32,15 +32,14 @@ static void drop_graph(ising_sim *h);
 static bool valid_model_L(int model, int64_t L)
 {
     if (model == ISING_MODEL_ISING_LUT) return L >= 256 && (L % 256) == 0 && L <= (1ll << 20);   // 128-bit vector = 128 sites
-    return (model == ISING_MODEL_ISING || model == ISING_MODEL_BLUME_CAPEL) && L >= 64 && (L % 64) == 0 &&
+    return (model == ISING_MODEL_ISING || is_blume_capel(model)) && L >= 64 && (L % 64) == 0 &&
            L <= (1ll << 20);
 }
 
 extern "C" size_t ising_workspace_bytes(int model, int64_t L)
 {
     if (!valid_model_L(model, L)) return 0;
-    if (model == ISING_MODEL_ISING_LUT) return (size_t)L * (size_t)L / 8 + kScratchBytes;   // 1 bit per spin
-    return (size_t)L * (size_t)L / 2 + kScratchBytes;
+    return (size_t)L * (size_t)L / (size_t)sites_per_word(model) * 8 + kScratchBytes;   // both colour arrays
 }
 
 // ------------------------------------------------------------ thresholds ---
@@ -126,7 +125,7 @@ extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_
 {
     if (!out) return set_error(ISING_EINVAL, "ising_create: out is NULL");
     if (!valid_model_L(model, L))
-        return set_error(ISING_EINVAL, "ising_create: model must be 0/1 and L a multiple of 64 in [64, 2^20]");
+        return set_error(ISING_EINVAL, "ising_create: unknown model, or L not a multiple of 64 (256 for the LUT model) in [64, 2^20]");
     if (!(beta >= 0.0) || !isfinite(beta)) return set_error(ISING_EINVAL, "ising_create: beta must be finite and >= 0");
     if (!isfinite(D)) return set_error(ISING_EINVAL, "ising_create: D must be finite");
     const size_t need = ising_workspace_bytes(model, L);
@@ -135,7 +134,7 @@ extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_
 
     ising_sim *h = new (std::nothrow) ising_sim();
     if (!h) return set_error(ISING_ENOMEM, "ising_create: host allocation failed");
-    h->model = model; h->L = L; h->beta = beta; h->D = (model == ISING_MODEL_BLUME_CAPEL) ? D : 0.0; h->seed = seed;
+    h->model = model; h->L = L; h->beta = beta; h->D = is_blume_capel(model) ? D : 0.0; h->seed = seed;
     h->stream = (cudaStream_t)cuda_stream;
     char *base = (char *)dev_buf;
     if (!base) {
@@ -148,7 +147,7 @@ extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_
         }
         base = (char *)h->owned;
     }
-    const size_t colour_bytes = (model == ISING_MODEL_ISING_LUT) ? (size_t)L * (size_t)L / 16 : (size_t)L * (size_t)L / 4;
+    const size_t colour_bytes = (size_t)L * (size_t)L / (size_t)sites_per_word(model) * 4;
     h->lat[0] = (uint64_t *)base;
     h->lat[1] = (uint64_t *)(base + colour_bytes);
     h->d_acc = (long long *)(base + 2 * colour_bytes);                 // 64 int64 = 512 B (+ 4 KiB sink area unused)
@@ -162,7 +161,7 @@ extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_
     }
     cudaError_t e = cudaMallocHost(&h->h_acc, 256 * sizeof(long long));
     if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "cudaMallocHost"); }
-    if (model == ISING_MODEL_BLUME_CAPEL) {
+    if (is_blume_capel(model)) {
         // [0, 66): thresholds clamped to 2^32-1 + "always" bit mask (compare/select variant).
         // [80, 80 + 132): carry form for the default variant, two halves of 66 words (264 bytes):
         // C[b][16 code + S] = 2^32 - T, 0 for T = 2^32 (never a carry -> always accepted).  T = 0 has
@@ -420,7 +419,7 @@ extern "C" int ising_observables(ising_t *h, ising_obs_t *out)
     o.bond_sum = h->h_acc[0]; o.M = h->h_acc[1]; o.Q = lut ? h->L * h->L : h->h_acc[2];
     o.n_sites = h->L * h->L; o.sweeps_done = h->t;
     const double N = (double)h->L * (double)h->L;
-    o.E = (h->model != ISING_MODEL_BLUME_CAPEL) ? -(double)o.bond_sum : -(double)o.bond_sum + h->D * (double)o.Q;
+    o.E = !is_blume_capel(h->model) ? -(double)o.bond_sum : -(double)o.bond_sum + h->D * (double)o.Q;
     o.e_per_site = o.E / N;
     o.m_per_site = (double)o.M / N;
     o.zero_density = (double)(o.n_sites - o.Q) / N;
@@ -451,7 +450,7 @@ static void fill_obs(const ising_sim *h, const long long *bmq, ising_obs_t *o)
     o->bond_sum = bmq[0]; o->M = bmq[1]; o->Q = (lut || h->model == ISING_MODEL_ISING) ? h->L * h->L : bmq[2];
     o->n_sites = h->L * h->L; o->sweeps_done = h->t;
     const double N = (double)h->L * (double)h->L;
-    o->E = (h->model != ISING_MODEL_BLUME_CAPEL) ? -(double)o->bond_sum : -(double)o->bond_sum + h->D * (double)o->Q;
+    o->E = !is_blume_capel(h->model) ? -(double)o->bond_sum : -(double)o->bond_sum + h->D * (double)o->Q;
     o->e_per_site = o->E / N;
     o->m_per_site = (double)o->M / N;
     o->zero_density = (double)(o->n_sites - o->Q) / N;
@@ -580,7 +579,7 @@ extern "C" int ising_write_packed(ising_t *h, int colour, int64_t word0, int64_t
 static int ensure_planes(ising_sim *h)
 {
     const size_t pw = (size_t)h->L * (size_t)(h->L / 64);
-    const size_t bytes = pw * 8 * (h->model != ISING_MODEL_BLUME_CAPEL ? 2 : 4);
+    const size_t bytes = pw * 8 * (is_blume_capel(h->model) ? 4 : 2);
     if (h->planes_bytes >= bytes) return ISING_OK;
     cudaError_t e = cudaMalloc((void **)&h->planes, bytes);
     if (e != cudaSuccess) { cudaGetLastError(); h->planes = nullptr; return set_error(ISING_ENOMEM, "bit planes: cudaMalloc failed"); }
@@ -591,7 +590,7 @@ static int ensure_planes(ising_sim *h)
 static int ensure_comb(ising_sim *h, int64_t stride)
 {
     const size_t bytes = (size_t)h->L * (size_t)comb_words_per_row(h->L, stride) * 8 *
-                         (h->model != ISING_MODEL_BLUME_CAPEL ? 2 : 4);
+                         (is_blume_capel(h->model) ? 4 : 2);
     if (h->comb_bytes >= bytes) return ISING_OK;
     if (h->comb) { cudaFree(h->comb); h->comb = nullptr; h->comb_bytes = 0; }
     cudaError_t e = cudaMalloc((void **)&h->comb, bytes);
@@ -635,7 +634,7 @@ static int run_corr(ising_sim *h, int64_t stride, int64_t count, const int64_t *
     CUDA_TRY(cudaMemcpyAsync(sx, d_sx, (size_t)count * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaMemcpyAsync(sy, d_sy, (size_t)count * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
-    if (h->model != ISING_MODEL_BLUME_CAPEL) {   // popcount of unequal pairs -> pair sum
+    if (!is_blume_capel(h->model)) {   // popcount of unequal pairs -> pair sum
         const int64_t s = stride > 0 ? stride : 1;
         const int64_t n_src = (h->L / s) * (h->L / s);
         for (int64_t i = 0; i < count; ++i) { sx[i] = n_src - 2 * sx[i]; sy[i] = n_src - 2 * sy[i]; }

@@ -657,7 +657,7 @@ cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, lon
 {
     const int L = (int)h->L, Wq = L / 64;
     const size_t pw = (size_t)L * Wq;
-    const bool ising = h->model != ISING_MODEL_BLUME_CAPEL;
+    const bool ising = !is_blume_capel(h->model);
     const int np = ising ? 1 : 2;
     EncodeTiledFn enc = encode_tiled();
     if (!enc) return cudaErrorNotSupported;

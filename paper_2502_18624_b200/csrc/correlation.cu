@@ -153,7 +153,7 @@ cudaError_t launch_corr(ising_sim *h, int64_t stride, int64_t count, const long 
 {
     const int L = (int)h->L, Wq = L / 64;
     const size_t pw = (size_t)L * Wq;
-    const bool ising = h->model != ISING_MODEL_BLUME_CAPEL;
+    const bool ising = !is_blume_capel(h->model);
     const int np = ising ? 1 : 2;
     const uint64_t *sg = h->planes, *nz = ising ? nullptr : h->planes + pw;
     const uint64_t *sgT = h->planes + np * pw, *nzT = ising ? nullptr : h->planes + (np + 1) * pw;

@@ -60,11 +60,14 @@ int cuda_fail(cudaError_t e, const char *what);
 
 static inline int64_t words_per_row(int64_t L) { return L / 32; }              // uint64 per colour row
 static inline int64_t words_per_colour(int64_t L) { return L * (L / 32); }
-// uint64 words of one colour array: 16 sites per word (4 bits each), or 64 for the 1-bit LUT model
-static inline int64_t colour_words(const ising_sim *h)
+static inline bool is_blume_capel(int model) { return model == ISING_MODEL_BLUME_CAPEL || model == ISING_MODEL_BLUME_CAPEL_2BIT; }
+// same-colour sites per uint64 word: 16 (4 bits each), 32 (2-bit Blume-Capel), 64 (1-bit LUT model)
+static inline int64_t sites_per_word(int model)
 {
-    return h->model == ISING_MODEL_ISING_LUT ? h->L * (h->L / 128) : h->L * (h->L / 32);
+    return model == ISING_MODEL_ISING_LUT ? 64 : model == ISING_MODEL_BLUME_CAPEL_2BIT ? 32 : 16;
 }
+// uint64 words of one colour array
+static inline int64_t colour_words(const ising_sim *h) { return h->L * (h->L / (2 * sites_per_word(h->model))); }
 // 64-bit words per row of a plane down-sampled to the bits x % stride == 0 (zero padded)
 static inline int64_t comb_words_per_row(int64_t L, int64_t stride) { return (L / stride + 63) / 64; }
 

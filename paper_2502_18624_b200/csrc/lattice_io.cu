@@ -23,6 +23,11 @@ __global__ void __launch_bounds__(256) unpack_kernel(const __grid_constant__ Unp
         p.out[idx] = (int8_t)(2 * (int)((word >> (k & 63)) & 1u) - 1);
         return;
     }
+    if (p.model == ISING_MODEL_BLUME_CAPEL_2BIT) {           // 2 bits per spin, 32 sites per word
+        uint64_t word = p.lat[c][y * (p.L / 64) + (k >> 5)];
+        p.out[idx] = (int8_t)((int)((word >> (2 * (k & 31))) & 3u) - 1);
+        return;
+    }
     uint64_t word = p.lat[c][y * (p.L / 32) + (k >> 4)];
     int nib = (int)((word >> (4 * (k & 15))) & 15u);
     p.out[idx] = (int8_t)(p.model == ISING_MODEL_ISING ? 2 * nib - 1 : nib - 1);
@@ -48,10 +53,11 @@ struct PackParams {
     int *bad;
 };
 
-// one thread per 32-bit half (8 same-colour sites) of rows [y0, y0 + ny)
+// one thread per 32-bit half (8 same-colour sites; 16 in the 2-bit layout) of rows [y0, y0 + ny)
 __global__ void __launch_bounds__(256) pack_kernel(const __grid_constant__ PackParams p)
 {
-    const int64_t halves_per_row = p.L / 16;
+    const int sites = p.model == ISING_MODEL_BLUME_CAPEL_2BIT ? 16 : 8, bits = 32 / sites;
+    const int64_t halves_per_row = p.L / (2 * sites);
     int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= p.ny * halves_per_row * 2) return;
     int c = (int)(idx & 1);
@@ -61,14 +67,13 @@ __global__ void __launch_bounds__(256) pack_kernel(const __grid_constant__ PackP
     int par = (int)((y + c) & 1);
     uint32_t w = 0;
     bool bad = false;
-#pragma unroll
-    for (int j = 0; j < 8; ++j) {
-        int64_t x = 2 * (hf * 8 + j) + par;
+    for (int j = 0; j < sites; ++j) {
+        int64_t x = 2 * (hf * sites + j) + par;
         int v = p.in[row * p.L + x];
         uint32_t nib;
         if (p.model == ISING_MODEL_ISING) { bad |= (v != 1 && v != -1); nib = (v > 0) ? 1u : 0u; }
         else { bad |= (v < -1 || v > 1); nib = (uint32_t)(v + 1) & 3u; }
-        w |= nib << (4 * j);
+        w |= nib << (bits * j);
     }
     if (bad) atomicOr(p.bad, 1);
     if (!p.dry) p.lat[c][y * halves_per_row + hf] = w;
@@ -105,7 +110,7 @@ cudaError_t launch_pack(ising_sim *h, int64_t y0, int64_t ny, const int8_t *dev_
     p.lat[1] = reinterpret_cast<uint32_t *>(h->lat[1]);
     p.L = h->L; p.y0 = y0; p.ny = ny; p.model = h->model; p.dry = !write; p.in = dev_in; p.bad = dev_bad;
     const bool lut = h->model == ISING_MODEL_ISING_LUT;
-    int64_t n = ny * (lut ? h->L / 64 : h->L / 16) * 2;
+    int64_t n = ny * (h->L / sites_per_word(h->model)) * 2;      // 32-bit halves of both colours
     cudaError_t e;
     if (!write) {
         e = cudaMemsetAsync(dev_bad, 0, sizeof(int), h->stream);
@@ -140,6 +145,17 @@ __device__ __forceinline__ uint32_t compress_nibble_bit(uint64_t w, int b)   // 
     return (uint32_t)x;
 }
 
+__device__ __forceinline__ uint32_t compress_pair_bit(uint64_t w, int b)     // bit b of 32 bit pairs -> 32 bits
+{
+    uint64_t x = (w >> b) & 0x5555555555555555ull;
+    x = (x | (x >> 1)) & 0x3333333333333333ull;
+    x = (x | (x >> 2)) & 0x0F0F0F0F0F0F0F0Full;
+    x = (x | (x >> 4)) & 0x00FF00FF00FF00FFull;
+    x = (x | (x >> 8)) & 0x0000FFFF0000FFFFull;
+    x = (x | (x >> 16)) & 0xFFFFFFFFull;
+    return (uint32_t)x;
+}
+
 __device__ __forceinline__ uint64_t spread_even(uint32_t v)   // bit i -> bit 2 i
 {
     uint64_t x = v;
@@ -171,6 +187,15 @@ __global__ void __launch_bounds__(256) planes_kernel(const __grid_constant__ Pla
             sg |= spread_even(row32[q]) << (int)((y + c) & 1);
         }
         p.sg[idx] = sg;
+        return;
+    }
+    if (p.model == ISING_MODEL_BLUME_CAPEL_2BIT) {           // 2-bit layout: one word = 32 sites of a colour
+        for (int c = 0; c < 2; ++c) {
+            const uint64_t w = p.lat[c][y * Wq + q];
+            sg |= spread_even(compress_pair_bit(w, 1)) << (int)((y + c) & 1);       // code 2 = +1
+            nz |= spread_even(compress_pair_bit(~w, 0)) << (int)((y + c) & 1);      // code != 1
+        }
+        p.sg[idx] = sg; p.nz[idx] = nz;
         return;
     }
     for (int c = 0; c < 2; ++c) {
@@ -209,7 +234,7 @@ __global__ void __launch_bounds__(64) transpose_kernel(const uint64_t *__restric
 cudaError_t launch_planes(ising_sim *h)
 {
     const int64_t L = h->L, Wq = L / 64, plane_words = L * Wq;
-    const int np = (h->model != ISING_MODEL_BLUME_CAPEL) ? 1 : 2;
+    const int np = is_blume_capel(h->model) ? 2 : 1;
     PlaneParams p;
     p.lat[0] = h->lat[0]; p.lat[1] = h->lat[1];
     p.L = L; p.model = h->model;

@@ -1,9 +1,10 @@
 // Integer observables (A8 of SURVEY.md Sec. 8(a)) and the Schwinger-Dyson
 // histogram (Eq. 3).  Same register sliding window as the update
-// kernel: each thread walks R rows of one 128-bit column of the BLACK array and
+// kernel: each thread walks R rows of one 128-bit column (64-bit at 2 bits per spin) of the BLACK array and
 // sees every bond exactly once (for even L every bond joins a black and a white
 // site).  Warp shuffle -> one int64 atomic per warp per quantity.
 #include "ising_internal.cuh"
+#include "row_format.cuh"
 
 #define ONES 0x11111111u
 
@@ -25,18 +26,6 @@ __device__ __forceinline__ long long warp_sum(long long v)
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
     return v;
-}
-
-template <int P>
-__device__ __forceinline__ void side4(const uint4 &sm, uint32_t edge, uint32_t sd[4])
-{
-    if (P == 0) {
-        sd[0] = __funnelshift_l(edge, sm.x, 4); sd[1] = __funnelshift_l(sm.x, sm.y, 4);
-        sd[2] = __funnelshift_l(sm.y, sm.z, 4); sd[3] = __funnelshift_l(sm.z, sm.w, 4);
-    } else {
-        sd[0] = __funnelshift_r(sm.x, sm.y, 4); sd[1] = __funnelshift_r(sm.y, sm.z, 4);
-        sd[2] = __funnelshift_r(sm.z, sm.w, 4); sd[3] = __funnelshift_r(sm.w, edge, 4);
-    }
 }
 
 // MODE 0: B, M, Q.  MODE 1: Schwinger-Dyson histogram of s*h over the centre sites.
@@ -92,20 +81,21 @@ __global__ void __launch_bounds__(256) observe_kernel(const __grid_constant__ Ob
     int hist[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     if (y0 < L) {
         int yend = min(L, y0 + p.R);
-        const uint32_t *n32 = reinterpret_cast<const uint32_t *>(p.nbr);
-        const size_t halves = (size_t)cols * 4;
-        const int e0 = (col == 0) ? cols * 4 - 1 : 4 * col - 1;        // parity 0: neighbour k-1
-        const int e1 = (col == cols - 1) ? 0 : 4 * col + 4;            // parity 1: neighbour k+1
+        constexpr int VB = RowFmt<MODEL>::kVecBytes;
+        const char *nbr = reinterpret_cast<const char *>(p.nbr), *ctr = reinterpret_cast<const char *>(p.ctr);
+        const size_t rs = (size_t)cols * VB, cb = (size_t)col * VB;
+        const size_t e0 = (size_t)edge_half<MODEL, 0>(col, cols) * 4;   // parity 0: neighbour k-1
+        const size_t e1 = (size_t)edge_half<MODEL, 1>(col, cols) * 4;   // parity 1: neighbour k+1
         int ym = (y0 == 0) ? L - 1 : y0 - 1;
-        uint4 up = p.nbr[(size_t)ym * cols + col];
-        uint4 sm = p.nbr[(size_t)y0 * cols + col];
+        uint4 up = load_row<MODEL>(nbr + (size_t)ym * rs + cb);
+        uint4 sm = load_row<MODEL>(nbr + (size_t)y0 * rs + cb);
         for (int y = y0; y < yend; ++y) {
             int yp = (y + 1 == L) ? 0 : y + 1;
-            uint4 dn = p.nbr[(size_t)yp * cols + col];
-            uint4 x = p.ctr[(size_t)y * cols + col];
+            uint4 dn = load_row<MODEL>(nbr + (size_t)yp * rs + cb);
+            uint4 x = load_row<MODEL>(ctr + (size_t)y * rs + cb);
             uint32_t sd[4];
-            if (((y + p.centre) & 1) == 0) side4<0>(sm, n32[(size_t)y * halves + e0], sd);
-            else side4<1>(sm, n32[(size_t)y * halves + e1], sd);
+            if (((y + p.centre) & 1) == 0) side_words<MODEL, 0>(sm, *reinterpret_cast<const uint32_t *>(nbr + (size_t)y * rs + e0), sd);
+            else side_words<MODEL, 1>(sm, *reinterpret_cast<const uint32_t *>(nbr + (size_t)y * rs + e1), sd);
             obs_half<MODEL, MODE>(x.x, up.x, dn.x, sm.x, sd[0], B, M, Q, hist);
             obs_half<MODEL, MODE>(x.y, up.y, dn.y, sm.y, sd[1], B, M, Q, hist);
             obs_half<MODEL, MODE>(x.z, up.z, dn.z, sm.z, sd[2], B, M, Q, hist);
@@ -144,7 +134,8 @@ static cudaError_t launch_obs(ising_sim *h, int centre)
     int block = 128;
     unsigned grid = (unsigned)((threads + block - 1) / block);
     if (h->model == ISING_MODEL_ISING) observe_kernel<ISING_MODEL_ISING, MODE><<<grid, block, 0, h->stream>>>(p);
-    else observe_kernel<ISING_MODEL_BLUME_CAPEL, MODE><<<grid, block, 0, h->stream>>>(p);
+    else if (h->model == ISING_MODEL_BLUME_CAPEL) observe_kernel<ISING_MODEL_BLUME_CAPEL, MODE><<<grid, block, 0, h->stream>>>(p);
+    else observe_kernel<ISING_MODEL_BLUME_CAPEL_2BIT, MODE><<<grid, block, 0, h->stream>>>(p);
     h->launches++;
     return cudaGetLastError();
 }

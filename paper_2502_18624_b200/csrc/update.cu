@@ -10,6 +10,7 @@
 // coding: neighbour sums of many spins in one add), PAPER.md:69 (two colour
 // buffers, two phases), PAPER.md:131 (128-bit accesses).
 #include "ising_internal.cuh"
+#include "row_format.cuh"
 
 #define ONES 0x11111111u
 
@@ -29,34 +30,6 @@ struct UpdParams {
     long long *tally;           // A7: running B, M, Q (device), updated when the kernel is built with TALLY
     RoundKeys rk;
 };
-
-// ------------------------------------------------------------ row helpers ---
-// side word: for row parity p = (y + colour) & 1 the in-row neighbour that is not
-// at the same compact index k is k-1 (p = 0) or k+1 (p = 1)  [SURVEY.md Sec. 8 conventions]
-template <int P>
-__device__ __forceinline__ void side_words(const uint4 &sm, uint32_t edge, uint32_t sd[4])
-{
-    if (P == 0) {  // neighbour k-1: shift nibbles up, carry in the top nibble of the previous half
-        sd[0] = __funnelshift_l(edge, sm.x, 4);
-        sd[1] = __funnelshift_l(sm.x, sm.y, 4);
-        sd[2] = __funnelshift_l(sm.y, sm.z, 4);
-        sd[3] = __funnelshift_l(sm.z, sm.w, 4);
-    } else {       // neighbour k+1: shift nibbles down, carry in the bottom nibble of the next half
-        sd[0] = __funnelshift_r(sm.x, sm.y, 4);
-        sd[1] = __funnelshift_r(sm.y, sm.z, 4);
-        sd[2] = __funnelshift_r(sm.z, sm.w, 4);
-        sd[3] = __funnelshift_r(sm.w, edge, 4);
-    }
-}
-
-// index (in 32-bit halves, within the row) of the half that supplies the carry nibble
-template <int P>
-__device__ __forceinline__ int edge_half(int col, int cols)
-{
-    int halves = cols * 4;
-    if (P == 0) return (col == 0) ? halves - 1 : 4 * col - 1;
-    return (col == cols - 1) ? 0 : 4 * col + 4;
-}
 
 __device__ __forceinline__ uint32_t lt_mask8(const uint4 &a, const uint4 &b, uint32_t T)
 {
@@ -125,7 +98,7 @@ __device__ __forceinline__ uint4 ising_row(const uint4 &src, const uint4 &up, co
                                            uint32_t edge, uint64_t g0, uint32_t t, uint32_t tag, const UpdParams &p)
 {
     uint32_t sd[4];
-    side_words<P>(sm, edge, sd);
+    side_words<ISING_MODEL_ISING, P>(sm, edge, sd);
     PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), t, tag, p.rk);
     uint32_t gl = (uint32_t)g0;     // g0 is a multiple of 8: gl | q == gl + q
     uint4 r0 = philox_site4(gl | 0, pr, p.rk), r1 = philox_site4(gl | 1, pr, p.rk);
@@ -176,7 +149,7 @@ __device__ __forceinline__ uint4 bc_row(const uint4 &src, const uint4 &up, const
                                         const uint32_t *tab, uint64_t always)
 {
     uint32_t sd[4];
-    side_words<P>(sm, edge, sd);
+    side_words<ISING_MODEL_BLUME_CAPEL, P>(sm, edge, sd);
     PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), t, tag, p.rk);
     uint32_t gl = (uint32_t)g0;
     uint4 o;
@@ -250,7 +223,7 @@ __device__ __forceinline__ uint4 bc_row_carry(const uint4 &src, const uint4 &up,
                                               const unsigned char *tab)
 {
     uint32_t sd[4];
-    side_words<P>(sm, edge, sd);
+    side_words<ISING_MODEL_BLUME_CAPEL, P>(sm, edge, sd);
     PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), t, tag, p.rk);
     uint32_t gl = (uint32_t)g0;
     uint4 o;
@@ -269,6 +242,49 @@ __device__ __forceinline__ uint4 bc_row_carry(const uint4 &src, const uint4 &up,
     {
         uint4 ra = philox_site4(gl | 6, pr, p.rk), rb = philox_site4(gl | 7, pr, p.rk);
         o.w = bc_half_carry(src.w, up.w, dn.w, sm.w, sd[3], ra, rb, tab);
+    }
+    return o;
+}
+
+// 2-bit storage (ISING_MODEL_BLUME_CAPEL_2BIT): the register words are (E_lo, O_lo, E_hi, O_hi)
+// (row_format.cuh); nibble j of an E word is site 2j of its half, so it takes word 2 (j & 1) of
+// Philox call j >> 1, and the O word takes the words 2 (j & 1) + 1 -- register renaming only.
+// The trajectory is that of the 4-bit model: same keying, same thresholds, same rule.
+template <int P, int V>
+__device__ __forceinline__ uint4 bc2_row(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
+                                         uint32_t edge, uint64_t g0, uint32_t t, uint32_t tag, const UpdParams &p,
+                                         const unsigned char *ctab, const uint32_t *tab, uint64_t always)
+{
+    uint32_t sd[4];
+    side_words<ISING_MODEL_BLUME_CAPEL_2BIT, P>(sm, edge, sd);
+    PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), t, tag, p.rk);
+    uint32_t gl = (uint32_t)g0;
+    uint4 o;
+    {
+        const uint4 q0 = philox_site4(gl | 0, pr, p.rk), q1 = philox_site4(gl | 1, pr, p.rk);
+        const uint4 q2 = philox_site4(gl | 2, pr, p.rk), q3 = philox_site4(gl | 3, pr, p.rk);
+        const uint4 ea = make_uint4(q0.x, q0.z, q1.x, q1.z), eb = make_uint4(q2.x, q2.z, q3.x, q3.z);
+        const uint4 oa = make_uint4(q0.y, q0.w, q1.y, q1.w), ob = make_uint4(q2.y, q2.w, q3.y, q3.w);
+        if (V == 0) {
+            o.x = bc_half_carry(src.x, up.x, dn.x, sm.x, sd[0], ea, eb, ctab);
+            o.y = bc_half_carry(src.y, up.y, dn.y, sm.y, sd[1], oa, ob, ctab);
+        } else {
+            o.x = bc_half(src.x, up.x, dn.x, sm.x, sd[0], ea, eb, tab, always);
+            o.y = bc_half(src.y, up.y, dn.y, sm.y, sd[1], oa, ob, tab, always);
+        }
+    }
+    {
+        const uint4 q0 = philox_site4(gl | 4, pr, p.rk), q1 = philox_site4(gl | 5, pr, p.rk);
+        const uint4 q2 = philox_site4(gl | 6, pr, p.rk), q3 = philox_site4(gl | 7, pr, p.rk);
+        const uint4 ea = make_uint4(q0.x, q0.z, q1.x, q1.z), eb = make_uint4(q2.x, q2.z, q3.x, q3.z);
+        const uint4 oa = make_uint4(q0.y, q0.w, q1.y, q1.w), ob = make_uint4(q2.y, q2.w, q3.y, q3.w);
+        if (V == 0) {
+            o.z = bc_half_carry(src.z, up.z, dn.z, sm.z, sd[2], ea, eb, ctab);
+            o.w = bc_half_carry(src.w, up.w, dn.w, sm.w, sd[3], oa, ob, ctab);
+        } else {
+            o.z = bc_half(src.z, up.z, dn.z, sm.z, sd[2], ea, eb, tab, always);
+            o.w = bc_half(src.w, up.w, dn.w, sm.w, sd[3], oa, ob, tab, always);
+        }
     }
     return o;
 }
@@ -311,7 +327,7 @@ __device__ __forceinline__ void tally_row(const uint4 &x, const uint4 &y, const 
                                           uint32_t edge, int &dB, int &dM, int &dQ)
 {
     uint32_t sd[4];
-    side_words<P>(sm, edge, sd);
+    side_words<MODEL, P>(sm, edge, sd);
     tally_half<MODEL>(x.x, y.x, up.x, dn.x, sm.x, sd[0], dB, dM, dQ);
     tally_half<MODEL>(x.y, y.y, up.y, dn.y, sm.y, sd[1], dB, dM, dQ);
     tally_half<MODEL>(x.z, y.z, up.z, dn.z, sm.z, sd[2], dB, dM, dQ);
@@ -326,7 +342,8 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
     const uint32_t t_eff = p.t + __ldg(p.t_base);
     __shared__ __align__(16) uint32_t s_tab[80 + 132];   // both table forms (api.cu)
     uint64_t always = 0;
-    if (MODEL == ISING_MODEL_BLUME_CAPEL) {
+    constexpr bool kIsing = MODEL == ISING_MODEL_ISING, kTwoBit = RowFmt<MODEL>::kTwoBit;
+    if (!kIsing) {
         for (int i = threadIdx.x; i < 80 + 132; i += blockDim.x) s_tab[i] = p.bc_table[i];
         __syncthreads();
         always = (uint64_t)s_tab[64] | ((uint64_t)s_tab[65] << 32);
@@ -342,20 +359,21 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
 
     // Running byte pointers, advanced by one row stride per row (no index multiplications in
     // the loop).  y0 is even (R even), so the row parity (y + C) & 1 is C on even offsets.
-    const size_t rs = (size_t)cols * 16;                               // bytes per colour row
+    constexpr int VB = RowFmt<MODEL>::kVecBytes;                       // 16, or 8 for the 2-bit layout
+    const size_t rs = (size_t)cols * VB;                               // bytes per colour row
     const char *oppb = reinterpret_cast<const char *>(p.opp);
     char *ownb = reinterpret_cast<char *>(p.own);
-    const size_t row0 = (size_t)y0 * rs, cb = (size_t)col * 16;
-    const size_t e_even = (size_t)edge_half<C>(col, cols) * 4, e_odd = (size_t)edge_half<1 - C>(col, cols) * 4;
+    const size_t row0 = (size_t)y0 * rs, cb = (size_t)col * VB;
+    const size_t e_even = (size_t)edge_half<MODEL, C>(col, cols) * 4, e_odd = (size_t)edge_half<MODEL, 1 - C>(col, cols) * 4;
     const char *o1 = oppb + row0 + rs + cb;        // opposite colour, row y + 1 (y + 1 < L: L is even)
     const char *ee = oppb + row0 + e_even;         // carry half, even offsets: row y
     const char *eo = oppb + row0 + rs + e_odd;     // carry half, odd offsets:  row y + 1
     char *w0 = ownb + row0 + cb;                   // own colour, row y
 
     const int ym = (y0 == 0) ? L - 1 : y0 - 1;
-    uint4 up = *reinterpret_cast<const uint4 *>(oppb + (size_t)ym * rs + cb);
-    uint4 sm = *reinterpret_cast<const uint4 *>(oppb + row0 + cb);
-    uint4 src = *reinterpret_cast<const uint4 *>(w0);
+    uint4 up = load_row<MODEL>(oppb + (size_t)ym * rs + cb);
+    uint4 sm = load_row<MODEL>(oppb + row0 + cb);
+    uint4 src = load_row<MODEL>(w0);
     uint32_t edge = *reinterpret_cast<const uint32_t *>(ee);
     uint64_t g0 = (uint64_t)y0 * (uint64_t)(cols * 8) + (uint64_t)(col * 8);
     const uint64_t gs = (uint64_t)(cols * 8);
@@ -363,30 +381,32 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
     for (int y = y0; y < yend; y += 2) {
         // ---- even offset: parity C
         const char *o2 = (y + 2 == L) ? oppb + cb : o1 + rs;           // row y + 2, wraps to row 0
-        uint4 dn = *reinterpret_cast<const uint4 *>(o1);
-        uint4 nsrc = *reinterpret_cast<const uint4 *>(w0 + rs);
+        uint4 dn = load_row<MODEL>(o1);
+        uint4 nsrc = load_row<MODEL>(w0 + rs);
         uint32_t nedge = *reinterpret_cast<const uint32_t *>(eo);
-        uint4 dn2 = *reinterpret_cast<const uint4 *>(o2);
+        uint4 dn2 = load_row<MODEL>(o2);
         uint4 o;
-        if (MODEL == ISING_MODEL_ISING) o = ising_row<C, V>(src, up, sm, dn, edge, g0, t_eff, p.colour, p);
+        if (kIsing) o = ising_row<C, V>(src, up, sm, dn, edge, g0, t_eff, p.colour, p);
+        else if (kTwoBit) o = bc2_row<C, V>(src, up, sm, dn, edge, g0, t_eff, p.colour, p, ctab, s_tab, always);
         else if (V == 0) o = bc_row_carry<C>(src, up, sm, dn, edge, g0, t_eff, p.colour, p, ctab);
         else o = bc_row<C>(src, up, sm, dn, edge, g0, t_eff, p.colour, p, s_tab, always);
         if (TALLY) tally_row<MODEL, C>(src, o, up, sm, dn, edge, dB, dM, dQ);
-        *reinterpret_cast<uint4 *>(w0) = o;
+        store_row<MODEL>(w0, o);
         g0 += gs;
         // ---- odd offset: parity 1 - C.  Prefetch the next even row first.
         uint4 nsrc2 = src;
         uint32_t nedge2 = 0;
         ee += 2 * rs;
         if (y + 2 < yend) {
-            nsrc2 = *reinterpret_cast<const uint4 *>(w0 + 2 * rs);
+            nsrc2 = load_row<MODEL>(w0 + 2 * rs);
             nedge2 = *reinterpret_cast<const uint32_t *>(ee);
         }
-        if (MODEL == ISING_MODEL_ISING) o = ising_row<1 - C, V>(nsrc, sm, dn, dn2, nedge, g0, t_eff, p.colour, p);
+        if (kIsing) o = ising_row<1 - C, V>(nsrc, sm, dn, dn2, nedge, g0, t_eff, p.colour, p);
+        else if (kTwoBit) o = bc2_row<1 - C, V>(nsrc, sm, dn, dn2, nedge, g0, t_eff, p.colour, p, ctab, s_tab, always);
         else if (V == 0) o = bc_row_carry<1 - C>(nsrc, sm, dn, dn2, nedge, g0, t_eff, p.colour, p, ctab);
         else o = bc_row<1 - C>(nsrc, sm, dn, dn2, nedge, g0, t_eff, p.colour, p, s_tab, always);
         if (TALLY) tally_row<MODEL, 1 - C>(nsrc, o, sm, dn, dn2, nedge, dB, dM, dQ);
-        *reinterpret_cast<uint4 *>(w0 + rs) = o;
+        store_row<MODEL>(w0 + rs, o);
         g0 += gs;
         up = dn; sm = dn2; src = nsrc2; edge = nedge2;
         o1 += 2 * rs; eo += 2 * rs; w0 += 2 * rs;
@@ -427,14 +447,15 @@ cudaError_t launch_update(ising_sim *h, int colour, uint32_t t)
     p.tally = h->d_acc + 40;
     p.t_base = reinterpret_cast<const uint32_t *>(h->d_acc + 48) + (h->graph_capture ? 1 : 0);   // [0] stays 0, [1] = base of a graph replay
     bool never = false;                           // Blume-Capel: a threshold that is exactly 0 -> compare/select form
-    if (h->model == ISING_MODEL_BLUME_CAPEL)
+    if (is_blume_capel(h->model))
         for (int i = 0; i < h->n_T; ++i) never = never || h->T[i] == 0;
     const int v = (h->variant == 0 && !never) ? 0 : 1;
 #define LAUNCH_UPD(MODEL, C, V, T) update_kernel<MODEL, C, V, T><<<grid, block, 0, h->stream>>>(p)
 #define PICK_T(MODEL, C, V) do { if (h->tally_on) LAUNCH_UPD(MODEL, C, V, 1); else LAUNCH_UPD(MODEL, C, V, 0); } while (0)
 #define PICK_V(MODEL, C) do { if (v == 0) PICK_T(MODEL, C, 0); else PICK_T(MODEL, C, 1); } while (0)
     if (h->model == ISING_MODEL_ISING) { if (colour == 0) PICK_V(ISING_MODEL_ISING, 0); else PICK_V(ISING_MODEL_ISING, 1); }
-    else { if (colour == 0) PICK_V(ISING_MODEL_BLUME_CAPEL, 0); else PICK_V(ISING_MODEL_BLUME_CAPEL, 1); }
+    else if (h->model == ISING_MODEL_BLUME_CAPEL) { if (colour == 0) PICK_V(ISING_MODEL_BLUME_CAPEL, 0); else PICK_V(ISING_MODEL_BLUME_CAPEL, 1); }
+    else { if (colour == 0) PICK_V(ISING_MODEL_BLUME_CAPEL_2BIT, 0); else PICK_V(ISING_MODEL_BLUME_CAPEL_2BIT, 1); }
 #undef PICK_V
 #undef PICK_T
 #undef LAUNCH_UPD
@@ -444,7 +465,7 @@ cudaError_t launch_update(ising_sim *h, int colour, uint32_t t)
 
 // ------------------------------------------------------------------- init ---
 // A2: spin of site n from r = draw(n, t = 0, tag = 2 + colour).  Ising: top bit;
-// Blume-Capel: code = (3 r) >> 32.  One thread per 32-bit half (8 sites, 2 calls).
+// Blume-Capel: code = (3 r) >> 32.  One thread per 32-bit half (8 sites, 2 calls; 16 and 4 at 2 bits).
 struct InitParams {
     uint32_t *lat[2];
     int64_t halves_per_colour;
@@ -461,16 +482,17 @@ __global__ void __launch_bounds__(256) init_kernel(const __grid_constant__ InitP
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= p.halves_per_colour) return;
+    // 8 sites per half = 2 groups of 4 (4 bits per site); 16 sites = 4 groups in the 2-bit layout
+    const int calls = p.model == ISING_MODEL_BLUME_CAPEL_2BIT ? 4 : 2, bits = p.model == ISING_MODEL_BLUME_CAPEL_2BIT ? 2 : 4;
     for (int c = 0; c < 2; ++c) {
-        uint64_t g = (uint64_t)i * 2;          // 8 sites per half = 2 groups of 4
+        uint64_t g = (uint64_t)i * calls;
         uint32_t w = 0;
-#pragma unroll
-        for (int q = 0; q < 2; ++q) {
+        for (int q = 0; q < calls; ++q) {
             uint4 r = philox4x32_10(make_uint4((uint32_t)(g + q), (uint32_t)((g + q) >> 32), 0u, 2u + c), p.rk);
-            w |= init_nibble(p.model, r.x) << (16 * q);
-            w |= init_nibble(p.model, r.y) << (16 * q + 4);
-            w |= init_nibble(p.model, r.z) << (16 * q + 8);
-            w |= init_nibble(p.model, r.w) << (16 * q + 12);
+            w |= init_nibble(p.model, r.x) << (bits * (4 * q));
+            w |= init_nibble(p.model, r.y) << (bits * (4 * q + 1));
+            w |= init_nibble(p.model, r.z) << (bits * (4 * q + 2));
+            w |= init_nibble(p.model, r.w) << (bits * (4 * q + 3));
         }
         p.lat[c][i] = w;
     }
@@ -481,7 +503,7 @@ cudaError_t launch_init(ising_sim *h)
     InitParams p;
     p.lat[0] = reinterpret_cast<uint32_t *>(h->lat[0]);
     p.lat[1] = reinterpret_cast<uint32_t *>(h->lat[1]);
-    p.halves_per_colour = words_per_colour(h->L) * 2;
+    p.halves_per_colour = colour_words(h) * 2;
     p.model = h->model;
     p.rk = h->rk;
     int block = 256;
@@ -559,7 +581,7 @@ __global__ void __launch_bounds__(256) copy_kernel(const uint4 *__restrict__ opp
 
 cudaError_t launch_copy(ising_sim *h)
 {
-    size_t n = (size_t)words_per_colour(h->L) / 2;
+    size_t n = (size_t)colour_words(h) / 2;
     copy_kernel<<<148 * 16, 256, 0, h->stream>>>(reinterpret_cast<const uint4 *>(h->lat[1]),
                                                 reinterpret_cast<uint4 *>(h->lat[0]), n,
                                                 reinterpret_cast<uint32_t *>(h->d_acc) + 512);

@@ -38,7 +38,8 @@ def test_workspace_bytes_and_validation(lib):
     for bad_L in (0, 32, 100, 65, -64, (1 << 20) + 64):
         assert lib.ising_workspace_bytes(0, bad_L) == 0
     assert lib.ising_workspace_bytes(2, 256) == 256 * 256 // 8 + 4096      # LUT model: one bit per spin
-    assert lib.ising_workspace_bytes(2, 192) == 0 and lib.ising_workspace_bytes(3, 256) == 0
+    assert lib.ising_workspace_bytes(3, 256) == 256 * 256 // 4 + 4096      # Blume-Capel at 2 bits per spin
+    assert lib.ising_workspace_bytes(2, 192) == 0 and lib.ising_workspace_bytes(4, 256) == 0
 
 
 def test_null_handle_errors(lib):

@@ -212,11 +212,13 @@ def test_config4_ising_L2p16_correlation_protocol(eng):
 
 # ------------------------------------------------------------ maximum sizes ---
 @pytest.mark.parametrize("model,L,beta,D", [(wl.ISING_LUT, 1 << 20, wl.BETA_C / 0.9, 0.0),
-                                            (ISING, 1 << 19, wl.BETA_C / 0.9, 0.0), (BC, 1 << 19, 1 / 1.4, 1.0)])
+                                            (ISING, 1 << 19, wl.BETA_C / 0.9, 0.0), (BC, 1 << 19, 1 / 1.4, 1.0),
+                                            (wl.BLUME_CAPEL_2BIT, 3 << 18, 1 / 1.4, 1.0)])
 def test_maximum_lattice_sizes(eng, model, L, beta, D):
     """The largest lattices one B200 holds -- the paper's single-GPU maxima: 2^40 spins at
-    one bit (137 GB) and 2^38 at four bits (137 GB).  Light-cone windows on the wraps and in the last rows
-    (64-bit offsets), Q and n_sites at 2^40."""
+    one bit (137 GB) and 2^38 at four bits (137 GB); Blume-Capel at two bits per spin (NEXT-3) reaches
+    L = 3 * 2^18 (6.2e11 spins, 155 GB) against the 4-bit oracle.  Light-cone windows on the wraps and in the
+    last rows (64-bit offsets), Q and n_sites at 2^40."""
     n = 3
     with eng.IsingSim(model, L, beta, D, 1) as sim:
         sim.sweep(n)
@@ -224,8 +226,8 @@ def test_maximum_lattice_sizes(eng, model, L, beta, D):
             if model == wl.ISING_LUT:
                 want = oracle.lut_window_after(L, beta, 1, n, x0, y0, W, W)
             else:
-                want = oracle.window_after(model, L, beta, D, 1, n, x0, y0, W, W)
+                want = oracle.window_after(BC if model == wl.BLUME_CAPEL_2BIT else model, L, beta, D, 1, n, x0, y0, W, W)
             assert (sim.read_window(x0, y0, W, W) == want).all(), (x0, y0)
         o = sim.observables()
         assert o.n_sites == L * L and o.sweeps_done == n and abs(o.M) < L * L // 1000
-        assert o.Q == L * L if model != BC else 0 < o.Q < L * L
+        assert o.Q == L * L if model not in (BC, wl.BLUME_CAPEL_2BIT) else 0 < o.Q < L * L

@@ -10,7 +10,7 @@ from __future__ import annotations
 import math
 from dataclasses import dataclass
 
-ISING, BLUME_CAPEL, ISING_LUT = 0, 1, 2   # ISING_LUT: the paper's 1-bit look-up-table kernel (NEXT-2)
+ISING, BLUME_CAPEL, ISING_LUT, BLUME_CAPEL_2BIT = 0, 1, 2, 3   # ISING_LUT: the paper's 1-bit look-up-table kernel (NEXT-2)
 
 # beta_c = ln(1 + sqrt(2)) / 2 (2D Ising, J = k_B = 1); the same double is
 # handed to both sides (reading R6).
