@@ -231,3 +231,13 @@ def test_maximum_lattice_sizes(eng, model, L, beta, D):
         o = sim.observables()
         assert o.n_sites == L * L and o.sweeps_done == n and abs(o.M) < L * L // 1000
         assert o.Q == L * L if model not in (BC, wl.BLUME_CAPEL_2BIT) else 0 < o.Q < L * L
+        # no room left for the bit planes of the correlation pass: a clean ISING_ENOMEM, and the handle stays usable
+        with pytest.raises(eng.IsingError) as err:
+            sim.correlation(4)
+        assert err.value.code == -2
+        sim.sweep(1)
+        x0, y0 = L - W // 2, L - W // 2
+        omodel = BC if model == wl.BLUME_CAPEL_2BIT else model
+        want = (oracle.lut_window_after(L, beta, 1, n + 1, x0, y0, W, W) if model == wl.ISING_LUT
+                else oracle.window_after(omodel, L, beta, D, 1, n + 1, x0, y0, W, W))
+        assert (sim.read_window(x0, y0, W, W) == want).all()
