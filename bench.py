@@ -13,7 +13,8 @@ flush is needed between iterations).  Prints ONE JSON line (rank 0).
 value     = L^2 * S * K / (device time of the K steps), lattice resident in HBM
 e2e       = same through the C ABI with HOST buffers: every step uploads the packed
             lattice from pinned host memory (ising_write_packed), runs S sweeps and
-            reads the observables back
+            reads the observables back; two handles on two streams alternate so that
+            the next step's upload overlaps this step's sweeps (serial figure beside it)
 roofline  = the update kernel against the bound that actually limits it: the integer
             ALU ("one Philox4x32-10 number per site" = 9.25 dispatch slots per site,
             DESIGN.md Sec. 5.1); peak derived from unit counts and the max SM clock, with
@@ -242,6 +243,14 @@ def run_e2e(eng, torch, model, L, beta, D, seed, S, steps, device):
         note = f"host memory too small for the 2^18 lattice; e2e measured at L={L}"
     words = colour_bytes // 8
     host = [torch.empty(words, dtype=torch.int64).pin_memory() for _ in range(2)]
+
+    def enqueue(sim):                               # one step, asynchronous on the handle's stream
+        for c in range(2):
+            sim.write_packed(c, host[c], 0, words)
+        sim.set_sweeps_done(2)
+        sim.sweep(S)
+
+    # serial: upload, sweeps, observables, one after the other on one handle
     with eng.IsingSim(model, L, beta, D, seed, device=device) as sim:
         sim.sweep(2)
         for c in range(2):
@@ -250,19 +259,50 @@ def run_e2e(eng, torch, model, L, beta, D, seed, S, steps, device):
         for i in range(1 + steps):
             torch.cuda.synchronize(device)
             t0 = time.perf_counter()
-            for c in range(2):
-                sim.write_packed(c, host[c], 0, words)
-            sim.set_sweeps_done(2)
-            sim.sweep(S)
+            enqueue(sim)
             o = sim.observables()                  # synchronises; D2H of B, M, Q
             torch.cuda.synchronize(device)
             if i >= 1:
                 times.append(time.perf_counter() - t0)
         assert o.n_sites == L * L
+        ref = (o.bond_sum, o.M, o.Q)
     dt = sum(times) / len(times)
     out = {"value": L * L * S / (dt * 1e9), "unit": "updates/ns", "h2d_bytes_per_step": 2 * colour_bytes,
            "d2h_bytes_per_step": 24, "L": L, "sweeps_per_step": S, "steps": steps, "ms_per_step": dt * 1e3,
            "what": "ising_write_packed(both colours, pinned host) + ising_sweep(S) + ising_observables"}
+    # pipelined: the steps are independent inputs, so two handles on two streams alternate and the upload of
+    # step i + 1 (copy engine) overlaps the sweeps of step i; fill and drain are inside the timed region
+    free_b, _ = torch.cuda.mem_get_info(device)
+    if free_b > 2 * need + (8 << 30):
+        streams = [torch.cuda.Stream(device=device) for _ in range(2)]
+        sims = []
+        for st in streams:
+            with torch.cuda.stream(st):
+                sims.append(eng.IsingSim(model, L, beta, D, seed, device=device))
+        n_pipe = max(2 * steps, 6)
+        for sim in sims:                            # warm-up: one step each
+            enqueue(sim)
+            sim.observables()
+        torch.cuda.synchronize(device)
+        t0 = time.perf_counter()
+        pending = None
+        for i in range(n_pipe):
+            sim = sims[i % 2]
+            enqueue(sim)
+            if pending is not None:
+                po = pending.observables()          # waits for step i - 1 while step i uploads
+                assert (po.bond_sum, po.M, po.Q) == ref
+            pending = sim
+        po = pending.observables()
+        torch.cuda.synchronize(device)
+        dtp = (time.perf_counter() - t0) / n_pipe
+        assert (po.bond_sum, po.M, po.Q) == ref
+        for sim in sims:
+            sim.close()
+        out.update({"serial_value": out["value"], "serial_ms_per_step": out["ms_per_step"],
+                    "value": L * L * S / (dtp * 1e9), "ms_per_step": dtp * 1e3, "steps": n_pipe,
+                    "what": out["what"] + "; two handles on two streams, the upload of step i + 1 overlaps the sweeps "
+                            "of step i (wall clock over all steps incl. pipeline fill and drain)"})
     if note:
         out["note"] = note
     return out
