@@ -145,6 +145,8 @@ def time_oracle(model: int, beta: float, D: float, seed: int, seconds: float, L:
     sample of the workload: same model / beta / seed, lattice cut to L x L, as many
     full sweeps as fit in `seconds` (at least 2).  Returns (updates/ns, cores, text)."""
     import oracle
+    if model == wl.BLUME_CAPEL_2BIT:                           # storage format only: the trajectory contract is model 1's
+        model = wl.BLUME_CAPEL
     if model == wl.ISING_LUT:
         init = lambda: oracle.lut_init(L, seed)
         sweep = lambda s, t, tl: oracle.lut_sweep(s, beta, seed, t, tl)

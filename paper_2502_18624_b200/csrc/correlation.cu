@@ -107,7 +107,13 @@ __global__ void __launch_bounds__(256) comb_kernel(const uint64_t *__restrict__ 
         const int q = cw * s + j;
         if (q >= Wq) break;
         uint64_t w = in[(size_t)y * Wq + q];
-        for (int k = 0; k < log2s; ++k) w = gather_even(w);
+        if (log2s == 4) {                     // the protocol's stride: bits 0, 16, 32, 48 -> 4 bits
+            uint32_t lo = (uint32_t)w & 0x00010001u, hi = (uint32_t)(w >> 32) & 0x00010001u;
+            lo = (lo | (lo >> 15)) & 3u; hi = (hi | (hi >> 15)) & 3u;
+            w = lo | (hi << 2);
+        } else {
+            for (int k = 0; k < log2s; ++k) w = gather_even(w);
+        }
         o |= w << (j * bits);
     }
     out[idx] = o;
@@ -122,17 +128,31 @@ __global__ void __launch_bounds__(256) corr_list_kernel(const uint64_t *__restri
     const int r = (int)rlist[blockIdx.x];
     long long acc = 0;
     const int rows = L / stride;
-    for (int idx = threadIdx.x; idx < rows * W; idx += blockDim.x) {
-        int yi = idx / W, q = idx - yi * W;
-        int y = yi * stride;
-        int yb = y + r;
-        if (yb >= L) yb -= L;
-        uint64_t a = sg[(size_t)y * W + q], b = sg[(size_t)yb * W + q];
-        if (MODEL == ISING_MODEL_ISING) acc += __popcll(a ^ b);
-        else {
-            uint64_t both = nz[(size_t)y * W + q] & nz[(size_t)yb * W + q];
-            acc += __popcll(both) - 2 * __popcll(both & (a ^ b));
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    // a warp per source row, lanes over the words of the row (no per-element division), two rows in flight
+    for (int yi = warp; yi < rows; yi += 2 * nwarp) {
+        const int yj = yi + nwarp;
+        const bool two = yj < rows;
+        const int y0 = yi * stride, y1 = two ? yj * stride : y0;
+        int yb0 = y0 + r, yb1 = y1 + r;
+        if (yb0 >= L) yb0 -= L;
+        if (yb1 >= L) yb1 -= L;
+        const uint64_t *a0 = sg + (size_t)y0 * W, *b0 = sg + (size_t)yb0 * W;
+        const uint64_t *a1 = sg + (size_t)y1 * W, *b1 = sg + (size_t)yb1 * W;
+        int cnt = 0;
+        for (int q = lane; q < W; q += 32) {
+            const uint64_t xa = a0[q] ^ b0[q], xb = a1[q] ^ b1[q];
+            if (MODEL == ISING_MODEL_ISING) cnt += __popcll(xa) + (two ? __popcll(xb) : 0);
+            else {
+                const uint64_t both0 = nz[(size_t)y0 * W + q] & nz[(size_t)yb0 * W + q];
+                cnt += __popcll(both0) - 2 * __popcll(both0 & xa);
+                if (two) {
+                    const uint64_t both1 = nz[(size_t)y1 * W + q] & nz[(size_t)yb1 * W + q];
+                    cnt += __popcll(both1) - 2 * __popcll(both1 & xb);
+                }
+            }
         }
+        acc += cnt;
     }
     __shared__ long long red[8];
 #pragma unroll
