@@ -135,25 +135,14 @@ cudaError_t launch_pack(ising_sim *h, int64_t y0, int64_t ny, const int8_t *dev_
 // and the transposed planes planeT[x][y/64] so that S_x(r) of the lattice is S_y(r) of
 // the transpose.  Layout of h->planes: [sg | sgT] (Ising) or [sg | nz | sgT | nzT] (BC),
 // each L*L/8 bytes.
-__device__ __forceinline__ uint32_t compress_nibble_bit(uint64_t w, int b)   // bit b of 16 nibbles -> 16 bits
+__device__ __forceinline__ uint64_t nibble_bit_to_even(uint64_t w, int b)   // bit b of nibble j -> bit 2 j (j = 0..15)
 {
     uint64_t x = (w >> b) & 0x1111111111111111ull;
-    x = (x | (x >> 3)) & 0x0303030303030303ull;
-    x = (x | (x >> 6)) & 0x000F000F000F000Full;
-    x = (x | (x >> 12)) & 0x000000FF000000FFull;
-    x = (x | (x >> 24)) & 0xFFFFull;
-    return (uint32_t)x;
-}
-
-__device__ __forceinline__ uint32_t compress_pair_bit(uint64_t w, int b)     // bit b of 32 bit pairs -> 32 bits
-{
-    uint64_t x = (w >> b) & 0x5555555555555555ull;
-    x = (x | (x >> 1)) & 0x3333333333333333ull;
-    x = (x | (x >> 2)) & 0x0F0F0F0F0F0F0F0Full;
-    x = (x | (x >> 4)) & 0x00FF00FF00FF00FFull;
-    x = (x | (x >> 8)) & 0x0000FFFF0000FFFFull;
-    x = (x | (x >> 16)) & 0xFFFFFFFFull;
-    return (uint32_t)x;
+    x = (x | (x >> 2)) & 0x0505050505050505ull;
+    x = (x | (x >> 4)) & 0x0055005500550055ull;
+    x = (x | (x >> 8)) & 0x0000555500005555ull;
+    x = (x | (x >> 16)) & 0x0000000055555555ull;
+    return x;
 }
 
 __device__ __forceinline__ uint64_t spread_even(uint32_t v)   // bit i -> bit 2 i
@@ -189,11 +178,11 @@ __global__ void __launch_bounds__(256) planes_kernel(const __grid_constant__ Pla
         p.sg[idx] = sg;
         return;
     }
-    if (p.model == ISING_MODEL_BLUME_CAPEL_2BIT) {           // 2-bit layout: one word = 32 sites of a colour
+    if (p.model == ISING_MODEL_BLUME_CAPEL_2BIT) {           // 2-bit layout: one word = 32 sites of a colour, pair j at bit 2 j
         for (int c = 0; c < 2; ++c) {
             const uint64_t w = p.lat[c][y * Wq + q];
-            sg |= spread_even(compress_pair_bit(w, 1)) << (int)((y + c) & 1);       // code 2 = +1
-            nz |= spread_even(compress_pair_bit(~w, 0)) << (int)((y + c) & 1);      // code != 1
+            sg |= ((w >> 1) & 0x5555555555555555ull) << (int)((y + c) & 1);       // code 2 = +1: high bit of the pair
+            nz |= (~w & 0x5555555555555555ull) << (int)((y + c) & 1);             // code != 1: low bit clear
         }
         p.sg[idx] = sg; p.nz[idx] = nz;
         return;
@@ -203,13 +192,10 @@ __global__ void __launch_bounds__(256) planes_kernel(const __grid_constant__ Pla
         const uint64_t *row = p.lat[c] + y * (p.L / 32);
         uint64_t w0 = row[2 * q], w1 = row[2 * q + 1];
         if (p.model == ISING_MODEL_ISING) {
-            uint32_t m = compress_nibble_bit(w0, 0) | (compress_nibble_bit(w1, 0) << 16);
-            sg |= spread_even(m) << par;
+            sg |= (nibble_bit_to_even(w0, 0) | (nibble_bit_to_even(w1, 0) << 32)) << par;
         } else {
-            uint32_t m = compress_nibble_bit(w0, 1) | (compress_nibble_bit(w1, 1) << 16);        // code 2 = +1
-            uint32_t z = compress_nibble_bit(~w0, 0) | (compress_nibble_bit(~w1, 0) << 16);      // code != 1
-            sg |= spread_even(m) << par;
-            nz |= spread_even(z) << par;
+            sg |= (nibble_bit_to_even(w0, 1) | (nibble_bit_to_even(w1, 1) << 32)) << par;        // code 2 = +1
+            nz |= (nibble_bit_to_even(~w0, 0) | (nibble_bit_to_even(~w1, 0) << 32)) << par;      // code != 1
         }
     }
     p.sg[idx] = sg;
@@ -220,8 +206,8 @@ __global__ void __launch_bounds__(256) planes_kernel(const __grid_constant__ Pla
 // consecutive 32-bit words, low half first, so the 32-bit view is the same matrix).  A warp holds one tile,
 // one row per lane, and transposes it with five rounds of block swaps between lanes (`shfl.xor` by 16, 8, 4,
 // 2, 1: about one instruction per word instead of the 3 per word of gathering 32 bits one by one).  A block
-// moves a panel of 8 x 8 tiles through shared memory so that both the reads (256 rows) and the writes (256
-// rows) are 32-byte contiguous pieces.  W32 = L / 32 words per row; L is a multiple of 64, panels may be ragged.
+// moves a panel of 8 x 32 tiles through shared memory.  W32 = L / 32 words per row; L is a multiple of 64,
+// panels may be ragged.
 __device__ __forceinline__ uint32_t transpose32(uint32_t a, int lane)
 {
     const uint32_t masks[5] = {0x0000FFFFu, 0x00FF00FFu, 0x0F0F0F0Fu, 0x33333333u, 0x55555555u};
@@ -238,32 +224,34 @@ __device__ __forceinline__ uint32_t transpose32(uint32_t a, int lane)
 __global__ void __launch_bounds__(256) transpose_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out,
                                                         int64_t L, int64_t W32)
 {
-    __shared__ uint32_t tile[256][9];                       // stride 9: lanes reading one column hit 32 banks
+    // panel: 256 input rows x 32 words (8 x 32 tiles) -> 1024 output rows x 8 words.  blockIdx.x walks the
+    // input rows (= the output words), so consecutive blocks write neighbouring 32-byte pieces of the same
+    // output rows and the L2 assembles full lines; the reads are 128 contiguous bytes per row.
+    __shared__ uint32_t buf[1024 * 9];                      // in: [256][33], out: [1024][9] (odd strides: no bank conflicts)
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-    const int64_t row0 = 256 * (int64_t)blockIdx.y, word0 = 8 * (int64_t)blockIdx.x;
-    {
-        const int64_t y = row0 + t;
-#pragma unroll
-        for (int k = 0; k < 8; k += 2) {
-            uint2 v = make_uint2(0u, 0u);
-            if (y < L && word0 + k < W32) v = *reinterpret_cast<const uint2 *>(in + y * W32 + word0 + k);
-            tile[t][k] = v.x; tile[t][k + 1] = v.y;
-        }
+    const int64_t row0 = 256 * (int64_t)blockIdx.x, word0 = 32 * (int64_t)blockIdx.y;
+#pragma unroll 8
+    for (int i = 0; i < 32; ++i) {
+        const int row = warp + 8 * i;
+        const int64_t y = row0 + row;
+        uint32_t v = 0;
+        if (y < L && word0 + lane < W32) v = in[y * W32 + word0 + lane];
+        buf[row * 33 + lane] = v;
     }
     __syncthreads();
-    uint32_t r[8];
+    uint32_t r[32];
 #pragma unroll
-    for (int ty = 0; ty < 8; ++ty) r[ty] = transpose32(tile[32 * ty + lane][warp], lane);   // tile (ty, tx = warp)
+    for (int tx = 0; tx < 32; ++tx) r[tx] = transpose32(buf[(32 * warp + lane) * 33 + tx], lane);   // tile (ty = warp, tx)
     __syncthreads();
 #pragma unroll
-    for (int ty = 0; ty < 8; ++ty) tile[32 * warp + lane][ty] = r[ty];                      // output row 32 tx + lane, word ty
+    for (int tx = 0; tx < 32; ++tx) buf[(32 * tx + lane) * 9 + warp] = r[tx];                      // output row 32 tx + lane, word ty
     __syncthreads();
-    {
-        const int64_t x = 256 * (int64_t)blockIdx.x + t, yw0 = 8 * (int64_t)blockIdx.y;    // output row, first output word
-#pragma unroll
-        for (int k = 0; k < 8; k += 2)
-            if (x < L && yw0 + k < W32)
-                *reinterpret_cast<uint2 *>(out + x * W32 + yw0 + k) = make_uint2(tile[t][k], tile[t][k + 1]);
+    const int64_t x0 = 1024 * (int64_t)blockIdx.y, yw = 8 * (int64_t)blockIdx.x + (lane & 7);
+#pragma unroll 8
+    for (int i = 0; i < 32; ++i) {
+        const int row = 32 * i + 4 * warp + (lane >> 3);
+        const int64_t x = x0 + row;
+        if (x < L && yw < W32) out[x * W32 + yw] = buf[row * 9 + (lane & 7)];
     }
 }
 
@@ -280,7 +268,7 @@ cudaError_t launch_planes(ising_sim *h)
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     const int64_t W32 = 2 * Wq;
-    dim3 grid((unsigned)((W32 + 7) / 8), (unsigned)((L + 255) / 256));
+    dim3 grid((unsigned)((L + 255) / 256), (unsigned)((W32 + 31) / 32));
     for (int k = 0; k < np; ++k) {
         transpose_kernel<<<grid, 256, 0, h->stream>>>(reinterpret_cast<const uint32_t *>(h->planes + k * plane_words),
                                                      reinterpret_cast<uint32_t *>(h->planes + (np + k) * plane_words), L, W32);
