@@ -72,7 +72,10 @@ size_t ising_workspace_bytes(int model, int64_t L);
  *               (finite; ignored for Ising);  seed = Philox key
  *   dev_buf     device memory of >= ising_workspace_bytes() bytes, 256-byte
  *               aligned, owned by the caller and alive until ising_destroy;
- *               NULL: the library allocates (cudaMalloc) and frees it
+ *               NULL: the library allocates (cudaMalloc) and frees it.
+ *               The simulation lives on dev_buf's device (the current device
+ *               when dev_buf is NULL); every later call on the handle switches
+ *               to that device and restores the caller's on return
  *   cuda_stream a cudaStream_t (e.g. torch's current stream); NULL = default
  * Builds the acceptance thresholds floor(min(1, exp(-beta dE)) 2^32) in double
  * (PAPER.md:93 for the Ising probabilities), fills the lattice from the seed

@@ -29,6 +29,21 @@ extern "C" const char *ising_last_error(void) { return g_err.c_str(); }
 
 static void drop_graph(ising_sim *h);
 
+// Every entry point that takes a handle runs on the handle's device, whatever the caller's current
+// device is, and puts the caller's device back on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const ising_sim *h) { if (h) enter(h->device); }
+    explicit DeviceGuard(int device) { enter(device); }
+    void enter(int device)
+    {
+        if (device < 0 || cudaGetDevice(&prev) != cudaSuccess || prev == device) return;
+        switched = cudaSetDevice(device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+
 static bool valid_model_L(int model, int64_t L)
 {
     if (model == ISING_MODEL_ISING_LUT) return L >= 256 && (L % 256) == 0 && L <= (1ll << 20);   // 128-bit vector = 128 sites
@@ -137,6 +152,17 @@ extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_
     h->model = model; h->L = L; h->beta = beta; h->D = is_blume_capel(model) ? D : 0.0; h->seed = seed;
     h->stream = (cudaStream_t)cuda_stream;
     char *base = (char *)dev_buf;
+    cudaGetDevice(&h->device);                       // NULL dev_buf: the caller's current device
+    if (base) {
+        cudaPointerAttributes attr;
+        if (cudaPointerGetAttributes(&attr, base) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+            cudaGetLastError();
+            delete h;
+            return set_error(ISING_EINVAL, "ising_create: dev_buf is not device memory");
+        }
+        h->device = attr.device;
+    }
+    DeviceGuard dev_guard(h->device);
     if (!base) {
         cudaError_t e = cudaMalloc(&h->owned, need);
         if (e != cudaSuccess) {
@@ -230,6 +256,7 @@ extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_
 
 extern "C" int ising_destroy(ising_t *h)
 {
+    DeviceGuard dev_guard(h);
     if (!h) return ISING_OK;
     cudaStreamSynchronize(h->stream);
     if (h->io_stage) cudaFree(h->io_stage);
@@ -248,6 +275,7 @@ extern "C" int ising_destroy(ising_t *h)
 
 extern "C" int ising_sync(ising_t *h)
 {
+    DeviceGuard dev_guard(h);
     if (!h) return set_error(ISING_EINVAL, "ising_sync: NULL handle");
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     return ISING_OK;
@@ -314,6 +342,7 @@ static int ensure_graph(ising_sim *h)
 
 extern "C" int ising_sweep(ising_t *h, int64_t n)
 {
+    DeviceGuard dev_guard(h);
     if (!h) return set_error(ISING_EINVAL, "ising_sweep: NULL handle");
     if (n < 0) return set_error(ISING_EINVAL, "ising_sweep: n < 0");
     if (h->t + (uint64_t)n > 0xFFFFFFFFull) return set_error(ISING_EINVAL, "ising_sweep: sweep counter would exceed 2^32-1");
@@ -363,6 +392,7 @@ extern "C" int ising_time_grid(uint64_t tmax, uint64_t *out, int64_t cap, int64_
 // else the observables pass).  One call for "E and M every k sweeps" (BASELINE.json configs 1-3).
 extern "C" int ising_run_schedule(ising_t *h, int64_t n_times, const uint64_t *times, ising_obs_t *out)
 {
+    DeviceGuard dev_guard(h);
     if (!h || !times || !out || n_times < 0) return set_error(ISING_EINVAL, "ising_run_schedule: bad argument");
     uint64_t prev = h->t;
     for (int64_t i = 0; i < n_times; ++i) {
@@ -380,6 +410,7 @@ extern "C" int ising_run_schedule(ising_t *h, int64_t n_times, const uint64_t *t
 
 extern "C" int ising_set_sweeps_done(ising_t *h, uint64_t t)
 {
+    DeviceGuard dev_guard(h);
     if (!h) return set_error(ISING_EINVAL, "ising_set_sweeps_done: NULL handle");
     if (t > 0xFFFFFFFFull) return set_error(ISING_EINVAL, "ising_set_sweeps_done: t > 2^32-1");
     h->t = t;
@@ -388,6 +419,7 @@ extern "C" int ising_set_sweeps_done(ising_t *h, uint64_t t)
 
 extern "C" int ising_set_launch(ising_t *h, int rows_per_thread, int block_threads)
 {
+    DeviceGuard dev_guard(h);
     if (!h) return set_error(ISING_EINVAL, "ising_set_launch: NULL handle");
     if (rows_per_thread < 0 || (rows_per_thread & 1) || rows_per_thread > 4096)
         return set_error(ISING_EINVAL, "ising_set_launch: rows_per_thread must be even, in [2, 4096] (0 = keep)");
@@ -400,6 +432,7 @@ extern "C" int ising_set_launch(ising_t *h, int rows_per_thread, int block_threa
 
 extern "C" int ising_set_variant(ising_t *h, int variant)
 {
+    DeviceGuard dev_guard(h);
     if (!h) return set_error(ISING_EINVAL, "ising_set_variant: NULL handle");
     if (variant < 0 || variant > (h->model == ISING_MODEL_ISING_LUT ? 2 : 1)) return set_error(ISING_EINVAL, "ising_set_variant: unknown variant");
     h->variant = variant;
@@ -409,6 +442,7 @@ extern "C" int ising_set_variant(ising_t *h, int variant)
 // ----------------------------------------------------------- observables ---
 extern "C" int ising_observables(ising_t *h, ising_obs_t *out)
 {
+    DeviceGuard dev_guard(h);
     if (!h || !out) return set_error(ISING_EINVAL, "ising_observables: NULL argument");
     const bool lut = h->model == ISING_MODEL_ISING_LUT;
     cudaError_t e = lut ? launch_lut_observables(h) : launch_observables(h);
@@ -439,6 +473,7 @@ static int tally_resync(ising_sim *h)
 
 extern "C" int ising_set_tally(ising_t *h, int on)
 {
+    DeviceGuard dev_guard(h);
     if (!h) return set_error(ISING_EINVAL, "ising_set_tally: NULL handle");
     h->tally_on = on != 0;
     return h->tally_on ? tally_resync(h) : ISING_OK;
@@ -458,6 +493,7 @@ static void fill_obs(const ising_sim *h, const long long *bmq, ising_obs_t *o)
 
 extern "C" int ising_tally(ising_t *h, ising_obs_t *out)
 {
+    DeviceGuard dev_guard(h);
     if (!h || !out) return set_error(ISING_EINVAL, "ising_tally: NULL argument");
     if (!h->tally_on) return set_error(ISING_EINVAL, "ising_tally: the tally is off (ising_set_tally)");
     CUDA_TRY(cudaMemcpyAsync(h->h_acc + 40, h->d_acc + 40, 3 * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
@@ -468,6 +504,7 @@ extern "C" int ising_tally(ising_t *h, ising_obs_t *out)
 
 extern "C" int ising_schwinger_dyson(ising_t *h, int64_t hist[9], double *value)
 {
+    DeviceGuard dev_guard(h);
     if (!h || !hist || !value) return set_error(ISING_EINVAL, "ising_schwinger_dyson: NULL argument");
     cudaError_t e = (h->model == ISING_MODEL_ISING_LUT) ? launch_lut_sd_hist(h) : launch_sd_hist(h);
     if (e != cudaSuccess) return cuda_fail(e, "Schwinger-Dyson kernel");
@@ -484,6 +521,7 @@ extern "C" int ising_schwinger_dyson(ising_t *h, int64_t hist[9], double *value)
 
 extern "C" int ising_thresholds(ising_t *h, uint64_t *out, int cap, int *count)
 {
+    DeviceGuard dev_guard(h);
     if (!h || !count) return set_error(ISING_EINVAL, "ising_thresholds: NULL argument");
     *count = h->n_T;
     if (!out || cap < h->n_T) return set_error(ISING_EINVAL, "ising_thresholds: cap too small");
@@ -506,6 +544,7 @@ static const int64_t kStageBytes = 64ll << 20;
 
 extern "C" int ising_read_window(ising_t *h, int64_t x0, int64_t y0, int64_t w, int64_t hgt, int8_t *host_out)
 {
+    DeviceGuard dev_guard(h);
     if (!h || !host_out) return set_error(ISING_EINVAL, "ising_read_window: NULL argument");
     if (w < 1 || hgt < 1 || w > h->L || hgt > h->L) return set_error(ISING_EINVAL, "ising_read_window: window size out of range");
     const int64_t L = h->L;
@@ -525,6 +564,7 @@ extern "C" int ising_read_window(ising_t *h, int64_t x0, int64_t y0, int64_t w, 
 
 extern "C" int ising_read_lattice(ising_t *h, int64_t y0, int64_t ny, int8_t *host_out)
 {
+    DeviceGuard dev_guard(h);
     if (!h || !host_out) return set_error(ISING_EINVAL, "ising_read_lattice: NULL argument");
     if (y0 < 0 || ny < 1 || y0 + ny > h->L) return set_error(ISING_EINVAL, "ising_read_lattice: rows outside [0, L]");
     return ising_read_window(h, 0, y0, h->L, ny, host_out);
@@ -532,6 +572,7 @@ extern "C" int ising_read_lattice(ising_t *h, int64_t y0, int64_t ny, int8_t *ho
 
 extern "C" int ising_write_lattice(ising_t *h, int64_t y0, int64_t ny, const int8_t *host_in)
 {
+    DeviceGuard dev_guard(h);
     if (!h || !host_in) return set_error(ISING_EINVAL, "ising_write_lattice: NULL argument");
     if (y0 < 0 || ny < 1 || y0 + ny > h->L) return set_error(ISING_EINVAL, "ising_write_lattice: rows outside [0, L]");
     const int64_t L = h->L;
@@ -557,6 +598,7 @@ extern "C" int ising_write_lattice(ising_t *h, int64_t y0, int64_t ny, const int
 
 extern "C" int ising_read_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, uint64_t *host_out)
 {
+    DeviceGuard dev_guard(h);
     if (!h || !host_out) return set_error(ISING_EINVAL, "ising_read_packed: NULL argument");
     if ((colour != 0 && colour != 1) || word0 < 0 || nwords < 0 || word0 + nwords > colour_words(h))
         return set_error(ISING_EINVAL, "ising_read_packed: range outside the colour array");
@@ -567,6 +609,7 @@ extern "C" int ising_read_packed(ising_t *h, int colour, int64_t word0, int64_t 
 
 extern "C" int ising_write_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, const uint64_t *host_in)
 {
+    DeviceGuard dev_guard(h);
     if (!h || !host_in) return set_error(ISING_EINVAL, "ising_write_packed: NULL argument");
     if ((colour != 0 && colour != 1) || word0 < 0 || nwords < 0 || word0 + nwords > colour_words(h))
         return set_error(ISING_EINVAL, "ising_write_packed: range outside the colour array");
@@ -671,6 +714,7 @@ static int run_corr_gram(ising_sim *h, int64_t count, int64_t *sx, int64_t *sy)
 
 extern "C" int ising_correlation(ising_t *h, int64_t rmax, int64_t *sx, int64_t *sy)
 {
+    DeviceGuard dev_guard(h);
     if (!h || !sx || !sy) return set_error(ISING_EINVAL, "ising_correlation: NULL argument");
     if (rmax < 1 || rmax > h->L / 2) return set_error(ISING_EINVAL, "ising_correlation: rmax outside [1, L/2]");
     int rc = ensure_planes(h);
@@ -686,6 +730,7 @@ extern "C" int ising_correlation(ising_t *h, int64_t rmax, int64_t *sx, int64_t 
 
 extern "C" int ising_set_corr_path(ising_t *h, int path)
 {
+    DeviceGuard dev_guard(h);
     if (!h) return set_error(ISING_EINVAL, "ising_set_corr_path: NULL handle");
     if (path < 0 || path > 4) return set_error(ISING_EINVAL, "ising_set_corr_path: path must be 0 (auto), 1 (bit planes), 2 (tensor cores), 3 (CTA pairs) or 4 (CTA pairs, fp4)");
     h->corr_path = path;
@@ -696,6 +741,7 @@ static bool valid_stride(int64_t s) { return s == 1 || s == 2 || s == 4 || s == 
 
 extern "C" int ising_correlation_list(ising_t *h, int64_t stride, int64_t count, const int64_t *r, int64_t *sx, int64_t *sy)
 {
+    DeviceGuard dev_guard(h);
     if (!h || !r || !sx || !sy) return set_error(ISING_EINVAL, "ising_correlation_list: NULL argument");
     if (!valid_stride(stride)) return set_error(ISING_EINVAL, "ising_correlation_list: stride must be 1 or a power of two <= 64");
     if (count < 1 || count > 65535) return set_error(ISING_EINVAL, "ising_correlation_list: count outside [1, 65535]");
@@ -731,6 +777,7 @@ static void protocol_distances(int64_t L, uint64_t t, std::vector<int64_t> &dens
 extern "C" int ising_correlation_protocol(ising_t *h, int64_t cap, int64_t *r, int64_t *sx, int64_t *sy,
                                           int64_t *n_src, int64_t *count)
 {
+    DeviceGuard dev_guard(h);
     if (!h || !count) return set_error(ISING_EINVAL, "ising_correlation_protocol: NULL argument");
     std::vector<int64_t> dense, sparse;
     protocol_distances(h->L, h->t, dense, sparse);
@@ -755,6 +802,7 @@ extern "C" int ising_correlation_protocol(ising_t *h, int64_t cap, int64_t *r, i
 // ----------------------------------------------------- measurement helpers ---
 extern "C" int ising_bench_philox_only(ising_t *h, int n)
 {
+    DeviceGuard dev_guard(h);
     if (!h || n < 0 || h->model == ISING_MODEL_ISING_LUT) return set_error(ISING_EINVAL, "ising_bench_philox_only: bad argument");
     for (int i = 0; i < n; ++i) {
         cudaError_t e = launch_philox_only(h, (uint32_t)i);
@@ -765,6 +813,7 @@ extern "C" int ising_bench_philox_only(ising_t *h, int n)
 
 extern "C" int ising_bench_copy(ising_t *h, int n)
 {
+    DeviceGuard dev_guard(h);
     if (!h || n < 0 || h->model == ISING_MODEL_ISING_LUT) return set_error(ISING_EINVAL, "ising_bench_copy: bad argument");
     for (int i = 0; i < n; ++i) {
         cudaError_t e = launch_copy(h);

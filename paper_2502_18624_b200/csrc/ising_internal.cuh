@@ -21,6 +21,7 @@ struct ising_sim {
     uint64_t seed = 0;
     uint64_t t = 0;  // sweeps done
     cudaStream_t stream = nullptr;
+    int device = -1;  // CUDA device of the lattice (the current device at ising_create, or dev_buf's)
     uint64_t *lat[2] = {nullptr, nullptr};  // black, white colour arrays (device)
     void *owned = nullptr;                  // non-null if the library allocated dev_buf
     long long *d_acc = nullptr;             // 64 int64 accumulators inside the scratch area

@@ -276,6 +276,13 @@ def test_argument_errors(eng):
                 bad()
         sim.sweep(0)
         assert sim.observables().sweeps_done == 0
+    import ctypes as C                                                # a host pointer is not a lattice buffer
+    lib, n = eng.load_library(), eng.workspace_bytes(ISING, 64)
+    host = np.zeros(n + 256, dtype=np.uint8)
+    hp = (host.ctypes.data + 255) & ~255
+    handle = C.c_void_p()
+    assert lib.ising_create(ISING, 64, 0.4, 0.0, 1, hp, n, None, C.byref(handle)) == -1
+    assert b"not device memory" in lib.ising_last_error()
     sim2 = eng.IsingSim(ISING, 64, 0.4, use_torch_memory=False)     # library-owned memory
     sim2.sweep(2)
     s = oracle.init(ISING, 64, 1)
