@@ -101,6 +101,38 @@ cudaError_t launch_debug_philox(int64_t count, const uint32_t *d_ctr, const uint
 #define PHILOX_W0 0x9E3779B9u
 #define PHILOX_W1 0xBB67AE85u
 
+// Block-level sum of N per-thread ints into the int64 accumulators dst[0..N): warp
+// reduction (warp sums must fit 32 bits), one shared-memory atomic per warp, ONE
+// global atomic per block and quantity.  Same-address global atomics serialise in
+// one L2 slice (about 1.3 ns each on B200): with one per warp the observables pass
+// at L = 2^18 spent 4 of its 9 ms waiting for 3.1 M of them.  Every live thread of
+// the block must call this; threads that returned earlier count as arrived at the
+// barriers, and thread 0 is alive whenever any thread of its block is (the threads
+// past the lattice are the highest ones).
+template <int N>
+__device__ __forceinline__ void block_accumulate(const int (&v)[N], long long *dst)
+{
+    __shared__ unsigned long long s_acc[N];
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < N; ++k) s_acc[k] = 0;
+    }
+    __syncthreads();
+    const unsigned m = __activemask();
+    const bool leader = (int)(threadIdx.x & 31) == __ffs(m) - 1;
+#pragma unroll
+    for (int k = 0; k < N; ++k) {
+        const int sum = __reduce_add_sync(m, v[k]);
+        if (leader && sum) atomicAdd(&s_acc[k], (unsigned long long)(long long)sum);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < N; ++k)
+            if (s_acc[k]) atomicAdd(reinterpret_cast<unsigned long long *>(&dst[k]), s_acc[k]);
+    }
+}
+
 // Generic Philox4x32-10: ten rounds of
 //   (c0,c1,c2,c3) <- (hi(M1*c2)^c1^k0, lo(M1*c2), hi(M0*c0)^c3^k1, lo(M0*c0)).
 __device__ __forceinline__ uint4 philox4x32_10(uint4 c, const RoundKeys &rk)

@@ -246,14 +246,8 @@ __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const _
         o1 += 2 * rs; eo += 2 * rs; w0 += 2 * rs;
     }
     if (TALLY) {
-        const unsigned m = __activemask();
         const int v[2] = {dB, dM};
-#pragma unroll
-        for (int k = 0; k < 2; ++k) {
-            const int sum = __reduce_add_sync(m, v[k]);
-            if ((int)(threadIdx.x & 31) == __ffs(m) - 1 && sum)
-                atomicAdd(reinterpret_cast<unsigned long long *>(&p.tally[k]), (unsigned long long)(long long)sum);
-        }
+        block_accumulate<2>(v, p.tally);
     }
 }
 

@@ -2,7 +2,7 @@
 // histogram (Eq. 3).  Same register sliding window as the update
 // kernel: each thread walks R rows of one 128-bit column (64-bit at 2 bits per spin) of the BLACK array and
 // sees every bond exactly once (for even L every bond joins a black and a white
-// site).  Warp shuffle -> one int64 atomic per warp per quantity.
+// site).  Warp reduction -> one int64 atomic per block per quantity (block_accumulate).
 #include "ising_internal.cuh"
 #include "row_format.cuh"
 
@@ -19,13 +19,6 @@ __device__ __forceinline__ uint32_t nibble_sum(uint32_t x)  // sum of the 8 nibb
 {
     uint32_t t = (x & 0x0F0F0F0Fu) + ((x >> 4) & 0x0F0F0F0Fu);
     return (t * 0x01010101u) >> 24;
-}
-
-__device__ __forceinline__ long long warp_sum(long long v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-    return v;
 }
 
 // MODE 0: B, M, Q.  MODE 1: Schwinger-Dyson histogram of s*h over the centre sites.
@@ -103,19 +96,11 @@ __global__ void __launch_bounds__(256) observe_kernel(const __grid_constant__ Ob
             up = sm; sm = dn;
         }
     }
-    if (MODE == 0) {
-        long long b = warp_sum(B), m = warp_sum(M), q = warp_sum(Q);
-        if ((threadIdx.x & 31) == 0) {
-            atomicAdd((unsigned long long *)&p.acc[0], (unsigned long long)b);
-            atomicAdd((unsigned long long *)&p.acc[1], (unsigned long long)m);
-            atomicAdd((unsigned long long *)&p.acc[2], (unsigned long long)q);
-        }
+    if (MODE == 0) {          // warp sums fit 32 bits: <= 32 lanes x R rows x 128 sites x 4
+        const int v[3] = {B, M, Q};
+        block_accumulate<3>(v, p.acc);
     } else {
-#pragma unroll
-        for (int k = 0; k < 9; ++k) {
-            long long v = warp_sum(hist[k]);
-            if ((threadIdx.x & 31) == 0 && v) atomicAdd((unsigned long long *)&p.acc[8 + k], (unsigned long long)v);
-        }
+        block_accumulate<9>(hist, p.acc + 8);
     }
 }
 
@@ -127,7 +112,7 @@ static cudaError_t launch_obs(ising_sim *h, int centre)
     p.nbr = reinterpret_cast<const uint4 *>(h->lat[1 - centre]);
     p.centre = centre;
     p.L = (int)h->L; p.cols = (int)(h->L / 64);
-    p.R = (h->L >= 2048) ? 32 : 4;
+    p.R = (h->L >= 65536) ? 64 : (h->L >= 2048) ? 32 : 4;   // rows per thread: halo re-reads 2/R, still >= 1 M threads at R = 64
     p.acc = h->d_acc;
     int64_t chunks = (h->L + p.R - 1) / p.R;
     int64_t threads = chunks * p.cols;

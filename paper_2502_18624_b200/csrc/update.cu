@@ -412,14 +412,8 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
         o1 += 2 * rs; eo += 2 * rs; w0 += 2 * rs;
     }
     if (TALLY) {            // warp sums fit 32 bits (<= 32 lanes x R rows x 32 sites x 8); threads past the lattice have returned
-        const unsigned m = __activemask();
         const int v[3] = {dB, dM, dQ};
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const int sum = __reduce_add_sync(m, v[k]);
-            if ((int)(threadIdx.x & 31) == __ffs(m) - 1 && sum)
-                atomicAdd(reinterpret_cast<unsigned long long *>(&p.tally[k]), (unsigned long long)(long long)sum);
-        }
+        block_accumulate<3>(v, p.tally);
     }
 }
 
