@@ -312,70 +312,102 @@ cudaError_t launch_lut_init(ising_sim *h)
 }
 
 // ----------------------------------------------------------- observables ---
-// One thread per 32-bit word of the CENTRE colour array: d = unequal neighbours per site from
-// four XORs.  MODE 0 (centre = black only): B = sum (4 - 2 d) over black sites (each bond once),
-// M from the black word and the white word of the same position.  MODE 1 (run for both
-// colours): histogram of s*h = 4 - 2 d, bit-sliced count of the four difference words.
+// Same register sliding window as the update kernel: a thread walks R rows of one 128-bit column
+// (128 sites) of the CENTRE colour array and reads every word of both arrays once (+2/R halo rows);
+// d = unequal neighbours per site from four XORs.  MODE 0 (centre = black only): B = sum (4 - 2 d)
+// over black sites (each bond once), M from the black word and the white word of the same position.
+// MODE 1 (run for both colours): histogram of s*h = 4 - 2 d, bit-sliced count of the four
+// difference words.  One global atomic per block and quantity (block_accumulate).
+struct LutObsParams {
+    const uint4 *ctr, *nbr;
+    int centre, L, cols, R;
+    long long *acc;
+};
+
 template <int MODE>
-__global__ void __launch_bounds__(256) lut_observe_kernel(const uint32_t *__restrict__ ctr, const uint32_t *__restrict__ nbr,
-                                                          int centre, int L, long long *acc)
+__global__ void __launch_bounds__(256) lut_observe_kernel(const __grid_constant__ LutObsParams p)
 {
-    const int W = L / 64;                                    // 32-bit words per colour row
-    const int64_t n = (int64_t)L * W, stride = (int64_t)gridDim.x * blockDim.x;
-    long long v[5] = {0, 0, 0, 0, 0};
-    // grid-stride loop: a few thousand threads keep private sums, so the atomics at the end are few
-    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += stride) {
-        const int y = (int)(idx / W), q = (int)(idx - (int64_t)y * W);
-        const int ym = (y == 0) ? L - 1 : y - 1, yp = (y + 1 == L) ? 0 : y + 1;
-        const uint32_t x = ctr[idx], up = nbr[(int64_t)ym * W + q], dn = nbr[(int64_t)yp * W + q], sm = nbr[idx];
-        uint32_t sd;
-        if (((y + centre) & 1) == 0) sd = (sm << 1) | (nbr[(int64_t)y * W + (q == 0 ? W - 1 : q - 1)] >> 31);
-        else sd = (sm >> 1) | (nbr[(int64_t)y * W + (q == W - 1 ? 0 : q + 1)] << 31);
-        const uint32_t a = up ^ x, b = dn ^ x, c = sm ^ x, d = sd ^ x;   // 1 where the neighbour differs
-        if (MODE == 0) {
-            v[0] += 128 - 2 * (__popc(a) + __popc(b) + __popc(c) + __popc(d));
-            v[1] += 2 * (__popc(x) + __popc(sm)) - 64;
-        } else {
-            const uint32_t s0 = a ^ b, c0 = a & b, s1 = c ^ d, c1 = c & d;
-            const uint32_t b0 = s0 ^ s1, t = s0 & s1, b1 = c0 ^ c1 ^ t, b2 = c0 & c1;   // d = b0 + 2 b1 + 4 b2
-            v[0] += __popc(~b0 & ~b1 & ~b2); v[1] += __popc(b0 & ~b1); v[2] += __popc(~b0 & b1);
-            v[3] += __popc(b0 & b1); v[4] += __popc(b2);
+    const int cols = p.cols, L = p.L;
+    const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned chunk = tid / (unsigned)cols;
+    const int col = (int)(tid - chunk * (unsigned)cols);
+    const int y0 = (int)chunk * p.R;
+    int v[5] = {0, 0, 0, 0, 0};
+    if (y0 < L) {
+        const int yend = min(L, y0 + p.R);
+        const char *nbr = reinterpret_cast<const char *>(p.nbr), *ctr = reinterpret_cast<const char *>(p.ctr);
+        const size_t rs = (size_t)cols * 16, cb = (size_t)col * 16;
+        const int halves = cols * 4;
+        const size_t e0 = (size_t)((col == 0) ? halves - 1 : 4 * col - 1) * 4;   // parity 0: top bit of the previous word
+        const size_t e1 = (size_t)((col == cols - 1) ? 0 : 4 * col + 4) * 4;     // parity 1: low bit of the next word
+        const int ym = (y0 == 0) ? L - 1 : y0 - 1;
+        uint4 up = *reinterpret_cast<const uint4 *>(nbr + (size_t)ym * rs + cb);
+        uint4 sm = *reinterpret_cast<const uint4 *>(nbr + (size_t)y0 * rs + cb);
+        for (int y = y0; y < yend; ++y) {
+            const int yp = (y + 1 == L) ? 0 : y + 1;
+            const uint4 dn = *reinterpret_cast<const uint4 *>(nbr + (size_t)yp * rs + cb);
+            const uint4 x4 = *reinterpret_cast<const uint4 *>(ctr + (size_t)y * rs + cb);
+            uint32_t sd[4];
+            if (((y + p.centre) & 1) == 0) lut_side<0>(sm, *reinterpret_cast<const uint32_t *>(nbr + (size_t)y * rs + e0), sd);
+            else lut_side<1>(sm, *reinterpret_cast<const uint32_t *>(nbr + (size_t)y * rs + e1), sd);
+            const uint32_t xs[4] = {x4.x, x4.y, x4.z, x4.w}, us[4] = {up.x, up.y, up.z, up.w};
+            const uint32_t ds[4] = {dn.x, dn.y, dn.z, dn.w}, ms[4] = {sm.x, sm.y, sm.z, sm.w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const uint32_t x = xs[k];
+                const uint32_t a = us[k] ^ x, b = ds[k] ^ x, c = ms[k] ^ x, d = sd[k] ^ x;   // 1 where the neighbour differs
+                if (MODE == 0) {
+                    v[0] += 128 - 2 * (__popc(a) + __popc(b) + __popc(c) + __popc(d));
+                    v[1] += 2 * (__popc(x) + __popc(ms[k])) - 64;
+                } else {
+                    const uint32_t s0 = a ^ b, c0 = a & b, s1 = c ^ d, c1 = c & d;
+                    const uint32_t b0 = s0 ^ s1, t = s0 & s1, b1 = c0 ^ c1 ^ t, b2 = c0 & c1;   // d = b0 + 2 b1 + 4 b2
+                    v[0] += __popc(~b0 & ~b1 & ~b2); v[1] += __popc(b0 & ~b1); v[2] += __popc(~b0 & b1);
+                    v[3] += __popc(b0 & b1); v[4] += __popc(b2);
+                }
+            }
+            up = sm; sm = dn;
         }
     }
-#pragma unroll
-    for (int k = 0; k < 5; ++k) {
-        long long s = v[k];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
-        if ((threadIdx.x & 31) == 0 && s) {
-            // MODE 0: acc[0] = B, acc[1] = M.  MODE 1: d = k  <->  s*h = 4 - 2k  <->  hist index 8 - 2k (acc + 8)
-            long long *dst = (MODE == 0) ? &acc[k] : &acc[8 + 8 - 2 * k];
-            if (MODE == 1 || k < 2) atomicAdd(reinterpret_cast<unsigned long long *>(dst), (unsigned long long)s);
-        }
+    if (MODE == 0) {          // acc[0] = B, acc[1] = M; warp sums fit 32 bits (<= 32 lanes x R rows x 512)
+        const int bm[2] = {v[0], v[1]};
+        block_accumulate<2>(bm, p.acc);
+    } else {                  // d = k  <->  s*h = 4 - 2k  <->  hist index 8 - 2k (acc + 8)
+        const int hist[9] = {v[4], 0, v[3], 0, v[2], 0, v[1], 0, v[0]};
+        block_accumulate<9>(hist, p.acc + 8);
     }
+}
+
+template <int MODE>
+static cudaError_t launch_lut_obs(ising_sim *h, int centre)
+{
+    LutObsParams p;
+    p.ctr = reinterpret_cast<const uint4 *>(h->lat[centre]);
+    p.nbr = reinterpret_cast<const uint4 *>(h->lat[1 - centre]);
+    p.centre = centre;
+    p.L = (int)h->L; p.cols = (int)(h->L / 256);
+    p.R = 64;                 // rows per thread: as long as the grid keeps two full waves of threads
+    while (p.R > 4 && (h->L / p.R) * p.cols < 148 * 2048 * 2) p.R >>= 1;
+    p.acc = h->d_acc;
+    const int64_t threads = ((h->L + p.R - 1) / p.R) * p.cols;
+    const int block = 128;
+    lut_observe_kernel<MODE><<<(unsigned)((threads + block - 1) / block), block, 0, h->stream>>>(p);
+    h->launches++;
+    return cudaGetLastError();
 }
 
 cudaError_t launch_lut_observables(ising_sim *h)
 {
     cudaError_t e = cudaMemsetAsync(h->d_acc, 0, 8 * sizeof(long long), h->stream);
     if (e != cudaSuccess) return e;
-    const int64_t n = h->L * (h->L / 64);
-    const unsigned grid_obs = (unsigned)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16);
-    lut_observe_kernel<0><<<grid_obs, 256, 0, h->stream>>>(
-        reinterpret_cast<const uint32_t *>(h->lat[0]), reinterpret_cast<const uint32_t *>(h->lat[1]), 0, (int)h->L, h->d_acc);
-    h->launches++;
-    return cudaGetLastError();
+    return launch_lut_obs<0>(h, 0);
 }
 
 cudaError_t launch_lut_sd_hist(ising_sim *h)
 {
     cudaError_t e = cudaMemsetAsync(h->d_acc + 8, 0, 9 * sizeof(long long), h->stream);
     if (e != cudaSuccess) return e;
-    const int64_t n = h->L * (h->L / 64);
-    for (int c = 0; c < 2; ++c) {
-        lut_observe_kernel<1><<<(unsigned)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16), 256, 0, h->stream>>>(
-            reinterpret_cast<const uint32_t *>(h->lat[c]), reinterpret_cast<const uint32_t *>(h->lat[1 - c]), c, (int)h->L, h->d_acc);
-        h->launches++;
-    }
-    return cudaGetLastError();
+    e = launch_lut_obs<1>(h, 0);
+    if (e != cudaSuccess) return e;
+    return launch_lut_obs<1>(h, 1);
 }
