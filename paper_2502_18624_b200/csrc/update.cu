@@ -312,13 +312,17 @@ __device__ __forceinline__ void tally_half(uint32_t x, uint32_t y, uint32_t up, 
         dB += 4 * (int)nibble_sum32(d & (F * 15u)) - 8 * cnt;
         dM += 2 * cnt - 4 * cnt_up;
     } else {
-        const uint32_t S = up + dn + sm + sd;
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            const int s0 = (int)((x >> (4 * j)) & 15u) - 1, s1 = (int)((y >> (4 * j)) & 15u) - 1;
-            const int h = (int)((S >> (4 * j)) & 15u) - 4;
-            dB += (s1 - s0) * h; dM += s1 - s0; dQ += s1 * s1 - s0 * s0;
-        }
+        // codes 0, 1, 2 <-> s = -1, 0, +1: bit 0 marks s = 0, bit 1 marks s = +1.  Word level:
+        // sum (s1 - s0) = sum (c1 - c0) from four POPCs, s^2 = 1 unless bit 0, and per site
+        // c * S = (S where bit 0) + 2 (S where bit 1), so sum (c1 - c0)(S - 4) is four masked nibble sums.
+        const uint32_t S = up + dn + sm + sd;                      // h + 4 per nibble, <= 8
+        const uint32_t x0 = x & ONES, x1 = (x >> 1) & ONES, y0 = y & ONES, y1 = (y >> 1) & ONES;
+        const int px0 = __popc(x0), py0 = __popc(y0);
+        const int m = py0 + 2 * __popc(y1) - px0 - 2 * __popc(x1);
+        dM += m;
+        dQ += px0 - py0;
+        dB += (int)nibble_sum32(S & (y0 * 15u)) + 2 * (int)nibble_sum32(S & (y1 * 15u))
+            - (int)nibble_sum32(S & (x0 * 15u)) - 2 * (int)nibble_sum32(S & (x1 * 15u)) - 4 * m;
     }
 }
 
