@@ -62,6 +62,8 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--L", type=int, default=0, help="override the lattice size (default: configs[2], 2^18)")
+    ap.add_argument("--config", type=int, default=-1, choices=[-1, 0, 1, 2, 3, 4],
+                    help="time BASELINE.json configs[i] (model, L, beta, D, seed of that config); -1: --model / --workload decide")
     ap.add_argument("--model", default="ising", choices=["ising", "bc", "lut", "bc2"],
                     help="ising / bc: the north_star kernels (configs[2] / [3]); lut: NEXT-2, the paper's 1-bit look-up-table kernel on configs[2]'s parameters")
     ap.add_argument("--sweeps-per-step", type=int, default=10)
@@ -71,7 +73,7 @@ def parse_args():
     ap.add_argument("--rows-per-thread", type=int, default=0, help="update-kernel launch geometry (0 = library default)")
     ap.add_argument("--block", type=int, default=0, help="update-kernel threads per block (0 = library default)")
     ap.add_argument("--variant", type=int, default=0, help="update-kernel variant (0 = default carry form)")
-    ap.add_argument("--corr-path", type=int, default=0, help="ising_set_corr_path: 0 auto (tensor cores, CTA pairs), 1 bit planes, 2 tensor cores one CTA per tile, 3 CTA pairs")
+    ap.add_argument("--corr-path", type=int, default=0, help="ising_set_corr_path: 0 auto (fp4 tensor cores, path 4, for wide bands), 1 bit planes, 2 int8 tensor cores one CTA per tile, 3 int8 CTA pairs, 4 fp4 CTA pairs")
     ap.add_argument("--tally", action="store_true", help="A7: keep E, M by the fused tally of the update kernels instead of the observables pass")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -80,6 +82,12 @@ def parse_args():
 
 
 def pick_workload(args):
+    if getattr(args, "config", -1) >= 0:
+        base = wl.config(args.config)
+        args.model = "bc" if base.model == wl.BLUME_CAPEL else "ising"
+        if args.config == 4:
+            args.workload = "corr"
+        return base, base.L, base.name
     base = wl.config(3) if args.model in ("bc", "bc2") else wl.config(2)
     if getattr(args, "workload", "sweep") == "corr":
         base = wl.config(4)

@@ -19,7 +19,11 @@
  *
  * Pointers: every pointer argument is a HOST pointer unless its name starts
  * with dev_.  All calls return ISING_OK (0) or a negative error; outputs are
- * written only on ISING_OK.  Nothing throws or aborts.  ising_last_error()
+ * written only on ISING_OK, with one documented exception: calls that fill
+ * caller arrays of a size only the library knows take a `count` pointer, which
+ * is written whenever the arguments up to it are valid -- pass NULL for the
+ * output arrays to ask for the size (returns ISING_OK), a too small `cap`
+ * gives ISING_EINVAL with *count still set.  Nothing throws or aborts.  ising_last_error()
  * gives a thread-local message for the last non-OK return on this thread.
  * A handle is not thread-safe; distinct handles are independent.  Work is
  * enqueued on the stream given at create; calls documented as "synchronises"
@@ -119,10 +123,18 @@ int ising_set_corr_path(ising_t *h, int path);
 /* The paper's down-sampled protocol at t = sweeps_done:
  * all sources for r <= 32; sources {x % 16 == 0, y % 16 == 0} for 32 < r <=
  * r_c(t) and for r on the logarithmic grid up to L/2.  Arrays of capacity cap;
- * *count receives the number of distances (also when cap is too small, with
- * ISING_EINVAL).  Synchronises.                                             */
+ * *count receives the number of distances (size query: all four arrays NULL).
+ * The arrays are written only when every kernel has succeeded.  Synchronises. */
 int ising_correlation_protocol(ising_t *h, int64_t cap, int64_t *r, int64_t *sx, int64_t *sy,
                                int64_t *n_src, int64_t *count);
+
+/* The distance list of that protocol on its own (host arithmetic, no handle, no GPU):
+ *   r = 1..2R, R = 16                                   every site a source   stride[i] = 1
+ *   r = 2R+1..r_c(t), r_c = max{256, [g(L) sqrt(t)]},
+ *       g(L) = 6 sqrt(ln(L / 2^16) / 3.3^2 + 1)         one source per R x R  stride[i] = 16
+ *   r = floor(2^(x/32)) > r_c(t) while 2^(x/32) <= L/2   stride[i] = 16
+ * ascending, clipped to L/2 (L even).  Size query: r == stride == NULL.          */
+int ising_protocol_distances(int64_t L, uint64_t t, int64_t cap, int64_t *r, int64_t *stride, int64_t *count);
 
 /* Same sums for an explicit strictly positive distance list (each <= L/2) and
  * a source stride (sources x % stride == 0 and y % stride == 0; stride 1 or a
@@ -150,20 +162,33 @@ int ising_read_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, uin
 int ising_write_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, const uint64_t *host_in);
 /* Schedule interleave (A11 of SURVEY.md Sec. 8(a)).  ising_time_grid: the paper's measurement
  * times t = floor(2^(x/8) + 0.5), x = 1, 2, ..., de-duplicated, t <= tmax, into the
- * host array out (capacity cap); *count = number of times (also when cap is too small, with
- * ISING_EINVAL).  ising_run_schedule: sweeps to each time of the ascending host array times
+ * host array out (capacity cap); *count = number of times (size query: out == NULL).  Host
+ * arithmetic only: no handle, no GPU.  ising_run_schedule: sweeps to each time of the ascending host array times
  * (all >= sweeps_done) and records the integer observables there in out[i] (by the fused tally
  * if it is on, else by the observables pass).  Synchronises at every measurement.        */
 int ising_time_grid(uint64_t tmax, uint64_t *out, int64_t cap, int64_t *count);
 int ising_run_schedule(ising_t *h, int64_t n_times, const uint64_t *times, ising_obs_t *out);
+/* The same interleave with the correlation measurement: sweeps to each time and runs
+ * the Sec. 3.3 protocol there.  r, sx, sy, n_src are host arrays of n_times x cap int64, row-major: row i
+ * receives counts[i] entries (as ising_correlation_protocol at times[i]); cap must hold the longest list
+ * (ising_protocol_distances at the last time).  obs (may be NULL): the integer observables at the same
+ * times.  Synchronises at every measurement.                                                  */
+int ising_run_protocol_schedule(ising_t *h, int64_t n_times, const uint64_t *times, int64_t cap,
+                                int64_t *r, int64_t *sx, int64_t *sy, int64_t *n_src, int64_t *counts,
+                                ising_obs_t *obs);
 
 /* Set the sweep counter t (exact resume: state = lattice + t).               */
 int ising_set_sweeps_done(ising_t *h, uint64_t t);
 
 /* Threshold table dump for the equality assert against the oracle: Ising 5
- * entries indexed (dE+8)/4; Blume-Capel 54 entries ((s+1)*2+b)*9 + (h+4).
- * Values in [0, 2^32].  *count = entries; ISING_EINVAL if cap too small.    */
+ * entries indexed (dE+8)/4; Blume-Capel 54 entries ((s+1)*2+b)*9 + (h+4); the
+ * 1-bit look-up-table model 16 entries, entry i = floor(2^32 P(pattern < i)),
+ * patterns of four independent bits that are 1 with probability e^{-4 beta}
+ * (PAPER.md:133-149).  Values in [0, 2^32].  *count = entries (size query: out
+ * == NULL).  ising_threshold_table computes the same table from (model, beta, D)
+ * alone: host arithmetic, no handle, no GPU.                                */
 int ising_thresholds(ising_t *h, uint64_t *out, int cap, int *count);
+int ising_threshold_table(int model, double beta, double D, uint64_t *out, int cap, int *count);
 
 /* Launch geometry of the update kernel (results never depend on it,
  * cf. PAPER.md:193): rows walked per thread and threads per block
@@ -181,26 +206,6 @@ int64_t ising_launch_count(const ising_t *h);
 int ising_sync(ising_t *h);
 int ising_destroy(ising_t *h);
 const char *ising_last_error(void);
-
-/* Measurement helpers (not part of a simulation): n calls of the Philox-only
- * kernel with the update kernel's grid (the ALU roof), and a plain
- * read+write pass over the colour arrays (the HBM roof).  Asynchronous.     */
-int ising_bench_philox_only(ising_t *h, int n);
-int ising_bench_copy(ising_t *h, int n);
-
-/* Integer-pipe probe: issue rates, in warp-instructions per SM
- * sub-partition per clock at sm_mhz (<= 0: the device's maximum clock), of dependent chains of
- * [0] IMAD.WIDE  [1] LOP3  [2] IMAD  [3] IMAD.WIDE+LOP3  [4] IMAD.WIDE+2 LOP3
- * [5] IADD3(carry)+IMAD.X  [6] IMAD.WIDE+IMAD  [7] POPC+IADD (sum of both kinds per entry).
- * rates: host array of capacity cap; *count = 8.  Runs on the current device, default
- * stream, synchronises.  The ALU roofline of the update kernel is derived from these.     */
-int ising_bench_pipes(double sm_mhz, double *rates, int cap, int *count);
-
-/* Debug / test entry: evaluates this library's device Philox4x32-10 for count
- * (ctr, key) pairs (host arrays: ctr 4*count, key 2*count, out 4*count words).
- * with_curand != 0 evaluates the CUDA toolkit's curand_Philox4x32_10 instead.  */
-int ising_debug_philox(int64_t count, const uint32_t *ctr, const uint32_t *key, uint32_t *out,
-                       int with_curand);
 
 #ifdef __cplusplus
 }

@@ -87,6 +87,24 @@ def observables(s: np.ndarray):
     return int(out[0]), int(out[1]), int(out[2])
 
 
+def observables_rows(L: int, band: np.ndarray):
+    """(B, M, Q) of the first ny rows of ``band`` ((ny + 1) x L: the last row is only the lower neighbour)."""
+    band = np.ascontiguousarray(band, dtype=np.int8)
+    assert band.ndim == 2 and band.shape[1] == L and band.shape[0] >= 2
+    out = np.zeros(3, dtype=np.int64)
+    lib().orc_observables_rows(C.c_int64(L), C.c_int64(band.shape[0] - 1), _p(band, C.c_int8), _p(out, C.c_int64))
+    return int(out[0]), int(out[1]), int(out[2])
+
+
+def sd_hist_rows(L: int, band: np.ndarray) -> np.ndarray:
+    """Schwinger-Dyson histogram of the inner rows of ``band`` ((ny + 2) x L: first and last row are halos)."""
+    band = np.ascontiguousarray(band, dtype=np.int8)
+    assert band.ndim == 2 and band.shape[1] == L and band.shape[0] >= 3
+    hist = np.zeros(9, dtype=np.int64)
+    lib().orc_sd_hist_rows(C.c_int64(L), C.c_int64(band.shape[0] - 2), _p(band, C.c_int8), _p(hist, C.c_int64))
+    return hist
+
+
 def normalised(model: int, L: int, D: float, bmq):
     """(E, E/N, M/N, zero density) in double from the integers."""
     b = np.asarray(bmq, dtype=np.int64).copy()

@@ -210,10 +210,15 @@ void orc_sweep_patch(int model, int64_t L, double beta, double D, uint64_t seed,
 {
     uint64_t T[54];
     orc_thresholds(model, beta, D, T);
-    int64_t dump[3] = { 0, 0, 0 };
-    for (uint32_t c = 0; c < 2; ++c)
+    /* rows of one colour are independent (no two same-colour sites are neighbours, L even): the row loop
+     * may be split over threads exactly as in orc_sweep */
+    for (uint32_t c = 0; c < 2; ++c) {
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) if ((L % 2) == 0 && h >= 16)
+#endif
         for (int64_t j = 0; j < h; ++j)
             for (int64_t i = 0; i < w; ++i) {
+                int64_t dump[3] = { 0, 0, 0 };
                 int64_t x = ((x0 + i) % L + L) % L, y = ((y0 + j) % L + L) % L;
                 if ((uint32_t)((x + y) & 1) != c) continue;
                 int hs = 0;
@@ -224,6 +229,7 @@ void orc_sweep_patch(int model, int64_t L, double beta, double D, uint64_t seed,
                 uint32_t r = orc_draw(seed, site_index(L, x, y), t, c);
                 attempt(model, T, r, hs, &s[j * w + i], &dump[0], &dump[1], &dump[2]);
             }
+    }
 }
 
 /* ------------------------------------------------------------------ O5 --- */
@@ -232,6 +238,9 @@ void orc_sweep_patch(int model, int64_t L, double beta, double D, uint64_t seed,
 void orc_observables(int64_t L, const int8_t *s, int64_t *out)
 {
     int64_t B = 0, M = 0, Q = 0;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) reduction(+ : B, M, Q) if (L >= 1024)
+#endif
     for (int64_t y = 0; y < L; ++y)
         for (int64_t x = 0; x < L; ++x) {
             int v = s[y * L + x];
@@ -239,6 +248,40 @@ void orc_observables(int64_t L, const int8_t *s, int64_t *out)
             M += v; Q += v * v;
         }
     out[0] = B; out[1] = M; out[2] = Q;
+}
+
+/* The same sums restricted to the rows [y0, y0 + ny) of the lattice, for lattices the host cannot hold
+ * (SURVEY.md Sec. 8(c) "Large-L parity": O5 applied to a lattice streamed out in row bands): band holds
+ * ny + 1 rows of L spins -- the rows y0 .. y0 + ny, the last one (row (y0 + ny) mod L) only as the lower
+ * neighbour of row y0 + ny - 1.  The bands of a partition of [0, L) add up to orc_observables.          */
+void orc_observables_rows(int64_t L, int64_t ny, const int8_t *band, int64_t *out)
+{
+    int64_t B = 0, M = 0, Q = 0;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) reduction(+ : B, M, Q) if (L >= 1024)
+#endif
+    for (int64_t j = 0; j < ny; ++j)
+        for (int64_t x = 0; x < L; ++x) {
+            int v = band[j * L + x];
+            B += v * (band[j * L + (x + 1) % L] + band[(j + 1) * L + x]);
+            M += v; Q += v * v;
+        }
+    out[0] = B; out[1] = M; out[2] = Q;
+}
+
+/* Schwinger-Dyson histogram (Eq. 3) of the rows [y0, y0 + ny): band holds ny + 2 rows, the rows
+ * y0 - 1 .. y0 + ny (mod L); hist[k+4] += #sites of the ny inner rows with s*h = k.                    */
+void orc_sd_hist_rows(int64_t L, int64_t ny, const int8_t *band, int64_t *hist)
+{
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) reduction(+ : hist[:9]) if (L >= 1024)
+#endif
+    for (int64_t j = 1; j <= ny; ++j)
+        for (int64_t x = 0; x < L; ++x) {
+            int h = band[(j - 1) * L + x] + band[(j + 1) * L + x]
+                  + band[j * L + (x + L - 1) % L] + band[j * L + (x + 1) % L];
+            hist[band[j * L + x] * h + 4] += 1;
+        }
 }
 
 /* E = -B (Ising, Eq. 1) or -B + D*Q (Blume-Capel, Eq. 2; R10), J = 1.
@@ -256,6 +299,9 @@ void orc_normalised(int model, int64_t L, double D, const int64_t *bmq, double *
 double orc_schwinger_dyson(int64_t L, double beta, const int8_t *s, int64_t *hist)
 {
     for (int k = 0; k < 9; ++k) hist[k] = 0;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) reduction(+ : hist[:9]) if (L >= 1024)
+#endif
     for (int64_t y = 0; y < L; ++y)
         for (int64_t x = 0; x < L; ++x) {
             int h = s[((y + L - 1) % L) * L + x] + s[((y + 1) % L) * L + x]
@@ -520,7 +566,10 @@ void orc_lut_sweep_patch(int64_t L, double beta, uint64_t seed, uint32_t t,
     orc_lut_table(beta, table);
     const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
     const int64_t Wr = lut_words_per_row(L);
-    for (uint32_t c = 0; c < 2; ++c)
+    for (uint32_t c = 0; c < 2; ++c) {
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) if ((L % 2) == 0 && h >= 16)
+#endif
         for (int64_t j = 0; j < h; ++j)
             for (int64_t i = 0; i < w; ++i) {
                 const int64_t x = ((x0 + i) % L + L) % L, y = ((y0 + j) % L + L) % L;
@@ -545,6 +594,7 @@ void orc_lut_sweep_patch(int64_t L, double beta, uint64_t seed, uint32_t t,
                 const int flip = (eq == 4 && b[0] && b[1]) || (eq == 3 && b[0]) || (eq <= 2);
                 if (flip) s[j * w + i] = (int8_t)(-sp);
             }
+    }
 }
 
 /* n sweeps t0..t0+n-1 of the LUT kernel with the (B, M, Q) trace after each (test helper). */

@@ -19,7 +19,8 @@ EXPORTS = [
     "ising_read_window", "ising_write_lattice", "ising_read_packed", "ising_write_packed",
     "ising_set_sweeps_done", "ising_thresholds", "ising_set_launch", "ising_set_variant", "ising_bench_pipes", "ising_set_corr_path", "ising_set_tally", "ising_tally", "ising_time_grid", "ising_run_schedule",
     "ising_launch_count", "ising_sync", "ising_destroy", "ising_last_error", "ising_bench_philox_only",
-    "ising_bench_copy", "ising_debug_philox",
+    "ising_bench_copy", "ising_debug_philox", "ising_protocol_distances", "ising_threshold_table",
+    "ising_run_protocol_schedule",
 ]
 
 
@@ -88,6 +89,15 @@ def load_library():
     lib.ising_bench_philox_only.argtypes = [vp, C.c_int]
     lib.ising_bench_copy.argtypes = [vp, C.c_int]
     lib.ising_debug_philox.argtypes = [i64, vp, vp, vp, C.c_int]
+    lib.ising_time_grid.argtypes = [u64, vp, i64, vp]
+    lib.ising_protocol_distances.argtypes = [i64, u64, i64, vp, vp, vp]
+    lib.ising_threshold_table.argtypes = [C.c_int, dbl, dbl, vp, C.c_int, vp]
+    lib.ising_run_protocol_schedule.argtypes = [vp, i64, vp, i64, vp, vp, vp, vp, vp, vp]
+    lib.ising_run_schedule.argtypes = [vp, i64, vp, vp]
+    lib.ising_set_tally.argtypes = [vp, C.c_int]
+    lib.ising_tally.argtypes = [vp, vp]
+    lib.ising_set_corr_path.argtypes = [vp, C.c_int]
+    lib.ising_bench_pipes.argtypes = [dbl, vp, C.c_int, vp]
     _lib = lib
     return lib
 
@@ -108,7 +118,6 @@ PIPE_PROBES = ["IMAD.WIDE", "LOP3", "IMAD", "IMAD.WIDE+LOP3", "IMAD.WIDE+2LOP3",
 def bench_pipes(sm_mhz: float = 0.0) -> dict:
     """Issue rates (warp-instructions per SM sub-partition per clock) of the integer-pipe probes."""
     lib = load_library()
-    lib.ising_bench_pipes.argtypes = [C.c_double, C.c_void_p, C.c_int, C.c_void_p]
     rates = np.zeros(len(PIPE_PROBES), dtype=np.float64)
     n = C.c_int(0)
     _check(lib.ising_bench_pipes(float(sm_mhz), rates.ctypes.data, len(rates), C.addressof(n)))
@@ -116,14 +125,34 @@ def bench_pipes(sm_mhz: float = 0.0) -> dict:
 
 
 def time_grid(tmax: int) -> np.ndarray:
-    """The paper's measurement times up to tmax."""
+    """The paper's measurement times up to tmax.  Host arithmetic: no GPU needed."""
     lib = load_library()
-    lib.ising_time_grid.argtypes = [C.c_uint64, C.c_void_p, C.c_int64, C.c_void_p]
     n = C.c_int64(0)
-    lib.ising_time_grid(int(tmax), None, 0, C.addressof(n))
+    _check(lib.ising_time_grid(int(tmax), None, 0, C.addressof(n)))
     out = np.zeros(n.value, dtype=np.uint64)
     _check(lib.ising_time_grid(int(tmax), out.ctypes.data, len(out), C.addressof(n)))
     return out
+
+
+def protocol_distances(L: int, t: int):
+    """(r, stride) of the Sec. 3.3 protocol at time t.  Host arithmetic: no GPU needed."""
+    lib = load_library()
+    n = C.c_int64(0)
+    _check(lib.ising_protocol_distances(int(L), int(t), 0, None, None, C.addressof(n)))
+    r = np.zeros(n.value, dtype=np.int64)
+    st = np.zeros(n.value, dtype=np.int64)
+    _check(lib.ising_protocol_distances(int(L), int(t), len(r), r.ctypes.data, st.ctypes.data, C.addressof(n)))
+    return r, st
+
+
+def threshold_table(model: int, beta: float, D: float = 0.0) -> np.ndarray:
+    """The integer acceptance table of (model, beta, D) (A1; the 16-entry cumulative table for the 1-bit
+    model).  Host arithmetic: no GPU needed."""
+    lib = load_library()
+    out = np.zeros(64, dtype=np.uint64)
+    n = C.c_int(0)
+    _check(lib.ising_threshold_table(int(model), float(beta), float(D), out.ctypes.data, 64, C.addressof(n)))
+    return out[: n.value].copy()
 
 
 def debug_philox(ctr: np.ndarray, key: np.ndarray, with_curand: bool = False) -> np.ndarray:
@@ -193,12 +222,10 @@ class IsingSim:
         return Observables(*(getattr(o, f[0]) for f in _Obs._fields_))
 
     def set_tally(self, on: bool = True):
-        self._lib.ising_set_tally.argtypes = [C.c_void_p, C.c_int]
         _check(self._lib.ising_set_tally(self._h, int(on)))
 
     def tally(self) -> Observables:
         o = _Obs()
-        self._lib.ising_tally.argtypes = [C.c_void_p, C.c_void_p]
         _check(self._lib.ising_tally(self._h, C.byref(o)))
         return Observables(*(getattr(o, f[0]) for f in _Obs._fields_))
 
@@ -206,7 +233,6 @@ class IsingSim:
         """Sweep to every time of the ascending list and record the observables there (one native call)."""
         times = np.ascontiguousarray(times, dtype=np.uint64)
         arr = (_Obs * len(times))()
-        self._lib.ising_run_schedule.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
         _check(self._lib.ising_run_schedule(self._h, len(times), times.ctypes.data, C.addressof(arr)))
         return [Observables(*(getattr(o, f[0]) for f in _Obs._fields_)) for o in arr]
 
@@ -224,9 +250,26 @@ class IsingSim:
                                                 sy.ctypes.data))
         return sx, sy
 
+    def run_protocol_schedule(self, times, with_observables: bool = True):
+        """Sweep to every time of the ascending list and run the Sec. 3.3 protocol there (one native call).
+        Returns a list of (r, sx, sy, n_src) per time and the list of observables (or None)."""
+        times = np.ascontiguousarray(times, dtype=np.uint64)
+        n = C.c_int64(0)
+        _check(self._lib.ising_protocol_distances(self.L, int(times[-1]) if len(times) else 0, 0, None, None, C.byref(n)))
+        cap = n.value
+        arrs = [np.zeros((len(times), cap), dtype=np.int64) for _ in range(4)]
+        counts = np.zeros(len(times), dtype=np.int64)
+        obs = (_Obs * len(times))() if with_observables else None
+        _check(self._lib.ising_run_protocol_schedule(self._h, len(times), times.ctypes.data, cap,
+                                                     *(a.ctypes.data for a in arrs), counts.ctypes.data,
+                                                     C.addressof(obs) if obs is not None else None))
+        rows = [tuple(a[i, : counts[i]].copy() for a in arrs) for i in range(len(times))]
+        o = [Observables(*(getattr(x, f[0]) for f in _Obs._fields_)) for x in obs] if obs is not None else None
+        return rows, o
+
     def correlation_protocol(self):
         n = C.c_int64(0)
-        self._lib.ising_correlation_protocol(self._h, 0, None, None, None, None, C.byref(n))
+        _check(self._lib.ising_correlation_protocol(self._h, 0, None, None, None, None, C.byref(n)))
         cap = n.value
         arrs = [np.zeros(cap, dtype=np.int64) for _ in range(4)]
         _check(self._lib.ising_correlation_protocol(self._h, cap, *(a.ctypes.data for a in arrs), C.byref(n)))
@@ -289,7 +332,6 @@ class IsingSim:
         _check(self._lib.ising_set_variant(self._h, variant))
 
     def set_corr_path(self, path: int):
-        self._lib.ising_set_corr_path.argtypes = [C.c_void_p, C.c_int]
         _check(self._lib.ising_set_corr_path(self._h, path))
 
     def launch_count(self) -> int:

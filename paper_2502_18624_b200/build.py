@@ -17,7 +17,7 @@ def sources():
 
 
 def _deps():
-    return sources() + glob.glob(os.path.join(HERE, "csrc", "*.cuh")) + [os.path.join(ROOT, "include", "ising.h")]
+    return sources() + glob.glob(os.path.join(HERE, "csrc", "*.cuh")) + glob.glob(os.path.join(ROOT, "include", "*.h"))
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

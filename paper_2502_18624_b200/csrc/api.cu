@@ -8,8 +8,6 @@
 #include <string>
 #include <vector>
 
-#include <curand_kernel.h>
-
 #include "ising_internal.cuh"
 
 static thread_local std::string g_err;
@@ -29,21 +27,6 @@ extern "C" const char *ising_last_error(void) { return g_err.c_str(); }
 
 static void drop_graph(ising_sim *h);
 
-// Every entry point that takes a handle runs on the handle's device, whatever the caller's current
-// device is, and puts the caller's device back on return.
-struct DeviceGuard {
-    int prev = -1;
-    bool switched = false;
-    explicit DeviceGuard(const ising_sim *h) { if (h) enter(h->device); }
-    explicit DeviceGuard(int device) { enter(device); }
-    void enter(int device)
-    {
-        if (device < 0 || cudaGetDevice(&prev) != cudaSuccess || prev == device) return;
-        switched = cudaSetDevice(device) == cudaSuccess;
-    }
-    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
-};
-
 static bool valid_model_L(int model, int64_t L)
 {
     if (model == ISING_MODEL_ISING_LUT) return L >= 256 && (L % 256) == 0 && L <= (1ll << 20);   // 128-bit vector = 128 sites
@@ -57,56 +40,10 @@ extern "C" size_t ising_workspace_bytes(int model, int64_t L)
     return (size_t)L * (size_t)L / (size_t)sites_per_word(model) * 8 + kScratchBytes;   // both colour arrays
 }
 
-// ------------------------------------------------------------ thresholds ---
-// A1: T = 2^32 if p >= 1 else floor(p 2^32), p = exp(-beta dE) evaluated in double.
-static uint64_t metropolis_threshold(double beta, double dE)
-{
-    const double p = exp(-(beta * dE));
-    if (p >= 1.0) return 1ull << 32;
-    return (uint64_t)floor(ldexp(p, 32));
-}
-
-// NEXT-2 (reading L2): table[i] = floor(2^32 sum_{j<i} P(j)),
-// P(j) = p^popc(j) (1-p)^(4-popc(j)), p = exp(-4 beta), sums in index order in double.
-static void build_lut_table(ising_sim *h)
-{
-    const double p = exp(-(4.0 * h->beta)), q = 1.0 - p;
-    double pw[5] = {1, 0, 0, 0, 0}, qw[5] = {1, 0, 0, 0, 0};
-    for (int k = 1; k <= 4; ++k) { pw[k] = pw[k - 1] * p; qw[k] = qw[k - 1] * q; }
-    double cum = 0.0;
-    h->n_T = 16;
-    for (int i = 0; i < 16; ++i) {
-        double v = floor(ldexp(cum, 32));
-        if (v > 4294967296.0) v = 4294967296.0;
-        h->T[i] = (uint64_t)v;
-        int ones = 0;
-        for (int b = 0; b < 4; ++b) ones += (i >> b) & 1;
-        volatile double term = pw[ones] * qw[4 - ones];      // rounded product, then the sum (no FMA)
-        cum += term;
-    }
-}
-
+// A1 / L2: the tables themselves are host arithmetic (host_logic.cu)
 static void build_thresholds(ising_sim *h)
 {
-    if (h->model == ISING_MODEL_ISING_LUT) { build_lut_table(h); return; }
-    if (h->model == ISING_MODEL_ISING) {
-        // entry i: dE = 4 i - 8, i.e. the spin agrees with i of... dE = 2 s h in {-8,-4,0,4,8}
-        h->n_T = 5;
-        for (int i = 0; i < 5; ++i) h->T[i] = metropolis_threshold(h->beta, 4.0 * i - 8.0);
-        return;
-    }
-    // Blume-Capel (Eq. 2): single-site energy e(s) = -s h + D s^2
-    h->n_T = 54;
-    for (int code = 0; code < 3; ++code)
-        for (int b = 0; b < 2; ++b)
-            for (int S = 0; S <= 8; ++S) {
-                const int s_old = code - 1, s_new = (code + 1 + b) % 3 - 1, field = S - 4;
-                const int d_lin = (s_new - s_old) * field;                 // change of s h
-                const int d_sq = s_new * s_new - s_old * s_old;            // change of s^2
-                volatile double crystal = h->D * (double)d_sq;             // rounded product, no FMA
-                const double dE = crystal - (double)d_lin;
-                h->T[(code * 2 + b) * 9 + S] = metropolis_threshold(h->beta, dE);
-            }
+    h->n_T = host_threshold_table(h->model, h->beta, h->D, h->T);
 }
 
 static void build_round_keys(ising_sim *h)
@@ -369,25 +306,6 @@ extern "C" int ising_sweep(ising_t *h, int64_t n)
     return ISING_OK;
 }
 
-// A11: measurement times of the paper, t = floor(2^(x/8) + 0.5), x = 1, 2, ..., de-duplicated
-extern "C" int ising_time_grid(uint64_t tmax, uint64_t *out, int64_t cap, int64_t *count)
-{
-    if (!count) return set_error(ISING_EINVAL, "ising_time_grid: count is NULL");
-    int64_t n = 0;
-    uint64_t last = 0;
-    for (int x = 1; x < 8 * 64; ++x) {
-        const double v = floor(exp2((double)x / 8.0) + 0.5);
-        if (v > (double)tmax) break;
-        const uint64_t t = (uint64_t)v;
-        if (t == last) continue;
-        if (out && n < cap) out[n] = t;
-        ++n; last = t;
-    }
-    *count = n;
-    if (!out || cap < n) return set_error(ISING_EINVAL, "ising_time_grid: cap too small");
-    return ISING_OK;
-}
-
 // A11: sweep to every time of an ascending schedule and record B, M, Q there (fused tally if it is on,
 // else the observables pass).  One call for "E and M every k sweeps" (BASELINE.json configs 1-3).
 extern "C" int ising_run_schedule(ising_t *h, int64_t n_times, const uint64_t *times, ising_obs_t *out)
@@ -524,7 +442,8 @@ extern "C" int ising_thresholds(ising_t *h, uint64_t *out, int cap, int *count)
     DeviceGuard dev_guard(h);
     if (!h || !count) return set_error(ISING_EINVAL, "ising_thresholds: NULL argument");
     *count = h->n_T;
-    if (!out || cap < h->n_T) return set_error(ISING_EINVAL, "ising_thresholds: cap too small");
+    if (!out) return ISING_OK;                                   // size query
+    if (cap < h->n_T) return set_error(ISING_EINVAL, "ising_thresholds: cap too small");
     memcpy(out, h->T, h->n_T * sizeof(uint64_t));
     return ISING_OK;
 }
@@ -754,24 +673,30 @@ extern "C" int ising_correlation_list(ising_t *h, int64_t stride, int64_t count,
     return run_corr(h, stride, count, r, sx, sy);
 }
 
-// Sec. 3.3: R = 16, r_c(t) = max{256, floor(g(L) sqrt(t) + 0.5)},
-// g(L) = 6 sqrt(ln(L / 2^16) / 3.3^2 + 1); log grid floor(2^(x/32)), x <= 32 (log2 L - 1).
-static void protocol_distances(int64_t L, uint64_t t, std::vector<int64_t> &dense, std::vector<int64_t> &sparse)
+// Sec. 3.3 at t = sweeps_done; the distance lists are host arithmetic (host_logic.cu).
+// Results are staged in host vectors and handed out only when every kernel has succeeded.
+static int protocol_measure(ising_sim *h, std::vector<int64_t> &r, std::vector<int64_t> &sx, std::vector<int64_t> &sy,
+                            std::vector<int64_t> &n_src)
 {
-    const int64_t R = 16, half = L / 2;
-    const double g = 6.0 * sqrt(log((double)L / 65536.0) / (3.3 * 3.3) + 1.0);
-    int64_t rc = (int64_t)floor(g * sqrt((double)t) + 0.5);
-    if (rc < 256) rc = 256;
-    for (int64_t d = 1; d <= std::min(2 * R, half); ++d) dense.push_back(d);
-    for (int64_t d = 2 * R + 1; d <= std::min(rc, half); ++d) sparse.push_back(d);
-    const int64_t xmax = (int64_t)floor(32.0 * (log2((double)L) - 1.0) + 1e-9);
-    int64_t last = std::max(rc, 2 * R);
-    for (int64_t x = 0; x <= xmax; ++x) {
-        const int64_t d = (int64_t)floor(exp2((double)x / 32.0));
-        if (d <= last || d > half) continue;
-        sparse.push_back(d);
-        last = d;
+    std::vector<int64_t> all_sources, block_sources;
+    host_protocol_lists(h->L, h->t, all_sources, block_sources);
+    const int64_t na = (int64_t)all_sources.size(), nb = (int64_t)block_sources.size();
+    r = all_sources;
+    r.insert(r.end(), block_sources.begin(), block_sources.end());
+    sx.assign(na + nb, 0); sy.assign(na + nb, 0); n_src.assign(na + nb, 0);
+    int rc = ensure_planes(h);
+    if (rc) return rc;
+    cudaError_t e = launch_planes(h);
+    if (e != cudaSuccess) return cuda_fail(e, "bit-plane kernels");
+    rc = run_corr(h, 0, na, nullptr, sx.data(), sy.data());                  // every site a source, r = 1..2R
+    if (rc) return rc;
+    for (int64_t i = 0; i < na; ++i) n_src[i] = h->L * h->L;
+    if (nb > 0) {
+        rc = run_corr(h, 16, nb, block_sources.data(), sx.data() + na, sy.data() + na);   // one source per 16 x 16 block
+        if (rc) return rc;
+        for (int64_t i = 0; i < nb; ++i) n_src[na + i] = (h->L / 16) * (h->L / 16);
     }
+    return ISING_OK;
 }
 
 extern "C" int ising_correlation_protocol(ising_t *h, int64_t cap, int64_t *r, int64_t *sx, int64_t *sy,
@@ -779,91 +704,52 @@ extern "C" int ising_correlation_protocol(ising_t *h, int64_t cap, int64_t *r, i
 {
     DeviceGuard dev_guard(h);
     if (!h || !count) return set_error(ISING_EINVAL, "ising_correlation_protocol: NULL argument");
-    std::vector<int64_t> dense, sparse;
-    protocol_distances(h->L, h->t, dense, sparse);
-    const int64_t nd = (int64_t)dense.size(), ns = (int64_t)sparse.size();
-    *count = nd + ns;
-    if (!r || !sx || !sy || !n_src || cap < nd + ns) return set_error(ISING_EINVAL, "ising_correlation_protocol: cap too small");
-    int rc = ensure_planes(h);
+    std::vector<int64_t> all_sources, block_sources;
+    host_protocol_lists(h->L, h->t, all_sources, block_sources);
+    const int64_t n = (int64_t)(all_sources.size() + block_sources.size());
+    *count = n;
+    if (!r && !sx && !sy && !n_src) return ISING_OK;             // size query
+    if (!r || !sx || !sy || !n_src || cap < n) return set_error(ISING_EINVAL, "ising_correlation_protocol: cap too small");
+    std::vector<int64_t> vr, vx, vy, vn;
+    int rc = protocol_measure(h, vr, vx, vy, vn);
     if (rc) return rc;
-    cudaError_t e = launch_planes(h);
-    if (e != cudaSuccess) return cuda_fail(e, "bit-plane kernels");
-    rc = run_corr(h, 0, nd, nullptr, sx, sy);                 // all sources, r = 1..2R
-    if (rc) return rc;
-    for (int64_t i = 0; i < nd; ++i) { r[i] = dense[i]; n_src[i] = h->L * h->L; }
-    if (ns > 0) {
-        rc = run_corr(h, 16, ns, sparse.data(), sx + nd, sy + nd);   // one source per 16 x 16 block
+    std::copy(vr.begin(), vr.end(), r); std::copy(vx.begin(), vx.end(), sx);
+    std::copy(vy.begin(), vy.end(), sy); std::copy(vn.begin(), vn.end(), n_src);
+    return ISING_OK;
+}
+
+// A11 with the correlation measurement: sweep to each time, run the Sec. 3.3 protocol there.
+extern "C" int ising_run_protocol_schedule(ising_t *h, int64_t n_times, const uint64_t *times, int64_t cap,
+                                           int64_t *r, int64_t *sx, int64_t *sy, int64_t *n_src, int64_t *counts,
+                                           ising_obs_t *obs)
+{
+    DeviceGuard dev_guard(h);
+    if (!h || !times || !r || !sx || !sy || !n_src || !counts || n_times < 0)
+        return set_error(ISING_EINVAL, "ising_run_protocol_schedule: bad argument");
+    uint64_t prev = h->t;
+    for (int64_t i = 0; i < n_times; ++i) {
+        if (times[i] < prev) return set_error(ISING_EINVAL, "ising_run_protocol_schedule: times must be ascending and >= sweeps_done");
+        prev = times[i];
+        std::vector<int64_t> a, b;
+        host_protocol_lists(h->L, times[i], a, b);
+        if ((int64_t)(a.size() + b.size()) > cap)
+            return set_error(ISING_EINVAL, "ising_run_protocol_schedule: cap smaller than the distance list of a scheduled time "
+                                           "(ising_protocol_distances gives the size)");
+    }
+    for (int64_t i = 0; i < n_times; ++i) {
+        int rc = ising_sweep(h, (int64_t)(times[i] - h->t));
         if (rc) return rc;
-        for (int64_t i = 0; i < ns; ++i) { r[nd + i] = sparse[i]; n_src[nd + i] = (h->L / 16) * (h->L / 16); }
-    }
-    return ISING_OK;
-}
-
-// ----------------------------------------------------- measurement helpers ---
-extern "C" int ising_bench_philox_only(ising_t *h, int n)
-{
-    DeviceGuard dev_guard(h);
-    if (!h || n < 0 || h->model == ISING_MODEL_ISING_LUT) return set_error(ISING_EINVAL, "ising_bench_philox_only: bad argument");
-    for (int i = 0; i < n; ++i) {
-        cudaError_t e = launch_philox_only(h, (uint32_t)i);
-        if (e != cudaSuccess) return cuda_fail(e, "philox-only kernel");
-    }
-    return ISING_OK;
-}
-
-extern "C" int ising_bench_copy(ising_t *h, int n)
-{
-    DeviceGuard dev_guard(h);
-    if (!h || n < 0 || h->model == ISING_MODEL_ISING_LUT) return set_error(ISING_EINVAL, "ising_bench_copy: bad argument");
-    for (int i = 0; i < n; ++i) {
-        cudaError_t e = launch_copy(h);
-        if (e != cudaSuccess) return cuda_fail(e, "copy kernel");
-    }
-    return ISING_OK;
-}
-
-// ------------------------------------------------------------ debug Philox ---
-__global__ void debug_philox_kernel(int64_t count, const uint32_t *ctr, const uint32_t *key, uint32_t *out, int with_curand)
-{
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= count) return;
-    uint4 c = make_uint4(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3]);
-    uint4 r;
-    if (with_curand) {
-        r = curand_Philox4x32_10(c, make_uint2(key[2 * i], key[2 * i + 1]));
-    } else {
-        RoundKeys rk;
-        uint32_t k0 = key[2 * i], k1 = key[2 * i + 1];
-        for (int j = 0; j < 10; ++j) { rk.k0[j] = k0; rk.k1[j] = k1; k0 += PHILOX_W0; k1 += PHILOX_W1; }
-        if (with_curand == 0 && (i & 1)) {
-            // odd entries go through the specialised path the update kernel uses
-            PhiloxRow pr = philox_row(c.y, c.z, c.w, rk);
-            r = philox_site4(c.x, pr, rk);
-        } else {
-            r = philox4x32_10(c, rk);
+        std::vector<int64_t> vr, vx, vy, vn;
+        rc = protocol_measure(h, vr, vx, vy, vn);
+        if (rc) return rc;
+        if (obs) {
+            rc = h->tally_on ? ising_tally(h, &obs[i]) : ising_observables(h, &obs[i]);
+            if (rc) return rc;
         }
+        counts[i] = (int64_t)vr.size();
+        std::copy(vr.begin(), vr.end(), r + i * cap); std::copy(vx.begin(), vx.end(), sx + i * cap);
+        std::copy(vy.begin(), vy.end(), sy + i * cap); std::copy(vn.begin(), vn.end(), n_src + i * cap);
     }
-    out[4 * i] = r.x; out[4 * i + 1] = r.y; out[4 * i + 2] = r.z; out[4 * i + 3] = r.w;
-}
-
-cudaError_t launch_debug_philox(int64_t count, const uint32_t *d_ctr, const uint32_t *d_key, uint32_t *d_out,
-                                int with_curand, cudaStream_t s)
-{
-    debug_philox_kernel<<<(unsigned)((count + 127) / 128), 128, 0, s>>>(count, d_ctr, d_key, d_out, with_curand);
-    return cudaGetLastError();
-}
-
-extern "C" int ising_debug_philox(int64_t count, const uint32_t *ctr, const uint32_t *key, uint32_t *out, int with_curand)
-{
-    if (count < 1 || !ctr || !key || !out) return set_error(ISING_EINVAL, "ising_debug_philox: bad argument");
-    uint32_t *d = nullptr;
-    CUDA_TRY(cudaMalloc((void **)&d, (size_t)count * 10 * sizeof(uint32_t)));
-    uint32_t *d_ctr = d, *d_key = d + 4 * count, *d_out = d + 6 * count;
-    cudaError_t e = cudaMemcpy(d_ctr, ctr, (size_t)count * 16, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemcpy(d_key, key, (size_t)count * 8, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = launch_debug_philox(count, d_ctr, d_key, d_out, with_curand, 0);
-    if (e == cudaSuccess) e = cudaMemcpy(out, d_out, (size_t)count * 16, cudaMemcpyDeviceToHost);
-    cudaFree(d);
-    if (e != cudaSuccess) return cuda_fail(e, "ising_debug_philox");
     return ISING_OK;
 }
+

@@ -6,8 +6,10 @@
 #include <stdint.h>
 
 #include <string>
+#include <vector>
 
 #include "ising.h"
+#include "ising_bench.h"
 
 // ----------------------------------------------------------------- handle ---
 struct RoundKeys {  // Philox key schedule (PAPER.md:149 names the generator): k(i) = seed + i*W
@@ -59,6 +61,27 @@ int cuda_fail(cudaError_t e, const char *what);
         if (e__ != cudaSuccess) return cuda_fail(e__, #x);     \
     } while (0)
 
+// Every entry point that takes a handle runs on the handle's device, whatever the caller's current
+// device is, and puts the caller's device back on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const ising_sim *h) { if (h) enter(h->device); }
+    explicit DeviceGuard(int device) { enter(device); }
+    void enter(int device)
+    {
+        if (device < 0 || cudaGetDevice(&prev) != cudaSuccess || prev == device) return;
+        switched = cudaSetDevice(device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+
+// host-only arithmetic (host_logic.cu)
+int host_threshold_table(int model, double beta, double D, uint64_t *T);     // returns the number of entries (<= 54)
+void host_time_grid(uint64_t tmax, std::vector<uint64_t> &times);
+int64_t host_protocol_crossover(int64_t L, uint64_t t);
+void host_protocol_lists(int64_t L, uint64_t t, std::vector<int64_t> &all_sources, std::vector<int64_t> &block_sources);
+
 static inline int64_t words_per_row(int64_t L) { return L / 32; }              // uint64 per colour row
 static inline int64_t words_per_colour(int64_t L) { return L * (L / 32); }
 static inline bool is_blume_capel(int model) { return model == ISING_MODEL_BLUME_CAPEL || model == ISING_MODEL_BLUME_CAPEL_2BIT; }
@@ -105,10 +128,9 @@ cudaError_t launch_debug_philox(int64_t count, const uint32_t *d_ctr, const uint
 // reduction (warp sums must fit 32 bits), one shared-memory atomic per warp, ONE
 // global atomic per block and quantity.  Same-address global atomics serialise in
 // one L2 slice (about 1.3 ns each on B200): with one per warp the observables pass
-// at L = 2^18 spent 4 of its 9 ms waiting for 3.1 M of them.  Every live thread of
-// the block must call this; threads that returned earlier count as arrived at the
-// barriers, and thread 0 is alive whenever any thread of its block is (the threads
-// past the lattice are the highest ones).
+// at L = 2^18 spent 4 of its 9 ms waiting for 3.1 M of them.  Every thread of the
+// block must call this (it contains two block barriers): kernels keep threads past
+// the lattice alive and let them add zeros.
 template <int N>
 __device__ __forceinline__ void block_accumulate(const int (&v)[N], long long *dst)
 {
@@ -118,8 +140,8 @@ __device__ __forceinline__ void block_accumulate(const int (&v)[N], long long *d
         for (int k = 0; k < N; ++k) s_acc[k] = 0;
     }
     __syncthreads();
-    const unsigned m = __activemask();
-    const bool leader = (int)(threadIdx.x & 31) == __ffs(m) - 1;
+    const unsigned m = 0xffffffffu;               // blocks are whole warps (ising_set_launch), all of them here
+    const bool leader = (threadIdx.x & 31) == 0;
 #pragma unroll
     for (int k = 0; k < N; ++k) {
         const int sum = __reduce_add_sync(m, v[k]);

@@ -195,7 +195,7 @@ __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const _
     unsigned chunk = tid / (unsigned)cols;
     int col = (int)(tid - chunk * (unsigned)cols);
     int y0 = (int)chunk * p.R;
-    if (y0 >= L) return;
+    if (y0 < L) {                                                      // no early return: every thread reaches block_accumulate
     int yend = min(L, y0 + p.R);
 
     const size_t rs = (size_t)cols * 16;                               // bytes per colour row
@@ -244,6 +244,7 @@ __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const _
         g0 += gs;
         up = dn; sm = dn2; src = nsrc2; edge = nedge2;
         o1 += 2 * rs; eo += 2 * rs; w0 += 2 * rs;
+    }
     }
     if (TALLY) {
         const int v[2] = {dB, dM};

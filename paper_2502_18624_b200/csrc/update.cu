@@ -358,7 +358,7 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
     unsigned chunk = tid / (unsigned)cols;
     int col = (int)(tid - chunk * (unsigned)cols);
     int y0 = (int)chunk * p.R;
-    if (y0 >= L) return;
+    if (y0 < L) {                                            // no early return: every thread reaches block_accumulate
     int yend = min(L, y0 + p.R);
 
     // Running byte pointers, advanced by one row stride per row (no index multiplications in
@@ -415,7 +415,8 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
         up = dn; sm = dn2; src = nsrc2; edge = nedge2;
         o1 += 2 * rs; eo += 2 * rs; w0 += 2 * rs;
     }
-    if (TALLY) {            // warp sums fit 32 bits (<= 32 lanes x R rows x 32 sites x 8); threads past the lattice have returned
+    }
+    if (TALLY) {            // warp sums fit 32 bits (<= 32 lanes x R rows x 32 sites x 8); threads past the lattice add zeros
         const int v[3] = {dB, dM, dQ};
         block_accumulate<3>(v, p.tally);
     }

@@ -89,6 +89,28 @@ def test_tally_equals_recompute_and_init_is_balanced(L, beta):
         assert tl == oracle.observables(s)
 
 
+def test_init_mapping_reading_L5():
+    """Reading L5, site by site with the KAT-pinned Philox and Python integers: colour c = (x + y) & 1,
+    compact index k = x >> 1, word w = y * ceil(L / 128) + (k >> 6) of colour c is (out[0] | out[1] << 32) of
+    Philox(ctr = (w_lo, w_hi, 0, 2 + c), key = seed); bit k & 63 set <-> spin +1.  Covers both colours, both
+    32-bit halves of a word, several words per row, the last row, and a patch that wraps."""
+    seed = 0x0123456789ABCDEF
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    for L in (256, 640, 96):
+        s = oracle.lut_init(L, seed)
+        Wr = (L // 2 + 63) // 64
+        sites = [(0, 0), (1, 0), (0, 1), (63, 0), (64, 0), (65, 1), (127, 5), (128, 5), (129, 6), (L - 1, L - 1),
+                 (L - 2, L - 1), (L - 1, 0), (L // 2 + 1, L // 3)]
+        for x, y in [(x, y) for x, y in sites if x < L and y < L]:
+            c, k = (x + y) & 1, x >> 1
+            w = y * Wr + (k >> 6)
+            out = oracle.philox4x32_10([w & 0xFFFFFFFF, w >> 32, 0, 2 + c], key)
+            bits = int(out[0]) | (int(out[1]) << 32)
+            assert s[y, x] == (1 if (bits >> (k & 63)) & 1 else -1), (L, x, y)
+        patch = oracle.lut_init_patch(L, seed, L - 3, L - 2, 7, 5)                     # wraps in x and y
+        assert (patch == np.roll(s, (2, 3), axis=(0, 1))[:5, :7]).all()
+
+
 def test_word_sweep_equals_per_site_patch_sweep():
     """The paper-order sweep (random words per 64 sites) and the per-site light-cone patch sweep are
     written independently; they must give the same spins where the patch is exact, including

@@ -133,6 +133,27 @@ def test_init_mapping_and_statistics():
 
 
 # ------------------------------------------------------------- observables ---
+@pytest.mark.parametrize("model,L", [(ISING, 64), (BC, 48), (ISING, 10)])
+def test_row_band_routines_add_up_to_the_full_lattice(model, L):
+    """orc_observables_rows / orc_sd_hist_rows (used to anchor B, M, Q and the Schwinger-Dyson histogram of
+    lattices the host cannot hold): any partition of [0, L) into bands, incl. ragged ones and the band whose
+    lower neighbour is row 0, adds up to the full-lattice routines; one band of L rows IS the full routine;
+    and a python double loop over one band."""
+    s = oracle.init(model, L, 5)
+    full = oracle.observables(s)
+    _, full_hist = oracle.schwinger_dyson(s, 0.4)
+    ext = np.concatenate([s[-1:], s, s[:1]])                       # rows -1 .. L
+    for cuts in ([0, L], [0, 1, L], sorted({0, 7, 8, min(30, L - 1), L}), list(range(0, L + 1, 2))):
+        tot, hist = np.zeros(3, dtype=np.int64), np.zeros(9, dtype=np.int64)
+        for a, b in zip(cuts, cuts[1:]):
+            tot += np.array(oracle.observables_rows(L, ext[a + 1:b + 2]))
+            hist += oracle.sd_hist_rows(L, ext[a:b + 2])
+        assert tuple(int(v) for v in tot) == full and (hist == full_hist).all(), cuts
+    a, b = 3, 6
+    B = sum(int(s[y, x]) * (int(s[y, (x + 1) % L]) + int(s[(y + 1) % L, x])) for y in range(a, b) for x in range(L))
+    assert oracle.observables_rows(L, ext[a + 1:b + 2])[0] == B
+
+
 def test_observables_closed_forms():
     """Eq. 1 / Eq. 2 on crafted lattices (each bond once: 2N bonds)."""
     L = 16
