@@ -74,6 +74,8 @@ def parse_args():
     ap.add_argument("--block", type=int, default=0, help="update-kernel threads per block (0 = library default)")
     ap.add_argument("--variant", type=int, default=0, help="update-kernel variant (0 = default carry form)")
     ap.add_argument("--corr-path", type=int, default=0, help="ising_set_corr_path: 0 auto (fp4 tensor cores, path 4, for wide bands), 1 bit planes, 2 int8 tensor cores one CTA per tile, 3 int8 CTA pairs, 4 fp4 CTA pairs")
+    ap.add_argument("--slabs", type=int, default=0, help="NEXT-4: cut the lattice into this many row slabs (allocations of their own, halo rows "
+                                                          "read from the neighbours; all on this GPU unless --gpus-as-slabs)")
     ap.add_argument("--tally", action="store_true", help="A7: keep E, M by the fused tally of the update kernels instead of the observables pass")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -358,7 +360,8 @@ def run_ours(args):
     base, L, name = pick_workload(args)
     model = MODEL_IDS[args.model]
     S, K, W = args.sweeps_per_step, args.steps, max(args.warmup, 0)
-    sim = eng.IsingSim(model, L, base.beta, base.D, replica_seed(base.seed, rank), device=device)
+    sim = eng.IsingSim(model, L, base.beta, base.D, replica_seed(base.seed, rank), device=device,
+                       slabs=args.slabs if args.slabs > 1 else None)
     if args.rows_per_thread or args.block:
         sim.set_launch(args.rows_per_thread, args.block)
     if args.variant:
@@ -407,7 +410,7 @@ def run_ours(args):
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
     lut = model == wl.ISING_LUT
     philox_ms = copy_ms = None
-    if not lut:                                            # the roof helpers work on the 4-bit layout
+    if not lut and args.slabs <= 1:                        # the roof helpers work on the 4-bit layout of an unsharded lattice
         sim.bench_philox_only(2); sim.bench_copy(2); torch.cuda.synchronize(device)
         ev[0].record(); sim.bench_philox_only(n_roof); ev[1].record(); sim.bench_copy(n_roof); ev[2].record()
         torch.cuda.synchronize(device)
@@ -474,7 +477,8 @@ def run_ours(args):
                    "seed": base.seed, "sweeps_per_step": S, "observables_every": S,
                    "step": "S sweeps + observables" if args.workload == "sweep" else "S sweeps + correlation protocol + observables",
                    "launch": {"rows_per_thread": args.rows_per_thread or "default", "block": args.block or "default",
-                              "variant": args.variant, "fused_tally": bool(args.tally), "corr_path": args.corr_path},
+                              "variant": args.variant, "fused_tally": bool(args.tally), "corr_path": args.corr_path,
+                              "slabs": max(1, args.slabs)},
                    "lattice_bytes": L * L * BITS_PER_SITE[model] // 8, "l2": "inputs larger than L2 (no flush needed)" if L * L // 2 > (256 << 20)
                    else "lattice fits L2: DRAM figures not meaningful", "parallelism": f"replicas x{world}"},
         "measurement_ms_per_step": (total_ms - sweep_ms) / K,

@@ -87,6 +87,25 @@ size_t ising_workspace_bytes(int model, int64_t L);
 int ising_create(int model, int64_t L, double beta, double D, uint64_t seed,
                  void *dev_buf, size_t dev_bytes, void *cuda_stream, ising_t **out);
 
+/* NEXT-4 of SURVEY.md Sec. 8(f): the same simulation with the lattice cut into n_slabs horizontal slabs
+ * ("partitioning each buffer into horizontal slabs, which are stored in device memory ...
+ * restricting [communication] to just two rows: the last row of the slab on the preceding GPU and the
+ * first row of the slab on the next GPU"; the first and last slab are neighbours too).  Slab k holds
+ * slab_rows[k] consecutive rows of both colour arrays (even, >= 2, adding up to L; NULL: an even split) in
+ * an allocation of its own on CUDA device devices[k] (NULL: all on the current device).  The library
+ * allocates; peer access between the devices involved is switched on, and the update / observables
+ * kernels of a slab read its two halo rows from the neighbouring slabs' memory with plain loads
+ * (PAPER.md:89).  Slabs of one colour phase run concurrently on streams of their own and wait only for
+ * the previous phase of their two neighbours; integer observables are summed over the slabs in int64.
+ * Random numbers are keyed by the global site index, so the trajectory is the unsharded lattice's bit for
+ * bit whatever the partition ("identical numerical results ... regardless of the number of
+ * GPUs used").  Every call of this header works on such a handle; cuda_stream is slab 0's stream.        */
+int ising_create_slabs(int model, int64_t L, double beta, double D, uint64_t seed, int n_slabs,
+                       const int64_t *slab_rows, const int *devices, void *cuda_stream, ising_t **out);
+/* Number of slabs (1 for ising_create), and rows [y0, y0 + rows) / device of one of them (NULL: skip). */
+int ising_slab_count(const ising_t *h);
+int ising_slab_info(const ising_t *h, int slab, int64_t *y0, int64_t *rows, int *device);
+
 /* n >= 0 full sweeps: colour 0 then colour 1 ("two update phases"),
  * one Philox number per site, accept iff r < T.  Asynchronous:
  * 2n kernel launches on the handle's stream, no host synchronisation; small

@@ -20,7 +20,7 @@ EXPORTS = [
     "ising_set_sweeps_done", "ising_thresholds", "ising_set_launch", "ising_set_variant", "ising_bench_pipes", "ising_set_corr_path", "ising_set_tally", "ising_tally", "ising_time_grid", "ising_run_schedule",
     "ising_launch_count", "ising_sync", "ising_destroy", "ising_last_error", "ising_bench_philox_only",
     "ising_bench_copy", "ising_debug_philox", "ising_protocol_distances", "ising_threshold_table",
-    "ising_run_protocol_schedule",
+    "ising_run_protocol_schedule", "ising_create_slabs", "ising_slab_count", "ising_slab_info",
 ]
 
 
@@ -66,6 +66,9 @@ def load_library():
     lib.ising_workspace_bytes.restype = C.c_size_t
     lib.ising_workspace_bytes.argtypes = [C.c_int, i64]
     lib.ising_create.argtypes = [C.c_int, i64, dbl, dbl, u64, vp, C.c_size_t, vp, C.POINTER(vp)]
+    lib.ising_create_slabs.argtypes = [C.c_int, i64, dbl, dbl, u64, C.c_int, vp, vp, vp, C.POINTER(vp)]
+    lib.ising_slab_count.argtypes = [vp]
+    lib.ising_slab_info.argtypes = [vp, C.c_int, vp, vp, vp]
     lib.ising_sweep.argtypes = [vp, i64]
     lib.ising_observables.argtypes = [vp, C.POINTER(_Obs)]
     lib.ising_correlation.argtypes = [vp, i64, vp, vp]
@@ -168,7 +171,9 @@ class IsingSim:
     """One lattice on one GPU.  Methods mirror the C ABI one to one."""
 
     def __init__(self, model: int, L: int, beta: float, D: float = 0.0, seed: int = 1, device="cuda:0",
-                 use_torch_memory: bool = True):
+                 use_torch_memory: bool = True, slabs=None, slab_devices=None):
+        """slabs: None = one lattice (ising_create); an int S or a list of row counts = ising_create_slabs
+        (row slabs in allocations of their own, optionally on the CUDA device indices slab_devices)."""
         import torch
         if not torch.cuda.is_available():
             raise IsingError(-3, "no CUDA device: the engine has no CPU fallback")
@@ -182,6 +187,15 @@ class IsingSim:
         self._h = C.c_void_p()
         with torch.cuda.device(self.device):
             self._stream = torch.cuda.current_stream(self.device)
+            if slabs is not None:
+                rows = None if isinstance(slabs, int) else np.ascontiguousarray(slabs, dtype=np.int64)
+                n = slabs if rows is None else len(rows)
+                devs = None if slab_devices is None else np.ascontiguousarray(slab_devices, dtype=np.int32)
+                self._buf = None
+                _check(self._lib.ising_create_slabs(model, L, beta, D, seed, n, None if rows is None else rows.ctypes.data,
+                                                    None if devs is None else devs.ctypes.data,
+                                                    self._stream.cuda_stream, C.byref(self._h)))
+                return
             if use_torch_memory:
                 self._buf = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
                 ptr, size = self._buf.data_ptr(), nbytes
@@ -208,6 +222,15 @@ class IsingSim:
 
     def __exit__(self, *a):
         self.close()
+
+    def slab_layout(self):
+        """[(y0, rows, device)] of the row slabs (one entry for an unsharded lattice)."""
+        out = []
+        for k in range(self._lib.ising_slab_count(self._h)):
+            y0, rows, dev = C.c_int64(0), C.c_int64(0), C.c_int(0)
+            _check(self._lib.ising_slab_info(self._h, k, C.addressof(y0), C.addressof(rows), C.addressof(dev)))
+            out.append((y0.value, rows.value, dev.value))
+        return out
 
     # -- the path
     def sweep(self, n: int = 1):

@@ -72,22 +72,146 @@ static void default_launch(ising_sim *h)
 }
 
 // ---------------------------------------------------------------- create ---
+// Device tables derived from the integer thresholds: Blume-Capel compare / carry tables, or the search
+// tree and bucket table of the 1-bit kernel's getMaxLE.  Built once on the host, copied to every slab's device.
+struct HostTables {
+    std::vector<uint32_t> table;     // -> Slab::d_table
+    std::vector<uint32_t> buckets;   // -> Slab::lut_buckets (LUT model only)
+};
+
+static int build_host_tables(const ising_sim *h, HostTables &ht)
+{
+    if (is_blume_capel(h->model)) {
+        // [0, 66): thresholds clamped to 2^32-1 + "always" bit mask (compare/select variant).
+        // [80, 80 + 132): carry form for the default variant, two halves of 66 words (264 bytes):
+        // C[b][16 code + S] = 2^32 - T, 0 for T = 2^32 (never a carry -> always accepted).  T = 0 has
+        // no 32-bit carry constant: launch_update then uses the compare/select variant.
+        ht.table.assign(80 + 132, 0u);
+        uint64_t always = 0;
+        for (int i = 0; i < 54; ++i) {
+            if (h->T[i] >> 32) { always |= 1ull << i; ht.table[i] = 0xFFFFFFFFu; }
+            else ht.table[i] = (uint32_t)h->T[i];
+        }
+        ht.table[64] = (uint32_t)always; ht.table[65] = (uint32_t)(always >> 32);
+        for (int code = 0; code < 3; ++code)
+            for (int S = 0; S <= 8; ++S)
+                for (int b = 0; b < 2; ++b) {
+                    const uint64_t T = h->T[(code * 2 + b) * 9 + S];
+                    ht.table[80 + 66 * b + 16 * code + S] = (T >> 32) ? 0u : (uint32_t)((1ull << 32) - T);
+                }
+    }
+    if (h->model == ISING_MODEL_ISING_LUT) {
+        // heap-ordered carry constants of the binary search: node n at level l splits at table index
+        // ((n - 2^l) << (4 - l)) | (1 << (3 - l));  rnd >= table[i]  <=>  rnd + (2^32 - table[i]) carries
+        for (int i = 1; i < 16; ++i)
+            if (h->T[i] == 0)        // "rnd >= 0" has no 32-bit carry constant (2^32 is fine: constant 0, never a carry)
+                return set_error(ISING_EINVAL, "ising_create: beta too small for the look-up-table model "
+                                               "(a table entry above index 0 is 0; needs beta > about 0.001)");
+        ht.table.assign(16, 0u);
+        for (int l = 0; l < 4; ++l)
+            for (int n = 1 << l; n < (2 << l); ++n) {
+                const int idx = ((n - (1 << l)) << (4 - l)) | (1 << (3 - l));
+                ht.table[n] = (uint32_t)((1ull << 32) - h->T[idx]);
+            }
+        // bucket table of the default kernel variant: entry b covers rnd in [b 2^20, (b+1) 2^20):
+        // {C, meta} with getMaxLE(rnd) = meta + carry(rnd + C) when the bucket holds at most one threshold,
+        // meta = 256 (recompute by binary search) when it holds more
+        ht.buckets.assign(2 * 4096, 0u);
+        for (uint64_t b = 0; b < 4096; ++b) {
+            const uint64_t lo = b << 20, hi = lo + (1ull << 20) - 1;
+            int base = 0, inside = 0;
+            for (int i = 1; i < 16; ++i) {
+                if (h->T[i] <= lo) base = i;
+                else if (h->T[i] <= hi) ++inside;
+            }
+            if (inside == 0) { ht.buckets[2 * b] = 0u; ht.buckets[2 * b + 1] = (uint32_t)base; }
+            else if (inside == 1) { ht.buckets[2 * b] = (uint32_t)((1ull << 32) - h->T[base + 1]); ht.buckets[2 * b + 1] = (uint32_t)base; }
+            else { ht.buckets[2 * b] = 0u; ht.buckets[2 * b + 1] = 256u; }
+        }
+    }
+    return ISING_OK;
+}
+
+// Scratch, tables and the seeded lattice of one slab (its memory and stream are in place).
+static int setup_slab(ising_sim *h, int k, const HostTables &ht)
+{
+    Slab &sl = h->slabs[k];
+    DeviceGuard dev_guard(sl.device);
+    CUDA_TRY(cudaEventCreateWithFlags(&sl.done, cudaEventDisableTiming));
+    CUDA_TRY(cudaMemsetAsync(sl.d_acc, 0, 1024, sl.stream));              // accumulators, tally, t_base words
+    if (!ht.table.empty())
+        CUDA_TRY(cudaMemcpyAsync(sl.d_table, ht.table.data(), ht.table.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, sl.stream));
+    if (!ht.buckets.empty()) {
+        CUDA_TRY(cudaMalloc(&sl.lut_buckets, ht.buckets.size() * sizeof(uint32_t)));
+        CUDA_TRY(cudaMemcpyAsync(sl.lut_buckets, ht.buckets.data(), ht.buckets.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, sl.stream));
+    }
+    cudaError_t e = (h->model == ISING_MODEL_ISING_LUT) ? launch_lut_init(h, k) : launch_init(h, k);
+    if (e != cudaSuccess) return cuda_fail(e, "init kernel");
+    CUDA_TRY(cudaStreamSynchronize(sl.stream));                           // the host tables go out of scope after create
+    return ISING_OK;
+}
+
+static void carve_slab(ising_sim *h, Slab &sl, char *base)
+{
+    const size_t colour_bytes = (size_t)sl.rows * (size_t)colour_row_words(h) * 8;
+    sl.lat[0] = (uint64_t *)base;
+    sl.lat[1] = (uint64_t *)(base + colour_bytes);
+    sl.d_acc = (long long *)(base + 2 * colour_bytes);                 // 64 int64 = 512 B (+ sink area)
+    sl.d_table = (uint32_t *)(base + 2 * colour_bytes + 1024);         // 212 uint32 (two table forms)
+}
+
+static int check_create_args(const char *who, int model, int64_t L, double beta, double D, ising_t **out)
+{
+    if (!out) return set_error(ISING_EINVAL, std::string(who) + ": out is NULL");
+    if (!valid_model_L(model, L))
+        return set_error(ISING_EINVAL, std::string(who) + ": unknown model, or L not a multiple of 64 (256 for the LUT model) in [64, 2^20]");
+    if (!(beta >= 0.0) || !isfinite(beta)) return set_error(ISING_EINVAL, std::string(who) + ": beta must be finite and >= 0");
+    if (!isfinite(D)) return set_error(ISING_EINVAL, std::string(who) + ": D must be finite");
+    return ISING_OK;
+}
+
+static ising_sim *new_handle(int model, int64_t L, double beta, double D, uint64_t seed, void *cuda_stream)
+{
+    ising_sim *h = new (std::nothrow) ising_sim();
+    if (!h) return nullptr;
+    h->model = model; h->L = L; h->beta = beta; h->D = is_blume_capel(model) ? D : 0.0; h->seed = seed;
+    h->stream = (cudaStream_t)cuda_stream;
+    build_thresholds(h);
+    build_round_keys(h);
+    default_launch(h);
+    return h;
+}
+
+// common tail of both create calls: slabs carved, streams in place
+static int finish_create(ising_sim *h, ising_t **out)
+{
+    HostTables ht;
+    int rc = build_host_tables(h, ht);
+    if (rc) { ising_destroy(h); return rc; }
+    cudaError_t e = cudaMallocHost(&h->h_acc, (size_t)ISING_MAX_SLABS * 64 * sizeof(long long));
+    if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "cudaMallocHost"); }
+    for (int k = 0; k < (int)h->slabs.size(); ++k) {
+        rc = setup_slab(h, k, ht);
+        if (rc) { ising_destroy(h); return rc; }
+    }
+    const Slab &s0 = h->slabs[0];
+    h->lat[0] = s0.lat[0]; h->lat[1] = s0.lat[1]; h->d_acc = s0.d_acc; h->d_bc_table = s0.d_table;
+    h->lut_buckets = s0.lut_buckets;
+    *out = h;
+    return ISING_OK;
+}
+
 extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_t seed, void *dev_buf,
                             size_t dev_bytes, void *cuda_stream, ising_t **out)
 {
-    if (!out) return set_error(ISING_EINVAL, "ising_create: out is NULL");
-    if (!valid_model_L(model, L))
-        return set_error(ISING_EINVAL, "ising_create: unknown model, or L not a multiple of 64 (256 for the LUT model) in [64, 2^20]");
-    if (!(beta >= 0.0) || !isfinite(beta)) return set_error(ISING_EINVAL, "ising_create: beta must be finite and >= 0");
-    if (!isfinite(D)) return set_error(ISING_EINVAL, "ising_create: D must be finite");
+    int rc = check_create_args("ising_create", model, L, beta, D, out);
+    if (rc) return rc;
     const size_t need = ising_workspace_bytes(model, L);
     if (dev_buf && dev_bytes < need) return set_error(ISING_EINVAL, "ising_create: dev_bytes < ising_workspace_bytes()");
     if (dev_buf && ((uintptr_t)dev_buf & 255u)) return set_error(ISING_EINVAL, "ising_create: dev_buf must be 256-byte aligned");
 
-    ising_sim *h = new (std::nothrow) ising_sim();
+    ising_sim *h = new_handle(model, L, beta, D, seed, cuda_stream);
     if (!h) return set_error(ISING_ENOMEM, "ising_create: host allocation failed");
-    h->model = model; h->L = L; h->beta = beta; h->D = is_blume_capel(model) ? D : 0.0; h->seed = seed;
-    h->stream = (cudaStream_t)cuda_stream;
     char *base = (char *)dev_buf;
     cudaGetDevice(&h->device);                       // NULL dev_buf: the caller's current device
     if (base) {
@@ -100,113 +224,183 @@ extern "C" int ising_create(int model, int64_t L, double beta, double D, uint64_
         h->device = attr.device;
     }
     DeviceGuard dev_guard(h->device);
+    Slab sl;                                         // the whole lattice is one slab; its halo rows are its own
+    sl.device = h->device; sl.stream = h->stream; sl.y0 = 0; sl.rows = L;
     if (!base) {
-        cudaError_t e = cudaMalloc(&h->owned, need);
+        cudaError_t e = cudaMalloc(&sl.owned, need);
         if (e != cudaSuccess) {
             delete h;
             cudaGetLastError();
             return set_error(e == cudaErrorMemoryAllocation ? ISING_ENOMEM : ISING_ECUDA,
                              std::string("ising_create: cudaMalloc: ") + cudaGetErrorString(e));
         }
-        base = (char *)h->owned;
+        base = (char *)sl.owned;
     }
-    const size_t colour_bytes = (size_t)L * (size_t)L / (size_t)sites_per_word(model) * 4;
-    h->lat[0] = (uint64_t *)base;
-    h->lat[1] = (uint64_t *)(base + colour_bytes);
-    h->d_acc = (long long *)(base + 2 * colour_bytes);                 // 64 int64 = 512 B (+ 4 KiB sink area unused)
-    h->d_bc_table = (uint32_t *)(base + 2 * colour_bytes + 1024);      // 212 uint32 (two table forms)
-    build_thresholds(h);
-    build_round_keys(h);
-    default_launch(h);
-    {
-        cudaError_t ez = cudaMemsetAsync(h->d_acc, 0, 1024, h->stream);   // accumulators, tally, t_base words
-        if (ez != cudaSuccess) { ising_destroy(h); return cuda_fail(ez, "cudaMemsetAsync(scratch)"); }
+    carve_slab(h, sl, base);
+    h->slabs.push_back(sl);
+    return finish_create(h, out);
+}
+
+// NEXT-4: the lattice as n_slabs row slabs, each an
+// allocation of its own on the device the caller names, with the two halo rows of a slab read straight from
+// its neighbours' memory (peer access between the devices involved is switched on here).
+extern "C" int ising_create_slabs(int model, int64_t L, double beta, double D, uint64_t seed, int n_slabs,
+                                  const int64_t *slab_rows, const int *devices, void *cuda_stream, ising_t **out)
+{
+    int rc = check_create_args("ising_create_slabs", model, L, beta, D, out);
+    if (rc) return rc;
+    if (n_slabs < 1 || n_slabs > ISING_MAX_SLABS || 2 * (int64_t)n_slabs > L)
+        return set_error(ISING_EINVAL, "ising_create_slabs: n_slabs must be in [1, 64] and leave every slab two rows");
+    std::vector<int64_t> rows(n_slabs);
+    int64_t total = 0;
+    for (int k = 0; k < n_slabs; ++k) {
+        // default: L/2 row pairs dealt as evenly as possible
+        rows[k] = slab_rows ? slab_rows[k] : 2 * ((L / 2) * (k + 1) / n_slabs - (L / 2) * k / n_slabs);
+        if (rows[k] < 2 || (rows[k] & 1)) return set_error(ISING_EINVAL, "ising_create_slabs: every slab needs an even number of rows >= 2");
+        total += rows[k];
     }
-    cudaError_t e = cudaMallocHost(&h->h_acc, 256 * sizeof(long long));
-    if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "cudaMallocHost"); }
-    if (is_blume_capel(model)) {
-        // [0, 66): thresholds clamped to 2^32-1 + "always" bit mask (compare/select variant).
-        // [80, 80 + 132): carry form for the default variant, two halves of 66 words (264 bytes):
-        // C[b][16 code + S] = 2^32 - T, 0 for T = 2^32 (never a carry -> always accepted).  T = 0 has
-        // no 32-bit carry constant: launch_update then uses the compare/select variant.
-        uint32_t tab[80 + 132] = {};
-        uint64_t always = 0;
-        for (int i = 0; i < 54; ++i) {
-            if (h->T[i] >> 32) { always |= 1ull << i; tab[i] = 0xFFFFFFFFu; }
-            else tab[i] = (uint32_t)h->T[i];
+    if (total != L) return set_error(ISING_EINVAL, "ising_create_slabs: slab_rows must add up to L");
+    int n_dev = 0, cur = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1 || cudaGetDevice(&cur) != cudaSuccess) {
+        cudaGetLastError();
+        return set_error(ISING_ECUDA, "ising_create_slabs: no CUDA device");
+    }
+    for (int k = 0; devices && k < n_slabs; ++k)
+        if (devices[k] < 0 || devices[k] >= n_dev) return set_error(ISING_EINVAL, "ising_create_slabs: device index out of range");
+
+    ising_sim *h = new_handle(model, L, beta, D, seed, cuda_stream);
+    if (!h) return set_error(ISING_ENOMEM, "ising_create_slabs: host allocation failed");
+    h->device = devices ? devices[0] : cur;
+    // plain loads across devices: every device used maps every other one
+    for (int a = 0; devices && a < n_slabs; ++a)
+        for (int b = 0; b < n_slabs; ++b) {
+            if (devices[a] == devices[b]) continue;
+            DeviceGuard g(devices[a]);
+            cudaError_t e = cudaDeviceEnablePeerAccess(devices[b], 0);
+            if (e == cudaErrorPeerAccessAlreadyEnabled) { cudaGetLastError(); continue; }
+            if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaDeviceEnablePeerAccess (slabs on devices without peer access)"); }
         }
-        tab[64] = (uint32_t)always; tab[65] = (uint32_t)(always >> 32);
-        for (int code = 0; code < 3; ++code)
-            for (int S = 0; S <= 8; ++S)
-                for (int b = 0; b < 2; ++b) {
-                    const uint64_t T = h->T[(code * 2 + b) * 9 + S];
-                    tab[80 + 66 * b + 16 * code + S] = (T >> 32) ? 0u : (uint32_t)((1ull << 32) - T);
-                }
-        memcpy(h->h_acc, tab, sizeof(tab));
-        e = cudaMemcpyAsync(h->d_bc_table, h->h_acc, sizeof(tab), cudaMemcpyHostToDevice, h->stream);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-        if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "upload of the Blume-Capel table"); }
-    }
-    if (model == ISING_MODEL_ISING_LUT) {
-        // heap-ordered carry constants of the binary search: node n at level l splits at table index
-        // ((n - 2^l) << (4 - l)) | (1 << (3 - l));  rnd >= table[i]  <=>  rnd + (2^32 - table[i]) carries
-        uint32_t tree[16] = {};
-        for (int i = 1; i < 16; ++i)
-            if (h->T[i] == 0) {      // "rnd >= 0" has no 32-bit carry constant (2^32 is fine: constant 0, never a carry)
-                ising_destroy(h);
-                return set_error(ISING_EINVAL, "ising_create: beta too small for the look-up-table model "
-                                               "(a table entry above index 0 is 0; needs beta > about 0.001)");
-            }
-        for (int l = 0; l < 4; ++l)
-            for (int n = 1 << l; n < (2 << l); ++n) {
-                const int idx = ((n - (1 << l)) << (4 - l)) | (1 << (3 - l));
-                tree[n] = (uint32_t)((1ull << 32) - h->T[idx]);
-            }
-        memcpy(h->h_acc, tree, sizeof(tree));
-        e = cudaMemcpyAsync(h->d_bc_table, h->h_acc, sizeof(tree), cudaMemcpyHostToDevice, h->stream);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-        if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "upload of the look-up table"); }
-        // bucket table of the default kernel variant: entry b covers rnd in [b 2^20, (b+1) 2^20):
-        // {C, meta} with getMaxLE(rnd) = meta + carry(rnd + C) when the bucket holds at most one threshold,
-        // meta = 256 (recompute by binary search) when it holds more
-        std::vector<uint32_t> bk(2 * 4096);
-        for (uint64_t b = 0; b < 4096; ++b) {
-            const uint64_t lo = b << 20, hi = lo + (1ull << 20) - 1;
-            int base = 0, inside = 0;
-            for (int i = 1; i < 16; ++i) {
-                if (h->T[i] <= lo) base = i;
-                else if (h->T[i] <= hi) ++inside;
-            }
-            if (inside == 0) { bk[2 * b] = 0u; bk[2 * b + 1] = (uint32_t)base; }
-            else if (inside == 1) { bk[2 * b] = (uint32_t)((1ull << 32) - h->T[base + 1]); bk[2 * b + 1] = (uint32_t)base; }
-            else { bk[2 * b] = 0u; bk[2 * b + 1] = 256u; }
+    int64_t y0 = 0;
+    for (int k = 0; k < n_slabs; ++k) {
+        Slab sl;
+        sl.device = devices ? devices[k] : cur;
+        sl.y0 = y0; sl.rows = rows[k];
+        y0 += rows[k];
+        DeviceGuard g(sl.device);
+        cudaError_t e = cudaSuccess;
+        if (k == 0) sl.stream = h->stream;
+        else { e = cudaStreamCreateWithFlags(&sl.stream, cudaStreamNonBlocking); sl.own_stream = e == cudaSuccess; }
+        const size_t bytes = (size_t)sl.rows * (size_t)colour_row_words(h) * 16 + kScratchBytes;
+        if (e == cudaSuccess) e = cudaMalloc(&sl.owned, bytes);
+        h->slabs.push_back(sl);                      // before the error check: ising_destroy frees what exists
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            ising_destroy(h);
+            return set_error(e == cudaErrorMemoryAllocation ? ISING_ENOMEM : ISING_ECUDA,
+                             std::string("ising_create_slabs: slab allocation: ") + cudaGetErrorString(e));
         }
-        e = cudaMalloc(&h->lut_buckets, bk.size() * sizeof(uint32_t));
-        if (e == cudaSuccess) e = cudaMemcpy(h->lut_buckets, bk.data(), bk.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
-        if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "upload of the bucket table"); }
+        carve_slab(h, h->slabs.back(), (char *)sl.owned);
     }
-    e = (model == ISING_MODEL_ISING_LUT) ? launch_lut_init(h) : launch_init(h);
-    if (e != cudaSuccess) { ising_destroy(h); return cuda_fail(e, "init kernel"); }
-    *out = h;
+    return finish_create(h, out);
+}
+
+extern "C" int ising_slab_count(const ising_t *h) { return h ? (int)h->slabs.size() : 0; }
+
+extern "C" int ising_slab_info(const ising_t *h, int slab, int64_t *y0, int64_t *rows, int *device)
+{
+    if (!h || slab < 0 || slab >= (int)h->slabs.size()) return set_error(ISING_EINVAL, "ising_slab_info: bad handle or slab index");
+    if (y0) *y0 = h->slabs[slab].y0;
+    if (rows) *rows = h->slabs[slab].rows;
+    if (device) *device = h->slabs[slab].device;
     return ISING_OK;
 }
 
 extern "C" int ising_destroy(ising_t *h)
 {
-    DeviceGuard dev_guard(h);
     if (!h) return ISING_OK;
-    cudaStreamSynchronize(h->stream);
-    if (h->io_stage) cudaFree(h->io_stage);
-    if (h->planes) cudaFree(h->planes);
-    if (h->comb) cudaFree(h->comb);
-    if (h->gram) cudaFree(h->gram);
-    drop_graph(h);
-    if (h->lut_buckets) cudaFree(h->lut_buckets);
-    if (h->d_corr) cudaFree(h->d_corr);
-    if (h->d_rlist) cudaFree(h->d_rlist);
-    if (h->h_acc) cudaFreeHost(h->h_acc);
-    if (h->owned) cudaFree(h->owned);
+    for (Slab &sl : h->slabs) {
+        DeviceGuard g(sl.device);
+        cudaStreamSynchronize(sl.stream);
+    }
+    {
+        DeviceGuard dev_guard(h);
+        if (h->io_stage) cudaFree(h->io_stage);
+        if (h->planes) cudaFree(h->planes);
+        if (h->comb) cudaFree(h->comb);
+        if (h->gram) cudaFree(h->gram);
+        drop_graph(h);
+        if (h->d_corr) cudaFree(h->d_corr);
+        if (h->d_rlist) cudaFree(h->d_rlist);
+        if (h->h_acc) cudaFreeHost(h->h_acc);
+    }
+    for (Slab &sl : h->slabs) {
+        DeviceGuard g(sl.device);
+        if (sl.lut_buckets) cudaFree(sl.lut_buckets);
+        if (sl.done) cudaEventDestroy(sl.done);
+        if (sl.own_stream) cudaStreamDestroy(sl.stream);
+        if (sl.owned) cudaFree(sl.owned);
+    }
     delete h;
+    return ISING_OK;
+}
+
+// ------------------------------------------------------- slab sequencing ---
+// Work that touches the whole lattice through one stream (IO, bit planes, copies) runs on the main stream
+// = slab 0's; per-slab kernels run on the slab's own stream and device.  fan_out: every slab stream waits
+// for what is queued on the main stream; fan_in: the main stream waits for every slab stream.  Both are
+// no-ops for an unsharded lattice.
+static int fan_out(ising_sim *h)
+{
+    if (h->slabs.size() < 2) return ISING_OK;
+    {
+        DeviceGuard g(h->slabs[0].device);
+        CUDA_TRY(cudaEventRecord(h->slabs[0].done, h->slabs[0].stream));
+    }
+    for (size_t k = 1; k < h->slabs.size(); ++k) {
+        DeviceGuard g(h->slabs[k].device);
+        CUDA_TRY(cudaStreamWaitEvent(h->slabs[k].stream, h->slabs[0].done, 0));
+    }
+    return ISING_OK;
+}
+
+static int fan_in(ising_sim *h)
+{
+    for (size_t k = 1; k < h->slabs.size(); ++k) {
+        {
+            DeviceGuard g(h->slabs[k].device);
+            CUDA_TRY(cudaEventRecord(h->slabs[k].done, h->slabs[k].stream));
+        }
+        DeviceGuard g(h->slabs[0].device);
+        CUDA_TRY(cudaStreamWaitEvent(h->slabs[0].stream, h->slabs[k].done, 0));
+    }
+    return ISING_OK;
+}
+
+// One per-slab pass (observables, histogram): launch(k) on every slab between fan_out and fan_in.
+template <typename F>
+static int for_each_slab(ising_sim *h, const char *what, F launch)
+{
+    int rc = fan_out(h);
+    if (rc) return rc;
+    for (int k = 0; k < (int)h->slabs.size(); ++k) {
+        DeviceGuard g(h->slabs[k].device);
+        cudaError_t e = launch(k);
+        if (e != cudaSuccess) return cuda_fail(e, what);
+    }
+    return fan_in(h);
+}
+
+// Mirror the accumulators [first, first + n) of every slab into h_acc[64 k + first ...] and add them up in int64.
+static int sum_over_slabs(ising_sim *h, int first, int n, long long *total)
+{
+    for (int k = 0; k < (int)h->slabs.size(); ++k)
+        CUDA_TRY(cudaMemcpyAsync(h->h_acc + 64 * k + first, h->slabs[k].d_acc + first, n * sizeof(long long),
+                                 cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    for (int j = 0; j < n; ++j) {
+        total[j] = 0;
+        for (int k = 0; k < (int)h->slabs.size(); ++k) total[j] += h->h_acc[64 * k + first + j];
+    }
     return ISING_OK;
 }
 
@@ -228,9 +422,31 @@ static const int kGraphSweeps = 16;
 
 __global__ void set_t_base_kernel(uint32_t *t_base, uint32_t value) { *t_base = value; }
 
+// One colour phase of sweep t on every slab.  A slab's kernel reads the boundary rows of its two neighbours
+// (written by their previous phase) and overwrites rows they read in that phase, so it waits for the previous
+// phase of both; slabs of the same phase run concurrently on their own streams.  Unsharded: one launch.
 static cudaError_t launch_colour(ising_sim *h, int c, uint32_t t)
 {
-    return (h->model == ISING_MODEL_ISING_LUT) ? launch_lut_update(h, c, t) : launch_update(h, c, t);
+    const int S = (int)h->slabs.size();
+    for (int k = 0; S > 1 && k < S; ++k) {
+        DeviceGuard g(h->slabs[k].device);
+        for (int nb : {(k + S - 1) % S, (k + 1) % S}) {
+            if (nb == k) continue;
+            cudaError_t e = cudaStreamWaitEvent(h->slabs[k].stream, h->slabs[nb].done, 0);
+            if (e != cudaSuccess) return e;
+        }
+    }
+    for (int k = 0; k < S; ++k) {
+        DeviceGuard g(h->slabs[k].device);
+        cudaError_t e = (h->model == ISING_MODEL_ISING_LUT) ? launch_lut_update(h, k, c, t) : launch_update(h, k, c, t);
+        if (e != cudaSuccess) return e;
+    }
+    for (int k = 0; S > 1 && k < S; ++k) {
+        DeviceGuard g(h->slabs[k].device);
+        cudaError_t e = cudaEventRecord(h->slabs[k].done, h->slabs[k].stream);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 static void drop_graph(ising_sim *h)
@@ -241,7 +457,7 @@ static void drop_graph(ising_sim *h)
 static bool graph_worthwhile(const ising_sim *h, int64_t n)
 {
     const int64_t sites = h->L * h->L;
-    return n >= 2 * kGraphSweeps && sites <= (1ll << 22);      // L <= 2048: a colour phase is launch-bound
+    return n >= 2 * kGraphSweeps && sites <= (1ll << 22) && h->slabs.size() == 1;      // L <= 2048: a colour phase is launch-bound
 }
 
 static int ensure_graph(ising_sim *h)
@@ -257,11 +473,11 @@ static int ensure_graph(ising_sim *h)
     cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
     if (e != cudaSuccess) { cudaStreamDestroy(cap); return cuda_fail(e, "cudaStreamBeginCapture"); }
     h->graph_capture = true;
-    h->stream = cap;
+    h->stream = h->slabs[0].stream = cap;
     const int64_t launches_before = h->launches;
     for (int j = 0; j < kGraphSweeps && e == cudaSuccess; ++j)
         for (int c = 0; c < 2 && e == cudaSuccess; ++c) e = launch_colour(h, c, (uint32_t)j);
-    h->stream = user;
+    h->stream = h->slabs[0].stream = user;
     h->graph_capture = false;
     h->launches = launches_before;                              // counted when the graph is replayed
     cudaError_t e2 = cudaStreamEndCapture(cap, &graph);
@@ -296,6 +512,10 @@ extern "C" int ising_sweep(ising_t *h, int64_t n)
             n -= kGraphSweeps;
         }
     }
+    if (n > 0) {
+        int rc = fan_out(h);
+        if (rc) return rc;
+    }
     for (int64_t i = 0; i < n; ++i) {
         for (int c = 0; c < 2; ++c) {
             cudaError_t e = launch_colour(h, c, (uint32_t)h->t);
@@ -303,7 +523,7 @@ extern "C" int ising_sweep(ising_t *h, int64_t n)
         }
         h->t++;
     }
-    return ISING_OK;
+    return n > 0 ? fan_in(h) : ISING_OK;
 }
 
 // A11: sweep to every time of an ascending schedule and record B, M, Q there (fused tally if it is on,
@@ -358,43 +578,10 @@ extern "C" int ising_set_variant(ising_t *h, int variant)
 }
 
 // ----------------------------------------------------------- observables ---
-extern "C" int ising_observables(ising_t *h, ising_obs_t *out)
-{
-    DeviceGuard dev_guard(h);
-    if (!h || !out) return set_error(ISING_EINVAL, "ising_observables: NULL argument");
-    const bool lut = h->model == ISING_MODEL_ISING_LUT;
-    cudaError_t e = lut ? launch_lut_observables(h) : launch_observables(h);
-    if (e != cudaSuccess) return cuda_fail(e, "observables kernel");
-    CUDA_TRY(cudaMemcpyAsync(h->h_acc, h->d_acc, 3 * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
-    CUDA_TRY(cudaStreamSynchronize(h->stream));
-    ising_obs_t o;
-    o.bond_sum = h->h_acc[0]; o.M = h->h_acc[1]; o.Q = lut ? h->L * h->L : h->h_acc[2];
-    o.n_sites = h->L * h->L; o.sweeps_done = h->t;
-    const double N = (double)h->L * (double)h->L;
-    o.E = !is_blume_capel(h->model) ? -(double)o.bond_sum : -(double)o.bond_sum + h->D * (double)o.Q;
-    o.e_per_site = o.E / N;
-    o.m_per_site = (double)o.M / N;
-    o.zero_density = (double)(o.n_sites - o.Q) / N;
-    *out = o;
-    return ISING_OK;
-}
-
-// A7: fused tally.  d_acc[40..42] hold running B, M, Q; the update kernels add the changes.
-static int tally_resync(ising_sim *h)
+static int observe_all_slabs(ising_sim *h)                // -> d_acc[0..2] of every slab
 {
     const bool lut = h->model == ISING_MODEL_ISING_LUT;
-    cudaError_t e = lut ? launch_lut_observables(h) : launch_observables(h);
-    if (e != cudaSuccess) return cuda_fail(e, "observables kernel");
-    CUDA_TRY(cudaMemcpyAsync(h->d_acc + 40, h->d_acc, 3 * sizeof(long long), cudaMemcpyDeviceToDevice, h->stream));
-    return ISING_OK;
-}
-
-extern "C" int ising_set_tally(ising_t *h, int on)
-{
-    DeviceGuard dev_guard(h);
-    if (!h) return set_error(ISING_EINVAL, "ising_set_tally: NULL handle");
-    h->tally_on = on != 0;
-    return h->tally_on ? tally_resync(h) : ISING_OK;
+    return for_each_slab(h, "observables kernel", [&](int k) { return lut ? launch_lut_observables(h, k) : launch_observables(h, k); });
 }
 
 static void fill_obs(const ising_sim *h, const long long *bmq, ising_obs_t *o)
@@ -409,14 +596,46 @@ static void fill_obs(const ising_sim *h, const long long *bmq, ising_obs_t *o)
     o->zero_density = (double)(o->n_sites - o->Q) / N;
 }
 
+extern "C" int ising_observables(ising_t *h, ising_obs_t *out)
+{
+    DeviceGuard dev_guard(h);
+    if (!h || !out) return set_error(ISING_EINVAL, "ising_observables: NULL argument");
+    int rc = observe_all_slabs(h);
+    if (rc) return rc;
+    long long bmq[3];                                    // every slab's sums, added in int64
+    rc = sum_over_slabs(h, 0, 3, bmq);
+    if (rc) return rc;
+    fill_obs(h, bmq, out);
+    return ISING_OK;
+}
+
+// A7: fused tally.  d_acc[40..42] hold running B, M, Q; the update kernels add the changes.
+static int tally_resync(ising_sim *h)
+{
+    int rc = observe_all_slabs(h);
+    if (rc) return rc;
+    for (const Slab &sl : h->slabs)                      // every slab keeps the running sums of its own rows
+        CUDA_TRY(cudaMemcpyAsync(sl.d_acc + 40, sl.d_acc, 3 * sizeof(long long), cudaMemcpyDeviceToDevice, h->stream));
+    return ISING_OK;
+}
+
+extern "C" int ising_set_tally(ising_t *h, int on)
+{
+    DeviceGuard dev_guard(h);
+    if (!h) return set_error(ISING_EINVAL, "ising_set_tally: NULL handle");
+    h->tally_on = on != 0;
+    return h->tally_on ? tally_resync(h) : ISING_OK;
+}
+
 extern "C" int ising_tally(ising_t *h, ising_obs_t *out)
 {
     DeviceGuard dev_guard(h);
     if (!h || !out) return set_error(ISING_EINVAL, "ising_tally: NULL argument");
     if (!h->tally_on) return set_error(ISING_EINVAL, "ising_tally: the tally is off (ising_set_tally)");
-    CUDA_TRY(cudaMemcpyAsync(h->h_acc + 40, h->d_acc + 40, 3 * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
-    CUDA_TRY(cudaStreamSynchronize(h->stream));
-    fill_obs(h, h->h_acc + 40, out);
+    long long bmq[3];
+    int rc = sum_over_slabs(h, 40, 3, bmq);
+    if (rc) return rc;
+    fill_obs(h, bmq, out);
     return ISING_OK;
 }
 
@@ -424,13 +643,15 @@ extern "C" int ising_schwinger_dyson(ising_t *h, int64_t hist[9], double *value)
 {
     DeviceGuard dev_guard(h);
     if (!h || !hist || !value) return set_error(ISING_EINVAL, "ising_schwinger_dyson: NULL argument");
-    cudaError_t e = (h->model == ISING_MODEL_ISING_LUT) ? launch_lut_sd_hist(h) : launch_sd_hist(h);
-    if (e != cudaSuccess) return cuda_fail(e, "Schwinger-Dyson kernel");
-    CUDA_TRY(cudaMemcpyAsync(h->h_acc + 8, h->d_acc + 8, 9 * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
-    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    const bool lut = h->model == ISING_MODEL_ISING_LUT;
+    int rc = for_each_slab(h, "Schwinger-Dyson kernel", [&](int k) { return lut ? launch_lut_sd_hist(h, k) : launch_sd_hist(h, k); });
+    if (rc) return rc;
+    long long bins[9];
+    rc = sum_over_slabs(h, 8, 9, bins);
+    if (rc) return rc;
     double acc = 0.0;
     for (int k = -4; k <= 4; ++k) {
-        hist[k + 4] = h->h_acc[8 + k + 4];
+        hist[k + 4] = bins[k + 4];
         acc += (double)hist[k + 4] * exp(-2.0 * h->beta * (double)k);
     }
     *value = acc / ((double)h->L * (double)h->L);
@@ -521,7 +742,11 @@ extern "C" int ising_read_packed(ising_t *h, int colour, int64_t word0, int64_t 
     if (!h || !host_out) return set_error(ISING_EINVAL, "ising_read_packed: NULL argument");
     if ((colour != 0 && colour != 1) || word0 < 0 || nwords < 0 || word0 + nwords > colour_words(h))
         return set_error(ISING_EINVAL, "ising_read_packed: range outside the colour array");
-    CUDA_TRY(cudaMemcpyAsync(host_out, h->lat[colour] + word0, (size_t)nwords * 8, cudaMemcpyDeviceToHost, h->stream));
+    for (const Slab &sl : h->slabs) {                    // the word range, slab by slab
+        const int64_t first = sl.y0 * colour_row_words(h), last = first + sl.rows * colour_row_words(h);
+        const int64_t a = std::max(word0, first), b = std::min(word0 + nwords, last);
+        if (a < b) CUDA_TRY(cudaMemcpyAsync(host_out + (a - word0), sl.lat[colour] + (a - first), (size_t)(b - a) * 8, cudaMemcpyDeviceToHost, h->stream));
+    }
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     return ISING_OK;
 }
@@ -532,7 +757,11 @@ extern "C" int ising_write_packed(ising_t *h, int colour, int64_t word0, int64_t
     if (!h || !host_in) return set_error(ISING_EINVAL, "ising_write_packed: NULL argument");
     if ((colour != 0 && colour != 1) || word0 < 0 || nwords < 0 || word0 + nwords > colour_words(h))
         return set_error(ISING_EINVAL, "ising_write_packed: range outside the colour array");
-    CUDA_TRY(cudaMemcpyAsync(h->lat[colour] + word0, host_in, (size_t)nwords * 8, cudaMemcpyHostToDevice, h->stream));
+    for (const Slab &sl : h->slabs) {
+        const int64_t first = sl.y0 * colour_row_words(h), last = first + sl.rows * colour_row_words(h);
+        const int64_t a = std::max(word0, first), b = std::min(word0 + nwords, last);
+        if (a < b) CUDA_TRY(cudaMemcpyAsync(sl.lat[colour] + (a - first), host_in + (a - word0), (size_t)(b - a) * 8, cudaMemcpyHostToDevice, h->stream));
+    }
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     return h->tally_on ? tally_resync(h) : ISING_OK;
 }

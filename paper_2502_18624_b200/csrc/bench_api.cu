@@ -8,7 +8,7 @@
 extern "C" int ising_bench_philox_only(ising_t *h, int n)
 {
     DeviceGuard dev_guard(h);
-    if (!h || n < 0 || h->model == ISING_MODEL_ISING_LUT) return set_error(ISING_EINVAL, "ising_bench_philox_only: bad argument");
+    if (!h || n < 0 || h->model == ISING_MODEL_ISING_LUT || h->slabs.size() != 1) return set_error(ISING_EINVAL, "ising_bench_philox_only: bad argument (4-bit and 2-bit models, unsharded lattice)");
     for (int i = 0; i < n; ++i) {
         cudaError_t e = launch_philox_only(h, (uint32_t)i);
         if (e != cudaSuccess) return cuda_fail(e, "philox-only kernel");
@@ -19,7 +19,7 @@ extern "C" int ising_bench_philox_only(ising_t *h, int n)
 extern "C" int ising_bench_copy(ising_t *h, int n)
 {
     DeviceGuard dev_guard(h);
-    if (!h || n < 0 || h->model == ISING_MODEL_ISING_LUT) return set_error(ISING_EINVAL, "ising_bench_copy: bad argument");
+    if (!h || n < 0 || h->model == ISING_MODEL_ISING_LUT || h->slabs.size() != 1) return set_error(ISING_EINVAL, "ising_bench_copy: bad argument (4-bit and 2-bit models, unsharded lattice)");
     for (int i = 0; i < n; ++i) {
         cudaError_t e = launch_copy(h);
         if (e != cudaSuccess) return cuda_fail(e, "copy kernel");

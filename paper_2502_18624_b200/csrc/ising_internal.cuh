@@ -16,7 +16,37 @@ struct RoundKeys {  // Philox key schedule (PAPER.md:149 names the generator): k
     uint32_t k0[10], k1[10];
 };
 
+// NEXT-4 ("partitioning each buffer into horizontal slabs ... restricting [communication] to
+// just two rows"): a slab = the consecutive rows [y0, y0 + rows) of both colour arrays in an allocation of
+// its own, on a device of its own choice.  The kernels of a slab take its base pointers and, separately,
+// pointers to the one row above and the one row below it in the neighbouring slabs (plain loads, peer
+// memory when the neighbour lives on another device).  An unsharded lattice is one slab whose
+// halo rows are its own last and first row.
+struct Slab {
+    int device = -1;
+    cudaStream_t stream = nullptr;          // slab 0: the caller's stream; others: created by the library
+    bool own_stream = false;
+    int64_t y0 = 0, rows = 0;               // global rows [y0, y0 + rows); both even
+    uint64_t *lat[2] = {nullptr, nullptr};  // black, white rows of this slab (device)
+    void *owned = nullptr;                  // allocation made by the library (lattice + scratch), or NULL
+    long long *d_acc = nullptr;             // 64 int64 accumulators in the slab's scratch area
+    uint32_t *d_table = nullptr;            // Blume-Capel tables / LUT search tree on the slab's device
+    void *lut_buckets = nullptr;            // LUT model: bucket table on the slab's device (cudaMalloc)
+    cudaEvent_t done = nullptr;             // recorded after every colour phase (and every per-slab pass)
+};
+
+#define ISING_MAX_SLABS 64
+
+// Row directory handed by value to the kernels that address the lattice by global row (IO, bit planes):
+// slab k holds the rows [y_end[k-1], y_end[k]).
+struct SlabDir {
+    int n;
+    long long y_end[ISING_MAX_SLABS];
+    uint64_t *lat[2][ISING_MAX_SLABS];
+};
+
 struct ising_sim {
+    std::vector<Slab> slabs;                // >= 1; slabs[0] aliases lat / d_acc / d_bc_table / stream below
     int model = 0;
     int64_t L = 0;
     double beta = 0, D = 0;
@@ -90,16 +120,29 @@ static inline int64_t sites_per_word(int model)
 {
     return model == ISING_MODEL_ISING_LUT ? 64 : model == ISING_MODEL_BLUME_CAPEL_2BIT ? 32 : 16;
 }
-// uint64 words of one colour array
+// uint64 words of one colour array / of one colour row
 static inline int64_t colour_words(const ising_sim *h) { return h->L * (h->L / (2 * sites_per_word(h->model))); }
+static inline int64_t colour_row_words(const ising_sim *h) { return h->L / (2 * sites_per_word(h->model)); }
+// Halo rows of slab k in colour array c: the last row of the slab above, the first row of the slab below (periodic).
+static inline const uint64_t *halo_up(const ising_sim *h, int k, int c)
+{
+    const Slab &a = h->slabs[(k + (int)h->slabs.size() - 1) % (int)h->slabs.size()];
+    return a.lat[c] + (a.rows - 1) * colour_row_words(h);
+}
+static inline const uint64_t *halo_down(const ising_sim *h, int k, int c)
+{
+    return h->slabs[(k + 1) % (int)h->slabs.size()].lat[c];
+}
 // 64-bit words per row of a plane down-sampled to the bits x % stride == 0 (zero padded)
 static inline int64_t comb_words_per_row(int64_t L, int64_t stride) { return (L / stride + 63) / 64; }
 
 // kernels' host launchers (each returns a cudaError_t from the launch)
-cudaError_t launch_init(ising_sim *h);
-cudaError_t launch_update(ising_sim *h, int colour, uint32_t t);
-cudaError_t launch_observables(ising_sim *h);                       // -> d_acc[0..2] = B, M, Q
-cudaError_t launch_sd_hist(ising_sim *h);                           // -> d_acc[8..16]
+// per-slab launchers run on the slab's stream (the caller has switched to the slab's device)
+cudaError_t launch_init(ising_sim *h, int slab);
+cudaError_t launch_update(ising_sim *h, int slab, int colour, uint32_t t);
+cudaError_t launch_observables(ising_sim *h, int slab);             // -> slab d_acc[0..2] = B, M, Q of the slab's rows
+cudaError_t launch_sd_hist(ising_sim *h, int slab);                 // -> slab d_acc[8..16]
+SlabDir slab_directory(const ising_sim *h);
 cudaError_t launch_unpack(ising_sim *h, int64_t x0, int64_t y0, int64_t w, int64_t hgt, int8_t *dev_out);
 cudaError_t launch_pack(ising_sim *h, int64_t y0, int64_t ny, const int8_t *dev_in, int *dev_bad, int write);
 cudaError_t launch_planes(ising_sim *h);                            // lattice -> bit planes
@@ -108,10 +151,10 @@ cudaError_t launch_corr(ising_sim *h, int64_t stride, int64_t count, const long 
 bool corr_gram_supported(const ising_sim *h, int64_t rmax);
 size_t corr_gram_bytes(const ising_sim *h);
 cudaError_t launch_corr_gram(ising_sim *h, int64_t count, long long *dev_sx, long long *dev_sy);
-cudaError_t launch_lut_init(ising_sim *h);
-cudaError_t launch_lut_update(ising_sim *h, int colour, uint32_t t);
-cudaError_t launch_lut_observables(ising_sim *h);                   // -> d_acc[0..1] = B, M
-cudaError_t launch_lut_sd_hist(ising_sim *h);                       // -> d_acc[8..16]
+cudaError_t launch_lut_init(ising_sim *h, int slab);
+cudaError_t launch_lut_update(ising_sim *h, int slab, int colour, uint32_t t);
+cudaError_t launch_lut_observables(ising_sim *h, int slab);         // -> slab d_acc[0..1] = B, M
+cudaError_t launch_lut_sd_hist(ising_sim *h, int slab);             // -> slab d_acc[8..16]
 cudaError_t launch_philox_only(ising_sim *h, uint32_t t);
 cudaError_t launch_copy(ising_sim *h);
 cudaError_t launch_debug_philox(int64_t count, const uint32_t *d_ctr, const uint32_t *d_key,
@@ -123,6 +166,15 @@ cudaError_t launch_debug_philox(int64_t count, const uint32_t *d_ctr, const uint
 #define PHILOX_M1 0xCD9E8D57u
 #define PHILOX_W0 0x9E3779B9u
 #define PHILOX_W1 0xBB67AE85u
+
+// Row y of colour array c through the row directory (kernels that address the lattice by global row)
+__device__ __forceinline__ uint64_t *slab_row(const SlabDir &d, int c, long long y, long long row_words)
+{
+    int k = 0;
+    while (k + 1 < d.n && y >= d.y_end[k]) ++k;
+    const long long first = k ? d.y_end[k - 1] : 0;
+    return d.lat[c][k] + (y - first) * row_words;
+}
 
 // Block-level sum of N per-thread ints into the int64 accumulators dst[0..N): warp
 // reduction (warp sums must fit 32 bits), one shared-memory atomic per warp, ONE

@@ -2,9 +2,21 @@
 // the correlation kernels read (A9: "Pair product via 1-bit planes").
 #include "ising_internal.cuh"
 
+SlabDir slab_directory(const ising_sim *h)
+{
+    SlabDir d;
+    d.n = (int)h->slabs.size();
+    for (int k = 0; k < ISING_MAX_SLABS; ++k) {
+        const bool live = k < d.n;
+        d.y_end[k] = live ? h->slabs[k].y0 + h->slabs[k].rows : h->L;
+        for (int c = 0; c < 2; ++c) d.lat[c][k] = live ? h->slabs[k].lat[c] : nullptr;
+    }
+    return d;
+}
+
 // ---------------------------------------------------------------- unpack ---
 struct UnpackParams {
-    const uint64_t *lat[2];
+    SlabDir dir;
     int64_t L, x0, y0, w, hgt;
     int model;
     int8_t *out;
@@ -19,16 +31,16 @@ __global__ void __launch_bounds__(256) unpack_kernel(const __grid_constant__ Unp
     int c = (int)((x + y) & 1);
     int64_t k = x >> 1;
     if (p.model == ISING_MODEL_ISING_LUT) {                  // 1 bit per spin, 64 sites per word
-        uint64_t word = p.lat[c][y * (p.L / 128) + (k >> 6)];
+        uint64_t word = slab_row(p.dir, c, y, p.L / 128)[k >> 6];
         p.out[idx] = (int8_t)(2 * (int)((word >> (k & 63)) & 1u) - 1);
         return;
     }
     if (p.model == ISING_MODEL_BLUME_CAPEL_2BIT) {           // 2 bits per spin, 32 sites per word
-        uint64_t word = p.lat[c][y * (p.L / 64) + (k >> 5)];
+        uint64_t word = slab_row(p.dir, c, y, p.L / 64)[k >> 5];
         p.out[idx] = (int8_t)((int)((word >> (2 * (k & 31))) & 3u) - 1);
         return;
     }
-    uint64_t word = p.lat[c][y * (p.L / 32) + (k >> 4)];
+    uint64_t word = slab_row(p.dir, c, y, p.L / 32)[k >> 4];
     int nib = (int)((word >> (4 * (k & 15))) & 15u);
     p.out[idx] = (int8_t)(p.model == ISING_MODEL_ISING ? 2 * nib - 1 : nib - 1);
 }
@@ -36,7 +48,7 @@ __global__ void __launch_bounds__(256) unpack_kernel(const __grid_constant__ Unp
 cudaError_t launch_unpack(ising_sim *h, int64_t x0, int64_t y0, int64_t w, int64_t hgt, int8_t *dev_out)
 {
     UnpackParams p;
-    p.lat[0] = h->lat[0]; p.lat[1] = h->lat[1];
+    p.dir = slab_directory(h);
     p.L = h->L; p.x0 = x0; p.y0 = y0; p.w = w; p.hgt = hgt; p.model = h->model; p.out = dev_out;
     int64_t n = w * hgt;
     unpack_kernel<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(p);
@@ -46,7 +58,7 @@ cudaError_t launch_unpack(ising_sim *h, int64_t x0, int64_t y0, int64_t w, int64
 
 // ------------------------------------------------------------------ pack ---
 struct PackParams {
-    uint32_t *lat[2];
+    SlabDir dir;
     int64_t L, y0, ny;
     int model, dry;
     const int8_t *in;
@@ -76,7 +88,7 @@ __global__ void __launch_bounds__(256) pack_kernel(const __grid_constant__ PackP
         w |= nib << (bits * j);
     }
     if (bad) atomicOr(p.bad, 1);
-    if (!p.dry) p.lat[c][y * halves_per_row + hf] = w;
+    if (!p.dry) reinterpret_cast<uint32_t *>(slab_row(p.dir, c, y, halves_per_row / 2))[hf] = w;
 }
 
 // 1-bit layout (ISING_MODEL_ISING_LUT): one thread per 32-bit half (32 same-colour sites)
@@ -98,7 +110,7 @@ __global__ void __launch_bounds__(256) pack_lut_kernel(const __grid_constant__ P
         w |= (v > 0 ? 1u : 0u) << j;
     }
     if (bad) atomicOr(p.bad, 1);
-    if (!p.dry) p.lat[c][y * halves_per_row + hf] = w;
+    if (!p.dry) reinterpret_cast<uint32_t *>(slab_row(p.dir, c, y, halves_per_row / 2))[hf] = w;
 }
 
 // write = 0: validate only (cudaErrorInvalidValue if a value is outside the model's set;
@@ -106,8 +118,7 @@ __global__ void __launch_bounds__(256) pack_lut_kernel(const __grid_constant__ P
 cudaError_t launch_pack(ising_sim *h, int64_t y0, int64_t ny, const int8_t *dev_in, int *dev_bad, int write)
 {
     PackParams p;
-    p.lat[0] = reinterpret_cast<uint32_t *>(h->lat[0]);
-    p.lat[1] = reinterpret_cast<uint32_t *>(h->lat[1]);
+    p.dir = slab_directory(h);
     p.L = h->L; p.y0 = y0; p.ny = ny; p.model = h->model; p.dry = !write; p.in = dev_in; p.bad = dev_bad;
     const bool lut = h->model == ISING_MODEL_ISING_LUT;
     int64_t n = ny * (h->L / sites_per_word(h->model)) * 2;      // 32-bit halves of both colours
@@ -157,7 +168,7 @@ __device__ __forceinline__ uint64_t spread_even(uint32_t v)   // bit i -> bit 2 
 }
 
 struct PlaneParams {
-    const uint64_t *lat[2];
+    SlabDir dir;
     int64_t L;
     int model;
     uint64_t *sg, *nz;
@@ -172,7 +183,7 @@ __global__ void __launch_bounds__(256) planes_kernel(const __grid_constant__ Pla
     uint64_t sg = 0, nz = 0;
     if (p.model == ISING_MODEL_ISING_LUT) {                  // 1-bit layout: 32 sites of each colour per plane word
         for (int c = 0; c < 2; ++c) {
-            const uint32_t *row32 = reinterpret_cast<const uint32_t *>(p.lat[c]) + y * Wq;
+            const uint32_t *row32 = reinterpret_cast<const uint32_t *>(slab_row(p.dir, c, y, Wq / 2));
             sg |= spread_even(row32[q]) << (int)((y + c) & 1);
         }
         p.sg[idx] = sg;
@@ -180,7 +191,7 @@ __global__ void __launch_bounds__(256) planes_kernel(const __grid_constant__ Pla
     }
     if (p.model == ISING_MODEL_BLUME_CAPEL_2BIT) {           // 2-bit layout: one word = 32 sites of a colour, pair j at bit 2 j
         for (int c = 0; c < 2; ++c) {
-            const uint64_t w = p.lat[c][y * Wq + q];
+            const uint64_t w = slab_row(p.dir, c, y, Wq)[q];
             sg |= ((w >> 1) & 0x5555555555555555ull) << (int)((y + c) & 1);       // code 2 = +1: high bit of the pair
             nz |= (~w & 0x5555555555555555ull) << (int)((y + c) & 1);             // code != 1: low bit clear
         }
@@ -189,7 +200,7 @@ __global__ void __launch_bounds__(256) planes_kernel(const __grid_constant__ Pla
     }
     for (int c = 0; c < 2; ++c) {
         int par = (int)((y + c) & 1);
-        const uint64_t *row = p.lat[c] + y * (p.L / 32);
+        const uint64_t *row = slab_row(p.dir, c, y, p.L / 32);
         uint64_t w0 = row[2 * q], w1 = row[2 * q + 1];
         if (p.model == ISING_MODEL_ISING) {
             sg |= (nibble_bit_to_even(w0, 0) | (nibble_bit_to_even(w1, 0) << 32)) << par;
@@ -260,7 +271,7 @@ cudaError_t launch_planes(ising_sim *h)
     const int64_t L = h->L, Wq = L / 64, plane_words = L * Wq;
     const int np = is_blume_capel(h->model) ? 2 : 1;
     PlaneParams p;
-    p.lat[0] = h->lat[0]; p.lat[1] = h->lat[1];
+    p.dir = slab_directory(h);
     p.L = L; p.model = h->model;
     p.sg = h->planes; p.nz = h->planes + plane_words;
     planes_kernel<<<(unsigned)((plane_words + 255) / 256), 256, 0, h->stream>>>(p);

@@ -12,9 +12,11 @@
 #include "ising_internal.cuh"
 
 struct LutParams {
-    const uint4 *opp;
+    const uint4 *opp;            // rows of this slab (NEXT-4; the whole lattice when unsharded)
     uint4 *own;
-    int L, cols, R;              // cols = uint4 per colour row = L / 256
+    const char *opp_up, *opp_dn; // the opposite-colour row above / below the slab (neighbouring slabs; see update.cu)
+    int y_base;                  // global row of the slab's first row (even)
+    int L, cols, R;              // L = rows of this slab; cols = uint4 per colour row = (lattice size) / 256
     uint32_t colour, t;
     const uint32_t *tree;        // 16 carry constants in heap order (device): tree[n] = 2^32 - threshold(node n)
     const uint2 *buckets;        // 4096 entries indexed by the top 12 bits of the number (device), see lut_bits32
@@ -212,17 +214,16 @@ __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const _
     const char *eo = oppb + row0 + rs + e_odd;
     char *w0 = ownb + row0 + cb;
 
-    const int ym = (y0 == 0) ? L - 1 : y0 - 1;
-    uint4 up = *reinterpret_cast<const uint4 *>(oppb + (size_t)ym * rs + cb);
+    uint4 up = *reinterpret_cast<const uint4 *>((y0 == 0) ? p.opp_up + cb : oppb + row0 - rs + cb);
     uint4 sm = *reinterpret_cast<const uint4 *>(oppb + row0 + cb);
     uint4 src = *reinterpret_cast<const uint4 *>(w0);
     uint32_t edge = *reinterpret_cast<const uint32_t *>(ee);
-    // g = 8 * (64-site word index): word = y * (2 cols) + 2 col
+    // g = 8 * (64-site word index): word = y * (2 cols) + 2 col, y the global row
     const uint64_t gs = (uint64_t)cols * 16;
-    uint64_t g0 = (uint64_t)y0 * gs + (uint64_t)col * 16;
+    uint64_t g0 = (uint64_t)(p.y_base + y0) * gs + (uint64_t)col * 16;
 
     for (int y = y0; y < yend; y += 2) {
-        const char *o2 = (y + 2 == L) ? oppb + cb : o1 + rs;
+        const char *o2 = (y + 2 == L) ? p.opp_dn + cb : o1 + rs;
         uint4 dn = *reinterpret_cast<const uint4 *>(o1);
         uint4 nsrc = *reinterpret_cast<const uint4 *>(w0 + rs);
         uint32_t nedge = *reinterpret_cast<const uint32_t *>(eo);
@@ -252,25 +253,29 @@ __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const _
     }
 }
 
-cudaError_t launch_lut_update(ising_sim *h, int colour, uint32_t t)
+cudaError_t launch_lut_update(ising_sim *h, int slab, int colour, uint32_t t)
 {
     LutParams p;
-    const int64_t L = h->L;
-    p.opp = reinterpret_cast<const uint4 *>(h->lat[1 - colour]);
-    p.own = reinterpret_cast<uint4 *>(h->lat[colour]);
-    p.L = (int)L; p.cols = (int)(L / 256); p.R = h->rows_per_thread;
+    const Slab &sl = h->slabs[slab];
+    const int64_t L = sl.rows;
+    p.opp = reinterpret_cast<const uint4 *>(sl.lat[1 - colour]);
+    p.own = reinterpret_cast<uint4 *>(sl.lat[colour]);
+    p.opp_up = reinterpret_cast<const char *>(halo_up(h, slab, 1 - colour));
+    p.opp_dn = reinterpret_cast<const char *>(halo_down(h, slab, 1 - colour));
+    p.y_base = (int)sl.y0;
+    p.L = (int)L; p.cols = (int)(h->L / 256); p.R = h->rows_per_thread;
     p.colour = (uint32_t)colour; p.t = t;
-    p.tree = h->d_bc_table;
+    p.tree = sl.d_table;
     p.rk = h->rk;
     int64_t chunks = (L + p.R - 1) / p.R;
     int64_t threads = chunks * p.cols;
     int block = h->block_threads;
     unsigned grid = (unsigned)((threads + block - 1) / block);
-    p.buckets = reinterpret_cast<const uint2 *>(h->lut_buckets);
+    p.buckets = reinterpret_cast<const uint2 *>(sl.lut_buckets);
     const size_t smem = 8 << LUT_BUCKET_BITS;
-    p.tally = h->d_acc + 40;
-    p.t_base = reinterpret_cast<const uint32_t *>(h->d_acc + 48) + (h->graph_capture ? 1 : 0);
-#define LUT_LAUNCH(C, V, T, SM) lut_update_kernel<C, V, T><<<grid, block, SM, h->stream>>>(p)
+    p.tally = sl.d_acc + 40;
+    p.t_base = reinterpret_cast<const uint32_t *>(sl.d_acc + 48) + (h->graph_capture ? 1 : 0);
+#define LUT_LAUNCH(C, V, T, SM) lut_update_kernel<C, V, T><<<grid, block, SM, sl.stream>>>(p)
     // variant 0 = automatic: the bucket table pays once its 32 KB fill per block is amortised over several
     // waves (L >= 8192); a single-wave launch starts faster with the table-free binary search.
     // 1 = binary search, 2 = bucket table
@@ -294,20 +299,22 @@ cudaError_t launch_lut_update(ising_sim *h, int colour, uint32_t t)
 }
 
 // L5: word w of colour c = (x | y << 32) of Philox(ctr = (w_lo, w_hi, 0, 2 + c))
-__global__ void __launch_bounds__(256) lut_init_kernel(uint64_t *lat0, uint64_t *lat1, int64_t words, RoundKeys rk)
+__global__ void __launch_bounds__(256) lut_init_kernel(uint64_t *lat0, uint64_t *lat1, int64_t words, int64_t word0, RoundKeys rk)
 {
-    const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (w >= words) return;
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= words) return;
+    const uint64_t w = (uint64_t)(word0 + i);                     // global word index of the slab's word i
     for (int c = 0; c < 2; ++c) {
-        const uint4 r = philox4x32_10(make_uint4((uint32_t)w, (uint32_t)((uint64_t)w >> 32), 0u, 2u + c), rk);
-        (c ? lat1 : lat0)[w] = (uint64_t)r.x | ((uint64_t)r.y << 32);
+        const uint4 r = philox4x32_10(make_uint4((uint32_t)w, (uint32_t)(w >> 32), 0u, 2u + c), rk);
+        (c ? lat1 : lat0)[i] = (uint64_t)r.x | ((uint64_t)r.y << 32);
     }
 }
 
-cudaError_t launch_lut_init(ising_sim *h)
+cudaError_t launch_lut_init(ising_sim *h, int slab)
 {
-    const int64_t words = h->L * (h->L / 128);
-    lut_init_kernel<<<(unsigned)((words + 255) / 256), 256, 0, h->stream>>>(h->lat[0], h->lat[1], words, h->rk);
+    const Slab &sl = h->slabs[slab];
+    const int64_t words = sl.rows * (h->L / 128), word0 = sl.y0 * (h->L / 128);
+    lut_init_kernel<<<(unsigned)((words + 255) / 256), 256, 0, sl.stream>>>(sl.lat[0], sl.lat[1], words, word0, h->rk);
     h->launches++;
     return cudaGetLastError();
 }
@@ -320,8 +327,9 @@ cudaError_t launch_lut_init(ising_sim *h)
 // MODE 1 (run for both colours): histogram of s*h = 4 - 2 d, bit-sliced count of the four
 // difference words.  One global atomic per block and quantity (block_accumulate).
 struct LutObsParams {
-    const uint4 *ctr, *nbr;
-    int centre, L, cols, R;
+    const uint4 *ctr, *nbr;       // rows of this slab
+    const char *nbr_up, *nbr_dn;  // the neighbour-colour row above / below the slab
+    int centre, L, cols, R;       // L = rows of this slab
     long long *acc;
 };
 
@@ -341,12 +349,10 @@ __global__ void __launch_bounds__(256) lut_observe_kernel(const __grid_constant_
         const int halves = cols * 4;
         const size_t e0 = (size_t)((col == 0) ? halves - 1 : 4 * col - 1) * 4;   // parity 0: top bit of the previous word
         const size_t e1 = (size_t)((col == cols - 1) ? 0 : 4 * col + 4) * 4;     // parity 1: low bit of the next word
-        const int ym = (y0 == 0) ? L - 1 : y0 - 1;
-        uint4 up = *reinterpret_cast<const uint4 *>(nbr + (size_t)ym * rs + cb);
+        uint4 up = *reinterpret_cast<const uint4 *>((y0 == 0) ? p.nbr_up + cb : nbr + (size_t)(y0 - 1) * rs + cb);
         uint4 sm = *reinterpret_cast<const uint4 *>(nbr + (size_t)y0 * rs + cb);
         for (int y = y0; y < yend; ++y) {
-            const int yp = (y + 1 == L) ? 0 : y + 1;
-            const uint4 dn = *reinterpret_cast<const uint4 *>(nbr + (size_t)yp * rs + cb);
+            const uint4 dn = *reinterpret_cast<const uint4 *>((y + 1 == L) ? p.nbr_dn + cb : nbr + (size_t)(y + 1) * rs + cb);
             const uint4 x4 = *reinterpret_cast<const uint4 *>(ctr + (size_t)y * rs + cb);
             uint32_t sd[4];
             if (((y + p.centre) & 1) == 0) lut_side<0>(sm, *reinterpret_cast<const uint32_t *>(nbr + (size_t)y * rs + e0), sd);
@@ -380,35 +386,38 @@ __global__ void __launch_bounds__(256) lut_observe_kernel(const __grid_constant_
 }
 
 template <int MODE>
-static cudaError_t launch_lut_obs(ising_sim *h, int centre)
+static cudaError_t launch_lut_obs(ising_sim *h, int slab, int centre)
 {
     LutObsParams p;
-    p.ctr = reinterpret_cast<const uint4 *>(h->lat[centre]);
-    p.nbr = reinterpret_cast<const uint4 *>(h->lat[1 - centre]);
+    const Slab &sl = h->slabs[slab];
+    p.ctr = reinterpret_cast<const uint4 *>(sl.lat[centre]);
+    p.nbr = reinterpret_cast<const uint4 *>(sl.lat[1 - centre]);
+    p.nbr_up = reinterpret_cast<const char *>(halo_up(h, slab, 1 - centre));
+    p.nbr_dn = reinterpret_cast<const char *>(halo_down(h, slab, 1 - centre));
     p.centre = centre;
-    p.L = (int)h->L; p.cols = (int)(h->L / 256);
+    p.L = (int)sl.rows; p.cols = (int)(h->L / 256);
     p.R = 64;                 // rows per thread: as long as the grid keeps two full waves of threads
-    while (p.R > 4 && (h->L / p.R) * p.cols < 148 * 2048 * 2) p.R >>= 1;
-    p.acc = h->d_acc;
-    const int64_t threads = ((h->L + p.R - 1) / p.R) * p.cols;
+    while (p.R > 4 && (sl.rows / p.R) * p.cols < 148 * 2048 * 2) p.R >>= 1;
+    p.acc = sl.d_acc;
+    const int64_t threads = ((sl.rows + p.R - 1) / p.R) * p.cols;
     const int block = 128;
-    lut_observe_kernel<MODE><<<(unsigned)((threads + block - 1) / block), block, 0, h->stream>>>(p);
+    lut_observe_kernel<MODE><<<(unsigned)((threads + block - 1) / block), block, 0, sl.stream>>>(p);
     h->launches++;
     return cudaGetLastError();
 }
 
-cudaError_t launch_lut_observables(ising_sim *h)
+cudaError_t launch_lut_observables(ising_sim *h, int slab)
 {
-    cudaError_t e = cudaMemsetAsync(h->d_acc, 0, 8 * sizeof(long long), h->stream);
+    cudaError_t e = cudaMemsetAsync(h->slabs[slab].d_acc, 0, 8 * sizeof(long long), h->slabs[slab].stream);
     if (e != cudaSuccess) return e;
-    return launch_lut_obs<0>(h, 0);
+    return launch_lut_obs<0>(h, slab, 0);
 }
 
-cudaError_t launch_lut_sd_hist(ising_sim *h)
+cudaError_t launch_lut_sd_hist(ising_sim *h, int slab)
 {
-    cudaError_t e = cudaMemsetAsync(h->d_acc + 8, 0, 9 * sizeof(long long), h->stream);
+    cudaError_t e = cudaMemsetAsync(h->slabs[slab].d_acc + 8, 0, 9 * sizeof(long long), h->slabs[slab].stream);
     if (e != cudaSuccess) return e;
-    e = launch_lut_obs<1>(h, 0);
+    e = launch_lut_obs<1>(h, slab, 0);
     if (e != cudaSuccess) return e;
-    return launch_lut_obs<1>(h, 1);
+    return launch_lut_obs<1>(h, slab, 1);
 }

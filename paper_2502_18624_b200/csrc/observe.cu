@@ -9,9 +9,10 @@
 #define ONES 0x11111111u
 
 struct ObsParams {
-    const uint4 *ctr, *nbr;   // centre-colour array, neighbour-colour array
+    const uint4 *ctr, *nbr;   // centre-colour array, neighbour-colour array: the rows of this slab
+    const char *nbr_up, *nbr_dn;   // neighbour-colour row above / below the slab (NEXT-4; own last / first row when unsharded)
     int centre;               // colour of the centre sites
-    int L, cols, R;
+    int L, cols, R;           // L = rows of this slab
     long long *acc;
 };
 
@@ -79,12 +80,10 @@ __global__ void __launch_bounds__(256) observe_kernel(const __grid_constant__ Ob
         const size_t rs = (size_t)cols * VB, cb = (size_t)col * VB;
         const size_t e0 = (size_t)edge_half<MODEL, 0>(col, cols) * 4;   // parity 0: neighbour k-1
         const size_t e1 = (size_t)edge_half<MODEL, 1>(col, cols) * 4;   // parity 1: neighbour k+1
-        int ym = (y0 == 0) ? L - 1 : y0 - 1;
-        uint4 up = load_row<MODEL>(nbr + (size_t)ym * rs + cb);
+        uint4 up = load_row<MODEL>((y0 == 0) ? p.nbr_up + cb : nbr + (size_t)(y0 - 1) * rs + cb);
         uint4 sm = load_row<MODEL>(nbr + (size_t)y0 * rs + cb);
         for (int y = y0; y < yend; ++y) {
-            int yp = (y + 1 == L) ? 0 : y + 1;
-            uint4 dn = load_row<MODEL>(nbr + (size_t)yp * rs + cb);
+            uint4 dn = load_row<MODEL>((y + 1 == L) ? p.nbr_dn + cb : nbr + (size_t)(y + 1) * rs + cb);
             uint4 x = load_row<MODEL>(ctr + (size_t)y * rs + cb);
             uint32_t sd[4];
             if (((y + p.centre) & 1) == 0) side_words<MODEL, 0>(sm, *reinterpret_cast<const uint32_t *>(nbr + (size_t)y * rs + e0), sd);
@@ -105,41 +104,44 @@ __global__ void __launch_bounds__(256) observe_kernel(const __grid_constant__ Ob
 }
 
 template <int MODE>
-static cudaError_t launch_obs(ising_sim *h, int centre)
+static cudaError_t launch_obs(ising_sim *h, int slab, int centre)
 {
     ObsParams p;
-    p.ctr = reinterpret_cast<const uint4 *>(h->lat[centre]);
-    p.nbr = reinterpret_cast<const uint4 *>(h->lat[1 - centre]);
+    const Slab &sl = h->slabs[slab];
+    p.ctr = reinterpret_cast<const uint4 *>(sl.lat[centre]);
+    p.nbr = reinterpret_cast<const uint4 *>(sl.lat[1 - centre]);
+    p.nbr_up = reinterpret_cast<const char *>(halo_up(h, slab, 1 - centre));
+    p.nbr_dn = reinterpret_cast<const char *>(halo_down(h, slab, 1 - centre));
     p.centre = centre;
-    p.L = (int)h->L; p.cols = (int)(h->L / 64);
+    p.L = (int)sl.rows; p.cols = (int)(h->L / 64);
     p.R = (h->L >= 65536) ? 64 : (h->L >= 2048) ? 32 : 4;   // rows per thread: halo re-reads 2/R, still >= 1 M threads at R = 64
-    p.acc = h->d_acc;
-    int64_t chunks = (h->L + p.R - 1) / p.R;
+    p.acc = sl.d_acc;
+    int64_t chunks = (sl.rows + p.R - 1) / p.R;
     int64_t threads = chunks * p.cols;
     int block = 128;
     unsigned grid = (unsigned)((threads + block - 1) / block);
-    if (h->model == ISING_MODEL_ISING) observe_kernel<ISING_MODEL_ISING, MODE><<<grid, block, 0, h->stream>>>(p);
-    else if (h->model == ISING_MODEL_BLUME_CAPEL) observe_kernel<ISING_MODEL_BLUME_CAPEL, MODE><<<grid, block, 0, h->stream>>>(p);
-    else observe_kernel<ISING_MODEL_BLUME_CAPEL_2BIT, MODE><<<grid, block, 0, h->stream>>>(p);
+    if (h->model == ISING_MODEL_ISING) observe_kernel<ISING_MODEL_ISING, MODE><<<grid, block, 0, sl.stream>>>(p);
+    else if (h->model == ISING_MODEL_BLUME_CAPEL) observe_kernel<ISING_MODEL_BLUME_CAPEL, MODE><<<grid, block, 0, sl.stream>>>(p);
+    else observe_kernel<ISING_MODEL_BLUME_CAPEL_2BIT, MODE><<<grid, block, 0, sl.stream>>>(p);
     h->launches++;
     return cudaGetLastError();
 }
 
 // B, M, Q: centre = black sees every bond once; M and Q also count the white words of
 // the centre row (`sm`), so one pass covers both arrays.
-cudaError_t launch_observables(ising_sim *h)
+cudaError_t launch_observables(ising_sim *h, int slab)
 {
-    cudaError_t e = cudaMemsetAsync(h->d_acc, 0, 8 * sizeof(long long), h->stream);
+    cudaError_t e = cudaMemsetAsync(h->slabs[slab].d_acc, 0, 8 * sizeof(long long), h->slabs[slab].stream);
     if (e != cudaSuccess) return e;
-    return launch_obs<0>(h, 0);
+    return launch_obs<0>(h, slab, 0);
 }
 
 // Schwinger-Dyson histogram over ALL sites: one pass centred on each colour.
-cudaError_t launch_sd_hist(ising_sim *h)
+cudaError_t launch_sd_hist(ising_sim *h, int slab)
 {
-    cudaError_t e = cudaMemsetAsync(h->d_acc + 8, 0, 9 * sizeof(long long), h->stream);
+    cudaError_t e = cudaMemsetAsync(h->slabs[slab].d_acc + 8, 0, 9 * sizeof(long long), h->slabs[slab].stream);
     if (e != cudaSuccess) return e;
-    e = launch_obs<1>(h, 0);
+    e = launch_obs<1>(h, slab, 0);
     if (e != cudaSuccess) return e;
-    return launch_obs<1>(h, 1);
+    return launch_obs<1>(h, slab, 1);
 }

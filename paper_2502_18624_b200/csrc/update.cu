@@ -15,9 +15,12 @@
 #define ONES 0x11111111u
 
 struct UpdParams {
-    const uint4 *opp;   // opposite colour (read only during this phase)
-    uint4 *own;         // colour being updated
-    int L;              // rows
+    const uint4 *opp;   // opposite colour, rows of this slab (read only during this phase)
+    uint4 *own;         // colour being updated, rows of this slab
+    const char *opp_up; // opposite colour, the row above the slab's first row (last row of the slab above: NEXT-4,
+    const char *opp_dn; // PAPER.md:69) and the row below its last row; the slab's own last / first row when unsharded
+    int y_base;         // global row of the slab's first row (even): keys the random numbers, not the addresses
+    int L;              // rows of this slab (even)
     int cols;           // uint4 per colour row = L / 64
     int R;              // rows per thread (even)
     uint32_t colour, t;
@@ -374,17 +377,16 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
     const char *eo = oppb + row0 + rs + e_odd;     // carry half, odd offsets:  row y + 1
     char *w0 = ownb + row0 + cb;                   // own colour, row y
 
-    const int ym = (y0 == 0) ? L - 1 : y0 - 1;
-    uint4 up = load_row<MODEL>(oppb + (size_t)ym * rs + cb);
+    uint4 up = load_row<MODEL>((y0 == 0) ? p.opp_up + cb : oppb + row0 - rs + cb);
     uint4 sm = load_row<MODEL>(oppb + row0 + cb);
     uint4 src = load_row<MODEL>(w0);
     uint32_t edge = *reinterpret_cast<const uint32_t *>(ee);
-    uint64_t g0 = (uint64_t)y0 * (uint64_t)(cols * 8) + (uint64_t)(col * 8);
+    uint64_t g0 = (uint64_t)(p.y_base + y0) * (uint64_t)(cols * 8) + (uint64_t)(col * 8);
     const uint64_t gs = (uint64_t)(cols * 8);
 
     for (int y = y0; y < yend; y += 2) {
         // ---- even offset: parity C
-        const char *o2 = (y + 2 == L) ? oppb + cb : o1 + rs;           // row y + 2, wraps to row 0
+        const char *o2 = (y + 2 == L) ? p.opp_dn + cb : o1 + rs;       // row y + 2; below the slab: the halo row
         uint4 dn = load_row<MODEL>(o1);
         uint4 nsrc = load_row<MODEL>(w0 + rs);
         uint32_t nedge = *reinterpret_cast<const uint32_t *>(eo);
@@ -422,13 +424,17 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
     }
 }
 
-cudaError_t launch_update(ising_sim *h, int colour, uint32_t t)
+cudaError_t launch_update(ising_sim *h, int slab, int colour, uint32_t t)
 {
     UpdParams p;
-    const int64_t L = h->L;
-    p.opp = reinterpret_cast<const uint4 *>(h->lat[1 - colour]);
-    p.own = reinterpret_cast<uint4 *>(h->lat[colour]);
-    p.L = (int)L; p.cols = (int)(L / 64); p.R = h->rows_per_thread;
+    const Slab &sl = h->slabs[slab];
+    const int64_t L = sl.rows;                                  // rows this launch walks
+    p.opp = reinterpret_cast<const uint4 *>(sl.lat[1 - colour]);
+    p.own = reinterpret_cast<uint4 *>(sl.lat[colour]);
+    p.opp_up = reinterpret_cast<const char *>(halo_up(h, slab, 1 - colour));
+    p.opp_dn = reinterpret_cast<const char *>(halo_down(h, slab, 1 - colour));
+    p.y_base = (int)sl.y0;
+    p.L = (int)L; p.cols = (int)(h->L / 64); p.R = h->rows_per_thread;
     p.colour = (uint32_t)colour; p.t = t;
     const uint64_t T4 = h->T[3], T8 = h->T[4];
     p.T4 = (uint32_t)T4; p.T8 = (uint32_t)T8;
@@ -437,19 +443,19 @@ cudaError_t launch_update(ising_sim *h, int colour, uint32_t t)
     p.C4 = (T4 == 0 || (T4 >> 32)) ? 0u : (uint32_t)((1ull << 32) - T4);
     p.C8 = (T8 == 0 || (T8 >> 32)) ? 0u : (uint32_t)((1ull << 32) - T8);
     p.Kc = ONES * (8u - (T4 == 0 ? 1u : 0u) - (T8 == 0 ? 1u : 0u));
-    p.bc_table = h->d_bc_table;
+    p.bc_table = sl.d_table;
     p.rk = h->rk;
     int64_t chunks = (L + p.R - 1) / p.R;
     int64_t threads = chunks * p.cols;
     int block = h->block_threads;
     unsigned grid = (unsigned)((threads + block - 1) / block);
-    p.tally = h->d_acc + 40;
-    p.t_base = reinterpret_cast<const uint32_t *>(h->d_acc + 48) + (h->graph_capture ? 1 : 0);   // [0] stays 0, [1] = base of a graph replay
+    p.tally = sl.d_acc + 40;
+    p.t_base = reinterpret_cast<const uint32_t *>(sl.d_acc + 48) + (h->graph_capture ? 1 : 0);   // [0] stays 0, [1] = base of a graph replay
     bool never = false;                           // Blume-Capel: a threshold that is exactly 0 -> compare/select form
     if (is_blume_capel(h->model))
         for (int i = 0; i < h->n_T; ++i) never = never || h->T[i] == 0;
     const int v = (h->variant == 0 && !never) ? 0 : 1;
-#define LAUNCH_UPD(MODEL, C, V, T) update_kernel<MODEL, C, V, T><<<grid, block, 0, h->stream>>>(p)
+#define LAUNCH_UPD(MODEL, C, V, T) update_kernel<MODEL, C, V, T><<<grid, block, 0, sl.stream>>>(p)
 #define PICK_T(MODEL, C, V) do { if (h->tally_on) LAUNCH_UPD(MODEL, C, V, 1); else LAUNCH_UPD(MODEL, C, V, 0); } while (0)
 #define PICK_V(MODEL, C) do { if (v == 0) PICK_T(MODEL, C, 0); else PICK_T(MODEL, C, 1); } while (0)
     if (h->model == ISING_MODEL_ISING) { if (colour == 0) PICK_V(ISING_MODEL_ISING, 0); else PICK_V(ISING_MODEL_ISING, 1); }
@@ -467,7 +473,8 @@ cudaError_t launch_update(ising_sim *h, int colour, uint32_t t)
 // Blume-Capel: code = (3 r) >> 32.  One thread per 32-bit half (8 sites, 2 calls; 16 and 4 at 2 bits).
 struct InitParams {
     uint32_t *lat[2];
-    int64_t halves_per_colour;
+    int64_t halves_per_colour;   // of this slab
+    int64_t half0;               // global index of the slab's first half (keys the random numbers)
     int model;
     RoundKeys rk;
 };
@@ -484,7 +491,7 @@ __global__ void __launch_bounds__(256) init_kernel(const __grid_constant__ InitP
     // 8 sites per half = 2 groups of 4 (4 bits per site); 16 sites = 4 groups in the 2-bit layout
     const int calls = p.model == ISING_MODEL_BLUME_CAPEL_2BIT ? 4 : 2, bits = p.model == ISING_MODEL_BLUME_CAPEL_2BIT ? 2 : 4;
     for (int c = 0; c < 2; ++c) {
-        uint64_t g = (uint64_t)i * calls;
+        uint64_t g = (uint64_t)(p.half0 + i) * calls;
         uint32_t w = 0;
         for (int q = 0; q < calls; ++q) {
             uint4 r = philox4x32_10(make_uint4((uint32_t)(g + q), (uint32_t)((g + q) >> 32), 0u, 2u + c), p.rk);
@@ -497,17 +504,19 @@ __global__ void __launch_bounds__(256) init_kernel(const __grid_constant__ InitP
     }
 }
 
-cudaError_t launch_init(ising_sim *h)
+cudaError_t launch_init(ising_sim *h, int slab)
 {
     InitParams p;
-    p.lat[0] = reinterpret_cast<uint32_t *>(h->lat[0]);
-    p.lat[1] = reinterpret_cast<uint32_t *>(h->lat[1]);
-    p.halves_per_colour = colour_words(h) * 2;
+    const Slab &sl = h->slabs[slab];
+    p.lat[0] = reinterpret_cast<uint32_t *>(sl.lat[0]);
+    p.lat[1] = reinterpret_cast<uint32_t *>(sl.lat[1]);
+    p.halves_per_colour = sl.rows * colour_row_words(h) * 2;
+    p.half0 = sl.y0 * colour_row_words(h) * 2;
     p.model = h->model;
     p.rk = h->rk;
     int block = 256;
     unsigned grid = (unsigned)((p.halves_per_colour + block - 1) / block);
-    init_kernel<<<grid, block, 0, h->stream>>>(p);
+    init_kernel<<<grid, block, 0, sl.stream>>>(p);
     h->launches++;
     return cudaGetLastError();
 }
