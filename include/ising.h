@@ -179,6 +179,18 @@ int ising_write_lattice(ising_t *h, int64_t y0, int64_t ny, const int8_t *host_i
  * c (row-major L x L/32).  For checkpoints and the end-to-end benchmark.    */
 int ising_read_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, uint64_t *host_out);
 int ising_write_packed(ising_t *h, int colour, int64_t word0, int64_t nwords, const uint64_t *host_in);
+/* Compact transport format: the rows [row0, row0 + nrows) of colour array `colour` at the information content
+ * of a spin instead of its storage size -- Ising: 1 bit per spin, bit j of word m of a row = compact site
+ * k = 64 m + j, 1 = spin +1, L/128 words per colour row (the layout of ISING_MODEL_ISING_LUT);
+ * Blume-Capel: 2 bits per spin, site j of a word at bits 2j..2j+1, code = spin + 1, L/64 words per colour row
+ * (the layout of ISING_MODEL_BLUME_CAPEL_2BIT; a code equal to 3 gives ISING_EINVAL and leaves the lattice
+ * unchanged).  The 4-bit models expand / gather on the device, so a whole-lattice upload moves L*L/8 bytes
+ * for Ising (L*L/4 for Blume-Capel) instead of L*L/2; for the 1-bit and 2-bit models the format is the
+ * packed layout itself.  Host arrays of nrows * (words per colour row) uint64, row-major; the Ising format
+ * needs L to be a multiple of 128 (whole words per colour row).  Synchronises.                              */
+int ising_write_bits(ising_t *h, int colour, int64_t row0, int64_t nrows, const uint64_t *host_in);
+int ising_read_bits(ising_t *h, int colour, int64_t row0, int64_t nrows, uint64_t *host_out);
+
 /* Schedule interleave (A11 of SURVEY.md Sec. 8(a)).  ising_time_grid: the paper's measurement
  * times t = floor(2^(x/8) + 0.5), x = 1, 2, ..., de-duplicated, t <= tmax, into the
  * host array out (capacity cap); *count = number of times (size query: out == NULL).  Host

@@ -21,6 +21,7 @@ EXPORTS = [
     "ising_launch_count", "ising_sync", "ising_destroy", "ising_last_error", "ising_bench_philox_only",
     "ising_bench_copy", "ising_debug_philox", "ising_protocol_distances", "ising_threshold_table",
     "ising_run_protocol_schedule", "ising_create_slabs", "ising_slab_count", "ising_slab_info",
+    "ising_write_bits", "ising_read_bits",
 ]
 
 
@@ -80,6 +81,8 @@ def load_library():
     lib.ising_write_lattice.argtypes = [vp, i64, i64, vp]
     lib.ising_read_packed.argtypes = [vp, C.c_int, i64, i64, vp]
     lib.ising_write_packed.argtypes = [vp, C.c_int, i64, i64, vp]
+    lib.ising_write_bits.argtypes = [vp, C.c_int, i64, i64, vp]
+    lib.ising_read_bits.argtypes = [vp, C.c_int, i64, i64, vp]
     lib.ising_set_sweeps_done.argtypes = [vp, u64]
     lib.ising_thresholds.argtypes = [vp, vp, C.c_int, C.POINTER(C.c_int)]
     lib.ising_set_launch.argtypes = [vp, C.c_int, C.c_int]
@@ -338,6 +341,29 @@ class IsingSim:
             words = np.ascontiguousarray(words, dtype=np.uint64)
             ptr, n = words.ctypes.data, len(words)
         _check(self._lib.ising_write_packed(self._h, colour, word0, n if nwords is None else nwords, ptr))
+
+    def bits_row_words(self) -> int:
+        """uint64 words per colour row of the compact transport format (ising_write_bits / ising_read_bits)."""
+        return self.L // 64 if self.model in (BLUME_CAPEL, BLUME_CAPEL_2BIT) else self.L // 128
+
+    def read_bits(self, colour: int, row0: int = 0, nrows: int | None = None, out=None):
+        nrows = self.L - row0 if nrows is None else nrows
+        if out is None:
+            out = np.empty(nrows * self.bits_row_words(), dtype=np.uint64)
+            ptr = out.ctypes.data
+        else:
+            ptr = out.data_ptr() if hasattr(out, "data_ptr") else out.ctypes.data
+        _check(self._lib.ising_read_bits(self._h, colour, row0, nrows, ptr))
+        return out
+
+    def write_bits(self, colour: int, words, row0: int = 0, nrows: int | None = None):
+        if hasattr(words, "data_ptr"):
+            ptr, n = words.data_ptr(), words.numel() * words.element_size() // 8
+        else:
+            words = np.ascontiguousarray(words, dtype=np.uint64)
+            ptr, n = words.ctypes.data, len(words)
+        nrows = n // self.bits_row_words() if nrows is None else nrows
+        _check(self._lib.ising_write_bits(self._h, colour, row0, nrows, ptr))
 
     def set_sweeps_done(self, t: int):
         _check(self._lib.ising_set_sweeps_done(self._h, t))

@@ -325,6 +325,8 @@ extern "C" int ising_destroy(ising_t *h)
     {
         DeviceGuard dev_guard(h);
         if (h->io_stage) cudaFree(h->io_stage);
+        if (h->io_stream) cudaStreamDestroy(h->io_stream);
+        if (h->io_event) cudaEventDestroy(h->io_event);
         if (h->planes) cudaFree(h->planes);
         if (h->comb) cudaFree(h->comb);
         if (h->gram) cudaFree(h->gram);
@@ -764,6 +766,92 @@ extern "C" int ising_write_packed(ising_t *h, int colour, int64_t word0, int64_t
     }
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     return h->tally_on ? tally_resync(h) : ISING_OK;
+}
+
+// Compact transport format: 1 bit per Ising spin, 2 bits per Blume-Capel spin, rows of one
+// colour array in the site order of the packed layout.  For the 1-bit and 2-bit models this IS the packed
+// layout (a plain copy); the 4-bit models expand / gather on the device, chunk by chunk through the staging
+// buffer, so that an upload moves the information content of the lattice and not its storage size.
+static int64_t bits_row_words(const ising_sim *h) { return is_blume_capel(h->model) ? h->L / 64 : h->L / 128; }
+
+static int bits_args(const ising_sim *h, const char *who, int colour, int64_t row0, int64_t nrows, const void *host)
+{
+    if (!h || !host) return set_error(ISING_EINVAL, std::string(who) + ": NULL argument");
+    if ((colour != 0 && colour != 1) || row0 < 0 || nrows < 0 || row0 + nrows > h->L)
+        return set_error(ISING_EINVAL, std::string(who) + ": colour or rows out of range");
+    if (!is_blume_capel(h->model) && (h->L % 128) != 0)
+        return set_error(ISING_EINVAL, std::string(who) + ": one bit per spin needs L to be a multiple of 128 (whole 64-bit words per colour row)");
+    return ISING_OK;
+}
+
+extern "C" int ising_write_bits(ising_t *h, int colour, int64_t row0, int64_t nrows, const uint64_t *host_in)
+{
+    DeviceGuard dev_guard(h);
+    int rc = bits_args(h, "ising_write_bits", colour, row0, nrows, host_in);
+    if (rc) return rc;
+    const int64_t rw = bits_row_words(h);
+    if (h->model == ISING_MODEL_ISING_LUT || h->model == ISING_MODEL_BLUME_CAPEL_2BIT) {
+        if (h->model == ISING_MODEL_BLUME_CAPEL_2BIT)                  // the code 3 does not exist
+            for (int64_t i = 0; i < nrows * rw; ++i)
+                if (host_in[i] & (host_in[i] >> 1) & 0x5555555555555555ull)
+                    return set_error(ISING_EINVAL, "ising_write_bits: a 2-bit code equal to 3");
+        return ising_write_packed(h, colour, row0 * rw, nrows * rw, host_in);
+    }
+    const bool bc = is_blume_capel(h->model);
+    const int64_t rows_per = std::max<int64_t>(1, std::min<int64_t>(nrows, kStageBytes / (rw * 8)));
+    rc = ensure_stage(h, (size_t)(rows_per * rw * 8));
+    if (rc) return rc;
+    int *d_bad = (int *)(h->d_acc + 32);
+    // The copies and the (small) expansion kernels run on a stream of the highest priority, ordered after what is
+    // queued on the handle's stream: when another handle's sweeps fill the GPU (bench.py's pipelined end-to-end
+    // run) an expansion kernel is then scheduled as soon as blocks retire, not after the running launch.
+    if (!h->io_stream) {
+        int lo = 0, hi = 0;
+        CUDA_TRY(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+        CUDA_TRY(cudaStreamCreateWithPriority(&h->io_stream, cudaStreamNonBlocking, hi));
+        CUDA_TRY(cudaEventCreateWithFlags(&h->io_event, cudaEventDisableTiming));
+    }
+    CUDA_TRY(cudaEventRecord(h->io_event, h->stream));
+    CUDA_TRY(cudaStreamWaitEvent(h->io_stream, h->io_event, 0));
+    cudaStream_t user = h->stream;
+    struct Swap {                                               // the launchers use h->stream
+        ising_sim *h; cudaStream_t user;
+        ~Swap() { h->stream = user; }
+    } swap{h, user};
+    h->stream = h->io_stream;
+    // Blume-Capel: a first pass validates every chunk, so that the lattice is untouched on bad input
+    for (int pass = bc ? 0 : 1; pass < 2; ++pass)
+        for (int64_t j = 0; j < nrows; j += rows_per) {
+            const int64_t nr = std::min(rows_per, nrows - j);
+            CUDA_TRY(cudaMemcpyAsync(h->io_stage, host_in + j * rw, (size_t)(nr * rw * 8), cudaMemcpyHostToDevice, h->stream));
+            cudaError_t e = launch_bits(h, colour, row0 + j, nr, (uint32_t *)h->io_stage, pass, d_bad);
+            if (e == cudaErrorInvalidValue) return set_error(ISING_EINVAL, "ising_write_bits: a 2-bit code equal to 3");
+            if (e != cudaSuccess) return cuda_fail(e, "bit expansion kernel");
+        }
+    CUDA_TRY(cudaStreamSynchronize(h->io_stream));              // the lattice is written: later work on the user's stream may follow
+    h->stream = user;
+    return h->tally_on ? tally_resync(h) : ISING_OK;
+}
+
+extern "C" int ising_read_bits(ising_t *h, int colour, int64_t row0, int64_t nrows, uint64_t *host_out)
+{
+    DeviceGuard dev_guard(h);
+    int rc = bits_args(h, "ising_read_bits", colour, row0, nrows, host_out);
+    if (rc) return rc;
+    const int64_t rw = bits_row_words(h);
+    if (h->model == ISING_MODEL_ISING_LUT || h->model == ISING_MODEL_BLUME_CAPEL_2BIT)
+        return ising_read_packed(h, colour, row0 * rw, nrows * rw, host_out);
+    const int64_t rows_per = std::max<int64_t>(1, std::min<int64_t>(nrows, kStageBytes / (rw * 8)));
+    rc = ensure_stage(h, (size_t)(rows_per * rw * 8));
+    if (rc) return rc;
+    for (int64_t j = 0; j < nrows; j += rows_per) {
+        const int64_t nr = std::min(rows_per, nrows - j);
+        cudaError_t e = launch_bits(h, colour, row0 + j, nr, (uint32_t *)h->io_stage, 2, nullptr);
+        if (e != cudaSuccess) return cuda_fail(e, "bit gather kernel");
+        CUDA_TRY(cudaMemcpyAsync(host_out + j * rw, h->io_stage, (size_t)(nr * rw * 8), cudaMemcpyDeviceToHost, h->stream));
+    }
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return ISING_OK;
 }
 
 // ----------------------------------------------------------- correlation ---

@@ -66,6 +66,8 @@ struct ising_sim {
     int64_t launches = 0;
     // lazily allocated (cudaMalloc, owned)
     void *io_stage = nullptr; size_t io_stage_bytes = 0;
+    cudaStream_t io_stream = nullptr;                         // highest-priority stream of ising_write_bits (its small expansion
+    cudaEvent_t io_event = nullptr;                           // kernels must not queue behind another handle's sweeps)
     uint64_t *planes = nullptr; size_t planes_bytes = 0;      // bit planes for the correlation
     uint64_t *comb = nullptr; size_t comb_bytes = 0;          // planes down-sampled to the source comb (stride >= 2)
     void *lut_buckets = nullptr;                              // LUT model: 4096 x {C, meta} bucket table (cudaMalloc)
@@ -145,6 +147,7 @@ cudaError_t launch_sd_hist(ising_sim *h, int slab);                 // -> slab d
 SlabDir slab_directory(const ising_sim *h);
 cudaError_t launch_unpack(ising_sim *h, int64_t x0, int64_t y0, int64_t w, int64_t hgt, int8_t *dev_out);
 cudaError_t launch_pack(ising_sim *h, int64_t y0, int64_t ny, const int8_t *dev_in, int *dev_bad, int write);
+cudaError_t launch_bits(ising_sim *h, int colour, int64_t row0, int64_t nrows, uint32_t *dev_buf, int mode, int *dev_bad);
 cudaError_t launch_planes(ising_sim *h);                            // lattice -> bit planes
 cudaError_t launch_corr(ising_sim *h, int64_t stride, int64_t count, const long long *dev_r,
                         long long *dev_sx, long long *dev_sy);

@@ -289,3 +289,110 @@ cudaError_t launch_planes(ising_sim *h)
     }
     return cudaSuccess;
 }
+
+// ------------------------------------------------------- compact transport ---
+// ising_write_bits / ising_read_bits: the lattice at the information content of a spin -- 1 bit per Ising
+// spin, 2 bits per Blume-Capel spin -- in the site order of the packed arrays (the layouts of the 1-bit and
+// 2-bit models), expanded to / gathered from the 4-bit nibbles on the device.  One thread per 128-bit
+// lattice vector (32 sites): 32 input bits (Ising) or 64 (Blume-Capel).
+__device__ __forceinline__ uint64_t bits16_to_nibbles(uint32_t v)          // bit j -> nibble j (j = 0..15)
+{
+    uint64_t x = v & 0xFFFFu;
+    x = (x | (x << 24)) & 0x000000FF000000FFull;
+    x = (x | (x << 12)) & 0x000F000F000F000Full;
+    x = (x | (x << 6)) & 0x0303030303030303ull;
+    x = (x | (x << 3)) & 0x1111111111111111ull;
+    return x;
+}
+
+__device__ __forceinline__ uint32_t nibbles_to_bits16(uint64_t x)          // bit 0 of nibble j -> bit j
+{
+    x &= 0x1111111111111111ull;
+    x = (x | (x >> 3)) & 0x0303030303030303ull;
+    x = (x | (x >> 6)) & 0x000F000F000F000Full;
+    x = (x | (x >> 12)) & 0x000000FF000000FFull;
+    x = (x | (x >> 24)) & 0xFFFFull;
+    return (uint32_t)x;
+}
+
+__device__ __forceinline__ uint64_t pairs16_to_nibbles(uint32_t v)         // bit pair j -> nibble j (j = 0..15)
+{
+    uint64_t x = v;
+    x = (x | (x << 16)) & 0x0000FFFF0000FFFFull;
+    x = (x | (x << 8)) & 0x00FF00FF00FF00FFull;
+    x = (x | (x << 4)) & 0x0F0F0F0F0F0F0F0Full;
+    x = (x | (x << 2)) & 0x3333333333333333ull;
+    return x;
+}
+
+__device__ __forceinline__ uint32_t nibbles_to_pairs16(uint64_t x)         // low two bits of nibble j -> bit pair j
+{
+    x &= 0x3333333333333333ull;
+    x = (x | (x >> 2)) & 0x0F0F0F0F0F0F0F0Full;
+    x = (x | (x >> 4)) & 0x00FF00FF00FF00FFull;
+    x = (x | (x >> 8)) & 0x0000FFFF0000FFFFull;
+    x = (x | (x >> 16)) & 0xFFFFFFFFull;
+    return (uint32_t)x;
+}
+
+struct BitsParams {
+    SlabDir dir;
+    int64_t L, row0, nrows;      // rows [row0, row0 + nrows) of colour `colour`
+    int colour, bc, mode;        // mode 0: validate only, 1: expand into the lattice, 2: gather from the lattice
+    uint32_t *buf;               // staging: nrows x (L/64) x {1 (Ising) | 2 (Blume-Capel)} uint32, row-major
+    int *bad;
+};
+
+__global__ void __launch_bounds__(256) bits_kernel(const __grid_constant__ BitsParams p)
+{
+    const int64_t vecs = p.L / 64;                               // 128-bit vectors per colour row
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= p.nrows * vecs) return;
+    const int64_t row = idx / vecs, v = idx - row * vecs;
+    uint64_t *lat = slab_row(p.dir, p.colour, p.row0 + row, p.L / 32) + 2 * v;
+    if (p.mode == 2) {
+        const uint64_t w0 = lat[0], w1 = lat[1];
+        if (p.bc) {
+            p.buf[2 * idx] = nibbles_to_pairs16(w0);
+            p.buf[2 * idx + 1] = nibbles_to_pairs16(w1);
+        } else {
+            p.buf[idx] = nibbles_to_bits16(w0) | (nibbles_to_bits16(w1) << 16);
+        }
+        return;
+    }
+    uint64_t w0, w1;
+    if (p.bc) {
+        const uint32_t a = p.buf[2 * idx], b = p.buf[2 * idx + 1];
+        if ((a & (a >> 1) & 0x55555555u) | (b & (b >> 1) & 0x55555555u)) atomicOr(p.bad, 1);      // a pair equal to 3
+        w0 = pairs16_to_nibbles(a); w1 = pairs16_to_nibbles(b);
+    } else {
+        const uint32_t a = p.buf[idx];
+        w0 = bits16_to_nibbles(a); w1 = bits16_to_nibbles(a >> 16);
+    }
+    if (p.mode == 1) { lat[0] = w0; lat[1] = w1; }
+}
+
+// mode 0 synchronises and returns cudaErrorInvalidValue on a bad Blume-Capel code; modes 1, 2 are asynchronous
+cudaError_t launch_bits(ising_sim *h, int colour, int64_t row0, int64_t nrows, uint32_t *dev_buf, int mode, int *dev_bad)
+{
+    BitsParams p;
+    p.dir = slab_directory(h);
+    p.L = h->L; p.row0 = row0; p.nrows = nrows; p.colour = colour; p.bc = is_blume_capel(h->model) ? 1 : 0;
+    p.mode = mode; p.buf = dev_buf; p.bad = dev_bad;
+    cudaError_t e;
+    if (mode == 0) {
+        e = cudaMemsetAsync(dev_bad, 0, sizeof(int), h->stream);
+        if (e != cudaSuccess) return e;
+    }
+    const int64_t n = nrows * (h->L / 64);
+    bits_kernel<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(p);
+    h->launches++;
+    e = cudaGetLastError();
+    if (e != cudaSuccess || mode != 0) return e;
+    int bad = 0;
+    e = cudaMemcpyAsync(&bad, dev_bad, sizeof(int), cudaMemcpyDeviceToHost, h->stream);
+    if (e != cudaSuccess) return e;
+    e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return e;
+    return bad ? cudaErrorInvalidValue : cudaSuccess;
+}

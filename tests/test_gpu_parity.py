@@ -504,3 +504,135 @@ def test_schwinger_dyson_histogram(eng, model):
         v, hist = sim.schwinger_dyson()
         ov, ohist = oracle.schwinger_dyson(sim.read_lattice(), beta)
         assert (hist == ohist).all() and _close(v, ov)
+
+
+# ------------------------------------------- memory safety without a sanitizer ---
+@pytest.mark.parametrize("model,L", [(ISING, 320), (BC, 192), (wl.ISING_LUT, 512), (wl.BLUME_CAPEL_2BIT, 192), (ISING, 64)])
+def test_no_write_outside_the_lattice_buffer(eng, model, L):
+    """compute-sanitizer is closed on this pool (profiles/r02_sanitizer.md), so out-of-bounds WRITES are looked for
+    with guard bands: the caller-owned buffer sits in the middle of a larger torch allocation filled with a canary
+    pattern; after every kind of call (sweeps in several launch geometries incl. threads past the lattice, fused
+    tally, observables, histogram, IO, bit planes and all correlation paths) the bands must be untouched and the
+    results still equal the oracle's."""
+    import ctypes as C
+    import torch
+    lib = eng.load_library()
+    need = eng.workspace_bytes(model, L)
+    guard = 1 << 20
+    buf = torch.full((need + 2 * guard,), 0xA5, dtype=torch.uint8, device="cuda:0")
+    handle = C.c_void_p()
+    stream = torch.cuda.current_stream().cuda_stream
+    beta, D, seed = (1 / 1.4, 1.0, 9) if model in (BC, wl.BLUME_CAPEL_2BIT) else (wl.BETA_C / 0.9, 0.0, 9)
+    assert (buf.data_ptr() + guard) % 256 == 0
+    assert lib.ising_create(model, L, beta, D, seed, buf.data_ptr() + guard, need, stream, C.byref(handle)) == 0
+    sim = eng.IsingSim.__new__(eng.IsingSim)                     # wrap the raw handle in the binding's class
+    sim._lib, sim._h, sim._buf, sim.model, sim.L = lib, handle, buf, model, L
+    try:
+        for rows, block in [(0, 0), (2, 32), (6, 96), (14, 256)]:
+            sim.set_launch(rows, block)
+            sim.sweep(2)
+        sim.set_tally(True)
+        sim.sweep(3)
+        o, tly = sim.observables(), sim.tally()
+        sim.schwinger_dyson()
+        lat = sim.read_lattice()
+        sim.write_lattice(lat)
+        sim.read_window(L - 3, L - 5, 17, 9)
+        for path in ((1,) if L % 256 else (1, 2, 3, 4)):
+            sim.set_corr_path(path)
+            sim.correlation(L // 2)
+        sim.correlation_protocol()
+        sim.sweep(40)                                            # CUDA-graph replay on small lattices
+        sim.sync()
+        assert bool((buf[:guard] == 0xA5).all()) and bool((buf[guard + need:] == 0xA5).all())
+        n = 11
+        if model == wl.ISING_LUT:
+            s = oracle.lut_init(L, seed)
+            for t in range(n):
+                oracle.lut_sweep(s, beta, seed, t)
+        else:
+            om = BC if model == wl.BLUME_CAPEL_2BIT else model
+            s = oracle.init(om, L, seed)
+            for t in range(n):
+                oracle.sweep(om, s, beta, D, seed, t)
+        assert (lat == s).all() and (o.bond_sum, o.M, o.Q) == oracle.observables(s) == (tly.bond_sum, tly.M, tly.Q)
+    finally:
+        sim.close()
+
+
+@pytest.mark.parametrize("model", [ISING, BC])
+def test_tensor_core_correlation_is_deterministic(eng, model):
+    """The tcgen05 kernels synchronise through mbarriers, TMA transaction counts, remote arrives and a cluster
+    multicast commit; a race there would show as run-to-run differences.  40 repeats of each path on one lattice
+    (L = 768: wrapping B tiles, ragged band) must give identical integers, equal to the oracle's."""
+    L = 768
+    beta, D = (wl.BETA_C / 0.5, 0.0) if model == ISING else (1 / 1.4, 1.0)
+    with eng.IsingSim(model, L, beta, D, 5) as sim:
+        sim.sweep(4)
+        ox, oy = oracle.correlation(sim.read_lattice(), L // 2)
+        for path in (2, 3, 4):
+            sim.set_corr_path(path)
+            for rep in range(40):
+                sx, sy = sim.correlation(L // 2 - (rep % 3) * 37)
+                n = len(sx)
+                assert (sx == ox[:n]).all() and (sy == oy[:n]).all(), (path, rep)
+
+
+# ------------------------------------------------------- compact transport format ---
+def _numpy_bits(lat, model, colour):
+    """The documented layout restated with numpy: colour row y holds the sites x = 2k + ((y + colour) & 1),
+    k = 0..L/2-1; Ising: bit k & 63 of word k >> 6 is 1 for spin +1; Blume-Capel: bits 2 (k & 31) .. +1 of word
+    k >> 5 hold spin + 1."""
+    L = lat.shape[0]
+    rows = []
+    for y in range(L):
+        v = lat[y, (y + colour) & 1::2].astype(np.int64)
+        if model in (BC, wl.BLUME_CAPEL_2BIT):
+            codes = (v + 1).astype(np.uint64).reshape(-1, 32)
+            rows.append((codes << (2 * np.arange(32, dtype=np.uint64))).sum(axis=1, dtype=np.uint64))
+        else:
+            bits = (v > 0).astype(np.uint64).reshape(-1, 64)
+            rows.append((bits << np.arange(64, dtype=np.uint64)).sum(axis=1, dtype=np.uint64))
+    return np.concatenate(rows)
+
+
+@pytest.mark.parametrize("model,L", [(ISING, 256), (BC, 192), (wl.ISING_LUT, 512), (wl.BLUME_CAPEL_2BIT, 192), (ISING, 128), (BC, 64)])
+@pytest.mark.parametrize("slabs", [None, 3])
+def test_bit_transport_format(eng, model, L, slabs):
+    """ising_read_bits / ising_write_bits: the documented layout (numpy restatement), lossless round trip
+    through another handle incl. row ranges, resume of the trajectory, rejection of the 2-bit code 3."""
+    beta, D = (1 / 1.4, 1.0) if model in (BC, wl.BLUME_CAPEL_2BIT) else (wl.BETA_C / 0.9, 0.0)
+    part = None if slabs is None else [2, L - 12, 10]
+    with eng.IsingSim(model, L, beta, D, 5, slabs=part) as a, eng.IsingSim(model, L, beta, D, 5) as b:
+        a.sweep(3)
+        b.sweep(1)                                                      # some other lattice, overwritten below
+        lat = a.read_lattice()
+        assert not (b.read_lattice() == lat).all()
+        rw = a.bits_row_words()
+        for c in range(2):
+            bits = a.read_bits(c)
+            assert len(bits) == L * rw and (bits == _numpy_bits(lat, model, c)).all()
+            assert (a.read_bits(c, 5, 9) == bits[5 * rw: 14 * rw]).all()
+            b.write_bits(c, bits[: 7 * rw], 0, 7)                       # in two pieces
+            b.write_bits(c, bits[7 * rw:], 7)
+        assert (b.read_lattice() == lat).all()
+        b.set_sweeps_done(3)
+        a.sweep(4)
+        b.sweep(4)
+        assert (a.read_lattice() == b.read_lattice()).all()
+        oa, ob = a.observables(), b.observables()
+        assert (oa.bond_sum, oa.M, oa.Q) == (ob.bond_sum, ob.M, ob.Q)
+        if model in (BC, wl.BLUME_CAPEL_2BIT):
+            before = b.read_lattice()
+            bad = b.read_bits(0)
+            bad[len(bad) // 2] |= np.uint64(3 << 10)
+            with pytest.raises(eng.IsingError):
+                b.write_bits(0, bad)
+            assert (b.read_lattice() == before).all()
+        for fn in (lambda: a.read_bits(2), lambda: a.read_bits(0, L - 2, 5), lambda: a.write_bits(0, np.zeros(rw, np.uint64), L, 1)):
+            with pytest.raises(eng.IsingError):
+                fn()
+    if model == ISING:                                                  # half a word per colour row: refused
+        with eng.IsingSim(ISING, 192, beta) as c:
+            with pytest.raises(eng.IsingError):
+                c.read_bits(0, 0, 1)
