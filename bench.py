@@ -25,9 +25,12 @@ roofline_hbm = the same kernel against the measured HBM copy rate (MEASURED_PEAK
             capture (profiles/update_kernel_dram.csv) when it was taken at this L
 cpu_baseline = the oracle, as it stands, timed on the host cores on a bounded sample
 
-N > 1 (torchrun): the path does not shard under north_star ("one GPU, no
-sharding"): N independent replicas (seed + rank), weak scaling, no collective on
-the data path; barrier + max-over-ranks timing only.
+N > 1 (torchrun): by default N independent replicas (seed + rank), weak scaling, no
+collective on the data path (north_star: "one GPU, no sharding"); barrier + max-over-
+ranks timing only.  --parallel slabs runs ONE lattice cut into N row slabs, slab k on
+GPU k (NEXT-4, ising_create_slabs), driven by rank 0: strong scaling.
+Unmeasured on hardware: this run's boxes have one GPU (--slabs S cuts the lattice into
+S slabs on the one GPU: same code path, same streams and events).
 """
 from __future__ import annotations
 
@@ -76,6 +79,11 @@ def parse_args():
     ap.add_argument("--corr-path", type=int, default=0, help="ising_set_corr_path: 0 auto (fp4 tensor cores, path 4, for wide bands), 1 bit planes, 2 int8 tensor cores one CTA per tile, 3 int8 CTA pairs, 4 fp4 CTA pairs")
     ap.add_argument("--slabs", type=int, default=0, help="NEXT-4: cut the lattice into this many row slabs (allocations of their own, halo rows "
                                                           "read from the neighbours; all on this GPU unless --gpus-as-slabs)")
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "slabs"],
+                    help="N > 1: replicas = N independent lattices, one per rank (weak scaling; the default, north_star's "
+                         "'no sharding'); slabs = ONE lattice cut into N row slabs, slab k on GPU k, driven by rank 0 through "
+                         "ising_create_slabs with peer access between the GPUs (NEXT-4, PAPER.md:69-89: one process per node "
+                         "manages the node's GPUs; strong scaling at fixed L; the other ranks only join the barriers)")
     ap.add_argument("--tally", action="store_true", help="A7: keep E, M by the fused tally of the update kernels instead of the observables pass")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -338,9 +346,19 @@ def max_over_ranks(values, dist, device):
     return [float(v) for v in t]
 
 
-def whole_job_updates_per_ns(world: int, L: int, sweeps: int, steps: int, total_ms: float) -> float:
-    """N independent replicas of the same size: every rank does L^2 * sweeps * steps updates."""
-    return world * L * L * sweeps * steps / (total_ms * 1e6)
+def whole_job_updates_per_ns(world: int, L: int, sweeps: int, steps: int, total_ms: float, parallel: str = "replicas") -> float:
+    """replicas: N independent lattices of the same size, every rank does L^2 * sweeps * steps updates.
+    slabs: one lattice shared by the N GPUs, L^2 * sweeps * steps updates in all."""
+    lattices = world if parallel == "replicas" else 1
+    return lattices * L * L * sweeps * steps / (total_ms * 1e6)
+
+
+def rank_plan(rank: int, world: int, parallel: str):
+    """(drives a simulation?, slabs, slab devices) of one rank.  replicas: every rank its own unsharded lattice on
+    its own GPU.  slabs (N > 1): rank 0 drives one lattice whose slab k lives on GPU k; the others idle."""
+    if parallel == "slabs" and world > 1:
+        return (rank == 0, world, list(range(world))) if rank == 0 else (False, 0, None)
+    return True, 0, None
 
 
 def replica_seed(base_seed: int, rank: int) -> int:
@@ -367,8 +385,19 @@ def run_ours(args):
     base, L, name = pick_workload(args)
     model = MODEL_IDS[args.model]
     S, K, W = args.sweeps_per_step, args.steps, max(args.warmup, 0)
+    drives, n_slabs, slab_devices = rank_plan(rank, world, args.parallel)
+    if args.slabs > 1 and not n_slabs:
+        n_slabs = args.slabs                                   # several slabs on this rank's own GPU
+    if not drives:                                             # --parallel slabs: ranks > 0 only keep the barriers company
+        for _ in range(2):
+            dist.barrier()
+            torch.cuda.synchronize(device)
+        max_over_ranks([0.0, 0.0], dist, device)
+        dist.barrier()
+        dist.destroy_process_group()
+        return
     sim = eng.IsingSim(model, L, base.beta, base.D, replica_seed(base.seed, rank), device=device,
-                       slabs=args.slabs if args.slabs > 1 else None)
+                       slabs=n_slabs if n_slabs > 1 else None, slab_devices=slab_devices)
     if args.rows_per_thread or args.block:
         sim.set_launch(args.rows_per_thread, args.block)
     if args.variant:
@@ -417,7 +446,7 @@ def run_ours(args):
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
     lut = model == wl.ISING_LUT
     philox_ms = copy_ms = None
-    if not lut and args.slabs <= 1:                        # the roof helpers work on the 4-bit layout of an unsharded lattice
+    if not lut and n_slabs <= 1:                           # the roof helpers work on the 4-bit layout of an unsharded lattice
         sim.bench_philox_only(2); sim.bench_copy(2); torch.cuda.synchronize(device)
         ev[0].record(); sim.bench_philox_only(n_roof); ev[1].record(); sim.bench_copy(n_roof); ev[2].record()
         torch.cuda.synchronize(device)
@@ -473,10 +502,11 @@ def run_ours(args):
                 "philox_only_kernel_updates_per_ns": sites_per_launch / (philox_ms * 1e6) if philox_ms else None,
                 "frac_of_philox_only_kernel": philox_ms / kern_ms if philox_ms else None,
                 "pipe_rates_warp_instr_per_subpartition_clk": pipes}
-    value = whole_job_updates_per_ns(world, L, S, K, total_ms)
+    value = whole_job_updates_per_ns(world, L, S, K, total_ms, args.parallel)
     line = {
         "metric": "spin updates/ns", "value": value, "unit": "updates/ns", "n_gpus": world, "steps": K,
-        "warmup": W, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
+        "warmup": W, "ms_per_step": total_ms / K, "higher_is_better": True,
+        "scaling": "strong" if (args.parallel == "slabs" and world > 1) else "weak",
         "vs_baseline": None,                      # BASELINE.json publishes no number for this metric on B200
         "vs_paper_gb200_context": (value / PAPER_UPDATES_PER_NS[(args.model, L)]) if (args.model, L) in PAPER_UPDATES_PER_NS and args.workload == "sweep" else None,
         "dtype": "u32 (Philox4x32-10, SWAR on 4-bit spins, integer compare)",
@@ -486,11 +516,12 @@ def run_ours(args):
                    "step": "S sweeps + observables" if args.workload == "sweep" else "S sweeps + correlation protocol + observables",
                    "launch": {"rows_per_thread": args.rows_per_thread or "default", "block": args.block or "default",
                               "variant": args.variant, "fused_tally": bool(args.tally), "corr_path": args.corr_path,
-                              "slabs": max(1, args.slabs)},
+                              "slabs": max(1, n_slabs)},
                    "lattice_bytes": L * L * BITS_PER_SITE[model] // 8, "l2": "inputs larger than L2 (no flush needed)" if L * L // 2 > (256 << 20)
-                   else "lattice fits L2: DRAM figures not meaningful", "parallelism": f"replicas x{world}"},
+                   else "lattice fits L2: DRAM figures not meaningful",
+                   "parallelism": f"slabs x{world} (one lattice, slab k on GPU k, halo rows by peer loads)" if (args.parallel == "slabs" and world > 1) else f"replicas x{world}"},
         "measurement_ms_per_step": (total_ms - sweep_ms) / K,
-        "sweep_only_updates_per_ns": world * L * L * S * K / (sweep_ms * 1e6),
+        "sweep_only_updates_per_ns": whole_job_updates_per_ns(world, L, S, K, sweep_ms, args.parallel),
         "roofline": alu_roof,
         "roofline_hbm": {"bound": "hbm", "kernel": "update_kernel (one colour phase)", "achieved": achieved,
                          "peak": peak, "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8000_gbs": achieved / 8000.0,

@@ -102,6 +102,9 @@ int ising_create(int model, int64_t L, double beta, double D, uint64_t seed,
  * GPUs used").  Every call of this header works on such a handle; cuda_stream is slab 0's stream.        */
 int ising_create_slabs(int model, int64_t L, double beta, double D, uint64_t seed, int n_slabs,
                        const int64_t *slab_rows, const int *devices, void *cuda_stream, ising_t **out);
+/* The default partition on its own (host arithmetic, no GPU): the L/2 row pairs dealt as evenly as possible
+ * over n_slabs slabs, rows[k] = height of slab k (even, >= 2).                                             */
+int ising_slab_partition(int64_t L, int n_slabs, int64_t *rows);
 /* Number of slabs (1 for ising_create), and rows [y0, y0 + rows) / device of one of them (NULL: skip). */
 int ising_slab_count(const ising_t *h);
 int ising_slab_info(const ising_t *h, int slab, int64_t *y0, int64_t *rows, int *device);

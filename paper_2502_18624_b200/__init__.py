@@ -4,5 +4,5 @@ models (hot path of arxiv 2502.18624).  The product is the CUDA library
 the thin ctypes binding (argument marshalling only).  There is no CPU fallback:
 creating a simulation without the library or without a CUDA device raises."""
 from .binding import (ISING, BLUME_CAPEL, ISING_LUT, BLUME_CAPEL_2BIT, PIPE_PROBES, IsingError, IsingSim, Observables,  # noqa: F401
-                      bench_pipes, debug_philox, time_grid, protocol_distances, threshold_table, lib_path, load_library,
+                      bench_pipes, debug_philox, time_grid, protocol_distances, threshold_table, slab_partition, lib_path, load_library,
                       workspace_bytes)

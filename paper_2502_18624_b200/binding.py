@@ -10,7 +10,8 @@ import numpy as np
 
 ISING, BLUME_CAPEL, ISING_LUT, BLUME_CAPEL_2BIT = 0, 1, 2, 3
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libising_b200.so")
+# ISING_B200_LIB: another build of the same library (build.py's `out` / `defines`), for A/B timing of kernel variants
+_LIB_PATH = os.environ.get("ISING_B200_LIB") or os.path.join(_HERE, "libising_b200.so")
 _lib = None
 
 EXPORTS = [
@@ -21,7 +22,7 @@ EXPORTS = [
     "ising_launch_count", "ising_sync", "ising_destroy", "ising_last_error", "ising_bench_philox_only",
     "ising_bench_copy", "ising_debug_philox", "ising_protocol_distances", "ising_threshold_table",
     "ising_run_protocol_schedule", "ising_create_slabs", "ising_slab_count", "ising_slab_info",
-    "ising_write_bits", "ising_read_bits",
+    "ising_write_bits", "ising_read_bits", "ising_slab_partition",
 ]
 
 
@@ -149,6 +150,15 @@ def protocol_distances(L: int, t: int):
     st = np.zeros(n.value, dtype=np.int64)
     _check(lib.ising_protocol_distances(int(L), int(t), len(r), r.ctypes.data, st.ctypes.data, C.addressof(n)))
     return r, st
+
+
+def slab_partition(L: int, n_slabs: int) -> np.ndarray:
+    """Default slab heights of ising_create_slabs.  Host arithmetic: no GPU needed."""
+    lib = load_library()
+    lib.ising_slab_partition.argtypes = [C.c_int64, C.c_int, C.c_void_p]
+    rows = np.zeros(n_slabs, dtype=np.int64)
+    _check(lib.ising_slab_partition(int(L), int(n_slabs), rows.ctypes.data))
+    return rows
 
 
 def threshold_table(model: int, beta: float, D: float = 0.0) -> np.ndarray:

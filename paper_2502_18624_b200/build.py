@@ -20,16 +20,18 @@ def _deps():
     return sources() + glob.glob(os.path.join(HERE, "csrc", "*.cuh")) + glob.glob(os.path.join(ROOT, "include", "*.h"))
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps()):
-        return LIB
+def build(force: bool = False, verbose: bool = False, out: str = LIB, defines=()) -> str:
+    """out / defines: an experimental build beside the product library (e.g. -DBC_LANE_TABLE=0), loaded by
+    setting ISING_B200_LIB (binding.py) -- for A/B timing of kernel variants on one GPU box."""
+    if not force and os.path.exists(out) and all(os.path.getmtime(out) >= os.path.getmtime(d) for d in _deps()):
+        return out
     cmd = [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
            "-Xcompiler", "-fPIC", "-shared", "-I" + os.path.join(ROOT, "include"),
-           "-I" + os.path.join(HERE, "csrc"), "-o", LIB] + sources()
+           "-I" + os.path.join(HERE, "csrc"), "-o", out] + ["-D" + d for d in defines] + sources()
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.check_call(cmd)
-    return LIB
+    return out
 
 
 if __name__ == "__main__":

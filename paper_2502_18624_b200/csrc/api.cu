@@ -253,9 +253,9 @@ extern "C" int ising_create_slabs(int model, int64_t L, double beta, double D, u
         return set_error(ISING_EINVAL, "ising_create_slabs: n_slabs must be in [1, 64] and leave every slab two rows");
     std::vector<int64_t> rows(n_slabs);
     int64_t total = 0;
+    if (!slab_rows) { rc = ising_slab_partition(L, n_slabs, rows.data()); if (rc) return rc; }
     for (int k = 0; k < n_slabs; ++k) {
-        // default: L/2 row pairs dealt as evenly as possible
-        rows[k] = slab_rows ? slab_rows[k] : 2 * ((L / 2) * (k + 1) / n_slabs - (L / 2) * k / n_slabs);
+        if (slab_rows) rows[k] = slab_rows[k];
         if (rows[k] < 2 || (rows[k] & 1)) return set_error(ISING_EINVAL, "ising_create_slabs: every slab needs an even number of rows >= 2");
         total += rows[k];
     }

@@ -183,3 +183,17 @@ extern "C" int ising_protocol_distances(int64_t L, uint64_t t, int64_t cap, int6
     for (int64_t i = 0; i < nb; ++i) { r[na + i] = block_sources[i]; stride[na + i] = kBlock; }
     return ISING_OK;
 }
+
+// ---------------------------------------------------------------- NEXT-4 ---
+// Default row partition of ising_create_slabs ("horizontal slabs"): the L/2 row pairs dealt as
+// evenly as possible, so every slab starts on an even row and has an even height (a row pair is the unit the
+// kernels walk: the row parity alternates inside it).
+extern "C" int ising_slab_partition(int64_t L, int n_slabs, int64_t *rows)
+{
+    if (!rows) return set_error(ISING_EINVAL, "ising_slab_partition: rows is NULL");
+    if (L < 2 || (L & 1) || n_slabs < 1 || n_slabs > ISING_MAX_SLABS || 2 * (int64_t)n_slabs > L)
+        return set_error(ISING_EINVAL, "ising_slab_partition: L must be even and n_slabs in [1, min(64, L/2)]");
+    const int64_t pairs = L / 2;
+    for (int k = 0; k < n_slabs; ++k) rows[k] = 2 * (pairs * (k + 1) / n_slabs - pairs * k / n_slabs);
+    return ISING_OK;
+}

@@ -20,6 +20,7 @@ struct LutParams {
     uint32_t colour, t;
     const uint32_t *tree;        // 16 carry constants in heap order (device): tree[n] = 2^32 - threshold(node n)
     const uint2 *buckets;        // 4096 entries indexed by the top 12 bits of the number (device), see lut_bits32
+    uint32_t bucket_stride;      // 8: bytes per bucket entry, as a run-time value (see lut_bucket_step)
     const uint32_t *t_base;      // sweep number = t + *t_base (see update.cu)
     long long *tally;            // A7: running B, M (device), updated when the kernel is built with TALLY
     RoundKeys rk;
@@ -52,20 +53,31 @@ __device__ __forceinline__ uint32_t lut_search(uint32_t rnd, uint32_t c_root, co
 #ifndef LUT_MIN_BLOCKS
 #define LUT_MIN_BLOCKS 2
 #endif
-__device__ __forceinline__ void lut_bucket_step(uint32_t &w, uint32_t &f, uint32_t rnd, const unsigned char *buckets)
+// The entry address is base + 8 (rnd >> 20): the shift is an ALU instruction, the scaling a multiply-add on the FMA
+// pipe whose factor 8 comes from a kernel parameter (p.bucket_stride) so that it stays a multiply: written as a
+// constant it becomes a second ALU instruction (shift by 17 and mask), and the dispatch slots of the ALU are what
+// bounds this kernel.
+struct BucketTable { uint32_t base, stride; };     // shared-memory address of entry 0, bytes per entry (= 8)
+
+__device__ __forceinline__ void lut_bucket_step(uint32_t &w, uint32_t &f, uint32_t rnd, const BucketTable bk)
 {
-    const uint2 e = *reinterpret_cast<const uint2 *>(buckets + (rnd >> (32 - LUT_BUCKET_BITS)) * 8u);
-    asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\tmadc.lo.u32 %0, %0, 16, %3;\n\t}" : "+r"(w) : "r"(rnd), "r"(e.x), "r"(e.y));
-    asm("mad.lo.u32 %0, %1, 1, %0;" : "+r"(f) : "r"(e.y));
+    uint32_t ex, ey;
+    asm("{\n\t.reg .u32 t, a;\n\t"
+        "shr.u32 t, %2, 20;\n\t"
+        "mad.lo.u32 a, t, %4, %3;\n\t"
+        "ld.shared.v2.u32 {%0, %1}, [a];\n\t}"
+        : "=r"(ex), "=r"(ey) : "r"(rnd), "r"(bk.base), "r"(bk.stride));
+    asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\tmadc.lo.u32 %0, %0, 16, %3;\n\t}" : "+r"(w) : "r"(rnd), "r"(ex), "r"(ey));
+    asm("mad.lo.u32 %0, %1, 1, %0;" : "+r"(f) : "r"(ey));
 }
 
 // bad: OR of the meta sums of the fast path (>= 256 iff some number fell into a multi-threshold bucket)
 template <int V>
 __device__ __forceinline__ uint32_t lut_bits32(uint32_t g_lo, const PhiloxRow &pr, const RoundKeys &rk,
-                                               uint32_t c_root, const uint32_t *tree, const unsigned char *buckets,
+                                               uint32_t c_root, const uint32_t *tree, const BucketTable buckets,
                                                uint32_t &bad)
 {
-    const uint4 a = philox_site4(g_lo, pr, rk), b = philox_site4(g_lo | 1u, pr, rk);
+    const uint4 a = philox_site4(philox_counter(g_lo), pr, rk), b = philox_site4(philox_counter(g_lo | 1u), pr, rk);
     if (V == 0) {
         uint32_t w = 0, f = 0;   // highest nibble first
         lut_bucket_step(w, f, b.w, buckets); lut_bucket_step(w, f, b.z, buckets);
@@ -87,12 +99,16 @@ __device__ __forceinline__ uint32_t lut_bits32(uint32_t g_lo, const PhiloxRow &p
 __device__ __forceinline__ uint32_t lut_flip(uint32_t x, uint32_t up, uint32_t dn, uint32_t sm, uint32_t sd,
                                              uint32_t e4, uint32_t e8)
 {
-    // 1 where the neighbour equals the spin; bit-sliced count of the four
-    const uint32_t a = ~(up ^ x), b = ~(dn ^ x), c = ~(sm ^ x), d = ~(sd ^ x);
-    const uint32_t s0 = a ^ b, c0 = a & b, s1 = c ^ d, c1 = c & d;
+    // Bit-sliced count of the neighbours equal to the spin, pair by pair: c = both of a pair equal, s = exactly
+    // one (the spin cancels: (up == x) ^ (dn == x) = up ^ dn).  Equal neighbours = 2 c0 + s0 + 2 c1 + s1, so
+    // eq4 = c0 & c1 and ">= 3 equal" = c0 & (c1 | s1) | c1 & s0 (c and s of a pair exclude each other).
+    const uint32_t c0 = ~(up ^ x) & ~(dn ^ x), c1 = ~(sm ^ x) & ~(sd ^ x);
+    const uint32_t s0 = up ^ dn, s1 = sm ^ sd;
     const uint32_t eq4 = c0 & c1;
-    const uint32_t eq3 = (c0 ^ c1) & (s0 ^ s1);
-    const uint32_t flip = (eq4 & e8 & e4) | (eq3 & e4) | ~(eq4 | eq3);
+    const uint32_t ge3 = (c0 & (c1 | s1)) | (c1 & s0);
+    // flip = (eq4 & exp8) | (eq3 & exp4) | (~eq4 & ~eq3), exp8 = e8 & e4, eq3 = ge3 & ~eq4
+    //                        = ~ge3 | (e4 & (~eq4 | e8))
+    const uint32_t flip = ~ge3 | (e4 & (~eq4 | e8));
     return x ^ flip;
 }
 
@@ -116,7 +132,7 @@ __device__ __noinline__ uint4 lut_row_slow(const uint4 &src, const uint4 &up, co
 template <int P, int V>
 __device__ __forceinline__ uint4 lut_row(const uint4 &src, const uint4 &up, const uint4 &sm, const uint4 &dn,
                                          uint32_t edge, uint64_t g0, uint32_t t, const LutParams &p, uint32_t c_root,
-                                         const uint32_t *tree, const unsigned char *bk)
+                                         const uint32_t *tree, const BucketTable bk)
 {
     uint32_t sd[4];
     lut_side<P>(sm, edge, sd);
@@ -152,7 +168,7 @@ __device__ __noinline__ uint4 lut_row_slow(const uint4 &src, const uint4 &up, co
                                            uint32_t edge, uint64_t g0, uint32_t t, const LutParams &p, uint32_t c_root,
                                            const uint32_t *tree)
 {
-    return lut_row<P, 1>(src, up, sm, dn, edge, g0, t, p, c_root, tree, nullptr);
+    return lut_row<P, 1>(src, up, sm, dn, edge, g0, t, p, c_root, tree, BucketTable{0u, 0u});
 }
 
 // A7 (optional): change of B and M caused by one updated row, from old / new words and the neighbours.
@@ -192,6 +208,7 @@ __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const _
     }
     __syncthreads();
     const uint32_t c_root = s_tree[1];
+    const BucketTable bk = {(uint32_t)__cvta_generic_to_shared(s_buckets), p.bucket_stride};
     const int cols = p.cols, L = p.L;
     unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
     unsigned chunk = tid / (unsigned)cols;
@@ -228,7 +245,7 @@ __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const _
         uint4 nsrc = *reinterpret_cast<const uint4 *>(w0 + rs);
         uint32_t nedge = *reinterpret_cast<const uint32_t *>(eo);
         uint4 dn2 = *reinterpret_cast<const uint4 *>(o2);
-        uint4 o = lut_row<C, V>(src, up, sm, dn, edge, g0, t_eff, p, c_root, s_tree, s_buckets);
+        uint4 o = lut_row<C, V>(src, up, sm, dn, edge, g0, t_eff, p, c_root, s_tree, bk);
         if (TALLY) lut_tally_row<C>(src, o, up, sm, dn, edge, dB, dM);
         *reinterpret_cast<uint4 *>(w0) = o;
         g0 += gs;
@@ -239,7 +256,7 @@ __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const _
             nsrc2 = *reinterpret_cast<const uint4 *>(w0 + 2 * rs);
             nedge2 = *reinterpret_cast<const uint32_t *>(ee);
         }
-        o = lut_row<1 - C, V>(nsrc, sm, dn, dn2, nedge, g0, t_eff, p, c_root, s_tree, s_buckets);
+        o = lut_row<1 - C, V>(nsrc, sm, dn, dn2, nedge, g0, t_eff, p, c_root, s_tree, bk);
         if (TALLY) lut_tally_row<1 - C>(nsrc, o, sm, dn, dn2, nedge, dB, dM);
         *reinterpret_cast<uint4 *>(w0 + rs) = o;
         g0 += gs;
@@ -272,6 +289,7 @@ cudaError_t launch_lut_update(ising_sim *h, int slab, int colour, uint32_t t)
     int block = h->block_threads;
     unsigned grid = (unsigned)((threads + block - 1) / block);
     p.buckets = reinterpret_cast<const uint2 *>(sl.lut_buckets);
+    p.bucket_stride = 8u;
     const size_t smem = 8 << LUT_BUCKET_BITS;
     p.tally = sl.d_acc + 40;
     p.t_base = reinterpret_cast<const uint32_t *>(sl.d_acc + 48) + (h->graph_capture ? 1 : 0);

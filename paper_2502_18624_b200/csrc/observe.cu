@@ -43,14 +43,18 @@ __device__ __forceinline__ void obs_half(uint32_t x, uint32_t up, uint32_t dn, u
         }
     } else {
         uint32_t S = up + dn + sm + sd;                            // h + 4 per site
-        uint32_t pos = (x >> 1) & ONES, neg = ~(x | (x >> 1)) & ONES;
         if (MODE == 0) {
-            int np = __popc(pos), nn = __popc(neg);
-            B += (int)nibble_sum(S & (pos * 15u)) - 4 * np - (int)nibble_sum(S & (neg * 15u)) + 4 * nn;
-            uint32_t wpos = (sm >> 1) & ONES, wneg = ~(sm | (sm >> 1)) & ONES;
-            int wp = __popc(wpos), wn = __popc(wneg);
-            M += np - nn + wp - wn;
-            Q += np + nn + wp + wn;
+            // Word level, in the codes c = s + 1 ("similar to an energy computation using a short look-up
+            // table" -- here no table at all): the nibbles are spread to bytes and summed by 4-way byte dot products
+            // (IDP4A).  B accumulates sum_black c S, M sum c and Q sum c^2 over the black word and the white word of
+            // the same position; the kernel turns them into B, M, Q at the end (observe_kernel).
+            const uint32_t lo = 0x0F0F0F0Fu, one = 0x01010101u;
+            const uint32_t Se = S & lo, So = (S >> 4) & lo, ce = x & lo, co = (x >> 4) & lo, we = sm & lo, wo = (sm >> 4) & lo;
+            uint32_t b = (uint32_t)B, m = (uint32_t)M, q = (uint32_t)Q;
+            b = __dp4a(ce, Se, b); b = __dp4a(co, So, b);
+            m = __dp4a(ce + co + we + wo, one, m);                 // bytes <= 8
+            q = __dp4a(ce, ce, q); q = __dp4a(co, co, q); q = __dp4a(we, we, q); q = __dp4a(wo, wo, q);
+            B = (int)b; M = (int)m; Q = (int)q;
         } else {
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
@@ -96,6 +100,16 @@ __global__ void __launch_bounds__(256) observe_kernel(const __grid_constant__ Ob
         }
     }
     if (MODE == 0) {          // warp sums fit 32 bits: <= 32 lanes x R rows x 128 sites x 4
+        if (MODEL != ISING_MODEL_ISING && y0 < L) {
+            // (B, M, Q) hold (sum_black c S, sum c, sum c^2) over this thread's n black and n white sites.  With
+            // s = c - 1, h = S - 4:  sum_black s h = sum cS - 4 sum_black c - sum_black S + 4 n, and over the whole
+            // lattice sum_black S = 4 sum_white c (every white site is the neighbour of four black ones), so the
+            // per-thread shares  B' = sum cS - 4 sum c + 4 n  add up to the bond sum;  M = sum c - 2 n;
+            // Q = sum (c - 1)^2 = sum c^2 - 2 sum c + 2 n.
+            const int n = (min(L, y0 + p.R) - y0) * 32;
+            const int cS = B, c1 = M, c2 = Q;
+            B = cS - 4 * c1 + 4 * n; M = c1 - 2 * n; Q = c2 - 2 * c1 + 2 * n;
+        }
         const int v[3] = {B, M, Q};
         block_accumulate<3>(v, p.acc);
     } else {

@@ -14,6 +14,9 @@
 
 #define ONES 0x11111111u
 
+// Philox counter of call q of a row: gl + q, gl a multiple of 8 (philox_counter: ising_internal.cuh).
+#define CTR(gl, q) philox_counter((gl) | (q))
+
 struct UpdParams {
     const uint4 *opp;   // opposite colour, rows of this slab (read only during this phase)
     uint4 *own;         // colour being updated, rows of this slab
@@ -104,10 +107,10 @@ __device__ __forceinline__ uint4 ising_row(const uint4 &src, const uint4 &up, co
     side_words<ISING_MODEL_ISING, P>(sm, edge, sd);
     PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), t, tag, p.rk);
     uint32_t gl = (uint32_t)g0;     // g0 is a multiple of 8: gl | q == gl + q
-    uint4 r0 = philox_site4(gl | 0, pr, p.rk), r1 = philox_site4(gl | 1, pr, p.rk);
-    uint4 r2 = philox_site4(gl | 2, pr, p.rk), r3 = philox_site4(gl | 3, pr, p.rk);
-    uint4 r4 = philox_site4(gl | 4, pr, p.rk), r5 = philox_site4(gl | 5, pr, p.rk);
-    uint4 r6 = philox_site4(gl | 6, pr, p.rk), r7 = philox_site4(gl | 7, pr, p.rk);
+    uint4 r0 = philox_site4(CTR(gl, 0), pr, p.rk), r1 = philox_site4(CTR(gl, 1), pr, p.rk);
+    uint4 r2 = philox_site4(CTR(gl, 2), pr, p.rk), r3 = philox_site4(CTR(gl, 3), pr, p.rk);
+    uint4 r4 = philox_site4(CTR(gl, 4), pr, p.rk), r5 = philox_site4(CTR(gl, 5), pr, p.rk);
+    uint4 r6 = philox_site4(CTR(gl, 6), pr, p.rk), r7 = philox_site4(CTR(gl, 7), pr, p.rk);
     uint4 o;
     if (V == 0) {
         o.x = ising_half_carry(src.x, up.x, dn.x, sm.x, sd[0], r0, r1, p);
@@ -157,19 +160,19 @@ __device__ __forceinline__ uint4 bc_row(const uint4 &src, const uint4 &up, const
     uint32_t gl = (uint32_t)g0;
     uint4 o;
     {
-        uint4 ra = philox_site4(gl | 0, pr, p.rk), rb = philox_site4(gl | 1, pr, p.rk);
+        uint4 ra = philox_site4(CTR(gl, 0), pr, p.rk), rb = philox_site4(CTR(gl, 1), pr, p.rk);
         o.x = bc_half(src.x, up.x, dn.x, sm.x, sd[0], ra, rb, tab, always);
     }
     {
-        uint4 ra = philox_site4(gl | 2, pr, p.rk), rb = philox_site4(gl | 3, pr, p.rk);
+        uint4 ra = philox_site4(CTR(gl, 2), pr, p.rk), rb = philox_site4(CTR(gl, 3), pr, p.rk);
         o.y = bc_half(src.y, up.y, dn.y, sm.y, sd[1], ra, rb, tab, always);
     }
     {
-        uint4 ra = philox_site4(gl | 4, pr, p.rk), rb = philox_site4(gl | 5, pr, p.rk);
+        uint4 ra = philox_site4(CTR(gl, 4), pr, p.rk), rb = philox_site4(CTR(gl, 5), pr, p.rk);
         o.z = bc_half(src.z, up.z, dn.z, sm.z, sd[2], ra, rb, tab, always);
     }
     {
-        uint4 ra = philox_site4(gl | 6, pr, p.rk), rb = philox_site4(gl | 7, pr, p.rk);
+        uint4 ra = philox_site4(CTR(gl, 6), pr, p.rk), rb = philox_site4(CTR(gl, 7), pr, p.rk);
         o.w = bc_half(src.w, up.w, dn.w, sm.w, sd[3], ra, rb, tab, always);
     }
     return o;
@@ -231,19 +234,19 @@ __device__ __forceinline__ uint4 bc_row_carry(const uint4 &src, const uint4 &up,
     uint32_t gl = (uint32_t)g0;
     uint4 o;
     {
-        uint4 ra = philox_site4(gl | 0, pr, p.rk), rb = philox_site4(gl | 1, pr, p.rk);
+        uint4 ra = philox_site4(CTR(gl, 0), pr, p.rk), rb = philox_site4(CTR(gl, 1), pr, p.rk);
         o.x = bc_half_carry(src.x, up.x, dn.x, sm.x, sd[0], ra, rb, tab);
     }
     {
-        uint4 ra = philox_site4(gl | 2, pr, p.rk), rb = philox_site4(gl | 3, pr, p.rk);
+        uint4 ra = philox_site4(CTR(gl, 2), pr, p.rk), rb = philox_site4(CTR(gl, 3), pr, p.rk);
         o.y = bc_half_carry(src.y, up.y, dn.y, sm.y, sd[1], ra, rb, tab);
     }
     {
-        uint4 ra = philox_site4(gl | 4, pr, p.rk), rb = philox_site4(gl | 5, pr, p.rk);
+        uint4 ra = philox_site4(CTR(gl, 4), pr, p.rk), rb = philox_site4(CTR(gl, 5), pr, p.rk);
         o.z = bc_half_carry(src.z, up.z, dn.z, sm.z, sd[2], ra, rb, tab);
     }
     {
-        uint4 ra = philox_site4(gl | 6, pr, p.rk), rb = philox_site4(gl | 7, pr, p.rk);
+        uint4 ra = philox_site4(CTR(gl, 6), pr, p.rk), rb = philox_site4(CTR(gl, 7), pr, p.rk);
         o.w = bc_half_carry(src.w, up.w, dn.w, sm.w, sd[3], ra, rb, tab);
     }
     return o;
@@ -264,8 +267,8 @@ __device__ __forceinline__ uint4 bc2_row(const uint4 &src, const uint4 &up, cons
     uint32_t gl = (uint32_t)g0;
     uint4 o;
     {
-        const uint4 q0 = philox_site4(gl | 0, pr, p.rk), q1 = philox_site4(gl | 1, pr, p.rk);
-        const uint4 q2 = philox_site4(gl | 2, pr, p.rk), q3 = philox_site4(gl | 3, pr, p.rk);
+        const uint4 q0 = philox_site4(CTR(gl, 0), pr, p.rk), q1 = philox_site4(CTR(gl, 1), pr, p.rk);
+        const uint4 q2 = philox_site4(CTR(gl, 2), pr, p.rk), q3 = philox_site4(CTR(gl, 3), pr, p.rk);
         const uint4 ea = make_uint4(q0.x, q0.z, q1.x, q1.z), eb = make_uint4(q2.x, q2.z, q3.x, q3.z);
         const uint4 oa = make_uint4(q0.y, q0.w, q1.y, q1.w), ob = make_uint4(q2.y, q2.w, q3.y, q3.w);
         if (V == 0) {
@@ -277,8 +280,8 @@ __device__ __forceinline__ uint4 bc2_row(const uint4 &src, const uint4 &up, cons
         }
     }
     {
-        const uint4 q0 = philox_site4(gl | 4, pr, p.rk), q1 = philox_site4(gl | 5, pr, p.rk);
-        const uint4 q2 = philox_site4(gl | 6, pr, p.rk), q3 = philox_site4(gl | 7, pr, p.rk);
+        const uint4 q0 = philox_site4(CTR(gl, 4), pr, p.rk), q1 = philox_site4(CTR(gl, 5), pr, p.rk);
+        const uint4 q2 = philox_site4(CTR(gl, 6), pr, p.rk), q3 = philox_site4(CTR(gl, 7), pr, p.rk);
         const uint4 ea = make_uint4(q0.x, q0.z, q1.x, q1.z), eb = make_uint4(q2.x, q2.z, q3.x, q3.z);
         const uint4 oa = make_uint4(q0.y, q0.w, q1.y, q1.w), ob = make_uint4(q2.y, q2.w, q3.y, q3.w);
         if (V == 0) {
@@ -384,6 +387,9 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
     uint64_t g0 = (uint64_t)(p.y_base + y0) * (uint64_t)(cols * 8) + (uint64_t)(col * 8);
     const uint64_t gs = (uint64_t)(cols * 8);
 
+    // two row pairs per iteration for the Ising kernel (+1.4 % measured: loop and pointer arithmetic per site halve);
+    // the Blume-Capel kernels lose 2 % to it (register pressure around the table look-ups)
+#pragma unroll(kIsing ? 2 : 1)
     for (int y = y0; y < yend; y += 2) {
         // ---- even offset: parity C
         const char *o2 = (y + 2 == L) ? p.opp_dn + cb : o1 + rs;       // row y + 2; below the slab: the halo row
@@ -541,7 +547,7 @@ __global__ void __launch_bounds__(256) philox_only_kernel(const __grid_constant_
         uint32_t gl = (uint32_t)g0;
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
-            uint4 r = philox_site4(gl | q, pr, p.rk);
+            uint4 r = philox_site4(CTR(gl, q), pr, p.rk);
             // consume all four words on the FMA pipe (IMAD), which has spare dispatch slots:
             // the roof kernel should cost nothing but the generator itself
             asm("mad.lo.u32 %0, %0, 3, %1;\n\tmad.lo.u32 %0, %0, 3, %2;\n\t"

@@ -244,6 +244,19 @@ def test_lut_table_extremes_and_errors(eng):
     assert lib.ising_threshold_table(0, float("nan"), 0.0, None, 0, C.addressof(n)) == -1
 
 
+# ------------------------------------------------------------- slab partition ---
+def test_slab_partition(eng):
+    """NEXT-4 host logic: even heights >= 2 that add up to L, as even as row pairs allow."""
+    for L, n in [(256, 1), (256, 3), (256, 8), (1 << 18, 8), (1 << 20, 64), (64, 32), (192, 7), (1 << 19, 6)]:
+        rows = [int(r) for r in eng.slab_partition(L, n)]
+        assert len(rows) == n and sum(rows) == L and all(r >= 2 and r % 2 == 0 for r in rows)
+        assert max(rows) - min(rows) <= 2
+    assert [int(r) for r in eng.slab_partition(256, 3)] == [84, 86, 86]
+    for L, n in [(256, 0), (256, 65), (64, 33), (255, 2)]:
+        with pytest.raises(eng.IsingError):
+            eng.slab_partition(L, n)
+
+
 # ------------------------------------------------ and, as a consequence, == oracle ---
 def test_host_logic_agrees_with_the_oracle(eng):
     import oracle

@@ -1,6 +1,8 @@
-"""N > 1 host logic of bench.py on CPU (gloo, world_size 2): the path does not shard under
-north_star (one GPU per simulation, replicas only -- DESIGN.md Sec. 8), so the only cross-rank
-steps are the barrier and the max-over-ranks of the device times."""
+"""N > 1 host logic of bench.py on CPU (gloo, world_size 2).  Default: replicas (north_star: one GPU per
+simulation), where the only cross-rank steps are the barrier and the max-over-ranks of the device times.
+--parallel slabs (NEXT-4): one lattice cut into row slabs, slab k on GPU k, driven by rank 0;
+its host logic -- who drives, which slabs on which devices, the partition, the whole-job value -- is checked here,
+the device side by tests/test_gpu_slabs.py."""
 import os
 import socket
 import sys
@@ -29,7 +31,9 @@ def _worker(rank, world, port, out):
         dist.barrier()
         total_ms, sweep_ms = bench.max_over_ranks(mine, dist, torch.device("cpu"))
         value = bench.whole_job_updates_per_ns(world, 256, 10, 4, total_ms)
-        out.put((rank, total_ms, sweep_ms, value, bench.replica_seed(1, rank)))
+        plan = bench.rank_plan(rank, world, "slabs")
+        sharded = bench.whole_job_updates_per_ns(world, 256, 10, 4, total_ms, "slabs")
+        out.put((rank, total_ms, sweep_ms, value, bench.replica_seed(1, rank), plan, sharded))
     finally:
         dist.destroy_process_group()
 
@@ -46,10 +50,13 @@ def test_max_over_ranks_and_whole_job_value_world2():
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    for rank, total_ms, sweep_ms, value, seed in res:
+    for rank, total_ms, sweep_ms, value, seed, plan, sharded in res:
         assert total_ms == 107.0 and sweep_ms == 90.0            # element-wise max, same on both ranks
         assert value == pytest.approx(2 * 256 * 256 * 10 * 4 / (107.0 * 1e6), rel=1e-15)
         assert seed == 1 + rank                                  # independent replicas
+        # --parallel slabs: rank 0 drives one lattice of 2 slabs on GPUs 0 and 1, rank 1 idles; one lattice's updates
+        assert plan == ((True, 2, [0, 1]) if rank == 0 else (False, 0, None))
+        assert sharded == pytest.approx(256 * 256 * 10 * 4 / (107.0 * 1e6), rel=1e-15)
 
 
 def test_single_process_passthrough():
@@ -57,3 +64,17 @@ def test_single_process_passthrough():
     import bench
     assert bench.max_over_ranks([3.5, 2], None, None) == [3.5, 2.0]
     assert bench.whole_job_updates_per_ns(1, 1 << 18, 10, 10, 1000.0) == (1 << 36) * 100 / 1e9
+    assert bench.rank_plan(0, 1, "slabs") == (True, 0, None) and bench.rank_plan(3, 8, "replicas") == (True, 0, None)
+
+
+def test_slab_partition_for_every_rank_count():
+    """The slab heights --parallel slabs hands to the GPUs at the paper's strong-scaling sizes (Table 3:
+    L = 2^19 and 2^20 on 1..64 GPUs): equal, even, adding up to L (host arithmetic of the C ABI, no GPU)."""
+    sys.path.insert(0, ROOT)
+    from paper_2502_18624_b200 import build as b
+    b.build()
+    import paper_2502_18624_b200 as eng
+    for L in (1 << 18, 1 << 19, 1 << 20):
+        for n in (1, 2, 4, 8, 16, 32, 64):
+            rows = eng.slab_partition(L, n)
+            assert (rows == L // n).all()
