@@ -84,6 +84,7 @@ def parse_args():
                          "'no sharding'); slabs = ONE lattice cut into N row slabs, slab k on GPU k, driven by rank 0 through "
                          "ising_create_slabs with peer access between the GPUs (NEXT-4, PAPER.md:69-89: one process per node "
                          "manages the node's GPUs; strong scaling at fixed L; the other ranks only join the barriers)")
+    ap.add_argument("--sweep-mode", type=int, default=0, help="ising_set_sweep_mode for launch-bound lattices: 0 auto (= 1), 1 CUDA graph, 2 plain launches, 3 persistent cooperative kernel")
     ap.add_argument("--tally", action="store_true", help="A7: keep E, M by the fused tally of the update kernels instead of the observables pass")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -404,6 +405,8 @@ def run_ours(args):
         sim.set_variant(args.variant)
     if args.tally:
         sim.set_tally(True)
+    if args.sweep_mode:
+        sim.set_sweep_mode(args.sweep_mode)
     if args.corr_path:
         sim.set_corr_path(args.corr_path)
 
@@ -515,7 +518,7 @@ def run_ours(args):
                    "seed": base.seed, "sweeps_per_step": S, "observables_every": S,
                    "step": "S sweeps + observables" if args.workload == "sweep" else "S sweeps + correlation protocol + observables",
                    "launch": {"rows_per_thread": args.rows_per_thread or "default", "block": args.block or "default",
-                              "variant": args.variant, "fused_tally": bool(args.tally), "corr_path": args.corr_path,
+                              "variant": args.variant, "fused_tally": bool(args.tally), "corr_path": args.corr_path, "sweep_mode": args.sweep_mode,
                               "slabs": max(1, n_slabs)},
                    "lattice_bytes": L * L * BITS_PER_SITE[model] // 8, "l2": "inputs larger than L2 (no flush needed)" if L * L // 2 > (256 << 20)
                    else "lattice fits L2: DRAM figures not meaningful",

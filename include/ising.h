@@ -112,7 +112,7 @@ int ising_slab_info(const ising_t *h, int slab, int64_t *y0, int64_t *rows, int 
 /* n >= 0 full sweeps: colour 0 then colour 1 ("two update phases"),
  * one Philox number per site, accept iff r < T.  Asynchronous:
  * 2n kernel launches on the handle's stream, no host synchronisation; small
- * lattices (L <= 2048) replay a CUDA graph of 16 sweeps when n >= 32.           */
+ * lattices (L <= 2048) replay a CUDA graph of 16 sweeps when n >= 32 (ising_set_sweep_mode). */
 int ising_sweep(ising_t *h, int64_t n);
 
 /* Full recompute of B, M, Q by warp-shuffle / block reduction over both colour
@@ -233,6 +233,13 @@ int ising_set_launch(ising_t *h, int rows_per_thread, int block_threads);
  * binary search; 2 (LUT model only) = bucket table; equivalent implementations
  * kept for parity / performance comparison).                                */
 int ising_set_variant(ising_t *h, int variant);
+
+/* How ising_sweep runs launch-bound lattices (L <= 2048, unsharded; results never depend on it): 0 = automatic
+ * (= 1), 1 = replay of a CUDA graph of 16 sweeps when n >= 32, 2 = one launch per colour phase, 3 = one
+ * cooperative launch for all n sweeps with a grid-wide barrier after every colour phase (4-bit and 2-bit
+ * models; measured a little slower than the graph; falls back to 1 if the device cannot
+ * keep the grid resident).                                                                                */
+int ising_set_sweep_mode(ising_t *h, int mode);
 
 /* Number of kernels this handle has launched since create.                  */
 int64_t ising_launch_count(const ising_t *h);

@@ -23,6 +23,7 @@ EXPORTS = [
     "ising_bench_copy", "ising_debug_philox", "ising_protocol_distances", "ising_threshold_table",
     "ising_run_protocol_schedule", "ising_create_slabs", "ising_slab_count", "ising_slab_info",
     "ising_write_bits", "ising_read_bits", "ising_slab_partition",
+    "ising_set_sweep_mode",
 ]
 
 
@@ -389,6 +390,10 @@ class IsingSim:
 
     def set_variant(self, variant: int):
         _check(self._lib.ising_set_variant(self._h, variant))
+
+    def set_sweep_mode(self, mode: int):
+        self._lib.ising_set_sweep_mode.argtypes = [C.c_void_p, C.c_int]
+        _check(self._lib.ising_set_sweep_mode(self._h, mode))
 
     def set_corr_path(self, path: int):
         _check(self._lib.ising_set_corr_path(self._h, path))

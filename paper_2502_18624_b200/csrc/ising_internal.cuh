@@ -78,6 +78,7 @@ struct ising_sim {
     cudaGraphExec_t graph_exec = nullptr;
     int graph_key[4] = {0, 0, 0, 0};                          // rows_per_thread, block_threads, variant, tally_on
     bool tally_on = false;                                    // A7: update kernels keep running B, M, Q at d_acc[40..42]
+    int sweep_mode = 0;                                       // small lattices: 0 auto (persistent kernel), 1 CUDA graph, 2 plain launches
     int corr_path = 0;                                        // 0 auto, 1 bit planes (XOR + POPC), 2 tensor cores
     long long *d_corr = nullptr; size_t d_corr_bytes = 0;
     long long *d_rlist = nullptr; size_t d_rlist_bytes = 0;
@@ -142,6 +143,7 @@ static inline int64_t comb_words_per_row(int64_t L, int64_t stride) { return (L 
 // per-slab launchers run on the slab's stream (the caller has switched to the slab's device)
 cudaError_t launch_init(ising_sim *h, int slab);
 cudaError_t launch_update(ising_sim *h, int slab, int colour, uint32_t t);
+cudaError_t launch_sweeps_persistent(ising_sim *h, uint32_t t0, int n_sweeps);   // unsharded small lattices, one cooperative launch
 cudaError_t launch_observables(ising_sim *h, int slab);             // -> slab d_acc[0..2] = B, M, Q of the slab's rows
 cudaError_t launch_sd_hist(ising_sim *h, int slab);                 // -> slab d_acc[8..16]
 SlabDir slab_directory(const ising_sim *h);

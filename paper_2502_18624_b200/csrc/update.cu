@@ -345,22 +345,15 @@ __device__ __forceinline__ void tally_row(const uint4 &x, const uint4 &y, const 
 }
 
 // ----------------------------------------------------------------- kernel ---
+// One thread's share of a colour phase: the rows [chunk R, chunk R + R) of column col, chunk and col from the
+// thread number tid.  Used by the one-phase kernel (update_kernel) and by the persistent kernel of small lattices.
 template <int MODEL, int C, int V, int TALLY>
-__global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ UpdParams p)
+__device__ __forceinline__ void update_chunk(const UpdParams &p, unsigned tid, uint32_t t_eff, const uint32_t *s_tab,
+                                             uint64_t always, int &dB, int &dM, int &dQ)
 {
-    int dB = 0, dM = 0, dQ = 0;                            // TALLY: this thread's share of the changes
-    const uint32_t t_eff = p.t + __ldg(p.t_base);
-    __shared__ __align__(16) uint32_t s_tab[80 + 132];   // both table forms (api.cu)
-    uint64_t always = 0;
     constexpr bool kIsing = MODEL == ISING_MODEL_ISING, kTwoBit = RowFmt<MODEL>::kTwoBit;
-    if (!kIsing) {
-        for (int i = threadIdx.x; i < 80 + 132; i += blockDim.x) s_tab[i] = p.bc_table[i];
-        __syncthreads();
-        always = (uint64_t)s_tab[64] | ((uint64_t)s_tab[65] << 32);
-    }
     const unsigned char *ctab = reinterpret_cast<const unsigned char *>(s_tab + 80);
     const int cols = p.cols, L = p.L;
-    unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
     unsigned chunk = tid / (unsigned)cols;
     int col = (int)(tid - chunk * (unsigned)cols);
     int y0 = (int)chunk * p.R;
@@ -424,13 +417,75 @@ __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ Upd
         o1 += 2 * rs; eo += 2 * rs; w0 += 2 * rs;
     }
     }
+}
+
+// Blume-Capel tables -> shared memory (both forms, api.cu); returns the mask of always-accepted entries
+template <int MODEL>
+__device__ __forceinline__ uint64_t load_tables(const UpdParams &p, uint32_t *s_tab)
+{
+    if (MODEL == ISING_MODEL_ISING) return 0;
+    for (int i = threadIdx.x; i < 80 + 132; i += blockDim.x) s_tab[i] = p.bc_table[i];
+    __syncthreads();
+    return (uint64_t)s_tab[64] | ((uint64_t)s_tab[65] << 32);
+}
+
+template <int MODEL, int C, int V, int TALLY>
+__global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ UpdParams p)
+{
+    int dB = 0, dM = 0, dQ = 0;                            // TALLY: this thread's share of the changes
+    const uint32_t t_eff = p.t + __ldg(p.t_base);
+    __shared__ __align__(16) uint32_t s_tab[80 + 132];
+    const uint64_t always = load_tables<MODEL>(p, s_tab);
+    update_chunk<MODEL, C, V, TALLY>(p, blockIdx.x * blockDim.x + threadIdx.x, t_eff, s_tab, always, dB, dM, dQ);
     if (TALLY) {            // warp sums fit 32 bits (<= 32 lanes x R rows x 32 sites x 8); threads past the lattice add zeros
         const int v[3] = {dB, dM, dQ};
         block_accumulate<3>(v, p.tally);
     }
 }
 
-cudaError_t launch_update(ising_sim *h, int slab, int colour, uint32_t t)
+// ------------------------------------------------------ persistent kernel ---
+// Launch-bound lattices (L <= 2048: a colour phase is a few microseconds of work): ONE cooperative launch runs n
+// sweeps, every block keeping its threads' rows for the whole call, with a grid-wide barrier after each colour
+// phase instead of a kernel boundary.  Same per-thread code (update_chunk), same random numbers, same results.
+// The barrier: a monotonically increasing arrival counter in global memory; thread 0 of a block adds 1 with
+// release semantics after the block's barrier and spins with acquire loads until all blocks of the phase have
+// arrived.  All blocks are co-resident (cooperative launch), so the spin cannot deadlock.
+__device__ __forceinline__ void grid_phase_barrier(unsigned *counter, unsigned &target)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        target += gridDim.x;
+        unsigned seen;
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");
+        } while ((int)(seen - target) < 0);
+    }
+    __syncthreads();
+}
+
+template <int MODEL, int V, int TALLY>
+__global__ void __launch_bounds__(256) sweep_persistent_kernel(const __grid_constant__ UpdParams p0, const __grid_constant__ UpdParams p1,
+                                                               int n_sweeps, unsigned *barrier_counter)
+{
+    int dB = 0, dM = 0, dQ = 0;
+    __shared__ __align__(16) uint32_t s_tab[80 + 132];
+    const uint64_t always = load_tables<MODEL>(p0, s_tab);
+    const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned target = 0;                                   // the counter is zeroed before the launch
+    for (int s = 0; s < n_sweeps; ++s) {
+        update_chunk<MODEL, 0, V, TALLY>(p0, tid, p0.t + (uint32_t)s, s_tab, always, dB, dM, dQ);
+        grid_phase_barrier(barrier_counter, target);
+        update_chunk<MODEL, 1, V, TALLY>(p1, tid, p1.t + (uint32_t)s, s_tab, always, dB, dM, dQ);
+        grid_phase_barrier(barrier_counter, target);
+    }
+    if (TALLY) {            // <= 32 lanes x 2 rows x 32 sites x 8 x 2 n_sweeps: launch_sweeps_persistent caps n_sweeps
+        const int v[3] = {dB, dM, dQ};
+        block_accumulate<3>(v, p0.tally);
+    }
+}
+
+static UpdParams fill_update_params(ising_sim *h, int slab, int colour, uint32_t t)
 {
     UpdParams p;
     const Slab &sl = h->slabs[slab];
@@ -451,16 +506,29 @@ cudaError_t launch_update(ising_sim *h, int slab, int colour, uint32_t t)
     p.Kc = ONES * (8u - (T4 == 0 ? 1u : 0u) - (T8 == 0 ? 1u : 0u));
     p.bc_table = sl.d_table;
     p.rk = h->rk;
-    int64_t chunks = (L + p.R - 1) / p.R;
-    int64_t threads = chunks * p.cols;
-    int block = h->block_threads;
-    unsigned grid = (unsigned)((threads + block - 1) / block);
     p.tally = sl.d_acc + 40;
     p.t_base = reinterpret_cast<const uint32_t *>(sl.d_acc + 48) + (h->graph_capture ? 1 : 0);   // [0] stays 0, [1] = base of a graph replay
-    bool never = false;                           // Blume-Capel: a threshold that is exactly 0 -> compare/select form
+    return p;
+}
+
+// 0 = carry forms; 1 = compare/select (asked for, or a Blume-Capel threshold that is exactly 0)
+static int effective_variant(const ising_sim *h)
+{
+    bool never = false;
     if (is_blume_capel(h->model))
         for (int i = 0; i < h->n_T; ++i) never = never || h->T[i] == 0;
-    const int v = (h->variant == 0 && !never) ? 0 : 1;
+    return (h->variant == 0 && !never) ? 0 : 1;
+}
+
+cudaError_t launch_update(ising_sim *h, int slab, int colour, uint32_t t)
+{
+    const UpdParams p = fill_update_params(h, slab, colour, t);
+    const Slab &sl = h->slabs[slab];
+    const int64_t chunks = (sl.rows + p.R - 1) / p.R;
+    const int64_t threads = chunks * p.cols;
+    const int block = h->block_threads;
+    const unsigned grid = (unsigned)((threads + block - 1) / block);
+    const int v = effective_variant(h);
 #define LAUNCH_UPD(MODEL, C, V, T) update_kernel<MODEL, C, V, T><<<grid, block, 0, sl.stream>>>(p)
 #define PICK_T(MODEL, C, V) do { if (h->tally_on) LAUNCH_UPD(MODEL, C, V, 1); else LAUNCH_UPD(MODEL, C, V, 0); } while (0)
 #define PICK_V(MODEL, C) do { if (v == 0) PICK_T(MODEL, C, 0); else PICK_T(MODEL, C, 1); } while (0)
@@ -472,6 +540,42 @@ cudaError_t launch_update(ising_sim *h, int slab, int colour, uint32_t t)
 #undef LAUNCH_UPD
     h->launches++;
     return cudaGetLastError();
+}
+
+// n sweeps t0, t0 + 1, ... of an unsharded small lattice in one cooperative launch (see sweep_persistent_kernel).
+// Returns cudaErrorNotSupported when the device cannot keep the whole grid resident (the caller then launches
+// phase by phase).
+cudaError_t launch_sweeps_persistent(ising_sim *h, uint32_t t0, int n_sweeps)
+{
+    UpdParams p0 = fill_update_params(h, 0, 0, t0), p1 = fill_update_params(h, 0, 1, t0);
+    p0.R = p1.R = 2;                                            // one row pair per thread: as many threads as the lattice gives
+    p0.t_base = p1.t_base = reinterpret_cast<const uint32_t *>(h->d_acc + 48);
+    const int64_t threads = (h->L / 2) * p0.cols;
+    int block = 32;                                             // spread the few warps over the SMs ...
+    while (block < 128 && threads / block > 4 * 148) block *= 2;   // ... until every SM has a few blocks
+    const unsigned grid = (unsigned)((threads + block - 1) / block);
+    unsigned *counter = reinterpret_cast<unsigned *>(h->d_acc + 50);
+    const int v = effective_variant(h);
+    const void *fn = nullptr;
+#define PK(MODEL, V, T) reinterpret_cast<const void *>(&sweep_persistent_kernel<MODEL, V, T>)
+#define PICK_PK(MODEL) (v == 0 ? (h->tally_on ? PK(MODEL, 0, 1) : PK(MODEL, 0, 0)) : (h->tally_on ? PK(MODEL, 1, 1) : PK(MODEL, 1, 0)))
+    if (h->model == ISING_MODEL_ISING) fn = PICK_PK(ISING_MODEL_ISING);
+    else if (h->model == ISING_MODEL_BLUME_CAPEL) fn = PICK_PK(ISING_MODEL_BLUME_CAPEL);
+    else fn = PICK_PK(ISING_MODEL_BLUME_CAPEL_2BIT);
+#undef PICK_PK
+#undef PK
+    int per_sm = 0, n_sm = 0, coop = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, block, 0);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, h->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device);
+    if (e != cudaSuccess) return e;
+    if (!coop || (int64_t)grid > (int64_t)per_sm * n_sm) return cudaErrorNotSupported;
+    e = cudaMemsetAsync(counter, 0, sizeof(unsigned), h->stream);
+    if (e != cudaSuccess) return e;
+    void *args[] = {&p0, &p1, &n_sweeps, &counter};
+    e = cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(block), args, 0, h->stream);
+    h->launches++;
+    return e;
 }
 
 // ------------------------------------------------------------------- init ---

@@ -446,7 +446,7 @@ def test_graph_replayed_sweeps_equal_plain_launches(eng, model, L, beta, D):
         for t in range(n + 40):
             oracle.sweep(model, s, beta, D, seed, t)
     with eng.IsingSim(model, L, beta, D, seed) as sim:
-        sim.sweep(n)                                         # graph path
+        sim.sweep(n)                                         # graph path (the automatic mode)
         sim.set_launch(4, 64)
         sim.set_tally(True)
         sim.sweep(40)                                        # rebuilt graph (2 replays + 8 plain), tally kernels
@@ -458,6 +458,44 @@ def test_graph_replayed_sweeps_equal_plain_launches(eng, model, L, beta, D):
         for _ in range(n + 40):
             sim.sweep(1)                                     # plain launches only
         assert (sim.read_lattice() == s).all()
+
+
+@pytest.mark.parametrize("model,L,beta,D", [(ISING, 256, wl.BETA_C, 0.0), (ISING, 64, wl.BETA_C / 0.9, 0.0), (ISING, 1088, wl.BETA_C / 0.5, 0.0),
+                                            (ISING, 2048, wl.BETA_C, 0.0), (BC, 192, 1 / 1.4, 1.0), (BC, 1024, 12.0, 0.5),
+                                            (wl.BLUME_CAPEL_2BIT, 320, 1 / 1.4, 1.0)])
+def test_persistent_sweep_kernel_equals_plain_launches_and_oracle(eng, model, L, beta, D):
+    """Launch-bound lattices, sweep mode 3: ising_sweep(n) runs all n sweeps in ONE cooperative launch with a grid barrier
+    per colour phase.  Lattice, fused tally and observables must equal those of one launch per colour phase (mode 2), of
+    the CUDA graph (mode 1, the automatic choice) and of the oracle; mixing the modes in one trajectory changes nothing."""
+    seed, n = 29, 37
+    om = BC if model == wl.BLUME_CAPEL_2BIT else model
+    s = oracle.init(om, L, seed)
+    tl = oracle.observables(s)
+    for t in range(n):
+        tl = oracle.sweep(om, s, beta, D, seed, t, tl)
+    lats = []
+    for mode in (3, 2, 1):
+        with eng.IsingSim(model, L, beta, D, seed) as sim:
+            sim.set_sweep_mode(mode)
+            sim.set_tally(True)
+            k0 = sim.launch_count()
+            sim.sweep(n)
+            launches = sim.launch_count() - k0
+            a, b = sim.tally(), sim.observables()
+            assert (a.bond_sum, a.M, a.Q) == (b.bond_sum, b.M, b.Q) == tl and b.sweeps_done == n, mode
+            lats.append(sim.read_lattice())
+            if mode == 3:
+                assert launches == 1                                # one kernel for the 37 sweeps
+                sim.sweep(1)                                        # n = 1: a plain pair of launches
+                sim.set_sweep_mode(2)
+                sim.sweep(2)
+                sim.set_sweep_mode(3)
+                sim.sweep(5)
+                s2 = s.copy()
+                for t in range(n, n + 8):
+                    oracle.sweep(om, s2, beta, D, seed, t)
+                assert (sim.read_lattice() == s2).all()
+    assert all((lat == s).all() for lat in lats)
 
 
 def test_run_schedule_matches_stepwise_run(eng):
