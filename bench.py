@@ -84,7 +84,7 @@ def parse_args():
                          "'no sharding'); slabs = ONE lattice cut into N row slabs, slab k on GPU k, driven by rank 0 through "
                          "ising_create_slabs with peer access between the GPUs (NEXT-4, PAPER.md:69-89: one process per node "
                          "manages the node's GPUs; strong scaling at fixed L; the other ranks only join the barriers)")
-    ap.add_argument("--sweep-mode", type=int, default=0, help="ising_set_sweep_mode for launch-bound lattices: 0 auto (= 1), 1 CUDA graph, 2 plain launches, 3 persistent cooperative kernel")
+    ap.add_argument("--sweep-mode", type=int, default=0, help="ising_set_sweep_mode for launch-bound lattices: 0 auto, 1 CUDA graph, 2 plain launches, 3 persistent cooperative kernel, 4 cluster kernel (lattice in DSMEM)")
     ap.add_argument("--tally", action="store_true", help="A7: keep E, M by the fused tally of the update kernels instead of the observables pass")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

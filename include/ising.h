@@ -112,7 +112,8 @@ int ising_slab_info(const ising_t *h, int slab, int64_t *y0, int64_t *rows, int 
 /* n >= 0 full sweeps: colour 0 then colour 1 ("two update phases"),
  * one Philox number per site, accept iff r < T.  Asynchronous:
  * 2n kernel launches on the handle's stream, no host synchronisation; small
- * lattices (L <= 2048) replay a CUDA graph of 16 sweeps when n >= 32 (ising_set_sweep_mode). */
+ * lattices run in one cluster kernel (L <= 512) or replay a CUDA graph of 16 sweeps (L <= 2048, n >= 32);
+ * see ising_set_sweep_mode.                                                                  */
 int ising_sweep(ising_t *h, int64_t n);
 
 /* Full recompute of B, M, Q by warp-shuffle / block reduction over both colour
@@ -235,10 +236,12 @@ int ising_set_launch(ising_t *h, int rows_per_thread, int block_threads);
 int ising_set_variant(ising_t *h, int variant);
 
 /* How ising_sweep runs launch-bound lattices (L <= 2048, unsharded; results never depend on it): 0 = automatic
- * (= 1), 1 = replay of a CUDA graph of 16 sweeps when n >= 32, 2 = one launch per colour phase, 3 = one
- * cooperative launch for all n sweeps with a grid-wide barrier after every colour phase (4-bit and 2-bit
- * models; measured a little slower than the graph; falls back to 1 if the device cannot
- * keep the grid resident).                                                                                */
+ * (4 for L <= 512, else 1), 1 = replay of a CUDA graph of 16 sweeps when n >= 32, 2 = one launch per colour
+ * phase, 3 = one cooperative launch for all n sweeps with a grid-wide barrier after every colour phase
+ * (measured a little slower than the graph), 4 = one thread-block cluster of 16 CTAs that
+ * keeps the lattice in distributed shared memory for all n sweeps, halo rows read from the neighbouring CTA's
+ * shared memory, hardware cluster barrier between the colour phases.  3 and 4: 4-bit and 2-bit models; they
+ * fall back to 1 when the device refuses the launch (4: also when the lattice does not fit the cluster).   */
 int ising_set_sweep_mode(ising_t *h, int mode);
 
 /* Number of kernels this handle has launched since create.                  */

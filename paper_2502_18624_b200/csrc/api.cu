@@ -505,6 +505,18 @@ extern "C" int ising_sweep(ising_t *h, int64_t n)
     // barrier per colour phase (update.cu).  Measured slower than the CUDA graph below (L = 256: 5.95 against 5.5
     // microseconds per sweep): a barrier through L2 costs what a kernel boundary inside a graph costs.
     const bool small = h->L * h->L <= (1ll << 22) && h->slabs.size() == 1;
+    // Tiny lattices (L <= 512; mode 4: whatever fits): one cluster of 16 CTAs keeps the lattice in distributed shared
+    // memory for all n sweeps, the colour phases separated by the hardware cluster barrier (update.cu).
+    if (small && n >= 2 && h->model != ISING_MODEL_ISING_LUT && ((h->sweep_mode == 0 && h->L <= 512) || h->sweep_mode == 4)) {
+        while (n > 0) {
+            const int chunk = (int)std::min<int64_t>(n, 4096);          // bounds the 32-bit per-warp tally sums
+            cudaError_t e = launch_sweeps_cluster(h, (uint32_t)h->t, chunk);
+            if (e == cudaErrorNotSupported) break;
+            if (e != cudaSuccess) return cuda_fail(e, "cluster sweep kernel");
+            h->t += (uint64_t)chunk;
+            n -= chunk;
+        }
+    }
     if (small && n >= 2 && h->sweep_mode == 3 && h->model != ISING_MODEL_ISING_LUT) {
         while (n > 0) {
             const int chunk = (int)std::min<int64_t>(n, 4096);          // bounds the 32-bit per-warp tally sums
@@ -515,7 +527,7 @@ extern "C" int ising_sweep(ising_t *h, int64_t n)
             n -= chunk;
         }
     }
-    if (graph_worthwhile(h, n) && h->sweep_mode <= 1) {
+    if (graph_worthwhile(h, n) && (h->sweep_mode <= 1 || h->sweep_mode >= 3)) {
         int rc = ensure_graph(h);
         if (rc) return rc;
         uint32_t *t_base = reinterpret_cast<uint32_t *>(h->d_acc + 48) + 1;
@@ -588,7 +600,7 @@ extern "C" int ising_set_sweep_mode(ising_t *h, int mode)
 {
     DeviceGuard dev_guard(h);
     if (!h) return set_error(ISING_EINVAL, "ising_set_sweep_mode: NULL handle");
-    if (mode < 0 || mode > 3) return set_error(ISING_EINVAL, "ising_set_sweep_mode: mode must be 0 (auto), 1 (CUDA graph), 2 (plain launches) or 3 (persistent kernel)");
+    if (mode < 0 || mode > 4) return set_error(ISING_EINVAL, "ising_set_sweep_mode: mode must be 0 (auto), 1 (CUDA graph), 2 (plain launches), 3 (persistent kernel) or 4 (cluster kernel)");
     h->sweep_mode = mode;
     return ISING_OK;
 }

@@ -144,6 +144,7 @@ static inline int64_t comb_words_per_row(int64_t L, int64_t stride) { return (L 
 cudaError_t launch_init(ising_sim *h, int slab);
 cudaError_t launch_update(ising_sim *h, int slab, int colour, uint32_t t);
 cudaError_t launch_sweeps_persistent(ising_sim *h, uint32_t t0, int n_sweeps);   // unsharded small lattices, one cooperative launch
+cudaError_t launch_sweeps_cluster(ising_sim *h, uint32_t t0, int n_sweeps);      // tiny lattices: one cluster, lattice in DSMEM
 cudaError_t launch_observables(ising_sim *h, int slab);             // -> slab d_acc[0..2] = B, M, Q of the slab's rows
 cudaError_t launch_sd_hist(ising_sim *h, int slab);                 // -> slab d_acc[8..16]
 SlabDir slab_directory(const ising_sim *h);

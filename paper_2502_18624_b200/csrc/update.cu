@@ -12,6 +12,8 @@
 #include "ising_internal.cuh"
 #include "row_format.cuh"
 
+#include <cooperative_groups.h>
+
 #define ONES 0x11111111u
 
 // Philox counter of call q of a row: gl + q, gl a multiple of 8 (philox_counter: ising_internal.cuh).
@@ -540,6 +542,154 @@ cudaError_t launch_update(ising_sim *h, int slab, int colour, uint32_t t)
 #undef LAUNCH_UPD
     h->launches++;
     return cudaGetLastError();
+}
+
+// ------------------------------------------- cluster kernel (tiny lattices) ---
+// L <= 512: the whole lattice fits the shared memory of one thread-block cluster, and a colour phase is a fraction
+// of a microsecond of arithmetic -- a kernel boundary (even inside a CUDA graph) or a barrier through L2 costs
+// several times that.  ONE cluster of 16 CTAs keeps the lattice in distributed shared memory for all n sweeps:
+// CTA k holds the rows [k L/16, (k+1) L/16) of both colour arrays, a thread updates one 128-bit vector of one row
+// per phase, the row above the first / below the last row of a CTA is read from the neighbouring CTA's shared
+// memory (DSMEM, about 215 cycles), and the phases are separated by the hardware cluster barrier (about 380
+// cycles).  Same row functions, same random numbers (keyed by the global site index), same results.
+namespace cg = cooperative_groups;
+
+struct ClusterParams {
+    uint4 *lat[2];              // the two colour arrays in global memory (read at the start, written back at the end)
+    int L, cols, rows_per_cta, n_sweeps;
+    uint32_t t;
+    UpdParams u;                // thresholds, carry constants, tables, round keys, tally (pointer members of the lattice unused)
+};
+
+template <int MODEL, int C, int V, int TALLY>
+__device__ __forceinline__ void cluster_phase(const ClusterParams &p, char *const *own_c, const char *const *opp_c,
+                                              const char *opp_above, const char *opp_below, uint32_t t_eff,
+                                              const uint32_t *s_tab, uint64_t always, int y_first, int &dB, int &dM, int &dQ)
+{
+    constexpr bool kIsing = MODEL == ISING_MODEL_ISING, kTwoBit = RowFmt<MODEL>::kTwoBit;
+    constexpr int VB = RowFmt<MODEL>::kVecBytes;
+    const unsigned char *ctab = reinterpret_cast<const unsigned char *>(s_tab + 80);
+    const int cols = p.cols, rows = p.rows_per_cta, items = rows * cols, half_items = items >> 1;
+    const size_t rs = (size_t)cols * VB;
+    char *own = *own_c;
+    const char *opp = *opp_c;
+    // items ordered so that a warp works on rows of one parity: first all even local rows, then all odd ones
+    for (int i = threadIdx.x; i < items; i += blockDim.x) {
+        const int par = i >= half_items, j = par ? i - half_items : i;
+        const int yl = 2 * (j / cols) + par, col = j - (j / cols) * cols;
+        const size_t cb = (size_t)col * VB;
+        const uint4 src = load_row<MODEL>(own + yl * rs + cb);
+        const uint4 sm = load_row<MODEL>(opp + yl * rs + cb);
+        const uint4 up = load_row<MODEL>(yl == 0 ? opp_above + cb : opp + (yl - 1) * rs + cb);
+        const uint4 dn = load_row<MODEL>(yl == rows - 1 ? opp_below + cb : opp + (yl + 1) * rs + cb);
+        const uint64_t g0 = (uint64_t)(y_first + yl) * (uint64_t)(cols * 8) + (uint64_t)(col * 8);
+        uint4 o;
+        // y_first is even, so the row parity (y + C) & 1 is C for par = 0 and 1 - C for par = 1
+        if (par == 0) {
+            const uint32_t edge = *reinterpret_cast<const uint32_t *>(opp + yl * rs + (size_t)edge_half<MODEL, C>(col, cols) * 4);
+            if (kIsing) o = ising_row<C, V>(src, up, sm, dn, edge, g0, t_eff, C, p.u);
+            else if (kTwoBit) o = bc2_row<C, V>(src, up, sm, dn, edge, g0, t_eff, C, p.u, ctab, s_tab, always);
+            else if (V == 0) o = bc_row_carry<C>(src, up, sm, dn, edge, g0, t_eff, C, p.u, ctab);
+            else o = bc_row<C>(src, up, sm, dn, edge, g0, t_eff, C, p.u, s_tab, always);
+            if (TALLY) tally_row<MODEL, C>(src, o, up, sm, dn, edge, dB, dM, dQ);
+        } else {
+            const uint32_t edge = *reinterpret_cast<const uint32_t *>(opp + yl * rs + (size_t)edge_half<MODEL, 1 - C>(col, cols) * 4);
+            if (kIsing) o = ising_row<1 - C, V>(src, up, sm, dn, edge, g0, t_eff, C, p.u);
+            else if (kTwoBit) o = bc2_row<1 - C, V>(src, up, sm, dn, edge, g0, t_eff, C, p.u, ctab, s_tab, always);
+            else if (V == 0) o = bc_row_carry<1 - C>(src, up, sm, dn, edge, g0, t_eff, C, p.u, ctab);
+            else o = bc_row<1 - C>(src, up, sm, dn, edge, g0, t_eff, C, p.u, s_tab, always);
+            if (TALLY) tally_row<MODEL, 1 - C>(src, o, up, sm, dn, edge, dB, dM, dQ);
+        }
+        store_row<MODEL>(own + yl * rs + cb, o);
+    }
+}
+
+template <int MODEL, int V, int TALLY>
+__global__ void __launch_bounds__(1024) sweep_cluster_kernel(const __grid_constant__ ClusterParams p)
+{
+    extern __shared__ __align__(16) char s_lat[];           // [colour 0 rows | colour 1 rows] of this CTA
+    __shared__ __align__(16) uint32_t s_tab[80 + 132];
+    cg::cluster_group cluster = cg::this_cluster();
+    const unsigned rank = cluster.block_rank(), nc = cluster.num_blocks();
+    constexpr int VB = RowFmt<MODEL>::kVecBytes;
+    const size_t rs = (size_t)p.cols * VB, colour_bytes = (size_t)p.rows_per_cta * rs;
+    const int y_first = (int)rank * p.rows_per_cta;
+    const uint64_t always = load_tables<MODEL>(p.u, s_tab);
+    // global -> shared
+    for (int c = 0; c < 2; ++c) {
+        const uint4 *src = reinterpret_cast<const uint4 *>(reinterpret_cast<const char *>(p.lat[c]) + (size_t)y_first * rs);
+        uint4 *dst = reinterpret_cast<uint4 *>(s_lat + c * colour_bytes);
+        for (int i = threadIdx.x; i < (int)(colour_bytes / 16); i += blockDim.x) dst[i] = src[i];
+    }
+    char *mine[2] = {s_lat, s_lat + colour_bytes};
+    // halo rows in the neighbouring CTAs' shared memory: last row of the CTA above, first row of the CTA below
+    const char *above[2], *below[2];
+    for (int c = 0; c < 2; ++c) {
+        above[c] = reinterpret_cast<const char *>(cluster.map_shared_rank(mine[c], (rank + nc - 1) % nc)) + (size_t)(p.rows_per_cta - 1) * rs;
+        below[c] = reinterpret_cast<const char *>(cluster.map_shared_rank(mine[c], (rank + 1) % nc));
+    }
+    cluster.sync();
+    int dB = 0, dM = 0, dQ = 0;
+    const char *opp0 = mine[1], *opp1 = mine[0];
+    for (int s = 0; s < p.n_sweeps; ++s) {
+        cluster_phase<MODEL, 0, V, TALLY>(p, &mine[0], &opp0, above[1], below[1], p.t + (uint32_t)s, s_tab, always, y_first, dB, dM, dQ);
+        cluster.sync();
+        cluster_phase<MODEL, 1, V, TALLY>(p, &mine[1], &opp1, above[0], below[0], p.t + (uint32_t)s, s_tab, always, y_first, dB, dM, dQ);
+        cluster.sync();
+    }
+    for (int c = 0; c < 2; ++c) {
+        uint4 *dst = reinterpret_cast<uint4 *>(reinterpret_cast<char *>(p.lat[c]) + (size_t)y_first * rs);
+        const uint4 *src = reinterpret_cast<const uint4 *>(s_lat + c * colour_bytes);
+        for (int i = threadIdx.x; i < (int)(colour_bytes / 16); i += blockDim.x) dst[i] = src[i];
+    }
+    if (TALLY) {
+        const int v[3] = {dB, dM, dQ};
+        block_accumulate<3>(v, p.u.tally);
+    }
+}
+
+// n sweeps of an unsharded lattice whose slabs fit the shared memory of one cluster.  cudaErrorNotSupported: the
+// lattice is too large for it (or the launch is refused); the caller falls back to the graph / plain launches.
+cudaError_t launch_sweeps_cluster(ising_sim *h, uint32_t t0, int n_sweeps)
+{
+    const int nc = 16;
+    ClusterParams p;
+    p.u = fill_update_params(h, 0, 0, t0);
+    p.u.t_base = reinterpret_cast<const uint32_t *>(h->d_acc + 48);
+    p.lat[0] = reinterpret_cast<uint4 *>(h->lat[0]); p.lat[1] = reinterpret_cast<uint4 *>(h->lat[1]);
+    p.L = (int)h->L; p.cols = (int)(h->L / 64); p.n_sweeps = n_sweeps; p.t = t0;
+    if (h->L % (2 * nc)) return cudaErrorNotSupported;
+    p.rows_per_cta = (int)(h->L / nc);
+    const size_t smem = (size_t)2 * p.rows_per_cta * colour_row_words(h) * 8;
+    if (smem > 200 * 1024) return cudaErrorNotSupported;
+    const int items = p.rows_per_cta * p.cols;
+    int block = 32;
+    while (block < items && block < 1024) block *= 2;
+    const int v = effective_variant(h);
+    const void *fn = nullptr;
+#define CK(MODEL, V, T) reinterpret_cast<const void *>(&sweep_cluster_kernel<MODEL, V, T>)
+#define PICK_CK(MODEL) (v == 0 ? (h->tally_on ? CK(MODEL, 0, 1) : CK(MODEL, 0, 0)) : (h->tally_on ? CK(MODEL, 1, 1) : CK(MODEL, 1, 0)))
+    if (h->model == ISING_MODEL_ISING) fn = PICK_CK(ISING_MODEL_ISING);
+    else if (h->model == ISING_MODEL_BLUME_CAPEL) fn = PICK_CK(ISING_MODEL_BLUME_CAPEL);
+    else fn = PICK_CK(ISING_MODEL_BLUME_CAPEL_2BIT);
+#undef PICK_CK
+#undef CK
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) { cudaGetLastError(); return cudaErrorNotSupported; }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(nc); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = h->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = nc; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    int max_clusters = 0;
+    e = cudaOccupancyMaxActiveClusters(&max_clusters, fn, &cfg);
+    if (e != cudaSuccess || max_clusters < 1) { cudaGetLastError(); return cudaErrorNotSupported; }
+    void *args[] = {&p};
+    e = cudaLaunchKernelExC(&cfg, fn, args);
+    h->launches++;
+    return e;
 }
 
 // n sweeps t0, t0 + 1, ... of an unsharded small lattice in one cooperative launch (see sweep_persistent_kernel).

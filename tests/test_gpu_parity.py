@@ -464,8 +464,9 @@ def test_graph_replayed_sweeps_equal_plain_launches(eng, model, L, beta, D):
                                             (ISING, 2048, wl.BETA_C, 0.0), (BC, 192, 1 / 1.4, 1.0), (BC, 1024, 12.0, 0.5),
                                             (wl.BLUME_CAPEL_2BIT, 320, 1 / 1.4, 1.0)])
 def test_persistent_sweep_kernel_equals_plain_launches_and_oracle(eng, model, L, beta, D):
-    """Launch-bound lattices, sweep mode 3: ising_sweep(n) runs all n sweeps in ONE cooperative launch with a grid barrier
-    per colour phase.  Lattice, fused tally and observables must equal those of one launch per colour phase (mode 2), of
+    """Launch-bound lattices.  Sweep mode 4 (automatic for L <= 512): ONE cluster of 16 CTAs keeps the lattice in
+    distributed shared memory for all n sweeps, colour phases separated by the hardware cluster barrier.  Sweep mode 3:
+    ising_sweep(n) runs all n sweeps in ONE cooperative launch with a grid barrier per colour phase.  Lattice, fused tally and observables must equal those of one launch per colour phase (mode 2), of
     the CUDA graph (mode 1, the automatic choice) and of the oracle; mixing the modes in one trajectory changes nothing."""
     seed, n = 29, 37
     om = BC if model == wl.BLUME_CAPEL_2BIT else model
@@ -474,7 +475,7 @@ def test_persistent_sweep_kernel_equals_plain_launches_and_oracle(eng, model, L,
     for t in range(n):
         tl = oracle.sweep(om, s, beta, D, seed, t, tl)
     lats = []
-    for mode in (3, 2, 1):
+    for mode in (4, 3, 2, 1):                                    # 4: one cluster, lattice in distributed shared memory
         with eng.IsingSim(model, L, beta, D, seed) as sim:
             sim.set_sweep_mode(mode)
             sim.set_tally(True)
@@ -484,12 +485,12 @@ def test_persistent_sweep_kernel_equals_plain_launches_and_oracle(eng, model, L,
             a, b = sim.tally(), sim.observables()
             assert (a.bond_sum, a.M, a.Q) == (b.bond_sum, b.M, b.Q) == tl and b.sweeps_done == n, mode
             lats.append(sim.read_lattice())
-            if mode == 3:
+            if mode in (3, 4):
                 assert launches == 1                                # one kernel for the 37 sweeps
                 sim.sweep(1)                                        # n = 1: a plain pair of launches
                 sim.set_sweep_mode(2)
                 sim.sweep(2)
-                sim.set_sweep_mode(3)
+                sim.set_sweep_mode(mode)
                 sim.sweep(5)
                 s2 = s.copy()
                 for t in range(n, n + 8):
