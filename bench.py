@@ -415,14 +415,18 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize(device)
 
+    done = [0]
+
     def step(ev=None):
         if ev:
             ev[0].record()
         sim.sweep(S)
+        done[0] += S
         if ev:
             ev[1].record()
-        if args.workload == "corr":
-            sim.correlation_protocol()             # r <= 32 all sources + stride-16 sources up to L/2
+        if args.workload == "corr":                # A11: the protocol at this time, one native call (no sweeps left to do):
+            _, obs = sim.run_protocol_schedule([done[0]])      # r <= 32 all sources + stride-16 sources up to L/2, and B, M, Q
+            return obs[0]
         return sim.tally() if args.tally else sim.observables()
 
     for _ in range(W):

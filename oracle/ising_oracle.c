@@ -20,7 +20,11 @@
  * vectors, closed-form thresholds, tally == recompute invariant, exact
  * enumeration of 4x4 Ising / 3x3 + 4x4 Blume-Capel, Onsager energy and
  * magnetisation, crafted-lattice closed forms for observables, brute force and
- * sum identities for correlation, Schwinger-Dyson -> 1.  Section O7 (the
+ * sum identities for correlation, Schwinger-Dyson -> 1; the row-band forms of
+ * the observables and of the histogram (orc_observables_rows, orc_sd_hist_rows:
+ * for lattices streamed out of the GPU in bands) by "the bands of any partition
+ * add up to the full-lattice routine" and a python double loop; the time grid and
+ * the Sec. 3.3 lists also by exact integer criteria (tests/test_oracle_correlation.py).  Section O7 (the
  * paper's 1-bit look-up-table kernel, tests/test_oracle_lut.py): table
  * marginals / independence / closed forms, getMaxLE against a library
  * search, per-word sweep == independently written per-site sweep, tally ==

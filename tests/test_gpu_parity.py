@@ -261,7 +261,9 @@ def test_argument_errors(eng):
     with pytest.raises(eng.IsingError):
         eng.IsingSim(ISING, 100, 0.4)              # L not a multiple of 64
     with pytest.raises(eng.IsingError):
-        eng.IsingSim(2, 64, 0.4)                   # unknown model
+        eng.IsingSim(2, 64, 0.4)                   # the 1-bit model needs L % 256 == 0
+    with pytest.raises(eng.IsingError):
+        eng.IsingSim(7, 256, 0.4)                  # unknown model
     with pytest.raises(eng.IsingError):
         eng.IsingSim(ISING, 64, -0.1)              # beta < 0
     with pytest.raises(eng.IsingError):

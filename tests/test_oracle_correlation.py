@@ -102,6 +102,39 @@ def test_protocol_lists(golden_dir):
                 assert r[r > rc][0] == want
 
 
+def test_time_grid_and_log_grid_exact_integer_criteria():
+    """Pins that need no floating point: t = nearest integer to 2^(x/8) <=> (2t - 1)^8 <= 2^(x+8) < (2t + 1)^8, and
+    d = floor(2^(x/32)) <=> d^32 <= 2^x < (d + 1)^32, in Python integers."""
+    tg = [int(t) for t in oracle.time_grid(1 << 20)]
+    x, want = 1, []
+    while True:
+        t = max(1, round(2.0 ** (x / 8.0)))
+        while (2 * t + 1) ** 8 <= 2 ** (x + 8):
+            t += 1
+        while (2 * t - 1) ** 8 > 2 ** (x + 8):
+            t -= 1
+        if t > 1 << 20:
+            break
+        if not want or want[-1] != t:
+            want.append(t)
+        x += 1
+    assert tg == want
+    L = 1 << 20
+    r, st = oracle.protocol_list(L, 1)
+    rc = oracle.protocol_rc(L, 1)
+    grid, x = [], 0
+    while 2 ** x <= (L // 2) ** 32:
+        d = int(2.0 ** (x / 32.0))
+        while (d + 1) ** 32 <= 2 ** x:
+            d += 1
+        while d ** 32 > 2 ** x:
+            d -= 1
+        if d > rc and (not grid or grid[-1] != d):
+            grid.append(d)
+        x += 1
+    assert [int(v) for v in r[r > rc]] == grid
+
+
 def test_protocol_structure():
     L, t = 1 << 16, 100
     r, st = oracle.protocol_list(L, t)
