@@ -677,3 +677,36 @@ def test_bit_transport_format(eng, model, L, slabs):
         with eng.IsingSim(ISING, 192, beta) as c:
             with pytest.raises(eng.IsingError):
                 c.read_bits(0, 0, 1)
+
+
+@pytest.mark.parametrize("model", [ISING, BC, wl.ISING_LUT])
+def test_run_protocol_schedule_matches_oracle(eng, model):
+    """A11 with the correlation measurement in one native call: at every time of the schedule the
+    rows (r, S_x, S_y, n_src) and B, M, Q equal the oracle's protocol and observables on the oracle's own trajectory."""
+    L, seed = 1024, 6
+    beta, D = (1 / 1.4, 1.0) if model == BC else (wl.BETA_C / 0.5, 0.0)
+    times = [1, 2, 5, 9]
+    if model == wl.ISING_LUT:
+        s = oracle.lut_init(L, seed)
+        step = lambda t: oracle.lut_sweep(s, beta, seed, t)
+    else:
+        s = oracle.init(model, L, seed)
+        step = lambda t: oracle.sweep(model, s, beta, D, seed, t)
+    with eng.IsingSim(model, L, beta, D, seed) as sim:
+        rows, obs = sim.run_protocol_schedule(times)
+        t = 0
+        for k, tt in enumerate(times):
+            while t < tt:
+                step(t)
+                t += 1
+            orr, ox, oy, on = oracle.correlation_protocol(s, tt)
+            r, sx, sy, ns = rows[k]
+            assert (r == orr).all() and (sx == ox).all() and (sy == oy).all() and (ns == on).all(), tt
+            assert (obs[k].bond_sum, obs[k].M, obs[k].Q) == oracle.observables(s) and obs[k].sweeps_done == tt
+        with pytest.raises(eng.IsingError):
+            sim.run_protocol_schedule([3])                       # earlier than sweeps_done
+        lib, n = eng.load_library(), __import__("ctypes").c_int64(0)
+        tm = np.array([20], dtype=np.uint64)
+        buf = [np.zeros(8, dtype=np.int64) for _ in range(5)]
+        assert lib.ising_run_protocol_schedule(sim._h, 1, tm.ctypes.data, 8, *(b.ctypes.data for b in buf), None) == -1   # cap too small
+        assert sim.observables().sweeps_done == 9                # nothing was swept
