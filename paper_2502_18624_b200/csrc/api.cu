@@ -196,7 +196,6 @@ static int finish_create(ising_sim *h, ising_t **out)
     }
     const Slab &s0 = h->slabs[0];
     h->lat[0] = s0.lat[0]; h->lat[1] = s0.lat[1]; h->d_acc = s0.d_acc; h->d_bc_table = s0.d_table;
-    h->lut_buckets = s0.lut_buckets;
     *out = h;
     return ISING_OK;
 }

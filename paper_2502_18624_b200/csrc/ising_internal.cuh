@@ -46,7 +46,7 @@ struct SlabDir {
 };
 
 struct ising_sim {
-    std::vector<Slab> slabs;                // >= 1; slabs[0] aliases lat / d_acc / d_bc_table / stream below
+    std::vector<Slab> slabs;                // >= 1; lat / d_acc / d_bc_table / stream below are slab 0's (single-slab code paths)
     int model = 0;
     int64_t L = 0;
     double beta = 0, D = 0;
@@ -55,7 +55,6 @@ struct ising_sim {
     cudaStream_t stream = nullptr;
     int device = -1;  // CUDA device of the lattice (the current device at ising_create, or dev_buf's)
     uint64_t *lat[2] = {nullptr, nullptr};  // black, white colour arrays (device)
-    void *owned = nullptr;                  // non-null if the library allocated dev_buf
     long long *d_acc = nullptr;             // 64 int64 accumulators inside the scratch area
     long long *h_acc = nullptr;             // pinned mirror
     uint64_t T[54] = {};                    // thresholds in [0, 2^32]
@@ -70,7 +69,6 @@ struct ising_sim {
     cudaEvent_t io_event = nullptr;                           // kernels must not queue behind another handle's sweeps)
     uint64_t *planes = nullptr; size_t planes_bytes = 0;      // bit planes for the correlation
     uint64_t *comb = nullptr; size_t comb_bytes = 0;          // planes down-sampled to the source comb (stride >= 2)
-    void *lut_buckets = nullptr;                              // LUT model: 4096 x {C, meta} bucket table (cudaMalloc)
     int8_t *gram = nullptr; size_t gram_bytes = 0;            // L x L int8 spin matrix for the tensor-core correlation
     // CUDA graph of K sweeps for launch-bound (small) lattices: kernels baked with t = 0..K-1, the base
     // sweep number lives in device memory (d_acc[48] as two uint32: [0] = 0 for plain launches, [1] = base)
@@ -78,8 +76,8 @@ struct ising_sim {
     cudaGraphExec_t graph_exec = nullptr;
     int graph_key[4] = {0, 0, 0, 0};                          // rows_per_thread, block_threads, variant, tally_on
     bool tally_on = false;                                    // A7: update kernels keep running B, M, Q at d_acc[40..42]
-    int sweep_mode = 0;                                       // small lattices: 0 auto (persistent kernel), 1 CUDA graph, 2 plain launches
-    int corr_path = 0;                                        // 0 auto, 1 bit planes (XOR + POPC), 2 tensor cores
+    int sweep_mode = 0;                                       // small lattices (ising_set_sweep_mode): 0 auto, 1 graph, 2 plain, 3 persistent, 4 cluster
+    int corr_path = 0;                                        // ising_set_corr_path: 0 auto, 1 bit planes, 2-4 tensor cores
     long long *d_corr = nullptr; size_t d_corr_bytes = 0;
     long long *d_rlist = nullptr; size_t d_rlist_bytes = 0;
 };
