@@ -52,10 +52,21 @@ def test_null_handle_errors(lib):
     assert lib.ising_create(0, 64, -1.0, 0.0, 1, None, 0, None, C.byref(out)) == -1
     assert lib.ising_create(0, 64, 0.4, 0.0, 1, None, 0, None, None) == -1
     assert lib.ising_create(2, 192, 0.4, 0.0, 1, None, 0, None, C.byref(out)) == -1      # LUT model: L % 256
+    lib.ising_create_slabs.argtypes = [C.c_int, C.c_int64, C.c_double, C.c_double, C.c_uint64, C.c_int, C.c_void_p, C.c_void_p,
+                                       C.c_void_p, C.POINTER(C.c_void_p)]
+    assert lib.ising_create_slabs(0, 100, 0.4, 0.0, 1, 2, None, None, None, C.byref(out)) == -1   # bad L, before any CUDA call
+    assert lib.ising_create_slabs(0, 256, 0.4, 0.0, 1, 0, None, None, None, C.byref(out)) == -1   # no slab
+    assert lib.ising_create_slabs(0, 256, 0.4, 0.0, 1, 2, None, None, None, None) == -1
+    assert lib.ising_slab_count(None) == 0
     for fn, args in [(lib.ising_set_tally, (None, 1)), (lib.ising_tally, (None, None)), (lib.ising_set_corr_path, (None, 1)),
                      (lib.ising_run_schedule, (None, 0, None, None)), (lib.ising_correlation, (None, 1, None, None)),
                      (lib.ising_set_variant, (None, 0)), (lib.ising_set_launch, (None, 0, 0)),
-                     (lib.ising_time_grid, (10, None, 0, None))]:
+                     (lib.ising_time_grid, (10, None, 0, None)), (lib.ising_write_bits, (None, 0, 0, 1, None)),
+                     (lib.ising_read_bits, (None, 0, 0, 1, None)), (lib.ising_set_sweep_mode, (None, 0)),
+                     (lib.ising_run_protocol_schedule, (None, 0, None, 0, None, None, None, None, None, None)),
+                     (lib.ising_slab_info, (None, 0, None, None, None)), (lib.ising_slab_partition, (256, 2, None)),
+                     (lib.ising_protocol_distances, (256, 1, 0, None, None, None)),
+                     (lib.ising_threshold_table, (0, 0.4, 0.0, None, 0, None))]:
         assert fn(*args) == -1, fn.__name__
         assert len(lib.ising_last_error()) > 0
 
