@@ -27,10 +27,11 @@ cpu_baseline = the oracle, as it stands, timed on the host cores on a bounded sa
 
 N > 1 (torchrun): by default N independent replicas (seed + rank), weak scaling, no
 collective on the data path (north_star: "one GPU, no sharding"); barrier + max-over-
-ranks timing only.  --parallel slabs runs ONE lattice cut into N row slabs, slab k on
-GPU k (NEXT-4, ising_create_slabs), driven by rank 0: strong scaling.
-Unmeasured on hardware: this run's boxes have one GPU (--slabs S cuts the lattice into
-S slabs on the one GPU: same code path, same streams and events).
+ranks timing only.  --parallel slabs runs ONE lattice cut into N row slabs, rank k owning
+slab k (NEXT-4, ising_create_part): halo rows by peer loads through CUDA
+IPC, one NCCL all-reduce of a word between colour phases, strong scaling.  Unmeasured across
+GPUs: this run's boxes have one (tests/test_gpu_parts.py runs the same protocol with 2 and
+3 processes on one GPU; --slabs S cuts the lattice into S slabs inside one process).
 """
 from __future__ import annotations
 
@@ -81,9 +82,9 @@ def parse_args():
                                                           "read from the neighbours; all on this GPU unless --gpus-as-slabs)")
     ap.add_argument("--parallel", default="replicas", choices=["replicas", "slabs"],
                     help="N > 1: replicas = N independent lattices, one per rank (weak scaling; the default, north_star's "
-                         "'no sharding'); slabs = ONE lattice cut into N row slabs, slab k on GPU k, driven by rank 0 through "
-                         "ising_create_slabs with peer access between the GPUs (NEXT-4, PAPER.md:69-89: one process per node "
-                         "manages the node's GPUs; strong scaling at fixed L; the other ranks only join the barriers)")
+                         "'no sharding'); slabs = ONE lattice cut into N row slabs, rank k owns slab k (ising_create_part), halo "
+                         "rows read from the neighbouring ranks' memory through CUDA IPC, one NCCL all-reduce of a word between "
+                         "colour phases (NEXT-4, PAPER.md:69-89; strong scaling at fixed L)")
     ap.add_argument("--sweep-mode", type=int, default=0, help="ising_set_sweep_mode for launch-bound lattices: 0 auto, 1 CUDA graph, 2 plain launches, 3 persistent cooperative kernel, 4 cluster kernel (lattice in DSMEM)")
     ap.add_argument("--tally", action="store_true", help="A7: keep E, M by the fused tally of the update kernels instead of the observables pass")
     ap.add_argument("--no-e2e", action="store_true")
@@ -354,12 +355,22 @@ def whole_job_updates_per_ns(world: int, L: int, sweeps: int, steps: int, total_
     return lattices * L * L * sweeps * steps / (total_ms * 1e6)
 
 
-def rank_plan(rank: int, world: int, parallel: str):
-    """(drives a simulation?, slabs, slab devices) of one rank.  replicas: every rank its own unsharded lattice on
-    its own GPU.  slabs (N > 1): rank 0 drives one lattice whose slab k lives on GPU k; the others idle."""
+def rank_plan(rank: int, world: int, parallel: str, heights):
+    """(seed offset, (y0, rows) or None) of one rank.  replicas: every rank its own unsharded lattice (seed + rank).
+    slabs (N > 1): ONE lattice, the same seed everywhere; rank k owns the k-th slab of `heights` (ising_slab_partition)
+    as a part handle (ising_create_part)."""
     if parallel == "slabs" and world > 1:
-        return (rank == 0, world, list(range(world))) if rank == 0 else (False, 0, None)
-    return True, 0, None
+        return 0, (int(sum(heights[:rank])), int(heights[rank]))
+    return rank, None
+
+
+def attach_neighbours(sim, rank: int, world: int, heights, all_gather_object):
+    """--parallel slabs: exchange the 64-byte CUDA IPC handles of the slab allocations (an all-gather through
+    torch.distributed) and map the slab above and the slab below (periodic)."""
+    handles = [None] * world
+    all_gather_object(handles, sim.part_export())
+    up, dn = (rank - 1) % world, (rank + 1) % world
+    sim.part_attach(handles[up], int(heights[up]), handles[dn], int(heights[dn]))
 
 
 def replica_seed(base_seed: int, rank: int) -> int:
@@ -379,26 +390,30 @@ def run_ours(args):
     if world > 1:
         import torch.distributed as dist
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+        if os.environ.get("ISING_BENCH_RANKS_ON_ONE_GPU") == "1":
+            # test hook (tests/test_gpu_parts.py): a box with one GPU runs all ranks on cuda:0 over gloo, whose
+            # collectives order the ranks on the host -- NCCL refuses two ranks on one GPU, and kernels of different
+            # processes must not wait for one another there.  Not a measurement mode.
+            local = 0
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     device = torch.device(f"cuda:{local}")
     torch.cuda.set_device(device)
 
     base, L, name = pick_workload(args)
     model = MODEL_IDS[args.model]
     S, K, W = args.sweeps_per_step, args.steps, max(args.warmup, 0)
-    drives, n_slabs, slab_devices = rank_plan(rank, world, args.parallel)
-    if args.slabs > 1 and not n_slabs:
-        n_slabs = args.slabs                                   # several slabs on this rank's own GPU
-    if not drives:                                             # --parallel slabs: ranks > 0 only keep the barriers company
-        for _ in range(2):
-            dist.barrier()
-            torch.cuda.synchronize(device)
-        max_over_ranks([0.0, 0.0], dist, device)
-        dist.barrier()
-        dist.destroy_process_group()
-        return
-    sim = eng.IsingSim(model, L, base.beta, base.D, replica_seed(base.seed, rank), device=device,
-                       slabs=n_slabs if n_slabs > 1 else None, slab_devices=slab_devices)
+    sharded = args.parallel == "slabs" and world > 1
+    heights = eng.slab_partition(L, world) if sharded else None
+    seed_offset, part = rank_plan(rank, world, args.parallel, heights)
+    n_slabs = args.slabs if (args.slabs > 1 and not sharded) else 0       # several slabs on this rank's own GPU
+    sim = eng.IsingSim(model, L, base.beta, base.D, base.seed + seed_offset, device=device,
+                       slabs=n_slabs if n_slabs > 1 else None, part=part)
+    if sharded:
+        attach_neighbours(sim, rank, world, heights, dist.all_gather_object)
+        phase_flag = torch.zeros(1, dtype=torch.int32, device=device)
+        sums = torch.zeros(3, dtype=torch.int64, device=device)
     if args.rows_per_thread or args.block:
         sim.set_launch(args.rows_per_thread, args.block)
     if args.variant:
@@ -420,10 +435,25 @@ def run_ours(args):
     def step(ev=None):
         if ev:
             ev[0].record()
-        sim.sweep(S)
+        if sharded:
+            # one lattice on N GPUs: a colour phase may start when the previous phase of both neighbours is done; the
+            # NCCL all-reduce of one word is enqueued behind this rank's phase and ahead of its next one (stream-ordered,
+            # no host synchronisation) and completes only when every rank has reached it
+            for _ in range(S):
+                for c in (0, 1):
+                    sim.sweep_phase(c)
+                    dist.all_reduce(phase_flag)
+        else:
+            sim.sweep(S)
         done[0] += S
         if ev:
             ev[1].record()
+        if sharded:                                # the parts' integer sums, added up across the ranks in int64
+            o = sim.tally() if args.tally else sim.observables()
+            sums.copy_(torch.tensor([o.bond_sum, o.M, o.Q], dtype=torch.int64))
+            dist.all_reduce(sums)
+            b, m, q = (int(v) for v in sums)
+            return eng.Observables(b, m, q, L * L, o.sweeps_done, float("nan"), float("nan"), m / float(L * L), float("nan"))
         if args.workload == "corr":                # A11: the protocol at this time, one native call (no sweeps left to do):
             _, obs = sim.run_protocol_schedule([done[0]])      # r <= 32 all sources + stride-16 sources up to L/2, and B, M, Q
             return obs[0]
@@ -453,7 +483,7 @@ def run_ours(args):
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
     lut = model == wl.ISING_LUT
     philox_ms = copy_ms = None
-    if not lut and n_slabs <= 1:                           # the roof helpers work on the 4-bit layout of an unsharded lattice
+    if not lut and n_slabs <= 1 and not sharded:           # the roof helpers work on the 4-bit layout of an unsharded lattice
         sim.bench_philox_only(2); sim.bench_copy(2); torch.cuda.synchronize(device)
         ev[0].record(); sim.bench_philox_only(n_roof); ev[1].record(); sim.bench_copy(n_roof); ev[2].record()
         torch.cuda.synchronize(device)
@@ -523,10 +553,10 @@ def run_ours(args):
                    "step": "S sweeps + observables" if args.workload == "sweep" else "S sweeps + correlation protocol + observables",
                    "launch": {"rows_per_thread": args.rows_per_thread or "default", "block": args.block or "default",
                               "variant": args.variant, "fused_tally": bool(args.tally), "corr_path": args.corr_path, "sweep_mode": args.sweep_mode,
-                              "slabs": max(1, n_slabs)},
+                              "slabs": world if sharded else max(1, n_slabs)},
                    "lattice_bytes": L * L * BITS_PER_SITE[model] // 8, "l2": "inputs larger than L2 (no flush needed)" if L * L // 2 > (256 << 20)
                    else "lattice fits L2: DRAM figures not meaningful",
-                   "parallelism": f"slabs x{world} (one lattice, slab k on GPU k, halo rows by peer loads)" if (args.parallel == "slabs" and world > 1) else f"replicas x{world}"},
+                   "parallelism": f"slabs x{world} (one lattice, rank k owns slab k, halo rows by peer loads through CUDA IPC, one NCCL all-reduce of a word per colour phase)" if sharded else f"replicas x{world}"},
         "measurement_ms_per_step": (total_ms - sweep_ms) / K,
         "sweep_only_updates_per_ns": whole_job_updates_per_ns(world, L, S, K, sweep_ms, args.parallel),
         "roofline": alu_roof,
@@ -542,7 +572,7 @@ def run_ours(args):
         "paper_context": "GB200: 1802 upd/ns (1-bit Ising, 1/2 RNG per spin), 948 upd/ns (Blume-Capel, 1 RNG per spin) -- other hardware/contract",
     }
     if rank == 0:
-        if not args.no_e2e:
+        if not args.no_e2e and not sharded:
             line["e2e"] = run_e2e(eng, torch, model, L, base.beta, base.D, base.seed, S, min(K, 3), device)
         if not args.no_cpu and world == 1:
             v, cores, info = time_oracle(model, base.beta, base.D, base.seed, args.cpu_seconds)

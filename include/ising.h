@@ -109,6 +109,27 @@ int ising_slab_partition(int64_t L, int n_slabs, int64_t *rows);
 int ising_slab_count(const ising_t *h);
 int ising_slab_info(const ising_t *h, int slab, int64_t *y0, int64_t *rows, int *device);
 
+/* One process per GPU (torch.distributed's arrangement): ONE slab of the lattice per handle.  ising_create_part
+ * makes the handle of the rows [y0, y0 + rows) (both even, rows >= 2; the library allocates on the current device)
+ * and fills them from the seed exactly as the whole lattice would be.  ising_part_export writes the
+ * ISING_IPC_HANDLE_BYTES-byte CUDA IPC handle of the slab's allocation; the ranks exchange these (an all-gather) and
+ * every rank calls ising_part_attach with the handles and heights of the slab above and the slab below (periodic; with
+ * two parts both are the other part): the allocations are mapped (cudaIpcOpenMemHandle, peer access over NVLink) and
+ * the kernels read their two halo rows from them with plain loads.  A part covering the whole
+ * lattice (rows == L) needs no attach.  ising_sweep_phase launches ONE colour phase (0, then 1; after colour 1 the sweep
+ * counter advances); between two phases the caller orders the ranks -- a stream-ordered collective on the handle's
+ * stream (an NCCL all-reduce of one word) or a host barrier after ising_sync: a phase may start once the previous phase
+ * of both neighbours has finished.  On a part handle the observables, the tally and the histogram are the sums over
+ * its own rows (bonds counted at their black site; n_sites = rows * L): the ranks add them up (an int64 all-reduce).
+ * Lattice IO addresses global rows inside the part; the correlation calls need the whole lattice and return
+ * ISING_EINVAL.  Results are those of the unsharded lattice bit for bit.                          */
+#define ISING_IPC_HANDLE_BYTES 64
+int ising_create_part(int model, int64_t L, double beta, double D, uint64_t seed, int64_t y0, int64_t rows,
+                      void *cuda_stream, ising_t **out);
+int ising_part_export(ising_t *h, void *ipc_handle);
+int ising_part_attach(ising_t *h, const void *ipc_above, int64_t rows_above, const void *ipc_below, int64_t rows_below);
+int ising_sweep_phase(ising_t *h, int colour);
+
 /* n >= 0 full sweeps: colour 0 then colour 1 ("two update phases"),
  * one Philox number per site, accept iff r < T.  Asynchronous:
  * 2n kernel launches on the handle's stream, no host synchronisation; small

@@ -23,7 +23,7 @@ EXPORTS = [
     "ising_bench_copy", "ising_debug_philox", "ising_protocol_distances", "ising_threshold_table",
     "ising_run_protocol_schedule", "ising_create_slabs", "ising_slab_count", "ising_slab_info",
     "ising_write_bits", "ising_read_bits", "ising_slab_partition",
-    "ising_set_sweep_mode",
+    "ising_set_sweep_mode", "ising_create_part", "ising_part_export", "ising_part_attach", "ising_sweep_phase",
 ]
 
 
@@ -72,6 +72,10 @@ def load_library():
     lib.ising_create_slabs.argtypes = [C.c_int, i64, dbl, dbl, u64, C.c_int, vp, vp, vp, C.POINTER(vp)]
     lib.ising_slab_count.argtypes = [vp]
     lib.ising_slab_info.argtypes = [vp, C.c_int, vp, vp, vp]
+    lib.ising_create_part.argtypes = [C.c_int, i64, dbl, dbl, u64, i64, i64, vp, C.POINTER(vp)]
+    lib.ising_part_export.argtypes = [vp, vp]
+    lib.ising_part_attach.argtypes = [vp, vp, i64, vp, i64]
+    lib.ising_sweep_phase.argtypes = [vp, C.c_int]
     lib.ising_sweep.argtypes = [vp, i64]
     lib.ising_observables.argtypes = [vp, C.POINTER(_Obs)]
     lib.ising_correlation.argtypes = [vp, i64, vp, vp]
@@ -185,9 +189,10 @@ class IsingSim:
     """One lattice on one GPU.  Methods mirror the C ABI one to one."""
 
     def __init__(self, model: int, L: int, beta: float, D: float = 0.0, seed: int = 1, device="cuda:0",
-                 use_torch_memory: bool = True, slabs=None, slab_devices=None):
+                 use_torch_memory: bool = True, slabs=None, slab_devices=None, part=None):
         """slabs: None = one lattice (ising_create); an int S or a list of row counts = ising_create_slabs
-        (row slabs in allocations of their own, optionally on the CUDA device indices slab_devices)."""
+        (row slabs in allocations of their own, optionally on the CUDA device indices slab_devices).
+        part = (y0, rows): this handle is ONE slab of the lattice (ising_create_part; one process per GPU)."""
         import torch
         if not torch.cuda.is_available():
             raise IsingError(-3, "no CUDA device: the engine has no CPU fallback")
@@ -201,6 +206,11 @@ class IsingSim:
         self._h = C.c_void_p()
         with torch.cuda.device(self.device):
             self._stream = torch.cuda.current_stream(self.device)
+            if part is not None:
+                self._buf = None
+                _check(self._lib.ising_create_part(model, L, beta, D, seed, int(part[0]), int(part[1]),
+                                                   self._stream.cuda_stream, C.byref(self._h)))
+                return
             if slabs is not None:
                 rows = None if isinstance(slabs, int) else np.ascontiguousarray(slabs, dtype=np.int64)
                 n = slabs if rows is None else len(rows)
@@ -245,6 +255,18 @@ class IsingSim:
             _check(self._lib.ising_slab_info(self._h, k, C.addressof(y0), C.addressof(rows), C.addressof(dev)))
             out.append((y0.value, rows.value, dev.value))
         return out
+
+    def part_export(self) -> bytes:
+        """The CUDA IPC handle of this part's allocation (64 bytes), for the neighbouring ranks."""
+        buf = C.create_string_buffer(64)
+        _check(self._lib.ising_part_export(self._h, buf))
+        return buf.raw
+
+    def part_attach(self, ipc_above: bytes, rows_above: int, ipc_below: bytes, rows_below: int):
+        _check(self._lib.ising_part_attach(self._h, C.c_char_p(ipc_above), rows_above, C.c_char_p(ipc_below), rows_below))
+
+    def sweep_phase(self, colour: int):
+        _check(self._lib.ising_sweep_phase(self._h, colour))
 
     # -- the path
     def sweep(self, n: int = 1):

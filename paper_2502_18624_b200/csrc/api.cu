@@ -314,6 +314,95 @@ extern "C" int ising_slab_info(const ising_t *h, int slab, int64_t *y0, int64_t 
     return ISING_OK;
 }
 
+// ------------------------------------------------- one slab per process ---
+// The torch.distributed arrangement (one process per GPU): every rank creates the handle of its own slab, the
+// ranks exchange 64-byte CUDA IPC handles of the slab allocations (an all-gather), map the slabs above and below,
+// and from then on the update / observables kernels read the two halo rows from the neighbours' memory with plain
+// loads.  What has to be ordered across ranks is one thing only: a colour phase may start when the
+// previous phase of both neighbours has finished -- ising_sweep_phase launches one phase, the caller puts a
+// stream-ordered collective (e.g. an NCCL all-reduce of one word) or a host barrier between two phases.
+extern "C" int ising_create_part(int model, int64_t L, double beta, double D, uint64_t seed, int64_t y0, int64_t rows,
+                                 void *cuda_stream, ising_t **out)
+{
+    int rc = check_create_args("ising_create_part", model, L, beta, D, out);
+    if (rc) return rc;
+    if (y0 < 0 || rows < 2 || (y0 & 1) || (rows & 1) || y0 + rows > L)
+        return set_error(ISING_EINVAL, "ising_create_part: y0 and rows must be even, rows >= 2, y0 + rows <= L");
+    ising_sim *h = new_handle(model, L, beta, D, seed, cuda_stream);
+    if (!h) return set_error(ISING_ENOMEM, "ising_create_part: host allocation failed");
+    h->part = true;
+    cudaGetDevice(&h->device);
+    Slab sl;
+    sl.device = h->device; sl.stream = h->stream; sl.y0 = y0; sl.rows = rows;
+    const size_t bytes = (size_t)rows * (size_t)colour_row_words(h) * 16 + kScratchBytes;
+    cudaError_t e = cudaMalloc(&sl.owned, bytes);
+    if (e != cudaSuccess) {
+        delete h;
+        cudaGetLastError();
+        return set_error(e == cudaErrorMemoryAllocation ? ISING_ENOMEM : ISING_ECUDA,
+                         std::string("ising_create_part: cudaMalloc: ") + cudaGetErrorString(e));
+    }
+    carve_slab(h, sl, (char *)sl.owned);
+    h->slabs.push_back(sl);
+    if (rows == L) {                                  // the only part: its halo rows are its own last and first row
+        for (int c = 0; c < 2; ++c) {
+            h->part_halo[0][c] = sl.lat[c] + (rows - 1) * colour_row_words(h);
+            h->part_halo[1][c] = sl.lat[c];
+        }
+    }
+    return finish_create(h, out);
+}
+
+extern "C" int ising_part_export(ising_t *h, void *ipc_handle)
+{
+    DeviceGuard dev_guard(h);
+    if (!h || !ipc_handle || !h->part) return set_error(ISING_EINVAL, "ising_part_export: needs a handle made by ising_create_part");
+    static_assert(sizeof(cudaIpcMemHandle_t) == ISING_IPC_HANDLE_BYTES, "ISING_IPC_HANDLE_BYTES");
+    cudaIpcMemHandle_t mh;
+    CUDA_TRY(cudaIpcGetMemHandle(&mh, h->slabs[0].owned));
+    memcpy(ipc_handle, &mh, sizeof(mh));
+    return ISING_OK;
+}
+
+extern "C" int ising_part_attach(ising_t *h, const void *ipc_above, int64_t rows_above, const void *ipc_below, int64_t rows_below)
+{
+    DeviceGuard dev_guard(h);
+    if (!h || !h->part || !ipc_above || !ipc_below) return set_error(ISING_EINVAL, "ising_part_attach: needs a part handle and both neighbours' IPC handles");
+    if (rows_above < 2 || rows_below < 2 || (rows_above & 1) || (rows_below & 1))
+        return set_error(ISING_EINVAL, "ising_part_attach: neighbour heights must be even and >= 2");
+    if (h->part_ipc[0] || h->part_ipc[1] || h->part_halo[0][0]) return set_error(ISING_EINVAL, "ising_part_attach: neighbours already attached");
+    const bool same = memcmp(ipc_above, ipc_below, ISING_IPC_HANDLE_BYTES) == 0;     // two parts: one neighbour on both sides
+    const void *src[2] = {ipc_above, ipc_below};
+    for (int k = 0; k < (same ? 1 : 2); ++k) {
+        cudaIpcMemHandle_t mh;
+        memcpy(&mh, src[k], sizeof(mh));
+        cudaError_t e = cudaIpcOpenMemHandle(&h->part_ipc[k], mh, cudaIpcMemLazyEnablePeerAccess);
+        if (e != cudaSuccess) { h->part_ipc[k] = nullptr; return cuda_fail(e, "cudaIpcOpenMemHandle (neighbour slab)"); }
+    }
+    // a part's allocation is [colour 0 rows | colour 1 rows | scratch] (carve_slab)
+    const int64_t rw = colour_row_words(h);
+    const uint64_t *above = (const uint64_t *)h->part_ipc[0], *below = (const uint64_t *)(same ? h->part_ipc[0] : h->part_ipc[1]);
+    for (int c = 0; c < 2; ++c) {
+        h->part_halo[0][c] = above + (int64_t)c * rows_above * rw + (rows_above - 1) * rw;     // last row of the slab above
+        h->part_halo[1][c] = below + (int64_t)c * rows_below * rw;                             // first row of the slab below
+    }
+    return ISING_OK;
+}
+
+extern "C" int ising_sweep_phase(ising_t *h, int colour)
+{
+    DeviceGuard dev_guard(h);
+    if (!h || (colour != 0 && colour != 1)) return set_error(ISING_EINVAL, "ising_sweep_phase: bad argument");
+    if (!h->part || !h->part_halo[0][0]) return set_error(ISING_EINVAL, "ising_sweep_phase: needs a part handle with its neighbours attached");
+    if (colour != h->part_phase) return set_error(ISING_EINVAL, "ising_sweep_phase: the phases of a sweep are colour 0, then colour 1");
+    if (h->t >= 0xFFFFFFFFull) return set_error(ISING_EINVAL, "ising_sweep_phase: sweep counter would exceed 2^32-1");
+    cudaError_t e = (h->model == ISING_MODEL_ISING_LUT) ? launch_lut_update(h, 0, colour, (uint32_t)h->t) : launch_update(h, 0, colour, (uint32_t)h->t);
+    if (e != cudaSuccess) return cuda_fail(e, "update kernel");
+    h->part_phase = 1 - colour;
+    if (colour == 1) h->t++;
+    return ISING_OK;
+}
+
 extern "C" int ising_destroy(ising_t *h)
 {
     if (!h) return ISING_OK;
@@ -334,6 +423,8 @@ extern "C" int ising_destroy(ising_t *h)
         if (h->d_rlist) cudaFree(h->d_rlist);
         if (h->h_acc) cudaFreeHost(h->h_acc);
     }
+    for (int k = 0; k < 2; ++k)
+        if (h->part_ipc[k]) { DeviceGuard g(h->device); cudaIpcCloseMemHandle(h->part_ipc[k]); }
     for (Slab &sl : h->slabs) {
         DeviceGuard g(sl.device);
         if (sl.lut_buckets) cudaFree(sl.lut_buckets);
@@ -458,7 +549,7 @@ static void drop_graph(ising_sim *h)
 static bool graph_worthwhile(const ising_sim *h, int64_t n)
 {
     const int64_t sites = h->L * h->L;
-    return n >= 2 * kGraphSweeps && sites <= (1ll << 22) && h->slabs.size() == 1;      // L <= 2048: a colour phase is launch-bound
+    return n >= 2 * kGraphSweeps && sites <= (1ll << 22) && h->slabs.size() == 1 && !h->part;      // L <= 2048: a colour phase is launch-bound
 }
 
 static int ensure_graph(ising_sim *h)
@@ -500,10 +591,13 @@ extern "C" int ising_sweep(ising_t *h, int64_t n)
     if (!h) return set_error(ISING_EINVAL, "ising_sweep: NULL handle");
     if (n < 0) return set_error(ISING_EINVAL, "ising_sweep: n < 0");
     if (h->t + (uint64_t)n > 0xFFFFFFFFull) return set_error(ISING_EINVAL, "ising_sweep: sweep counter would exceed 2^32-1");
+    if (h->part && (h->slabs[0].rows != h->L || h->part_phase != 0))
+        return set_error(ISING_EINVAL, "ising_sweep: one part of a lattice is swept phase by phase (ising_sweep_phase), with the "
+                                       "caller's barrier between the phases");
     // Launch-bound lattices, on request (ising_set_sweep_mode 3): n sweeps in one cooperative launch with a grid
     // barrier per colour phase (update.cu).  Measured slower than the CUDA graph below (L = 256: 5.95 against 5.5
     // microseconds per sweep): a barrier through L2 costs what a kernel boundary inside a graph costs.
-    const bool small = h->L * h->L <= (1ll << 22) && h->slabs.size() == 1;
+    const bool small = h->L * h->L <= (1ll << 22) && h->slabs.size() == 1 && !h->part;
     // Tiny lattices (L <= 512; mode 4: whatever fits): one cluster of 16 CTAs keeps the lattice in distributed shared
     // memory for all n sweeps, the colour phases separated by the hardware cluster barrier (update.cu).
     if (small && n >= 2 && h->model != ISING_MODEL_ISING_LUT && ((h->sweep_mode == 0 && h->L <= 512) || h->sweep_mode == 4)) {
@@ -613,9 +707,29 @@ extern "C" int ising_set_variant(ising_t *h, int variant)
     return ISING_OK;
 }
 
+// Rows a handle holds: all of them, or [y0, y0 + rows) for one part of a lattice (ising_create_part).
+static int64_t local_sites(const ising_sim *h) { return (h->part ? h->slabs[0].rows : h->L) * h->L; }
+
+static int check_local_rows(const ising_sim *h, const char *who, int64_t y0, int64_t ny)
+{
+    if (!h->part) return ISING_OK;
+    const Slab &sl = h->slabs[0];
+    if (y0 < sl.y0 || y0 + ny > sl.y0 + sl.rows)
+        return set_error(ISING_EINVAL, std::string(who) + ": rows outside this part of the lattice (ising_slab_info gives its range)");
+    return ISING_OK;
+}
+
+static int no_parts(const ising_sim *h, const char *who)
+{
+    if (h->part && h->slabs[0].rows != h->L)
+        return set_error(ISING_EINVAL, std::string(who) + ": needs the whole lattice, this handle holds one part of it");
+    return ISING_OK;
+}
+
 // ----------------------------------------------------------- observables ---
 static int observe_all_slabs(ising_sim *h)                // -> d_acc[0..2] of every slab
 {
+    if (h->part && !h->part_halo[0][0]) return set_error(ISING_EINVAL, "observables of a part need its neighbours (ising_part_attach)");
     const bool lut = h->model == ISING_MODEL_ISING_LUT;
     return for_each_slab(h, "observables kernel", [&](int k) { return lut ? launch_lut_observables(h, k) : launch_observables(h, k); });
 }
@@ -623,9 +737,9 @@ static int observe_all_slabs(ising_sim *h)                // -> d_acc[0..2] of e
 static void fill_obs(const ising_sim *h, const long long *bmq, ising_obs_t *o)
 {
     const bool lut = h->model == ISING_MODEL_ISING_LUT;
-    o->bond_sum = bmq[0]; o->M = bmq[1]; o->Q = (lut || h->model == ISING_MODEL_ISING) ? h->L * h->L : bmq[2];
-    o->n_sites = h->L * h->L; o->sweeps_done = h->t;
-    const double N = (double)h->L * (double)h->L;
+    o->bond_sum = bmq[0]; o->M = bmq[1]; o->Q = (lut || h->model == ISING_MODEL_ISING) ? local_sites(h) : bmq[2];
+    o->n_sites = local_sites(h); o->sweeps_done = h->t;       // one part of a lattice: the sums and N of its own rows
+    const double N = (double)local_sites(h);
     o->E = !is_blume_capel(h->model) ? -(double)o->bond_sum : -(double)o->bond_sum + h->D * (double)o->Q;
     o->e_per_site = o->E / N;
     o->m_per_site = (double)o->M / N;
@@ -680,6 +794,7 @@ extern "C" int ising_schwinger_dyson(ising_t *h, int64_t hist[9], double *value)
     DeviceGuard dev_guard(h);
     if (!h || !hist || !value) return set_error(ISING_EINVAL, "ising_schwinger_dyson: NULL argument");
     const bool lut = h->model == ISING_MODEL_ISING_LUT;
+    if (h->part && !h->part_halo[0][0]) return set_error(ISING_EINVAL, "ising_schwinger_dyson: a part needs its neighbours (ising_part_attach)");
     int rc = for_each_slab(h, "Schwinger-Dyson kernel", [&](int k) { return lut ? launch_lut_sd_hist(h, k) : launch_sd_hist(h, k); });
     if (rc) return rc;
     long long bins[9];
@@ -690,7 +805,7 @@ extern "C" int ising_schwinger_dyson(ising_t *h, int64_t hist[9], double *value)
         hist[k + 4] = bins[k + 4];
         acc += (double)hist[k + 4] * exp(-2.0 * h->beta * (double)k);
     }
-    *value = acc / ((double)h->L * (double)h->L);
+    *value = acc / (double)local_sites(h);
     return ISING_OK;
 }
 
@@ -723,6 +838,7 @@ extern "C" int ising_read_window(ising_t *h, int64_t x0, int64_t y0, int64_t w, 
     DeviceGuard dev_guard(h);
     if (!h || !host_out) return set_error(ISING_EINVAL, "ising_read_window: NULL argument");
     if (w < 1 || hgt < 1 || w > h->L || hgt > h->L) return set_error(ISING_EINVAL, "ising_read_window: window size out of range");
+    if (int rcp = check_local_rows(h, "ising_read_window", y0, hgt)) return rcp;
     const int64_t L = h->L;
     x0 = ((x0 % L) + L) % L; y0 = ((y0 % L) + L) % L;
     const int64_t rows_per = std::max<int64_t>(1, std::min<int64_t>(hgt, kStageBytes / w));
@@ -751,6 +867,7 @@ extern "C" int ising_write_lattice(ising_t *h, int64_t y0, int64_t ny, const int
     DeviceGuard dev_guard(h);
     if (!h || !host_in) return set_error(ISING_EINVAL, "ising_write_lattice: NULL argument");
     if (y0 < 0 || ny < 1 || y0 + ny > h->L) return set_error(ISING_EINVAL, "ising_write_lattice: rows outside [0, L]");
+    if (int rcp = check_local_rows(h, "ising_write_lattice", y0, ny)) return rcp;
     const int64_t L = h->L;
     const int64_t rows_per = std::max<int64_t>(1, std::min<int64_t>(ny, kStageBytes / L));
     int rc = ensure_stage(h, (size_t)(rows_per * L) + 16);
@@ -778,6 +895,8 @@ extern "C" int ising_read_packed(ising_t *h, int colour, int64_t word0, int64_t 
     if (!h || !host_out) return set_error(ISING_EINVAL, "ising_read_packed: NULL argument");
     if ((colour != 0 && colour != 1) || word0 < 0 || nwords < 0 || word0 + nwords > colour_words(h))
         return set_error(ISING_EINVAL, "ising_read_packed: range outside the colour array");
+    if (h->part && (word0 < h->slabs[0].y0 * colour_row_words(h) || word0 + nwords > (h->slabs[0].y0 + h->slabs[0].rows) * colour_row_words(h)))
+        return set_error(ISING_EINVAL, "ising_read_packed: words outside this part of the lattice");
     for (const Slab &sl : h->slabs) {                    // the word range, slab by slab
         const int64_t first = sl.y0 * colour_row_words(h), last = first + sl.rows * colour_row_words(h);
         const int64_t a = std::max(word0, first), b = std::min(word0 + nwords, last);
@@ -793,6 +912,8 @@ extern "C" int ising_write_packed(ising_t *h, int colour, int64_t word0, int64_t
     if (!h || !host_in) return set_error(ISING_EINVAL, "ising_write_packed: NULL argument");
     if ((colour != 0 && colour != 1) || word0 < 0 || nwords < 0 || word0 + nwords > colour_words(h))
         return set_error(ISING_EINVAL, "ising_write_packed: range outside the colour array");
+    if (h->part && (word0 < h->slabs[0].y0 * colour_row_words(h) || word0 + nwords > (h->slabs[0].y0 + h->slabs[0].rows) * colour_row_words(h)))
+        return set_error(ISING_EINVAL, "ising_write_packed: words outside this part of the lattice");
     for (const Slab &sl : h->slabs) {
         const int64_t first = sl.y0 * colour_row_words(h), last = first + sl.rows * colour_row_words(h);
         const int64_t a = std::max(word0, first), b = std::min(word0 + nwords, last);
@@ -813,6 +934,7 @@ static int bits_args(const ising_sim *h, const char *who, int colour, int64_t ro
     if (!h || !host) return set_error(ISING_EINVAL, std::string(who) + ": NULL argument");
     if ((colour != 0 && colour != 1) || row0 < 0 || nrows < 0 || row0 + nrows > h->L)
         return set_error(ISING_EINVAL, std::string(who) + ": colour or rows out of range");
+    if (int rcp = check_local_rows(h, who, row0, nrows)) return rcp;
     if (!is_blume_capel(h->model) && (h->L % 128) != 0)
         return set_error(ISING_EINVAL, std::string(who) + ": one bit per spin needs L to be a multiple of 128 (whole 64-bit words per colour row)");
     return ISING_OK;
@@ -987,6 +1109,7 @@ extern "C" int ising_correlation(ising_t *h, int64_t rmax, int64_t *sx, int64_t 
     DeviceGuard dev_guard(h);
     if (!h || !sx || !sy) return set_error(ISING_EINVAL, "ising_correlation: NULL argument");
     if (rmax < 1 || rmax > h->L / 2) return set_error(ISING_EINVAL, "ising_correlation: rmax outside [1, L/2]");
+    if (int rcp = no_parts(h, "ising_correlation")) return rcp;
     int rc = ensure_planes(h);
     if (rc) return rc;
     cudaError_t e = launch_planes(h);
@@ -1014,6 +1137,7 @@ extern "C" int ising_correlation_list(ising_t *h, int64_t stride, int64_t count,
     DeviceGuard dev_guard(h);
     if (!h || !r || !sx || !sy) return set_error(ISING_EINVAL, "ising_correlation_list: NULL argument");
     if (!valid_stride(stride)) return set_error(ISING_EINVAL, "ising_correlation_list: stride must be 1 or a power of two <= 64");
+    if (int rcp = no_parts(h, "ising_correlation_list")) return rcp;
     if (count < 1 || count > 65535) return set_error(ISING_EINVAL, "ising_correlation_list: count outside [1, 65535]");
     for (int64_t i = 0; i < count; ++i)
         if (r[i] < 1 || r[i] > h->L / 2) return set_error(ISING_EINVAL, "ising_correlation_list: distance outside [1, L/2]");
@@ -1029,6 +1153,7 @@ extern "C" int ising_correlation_list(ising_t *h, int64_t stride, int64_t count,
 static int protocol_measure(ising_sim *h, std::vector<int64_t> &r, std::vector<int64_t> &sx, std::vector<int64_t> &sy,
                             std::vector<int64_t> &n_src)
 {
+    if (int rcp = no_parts(h, "the correlation protocol")) return rcp;
     std::vector<int64_t> all_sources, block_sources;
     host_protocol_lists(h->L, h->t, all_sources, block_sources);
     const int64_t na = (int64_t)all_sources.size(), nb = (int64_t)block_sources.size();

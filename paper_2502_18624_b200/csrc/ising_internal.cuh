@@ -41,12 +41,19 @@ struct Slab {
 // slab k holds the rows [y_end[k-1], y_end[k]).
 struct SlabDir {
     int n;
+    long long y_first;                      // first row of slab 0 (0 unless the handle is one part of a lattice)
     long long y_end[ISING_MAX_SLABS];
     uint64_t *lat[2][ISING_MAX_SLABS];
 };
 
 struct ising_sim {
     std::vector<Slab> slabs;                // >= 1; lat / d_acc / d_bc_table / stream below are slab 0's (single-slab code paths)
+    // One process per GPU (ising_create_part): the handle owns ONE slab of the lattice, the slabs above and below belong
+    // to other handles -- other processes -- and their boundary rows are mapped through CUDA IPC (plain loads over NVLink).
+    bool part = false;
+    const uint64_t *part_halo[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};   // [above / below][colour]; NULL until attached
+    void *part_ipc[2] = {nullptr, nullptr};                                        // mapped neighbour allocations (cudaIpcOpenMemHandle)
+    int part_phase = 0;                                                            // colour the next ising_sweep_phase must update
     int model = 0;
     int64_t L = 0;
     double beta = 0, D = 0;
@@ -127,11 +134,13 @@ static inline int64_t colour_row_words(const ising_sim *h) { return h->L / (2 * 
 // Halo rows of slab k in colour array c: the last row of the slab above, the first row of the slab below (periodic).
 static inline const uint64_t *halo_up(const ising_sim *h, int k, int c)
 {
+    if (h->part) return h->part_halo[0][c];
     const Slab &a = h->slabs[(k + (int)h->slabs.size() - 1) % (int)h->slabs.size()];
     return a.lat[c] + (a.rows - 1) * colour_row_words(h);
 }
 static inline const uint64_t *halo_down(const ising_sim *h, int k, int c)
 {
+    if (h->part) return h->part_halo[1][c];
     return h->slabs[(k + 1) % (int)h->slabs.size()].lat[c];
 }
 // 64-bit words per row of a plane down-sampled to the bits x % stride == 0 (zero padded)
@@ -176,7 +185,7 @@ __device__ __forceinline__ uint64_t *slab_row(const SlabDir &d, int c, long long
 {
     int k = 0;
     while (k + 1 < d.n && y >= d.y_end[k]) ++k;
-    const long long first = k ? d.y_end[k - 1] : 0;
+    const long long first = k ? d.y_end[k - 1] : d.y_first;
     return d.lat[c][k] + (y - first) * row_words;
 }
 

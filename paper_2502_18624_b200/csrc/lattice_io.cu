@@ -6,6 +6,7 @@ SlabDir slab_directory(const ising_sim *h)
 {
     SlabDir d;
     d.n = (int)h->slabs.size();
+    d.y_first = h->slabs[0].y0;
     for (int k = 0; k < ISING_MAX_SLABS; ++k) {
         const bool live = k < d.n;
         d.y_end[k] = live ? h->slabs[k].y0 + h->slabs[k].rows : h->L;

@@ -1,8 +1,8 @@
 """N > 1 host logic of bench.py on CPU (gloo, world_size 2).  Default: replicas (north_star: one GPU per
 simulation), where the only cross-rank steps are the barrier and the max-over-ranks of the device times.
---parallel slabs (NEXT-4): one lattice cut into row slabs, slab k on GPU k, driven by rank 0;
-its host logic -- who drives, which slabs on which devices, the partition, the whole-job value -- is checked here,
-the device side by tests/test_gpu_slabs.py."""
+--parallel slabs (NEXT-4): one lattice cut into row slabs, rank k owning slab k; its host logic --
+which rows a rank owns, the exchange of the IPC handles and who is whose neighbour, the partition, the whole-job value
+-- is checked here, the device side (IPC mapping, halo loads, phase protocol) by tests/test_gpu_parts.py."""
 import os
 import socket
 import sys
@@ -31,7 +31,19 @@ def _worker(rank, world, port, out):
         dist.barrier()
         total_ms, sweep_ms = bench.max_over_ranks(mine, dist, torch.device("cpu"))
         value = bench.whole_job_updates_per_ns(world, 256, 10, 4, total_ms)
-        plan = bench.rank_plan(rank, world, "slabs")
+        heights = [130, 126]
+        plan = bench.rank_plan(rank, world, "slabs", heights)
+        got = {}
+
+        class FakePart:                                        # the exchange of attach_neighbours over gloo, no GPU
+            def part_export(self):
+                return bytes([rank]) * 64
+
+            def part_attach(self, up, rows_up, dn, rows_dn):
+                got["attach"] = (up[0], rows_up, dn[0], rows_dn)
+
+        bench.attach_neighbours(FakePart(), rank, world, heights, dist.all_gather_object)
+        plan = (plan, got["attach"])
         sharded = bench.whole_job_updates_per_ns(world, 256, 10, 4, total_ms, "slabs")
         out.put((rank, total_ms, sweep_ms, value, bench.replica_seed(1, rank), plan, sharded))
     finally:
@@ -54,8 +66,10 @@ def test_max_over_ranks_and_whole_job_value_world2():
         assert total_ms == 107.0 and sweep_ms == 90.0            # element-wise max, same on both ranks
         assert value == pytest.approx(2 * 256 * 256 * 10 * 4 / (107.0 * 1e6), rel=1e-15)
         assert seed == 1 + rank                                  # independent replicas
-        # --parallel slabs: rank 0 drives one lattice of 2 slabs on GPUs 0 and 1, rank 1 idles; one lattice's updates
-        assert plan == ((True, 2, [0, 1]) if rank == 0 else (False, 0, None))
+        # --parallel slabs: one lattice, the same seed on both ranks, rank k owns slab k; with two parts the other rank is
+        # the neighbour above and below; the whole-job value counts one lattice's updates
+        other = 1 - rank
+        assert plan == ((0, ((0, 130) if rank == 0 else (130, 126))), (other, [130, 126][other], other, [130, 126][other]))
         assert sharded == pytest.approx(256 * 256 * 10 * 4 / (107.0 * 1e6), rel=1e-15)
 
 
@@ -64,7 +78,7 @@ def test_single_process_passthrough():
     import bench
     assert bench.max_over_ranks([3.5, 2], None, None) == [3.5, 2.0]
     assert bench.whole_job_updates_per_ns(1, 1 << 18, 10, 10, 1000.0) == (1 << 36) * 100 / 1e9
-    assert bench.rank_plan(0, 1, "slabs") == (True, 0, None) and bench.rank_plan(3, 8, "replicas") == (True, 0, None)
+    assert bench.rank_plan(0, 1, "slabs", None) == (0, None) and bench.rank_plan(3, 8, "replicas", None) == (3, None)
 
 
 def test_slab_partition_for_every_rank_count():
