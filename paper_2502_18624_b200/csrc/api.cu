@@ -71,6 +71,34 @@ static void default_launch(ising_sim *h)
     h->block_threads = lut ? 256 : 128;           // LUT: 32 KB bucket table per block, fewer and larger blocks
 }
 
+// Wave quantisation.  A colour phase of a mid-size lattice is a handful of waves of blocks (a wave = the blocks the
+// GPU holds at once), and a last wave that is nearly empty costs as much as a full one: at L = 2^14 the first
+// choice R = 26 gives 1262 blocks for 1184 places -- R = 28 (1172 blocks, one wave) runs 4.6 % faster, R = 14 (two
+// full waves) the same.  So among the even R up to the first choice's ceiling the one with the least
+// waves x (R + halo) is taken; lattices of many waves keep the first choice.
+static void tune_rows_for_waves(ising_sim *h)
+{
+    const bool lut = h->model == ISING_MODEL_ISING_LUT;
+    int n_sm = 0;
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, h->device) != cudaSuccess) { cudaGetLastError(); return; }
+    const int block = h->block_threads;
+    const int per_sm = lut ? lut_blocks_per_sm(h, block) : update_blocks_per_sm(h, block);
+    if (per_sm <= 0 || n_sm <= 0) return;
+    const int64_t capacity = (int64_t)per_sm * n_sm, cols = lut ? h->L / 256 : h->L / 64, rmax = lut ? 64 : 32;
+    int64_t rows = 0;
+    for (const Slab &sl : h->slabs) rows = std::max(rows, sl.rows);
+    auto blocks = [&](int64_t r) { return (((rows + r - 1) / r) * cols + block - 1) / block; };
+    if (blocks(rmax) > 16 * capacity) return;                   // many waves: the tail is a few per cent at most
+    double best = 0.0;
+    int64_t best_r = h->rows_per_thread;
+    for (int64_t r = 2; r <= rmax; r += 2) {
+        const int64_t waves = (blocks(r) + capacity - 1) / capacity;
+        const double cost = (double)waves * ((double)r + 0.7);      // two halo rows cost about a third of a row each
+        if (best == 0.0 || cost <= best) { best = cost; best_r = r; }
+    }
+    h->rows_per_thread = (int)best_r;
+}
+
 // ---------------------------------------------------------------- create ---
 // Device tables derived from the integer thresholds: Blume-Capel compare / carry tables, or the search
 // tree and bucket table of the 1-bit kernel's getMaxLE.  Built once on the host, copied to every slab's device.
@@ -193,6 +221,10 @@ static int finish_create(ising_sim *h, ising_t **out)
     for (int k = 0; k < (int)h->slabs.size(); ++k) {
         rc = setup_slab(h, k, ht);
         if (rc) { ising_destroy(h); return rc; }
+    }
+    {
+        DeviceGuard g(h->device);
+        tune_rows_for_waves(h);
     }
     const Slab &s0 = h->slabs[0];
     h->lat[0] = s0.lat[0]; h->lat[1] = s0.lat[1]; h->d_acc = s0.d_acc; h->d_bc_table = s0.d_table;

@@ -150,6 +150,8 @@ static inline int64_t comb_words_per_row(int64_t L, int64_t stride) { return (L 
 // per-slab launchers run on the slab's stream (the caller has switched to the slab's device)
 cudaError_t launch_init(ising_sim *h, int slab);
 cudaError_t launch_update(ising_sim *h, int slab, int colour, uint32_t t);
+int update_blocks_per_sm(const ising_sim *h, int block);         // occupancy of the update kernel this handle launches
+int lut_blocks_per_sm(const ising_sim *h, int block);
 cudaError_t launch_sweeps_persistent(ising_sim *h, uint32_t t0, int n_sweeps);   // unsharded small lattices, one cooperative launch
 cudaError_t launch_sweeps_cluster(ising_sim *h, uint32_t t0, int n_sweeps);      // tiny lattices: one cluster, lattice in DSMEM
 cudaError_t launch_observables(ising_sim *h, int slab);             // -> slab d_acc[0..2] = B, M, Q of the slab's rows

@@ -316,6 +316,18 @@ cudaError_t launch_lut_update(ising_sim *h, int slab, int colour, uint32_t t)
     return cudaGetLastError();
 }
 
+// Resident blocks per SM of the kernel launch_lut_update picks for this handle (0 if the query fails).
+int lut_blocks_per_sm(const ising_sim *h, int block)
+{
+    const bool bucket = h->variant == 2 || (h->variant == 0 && h->L >= 8192);
+    const size_t smem = bucket ? (8 << LUT_BUCKET_BITS) : 0;
+    const void *fn = bucket ? reinterpret_cast<const void *>(&lut_update_kernel<0, 0, 0>) : reinterpret_cast<const void *>(&lut_update_kernel<0, 1, 0>);
+    if (bucket && cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); return 0; }
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, block, smem) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return per_sm;
+}
+
 // L5: word w of colour c = (x | y << 32) of Philox(ctr = (w_lo, w_hi, 0, 2 + c))
 __global__ void __launch_bounds__(256) lut_init_kernel(uint64_t *lat0, uint64_t *lat1, int64_t words, int64_t word0, RoundKeys rk)
 {

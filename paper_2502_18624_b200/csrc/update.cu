@@ -692,6 +692,21 @@ cudaError_t launch_sweeps_cluster(ising_sim *h, uint32_t t0, int n_sweeps)
     return e;
 }
 
+// Resident blocks per SM of the one-phase kernel ising_sweep launches for this handle (0 if the query fails).
+int update_blocks_per_sm(const ising_sim *h, int block)
+{
+    const int v = effective_variant(h);
+    const void *fn = nullptr;
+#define UK(MODEL, V) (h->tally_on ? reinterpret_cast<const void *>(&update_kernel<MODEL, 0, V, 1>) : reinterpret_cast<const void *>(&update_kernel<MODEL, 0, V, 0>))
+    if (h->model == ISING_MODEL_ISING) fn = v == 0 ? UK(ISING_MODEL_ISING, 0) : UK(ISING_MODEL_ISING, 1);
+    else if (h->model == ISING_MODEL_BLUME_CAPEL) fn = v == 0 ? UK(ISING_MODEL_BLUME_CAPEL, 0) : UK(ISING_MODEL_BLUME_CAPEL, 1);
+    else fn = v == 0 ? UK(ISING_MODEL_BLUME_CAPEL_2BIT, 0) : UK(ISING_MODEL_BLUME_CAPEL_2BIT, 1);
+#undef UK
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, block, 0) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return per_sm;
+}
+
 // n sweeps t0, t0 + 1, ... of an unsharded small lattice in one cooperative launch (see sweep_persistent_kernel).
 // Returns cudaErrorNotSupported when the device cannot keep the whole grid resident (the caller then launches
 // phase by phase).
