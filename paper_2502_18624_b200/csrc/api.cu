@@ -986,7 +986,11 @@ extern "C" int ising_write_bits(ising_t *h, int colour, int64_t row0, int64_t nr
         return ising_write_packed(h, colour, row0 * rw, nrows * rw, host_in);
     }
     const bool bc = is_blume_capel(h->model);
-    const int64_t rows_per = std::max<int64_t>(1, std::min<int64_t>(nrows, kStageBytes / (rw * 8)));
+    // Blume-Capel input is validated before anything is written; up to 256 MB it stays in the staging buffer between
+    // the two passes (one upload), beyond that every chunk is uploaded twice
+    const int64_t stage_cap = bc ? 4 * kStageBytes : kStageBytes;
+    const int64_t rows_per = std::max<int64_t>(1, std::min<int64_t>(nrows, stage_cap / (rw * 8)));
+    const bool one_chunk = rows_per >= nrows;
     rc = ensure_stage(h, (size_t)(rows_per * rw * 8));
     if (rc) return rc;
     int *d_bad = (int *)(h->d_acc + 32);
@@ -1011,7 +1015,8 @@ extern "C" int ising_write_bits(ising_t *h, int colour, int64_t row0, int64_t nr
     for (int pass = bc ? 0 : 1; pass < 2; ++pass)
         for (int64_t j = 0; j < nrows; j += rows_per) {
             const int64_t nr = std::min(rows_per, nrows - j);
-            CUDA_TRY(cudaMemcpyAsync(h->io_stage, host_in + j * rw, (size_t)(nr * rw * 8), cudaMemcpyHostToDevice, h->stream));
+            if (pass == 0 || !bc || !one_chunk)
+                CUDA_TRY(cudaMemcpyAsync(h->io_stage, host_in + j * rw, (size_t)(nr * rw * 8), cudaMemcpyHostToDevice, h->stream));
             cudaError_t e = launch_bits(h, colour, row0 + j, nr, (uint32_t *)h->io_stage, pass, d_bad);
             if (e == cudaErrorInvalidValue) return set_error(ISING_EINVAL, "ising_write_bits: a 2-bit code equal to 3");
             if (e != cudaSuccess) return cuda_fail(e, "bit expansion kernel");
