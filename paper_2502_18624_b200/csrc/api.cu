@@ -626,10 +626,7 @@ extern "C" int ising_sweep(ising_t *h, int64_t n)
     if (h->part && (h->slabs[0].rows != h->L || h->part_phase != 0))
         return set_error(ISING_EINVAL, "ising_sweep: one part of a lattice is swept phase by phase (ising_sweep_phase), with the "
                                        "caller's barrier between the phases");
-    // Launch-bound lattices, on request (ising_set_sweep_mode 3): n sweeps in one cooperative launch with a grid
-    // barrier per colour phase (update.cu).  Measured slower than the CUDA graph below (L = 256: 5.95 against 5.5
-    // microseconds per sweep): a barrier through L2 costs what a kernel boundary inside a graph costs.
-    const bool small = h->L * h->L <= (1ll << 22) && h->slabs.size() == 1 && !h->part;
+    const bool small = h->L * h->L <= (1ll << 22) && h->slabs.size() == 1 && !h->part;      // launch-bound: L <= 2048
     // Tiny lattices (L <= 512; mode 4: whatever fits): one cluster of 16 CTAs keeps the lattice in distributed shared
     // memory for all n sweeps, the colour phases separated by the hardware cluster barrier (update.cu).
     if (small && n >= 2 && h->model != ISING_MODEL_ISING_LUT && ((h->sweep_mode == 0 && h->L <= 512) || h->sweep_mode == 4)) {
@@ -642,6 +639,9 @@ extern "C" int ising_sweep(ising_t *h, int64_t n)
             n -= chunk;
         }
     }
+    // On request (ising_set_sweep_mode 3): n sweeps in one cooperative launch with a grid barrier per colour phase
+    // (update.cu).  Measured slower than the CUDA graph below (L = 256: 5.95 against 5.5 microseconds per sweep): a
+    // barrier through L2 costs what a kernel boundary inside a graph costs.
     if (small && n >= 2 && h->sweep_mode == 3 && h->model != ISING_MODEL_ISING_LUT) {
         while (n > 0) {
             const int chunk = (int)std::min<int64_t>(n, 4096);          // bounds the 32-bit per-warp tally sums
