@@ -978,13 +978,8 @@ extern "C" int ising_write_bits(ising_t *h, int colour, int64_t row0, int64_t nr
     int rc = bits_args(h, "ising_write_bits", colour, row0, nrows, host_in);
     if (rc) return rc;
     const int64_t rw = bits_row_words(h);
-    if (h->model == ISING_MODEL_ISING_LUT || h->model == ISING_MODEL_BLUME_CAPEL_2BIT) {
-        if (h->model == ISING_MODEL_BLUME_CAPEL_2BIT)                  // the code 3 does not exist
-            for (int64_t i = 0; i < nrows * rw; ++i)
-                if (host_in[i] & (host_in[i] >> 1) & 0x5555555555555555ull)
-                    return set_error(ISING_EINVAL, "ising_write_bits: a 2-bit code equal to 3");
+    if (h->model == ISING_MODEL_ISING_LUT)                       // any bit pattern is a lattice: a plain copy
         return ising_write_packed(h, colour, row0 * rw, nrows * rw, host_in);
-    }
     const bool bc = is_blume_capel(h->model);
     // Blume-Capel input is validated before anything is written; up to 256 MB it stays in the staging buffer between
     // the two passes (one upload), beyond that every chunk is uploaded twice

@@ -340,6 +340,7 @@ struct BitsParams {
     SlabDir dir;
     int64_t L, row0, nrows;      // rows [row0, row0 + nrows) of colour `colour`
     int colour, bc, mode;        // mode 0: validate only, 1: expand into the lattice, 2: gather from the lattice
+    int two_bit;                 // the lattice itself is stored at 2 bits per spin: the format is the layout, no expansion
     uint32_t *buf;               // staging: nrows x (L/64) x {1 (Ising) | 2 (Blume-Capel)} uint32, row-major
     int *bad;
 };
@@ -350,6 +351,12 @@ __global__ void __launch_bounds__(256) bits_kernel(const __grid_constant__ BitsP
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= p.nrows * vecs) return;
     const int64_t row = idx / vecs, v = idx - row * vecs;
+    if (p.two_bit) {                                             // validate / store one 64-bit word (32 sites) as it is
+        const uint32_t a = p.buf[2 * idx], b = p.buf[2 * idx + 1];
+        if ((a & (a >> 1) & 0x55555555u) | (b & (b >> 1) & 0x55555555u)) atomicOr(p.bad, 1);
+        if (p.mode == 1) slab_row(p.dir, p.colour, p.row0 + row, vecs)[v] = (uint64_t)a | ((uint64_t)b << 32);
+        return;
+    }
     uint64_t *lat = slab_row(p.dir, p.colour, p.row0 + row, p.L / 32) + 2 * v;
     if (p.mode == 2) {
         const uint64_t w0 = lat[0], w1 = lat[1];
@@ -380,6 +387,7 @@ cudaError_t launch_bits(ising_sim *h, int colour, int64_t row0, int64_t nrows, u
     p.dir = slab_directory(h);
     p.L = h->L; p.row0 = row0; p.nrows = nrows; p.colour = colour; p.bc = is_blume_capel(h->model) ? 1 : 0;
     p.mode = mode; p.buf = dev_buf; p.bad = dev_bad;
+    p.two_bit = h->model == ISING_MODEL_BLUME_CAPEL_2BIT ? 1 : 0;
     cudaError_t e;
     if (mode == 0) {
         e = cudaMemsetAsync(dev_bad, 0, sizeof(int), h->stream);
