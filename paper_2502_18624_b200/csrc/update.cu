@@ -425,10 +425,13 @@ __device__ __forceinline__ void update_chunk(const UpdParams &p, unsigned tid, u
 template <int MODEL>
 __device__ __forceinline__ uint64_t load_tables(const UpdParams &p, uint32_t *s_tab)
 {
-    if (MODEL == ISING_MODEL_ISING) return 0;
-    for (int i = threadIdx.x; i < 80 + 132; i += blockDim.x) s_tab[i] = p.bc_table[i];
-    __syncthreads();
-    return (uint64_t)s_tab[64] | ((uint64_t)s_tab[65] << 32);
+    uint64_t always = 0;
+    if (MODEL != ISING_MODEL_ISING) {
+        for (int i = threadIdx.x; i < 80 + 132; i += blockDim.x) s_tab[i] = p.bc_table[i];
+        __syncthreads();
+        always = (uint64_t)s_tab[64] | ((uint64_t)s_tab[65] << 32);
+    }
+    return always;
 }
 
 template <int MODEL, int C, int V, int TALLY>
