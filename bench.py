@@ -308,7 +308,7 @@ def run_e2e(eng, torch, model, L, beta, D, seed, S, steps, device):
         for st in streams:
             with torch.cuda.stream(st):
                 sims.append(eng.IsingSim(model, L, beta, D, seed, device=device))
-        n_pipe = max(5 * steps, 15)                 # the fill (one upload that overlaps nothing) is inside the timed region
+        n_pipe = max(6 * steps, 18)                 # the fill (one upload that overlaps nothing) is inside the timed region
         for sim in sims:                            # warm-up: one step each
             enqueue(sim)
             sim.observables()
