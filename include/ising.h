@@ -156,6 +156,17 @@ int ising_tally(ising_t *h, ising_obs_t *out);
  * Host arrays of length rmax.  Synchronises.                                */
 int ising_correlation(ising_t *h, int64_t rmax, int64_t *sx, int64_t *sy);
 
+/* The same sums for callers that may not allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): ising_correlation keeps its scratch -- bit planes, transposed planes,
+ * accumulators -- in buffers it cudaMallocs on first use; this entry point runs the same bit-plane kernels on
+ * a static device array of 532480 bytes (held by every GPU that loads the library until exit) and calls no
+ * cudaMalloc, cudaFree or allocating library routine.  Limit: L <= ISING_NOALLOC_MAX_L (ISING_EINVAL beyond
+ * it).  Every call on a device shares the array, which keeps the last call's contents: what must start at
+ * zero is cleared by the call itself, but two calls that OVERLAP on the GPU (two handles on two streams, two
+ * host threads) race on it.  Same arguments, same integers as ising_correlation.  Synchronises.          */
+#define ISING_NOALLOC_MAX_L 1024
+int ising_correlation_noalloc(ising_t *h, int64_t rmax, int64_t *sx, int64_t *sy);
+
 /* Which kernels ising_correlation uses: 0 = automatic (tensor cores at the fp4 rate, path 4, when
  * rmax >= 512 and L is a multiple of 256; bit planes otherwise), 1 = bit planes (XOR + POPC),
  * 2 = tensor cores, int8, one CTA per 128 x 256 tile, 3 = int8, CTA pairs (cta_group::2, 256 x 256

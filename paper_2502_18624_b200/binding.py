@@ -24,6 +24,7 @@ EXPORTS = [
     "ising_run_protocol_schedule", "ising_create_slabs", "ising_slab_count", "ising_slab_info",
     "ising_write_bits", "ising_read_bits", "ising_slab_partition",
     "ising_set_sweep_mode", "ising_create_part", "ising_part_export", "ising_part_attach", "ising_sweep_phase",
+    "ising_correlation_noalloc",
 ]
 
 
@@ -79,6 +80,7 @@ def load_library():
     lib.ising_sweep.argtypes = [vp, i64]
     lib.ising_observables.argtypes = [vp, C.POINTER(_Obs)]
     lib.ising_correlation.argtypes = [vp, i64, vp, vp]
+    lib.ising_correlation_noalloc.argtypes = [vp, i64, vp, vp]
     lib.ising_correlation_protocol.argtypes = [vp, i64, vp, vp, vp, vp, C.POINTER(i64)]
     lib.ising_correlation_list.argtypes = [vp, i64, i64, vp, vp, vp]
     lib.ising_schwinger_dyson.argtypes = [vp, vp, C.POINTER(dbl)]
@@ -299,6 +301,13 @@ class IsingSim:
         sx = np.zeros(rmax, dtype=np.int64)
         sy = np.zeros(rmax, dtype=np.int64)
         _check(self._lib.ising_correlation(self._h, rmax, sx.ctypes.data, sy.ctypes.data))
+        return sx, sy
+
+    def correlation_noalloc(self, rmax: int):
+        """ising_correlation on a static device scratch array: no allocation, L <= 1024 (ISING_NOALLOC_MAX_L)."""
+        sx = np.zeros(rmax, dtype=np.int64)
+        sy = np.zeros(rmax, dtype=np.int64)
+        _check(self._lib.ising_correlation_noalloc(self._h, rmax, sx.ctypes.data, sy.ctypes.data))
         return sx, sy
 
     def correlation_list(self, stride: int, r):
