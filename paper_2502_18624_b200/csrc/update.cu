@@ -560,6 +560,7 @@ namespace cg = cooperative_groups;
 struct ClusterParams {
     uint4 *lat[2];              // the two colour arrays in global memory (read at the start, written back at the end)
     int L, cols, rows_per_cta, n_sweeps;
+    int by_vector;              // 1: a thread per 128-bit vector (the 2-bit layout always); 0: a thread per 32-bit half
     uint32_t t;
     UpdParams u;                // thresholds, carry constants, tables, round keys, tally (pointer members of the lattice unused)
 };
@@ -607,6 +608,46 @@ __device__ __forceinline__ void cluster_phase(const ClusterParams &p, char *cons
     }
 }
 
+// The same phase at the granularity of a 32-bit half (8 sites, two Philox calls) per thread, for the 4-bit models:
+// four times the threads of cluster_phase and a quarter of its serial work per thread.  A phase of a tiny lattice is
+// a latency chain, not a throughput problem (2 warps per CTA at L = 256), so this is what shortens it.  The in-row
+// neighbour half comes straight from shared memory: index (hq -+ 1) mod (halves per row) IS the wrap of the row.
+template <int MODEL, int C, int V, int TALLY>
+__device__ __forceinline__ void cluster_phase_halves(const ClusterParams &p, char *own, const char *opp,
+                                                     const char *opp_above, const char *opp_below, uint32_t t_eff,
+                                                     const uint32_t *s_tab, uint64_t always, int y_first, int &dB, int &dM, int &dQ)
+{
+    constexpr bool kIsing = MODEL == ISING_MODEL_ISING;
+    const unsigned char *ctab = reinterpret_cast<const unsigned char *>(s_tab + 80);
+    const int cols = p.cols, rows = p.rows_per_cta, H = cols * 4;          // H = 32-bit halves per colour row
+    const int items = rows * H, half_items = items >> 1;
+    const size_t rs = (size_t)H * 4;
+    // items ordered so that a warp works on rows of one parity: first all even local rows, then all odd ones
+    for (int i = threadIdx.x; i < items; i += blockDim.x) {
+        const int par = i >= half_items, j = par ? i - half_items : i;
+        const int yl = 2 * (j / H) + par, hq = j - (j / H) * H, col = hq >> 2, q = hq & 3;
+        const uint32_t *own_row = reinterpret_cast<const uint32_t *>(own + yl * rs);
+        const uint32_t *opp_row = reinterpret_cast<const uint32_t *>(opp + yl * rs);
+        const uint32_t *up_row = reinterpret_cast<const uint32_t *>(yl == 0 ? opp_above : opp + (yl - 1) * rs);
+        const uint32_t *dn_row = reinterpret_cast<const uint32_t *>(yl == rows - 1 ? opp_below : opp + (yl + 1) * rs);
+        const uint32_t x = own_row[hq], sm = opp_row[hq], up = up_row[hq], dn = dn_row[hq];
+        // y_first is even: the row parity (y + C) & 1 is C for par = 0 and 1 - C for par = 1.  Parity 0: the other in-row
+        // neighbour is k - 1 (nibbles shifted up, the top nibble of the previous half comes in), parity 1: k + 1.
+        const bool p0 = (par == 0) == (C == 0);
+        const uint32_t nb = opp_row[p0 ? (hq == 0 ? H - 1 : hq - 1) : (hq == H - 1 ? 0 : hq + 1)];
+        const uint32_t sd = p0 ? __funnelshift_l(nb, sm, 4) : __funnelshift_r(sm, nb, 4);
+        const uint64_t g0 = (uint64_t)(y_first + yl) * (uint64_t)(cols * 8) + (uint64_t)(col * 8);
+        const PhiloxRow pr = philox_row((uint32_t)(g0 >> 32), t_eff, C, p.u.rk);
+        const uint32_t gl = (uint32_t)g0 | (uint32_t)(2 * q);
+        const uint4 ra = philox_site4(CTR(gl, 0), pr, p.u.rk), rb = philox_site4(CTR(gl, 1), pr, p.u.rk);
+        uint32_t o;
+        if (kIsing) o = V == 0 ? ising_half_carry(x, up, dn, sm, sd, ra, rb, p.u) : ising_half(x, up, dn, sm, sd, ra, rb, p.u);
+        else o = V == 0 ? bc_half_carry(x, up, dn, sm, sd, ra, rb, ctab) : bc_half(x, up, dn, sm, sd, ra, rb, s_tab, always);
+        if (TALLY) tally_half<MODEL>(x, o, up, dn, sm, sd, dB, dM, dQ);
+        reinterpret_cast<uint32_t *>(own + yl * rs)[hq] = o;
+    }
+}
+
 template <int MODEL, int V, int TALLY>
 __global__ void __launch_bounds__(1024) sweep_cluster_kernel(const __grid_constant__ ClusterParams p)
 {
@@ -635,9 +676,15 @@ __global__ void __launch_bounds__(1024) sweep_cluster_kernel(const __grid_consta
     int dB = 0, dM = 0, dQ = 0;
     const char *opp0 = mine[1], *opp1 = mine[0];
     for (int s = 0; s < p.n_sweeps; ++s) {
-        cluster_phase<MODEL, 0, V, TALLY>(p, &mine[0], &opp0, above[1], below[1], p.t + (uint32_t)s, s_tab, always, y_first, dB, dM, dQ);
+        if (RowFmt<MODEL>::kTwoBit || p.by_vector)
+            cluster_phase<MODEL, 0, V, TALLY>(p, &mine[0], &opp0, above[1], below[1], p.t + (uint32_t)s, s_tab, always, y_first, dB, dM, dQ);
+        else
+            cluster_phase_halves<MODEL, 0, V, TALLY>(p, mine[0], opp0, above[1], below[1], p.t + (uint32_t)s, s_tab, always, y_first, dB, dM, dQ);
         cluster.sync();
-        cluster_phase<MODEL, 1, V, TALLY>(p, &mine[1], &opp1, above[0], below[0], p.t + (uint32_t)s, s_tab, always, y_first, dB, dM, dQ);
+        if (RowFmt<MODEL>::kTwoBit || p.by_vector)
+            cluster_phase<MODEL, 1, V, TALLY>(p, &mine[1], &opp1, above[0], below[0], p.t + (uint32_t)s, s_tab, always, y_first, dB, dM, dQ);
+        else
+            cluster_phase_halves<MODEL, 1, V, TALLY>(p, mine[1], opp1, above[0], below[0], p.t + (uint32_t)s, s_tab, always, y_first, dB, dM, dQ);
         cluster.sync();
     }
     for (int c = 0; c < 2; ++c) {
@@ -665,7 +712,17 @@ cudaError_t launch_sweeps_cluster(ising_sim *h, uint32_t t0, int n_sweeps)
     p.rows_per_cta = (int)(h->L / nc);
     const size_t smem = (size_t)2 * p.rows_per_cta * colour_row_words(h) * 8;
     if (smem > 200 * 1024) return cudaErrorNotSupported;
-    const int items = p.rows_per_cta * p.cols;
+    // a thread per half below L = 512: there a phase is a latency chain and a quarter of the serial work per thread
+    // wins (per 200 sweeps: L = 128 0.91 -> 0.31 ms, 256 0.60 -> 0.36, 384 0.92 -> 0.65, 448 0.87 -> 0.77); at L = 512 a
+    // CTA of 1024 half-threads is throughput-bound and the vector form, which shares the side-word and Philox-row
+    // work of four halves, is faster (0.68 vs 0.85 ms)
+    p.by_vector = (h->model == ISING_MODEL_BLUME_CAPEL_2BIT || p.rows_per_cta * p.cols >= 256) ? 1 : 0;
+#if defined(CLUSTER_BY_VECTOR)
+    p.by_vector = 1;
+#elif defined(CLUSTER_BY_HALVES)
+    p.by_vector = h->model == ISING_MODEL_BLUME_CAPEL_2BIT ? 1 : 0;
+#endif
+    const int items = p.rows_per_cta * p.cols * (p.by_vector ? 1 : 4);
     int block = 32;
     while (block < items && block < 1024) block *= 2;
     const int v = effective_variant(h);

@@ -710,3 +710,26 @@ def test_run_protocol_schedule_matches_oracle(eng, model):
         buf = [np.zeros(8, dtype=np.int64) for _ in range(5)]
         assert lib.ising_run_protocol_schedule(sim._h, 1, tm.ctypes.data, 8, *(b.ctypes.data for b in buf), None) == -1   # cap too small
         assert sim.observables().sweeps_done == 9                # nothing was swept
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("model,L,beta,D", [(ISING, 192, 0.0, 0.0), (ISING, 384, wl.BETA_C, 0.0), (ISING, 128, 3.0, 0.0), (ISING, 64, 40.0, 0.0),
+                                            (BC, 128, 1 / 1.4, 1.0), (BC, 448, 0.0, 1.0), (BC, 192, 12.0, 0.5), (BC, 512, 1 / 1.4, 1.0)])
+def test_cluster_kernel_half_granularity_variants_and_edge_thresholds(eng, variant, model, L, beta, D):
+    """The cluster kernel below L = 512 gives every 32-bit half a thread (cluster_phase_halves; L = 512: a thread per
+    vector): both flip-rule variants, thresholds that are 2^32 (beta = 0), exactly 0 (beta = 3, 12, 40: the carry forms fold
+    or fall back) and ordinary, with the fused tally, sizes whose halves do not fill the block -- against the oracle."""
+    seed, n = 31, 9
+    s = oracle.init(model, L, seed)
+    tl = oracle.observables(s)
+    for t in range(n):
+        tl = oracle.sweep(model, s, beta, D, seed, t, tl)
+    with eng.IsingSim(model, L, beta, D, seed) as sim:
+        sim.set_variant(variant)
+        sim.set_tally(True)
+        k0 = sim.launch_count()
+        sim.sweep(n)                                             # automatic mode: one cluster launch
+        assert sim.launch_count() - k0 == 1
+        assert (sim.read_lattice() == s).all()
+        a, b = sim.tally(), sim.observables()
+        assert (a.bond_sum, a.M, a.Q) == (b.bond_sum, b.M, b.Q) == tl
