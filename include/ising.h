@@ -133,7 +133,7 @@ int ising_sweep_phase(ising_t *h, int colour);
 /* n >= 0 full sweeps: colour 0 then colour 1 ("two update phases"),
  * one Philox number per site, accept iff r < T.  Asynchronous:
  * 2n kernel launches on the handle's stream, no host synchronisation; small
- * lattices run in one cluster kernel (L <= 512) or replay a CUDA graph of 16 sweeps (L <= 2048, n >= 32);
+ * lattices run in one cluster kernel (L <= 512) or replay a CUDA graph (L <= 2^14);
  * see ising_set_sweep_mode.                                                                  */
 int ising_sweep(ising_t *h, int64_t n);
 
@@ -267,8 +267,10 @@ int ising_set_launch(ising_t *h, int rows_per_thread, int block_threads);
  * kept for parity / performance comparison).                                */
 int ising_set_variant(ising_t *h, int variant);
 
-/* How ising_sweep runs launch-bound lattices (L <= 2048, unsharded; results never depend on it): 0 = automatic
- * (4 for L <= 512, else 1), 1 = replay of a CUDA graph of 16 sweeps when n >= 32, 2 = one launch per colour
+/* How ising_sweep runs launch-bound lattices (unsharded; results never depend on it): 0 = automatic
+ * (4 for L <= 512, else 1), 1 = replay of a CUDA graph (L <= 2^14, where a launch gap of about 2.4 microseconds
+ * still shows: a graph of 16 sweeps when n >= 32, a graph of exactly n sweeps when the same 4 <= n < 32 is asked
+ * for twice in a row -- "E, M every 10 sweeps"), 2 = one launch per colour
  * phase, 3 = one cooperative launch for all n sweeps with a grid-wide barrier after every colour phase
  * (measured a little slower than the graph), 4 = one thread-block cluster of 16 CTAs that
  * keeps the lattice in distributed shared memory for all n sweeps, halo rows read from the neighbouring CTA's

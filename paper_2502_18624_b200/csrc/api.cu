@@ -543,6 +543,10 @@ extern "C" int64_t ising_launch_count(const ising_t *h) { return h ? h->launches
 // of kGraphSweeps sweeps whose kernels carry t = 0..K-1; the base sweep number is a device word that
 // a one-thread kernel sets before every replay.  Same kernels, same numbers, fewer launch gaps.
 static const int kGraphSweeps = 16;
+#ifndef GRAPH_MAX_SITES
+#define GRAPH_MAX_SITES (1ll << 28)
+#endif
+static const int64_t kGraphMaxSites = GRAPH_MAX_SITES;      // L <= 2^14
 
 __global__ void set_t_base_kernel(uint32_t *t_base, uint32_t value) { *t_base = value; }
 
@@ -575,20 +579,24 @@ static cudaError_t launch_colour(ising_sim *h, int c, uint32_t t)
 
 static void drop_graph(ising_sim *h)
 {
-    if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
+    for (int k = 0; k < 2; ++k)
+        if (h->graph_exec[k]) { cudaGraphExecDestroy(h->graph_exec[k]); h->graph_exec[k] = nullptr; }
 }
 
-static bool graph_worthwhile(const ising_sim *h, int64_t n)
+// A dependent plain launch costs about 2.4 microseconds on B200; a colour phase takes 1.5 us at L = 1024, 10 us at
+// L = 4096, 104 us at L = 2^14.  Replaying the sweeps from a graph removes that gap: +30 % at L = 4096, +9 % at 8192,
+// +2.3 % at 2^14 (profiles/r02_README.md); above that it is below 1 % and the graph is not built.
+static bool graph_allowed(const ising_sim *h)
 {
-    const int64_t sites = h->L * h->L;
-    return n >= 2 * kGraphSweeps && sites <= (1ll << 22) && h->slabs.size() == 1 && !h->part;      // L <= 2048: a colour phase is launch-bound
+    return h->L * h->L <= kGraphMaxSites && h->slabs.size() == 1 && !h->part && (h->sweep_mode <= 1 || h->sweep_mode >= 3);
 }
 
-static int ensure_graph(ising_sim *h)
+// Graph `slot` holding `sweeps` sweeps whose kernels carry t = 0..sweeps-1 (the base sweep number is a device word).
+static int ensure_graph(ising_sim *h, int slot, int sweeps)
 {
-    const int key[4] = {h->rows_per_thread, h->block_threads, h->variant, h->tally_on ? 1 : 0};
-    if (h->graph_exec && memcmp(key, h->graph_key, sizeof(key)) == 0) return ISING_OK;
-    drop_graph(h);
+    const int key[5] = {h->rows_per_thread, h->block_threads, h->variant, h->tally_on ? 1 : 0, sweeps};
+    if (h->graph_exec[slot] && memcmp(key, h->graph_key[slot], sizeof(key)) == 0) return ISING_OK;
+    if (h->graph_exec[slot]) { cudaGraphExecDestroy(h->graph_exec[slot]); h->graph_exec[slot] = nullptr; }
     // captured on a private stream (the caller's may be the legacy default stream, which cannot be
     // captured); the instantiated graph is then launched on the caller's stream
     cudaGraph_t graph = nullptr;
@@ -599,7 +607,7 @@ static int ensure_graph(ising_sim *h)
     h->graph_capture = true;
     h->stream = h->slabs[0].stream = cap;
     const int64_t launches_before = h->launches;
-    for (int j = 0; j < kGraphSweeps && e == cudaSuccess; ++j)
+    for (int j = 0; j < sweeps && e == cudaSuccess; ++j)
         for (int c = 0; c < 2 && e == cudaSuccess; ++c) e = launch_colour(h, c, (uint32_t)j);
     h->stream = h->slabs[0].stream = user;
     h->graph_capture = false;
@@ -610,10 +618,21 @@ static int ensure_graph(ising_sim *h)
         if (graph) cudaGraphDestroy(graph);
         return cuda_fail(e != cudaSuccess ? e : e2, "CUDA graph capture of the sweep loop");
     }
-    e = cudaGraphInstantiate(&h->graph_exec, graph, 0);
+    e = cudaGraphInstantiate(&h->graph_exec[slot], graph, 0);
     cudaGraphDestroy(graph);
-    if (e != cudaSuccess) { h->graph_exec = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
-    memcpy(h->graph_key, key, sizeof(key));
+    if (e != cudaSuccess) { h->graph_exec[slot] = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
+    memcpy(h->graph_key[slot], key, sizeof(key));
+    return ISING_OK;
+}
+
+static int replay_graph(ising_sim *h, int slot, int sweeps)
+{
+    uint32_t *t_base = reinterpret_cast<uint32_t *>(h->d_acc + 48) + 1;
+    set_t_base_kernel<<<1, 1, 0, h->stream>>>(t_base, (uint32_t)h->t);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaGraphLaunch(h->graph_exec[slot], h->stream));
+    h->launches += 1 + 2 * sweeps;
+    h->t += sweeps;
     return ISING_OK;
 }
 
@@ -652,17 +671,24 @@ extern "C" int ising_sweep(ising_t *h, int64_t n)
             n -= chunk;
         }
     }
-    if (graph_worthwhile(h, n) && (h->sweep_mode <= 1 || h->sweep_mode >= 3)) {
-        int rc = ensure_graph(h);
+    if (graph_allowed(h) && n >= 2 * kGraphSweeps) {
+        int rc = ensure_graph(h, 0, kGraphSweeps);
         if (rc) return rc;
-        uint32_t *t_base = reinterpret_cast<uint32_t *>(h->d_acc + 48) + 1;
         while (n >= kGraphSweeps) {
-            set_t_base_kernel<<<1, 1, 0, h->stream>>>(t_base, (uint32_t)h->t);
-            CUDA_TRY(cudaGetLastError());
-            CUDA_TRY(cudaGraphLaunch(h->graph_exec, h->stream));
-            h->launches += 1 + 2 * kGraphSweeps;
-            h->t += kGraphSweeps;
+            rc = replay_graph(h, 0, kGraphSweeps);
+            if (rc) return rc;
             n -= kGraphSweeps;
+        }
+    } else if (graph_allowed(h) && n >= 4) {
+        // a short count asked for a second time in a row gets a graph of exactly that many sweeps
+        if (n == h->last_short_n) {
+            int rc = ensure_graph(h, 1, (int)n);
+            if (rc) return rc;
+            rc = replay_graph(h, 1, (int)n);
+            if (rc) return rc;
+            n = 0;
+        } else {
+            h->last_short_n = n;
         }
     }
     if (n > 0) {

@@ -80,8 +80,11 @@ struct ising_sim {
     // CUDA graph of K sweeps for launch-bound (small) lattices: kernels baked with t = 0..K-1, the base
     // sweep number lives in device memory (d_acc[48] as two uint32: [0] = 0 for plain launches, [1] = base)
     bool graph_capture = false;
-    cudaGraphExec_t graph_exec = nullptr;
-    int graph_key[4] = {0, 0, 0, 0};                          // rows_per_thread, block_threads, variant, tally_on
+    // two cached graphs: [0] of kGraphSweeps sweeps (long runs), [1] of a short sweep count that is asked for again and
+    // again ("E, M every 10 sweeps": ising_run_schedule, the bench step)
+    cudaGraphExec_t graph_exec[2] = {nullptr, nullptr};
+    int graph_key[2][5] = {{0, 0, 0, 0, 0}, {0, 0, 0, 0, 0}};  // rows_per_thread, block_threads, variant, tally_on, sweeps in the graph
+    int64_t last_short_n = 0;                                 // the previous call's n when it was too short for graph [0]
     bool tally_on = false;                                    // A7: update kernels keep running B, M, Q at d_acc[40..42]
     int sweep_mode = 0;                                       // small lattices (ising_set_sweep_mode): 0 auto, 1 graph, 2 plain, 3 persistent, 4 cluster
     int corr_path = 0;                                        // ising_set_corr_path: 0 auto, 1 bit planes, 2-4 tensor cores

@@ -733,3 +733,46 @@ def test_cluster_kernel_half_granularity_variants_and_edge_thresholds(eng, varia
         assert (sim.read_lattice() == s).all()
         a, b = sim.tally(), sim.observables()
         assert (a.bond_sum, a.M, a.Q) == (b.bond_sum, b.M, b.Q) == tl
+
+
+@pytest.mark.parametrize("model,L,beta,D", [(ISING, 1024, wl.BETA_C / 0.5, 0.0), (BC, 576, 1 / 1.4, 1.0), (wl.ISING_LUT, 512, wl.BETA_C / 0.9, 0.0),
+                                            (ISING, 4096, wl.BETA_C / 0.9, 0.0)])
+def test_short_repeated_sweep_counts_replay_a_graph_of_their_own(eng, model, L, beta, D):
+    """"E, M every 10 sweeps": the second call in a row with the same short count runs from a graph of exactly that many
+    sweeps (one set-base kernel + 2n update kernels per call, the same launch count as plain launches + 1).  Changing the
+    count, the launch geometry or the tally in between must rebuild it; the trajectory is the oracle's throughout."""
+    seed = 19
+    if model == wl.ISING_LUT:
+        s = oracle.lut_init(L, seed)
+        step = lambda t, tl: oracle.lut_sweep(s, beta, seed, t, tl)
+    else:
+        s = oracle.init(model, L, seed)
+        step = lambda t, tl: oracle.sweep(model, s, beta, D, seed, t, tl)
+    tl = oracle.observables(s)
+    plan = [10, 10, 10, 7, 7, 10, 10, 5, 5, 5]                  # counts per call
+    with eng.IsingSim(model, L, beta, D, seed) as sim:
+        t = 0
+        for i, n in enumerate(plan):
+            if i == 5:
+                sim.set_launch(4, 64)                            # another key: the graph of 10 is rebuilt
+            if i == 7:
+                sim.set_tally(True)
+            k0 = sim.launch_count()
+            sim.sweep(n)
+            replayed = i > 0 and plan[i - 1] == n
+            assert sim.launch_count() - k0 == 2 * n + (1 if replayed else 0), (i, n)
+            for _ in range(n):
+                tl = step(t, tl)
+                t += 1
+            o = sim.observables()
+            assert (o.bond_sum, o.M, o.Q) == tl and o.sweeps_done == t, (i, n)
+        a = sim.tally()
+        assert (a.bond_sum, a.M, a.Q) == tl
+        assert (sim.read_lattice() == s).all()
+        times = list(range(t + 10, t + 60, 10))                  # the native schedule call: every 10 sweeps
+        got = sim.run_schedule(times)
+        for o in got:
+            for _ in range(10):
+                tl = step(t, tl)
+                t += 1
+            assert (o.bond_sum, o.M, o.Q) == tl
