@@ -147,25 +147,33 @@ def test_parts_in_separate_processes_equal_the_oracle(eng, heights):
         assert covered == L
 
 
-def test_bench_parallel_slabs_two_ranks_on_one_gpu(eng):
-    """bench.py --gpus 2 --parallel slabs under torchrun, both ranks on the one GPU of the box (test hook: gloo instead
-    of NCCL): the sharded step -- part handles, IPC exchange, a collective between colour phases, int64 reduction of
-    the parts' sums -- must print one JSON line whose observables are the oracle's after (warmup + steps) * S sweeps."""
+@pytest.mark.parametrize("parallel", ["slabs", "replicas"])
+def test_bench_two_ranks_on_one_gpu(eng, parallel):
+    """bench.py --gpus 2 under torchrun, both ranks on the one GPU of the box (test hook: gloo instead of NCCL).
+    --parallel slabs: the sharded step -- part handles, IPC exchange, a collective between colour phases, int64
+    reduction of the parts' sums -- must print one JSON line whose observables are the oracle's after
+    (warmup + steps) * S sweeps, and count ONE lattice's updates.  --parallel replicas (the default): two independent
+    lattices (seed + rank), rank 0's observables are the oracle's for the base seed, the value counts both."""
     import json
     import subprocess
     L, S, K, W = 2048, 3, 2, 1
     env = dict(os.environ, ISING_BENCH_RANKS_ON_ONE_GPU="1")
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
-           "--master-port", str(_free_port()), os.path.join(ROOT, "bench.py"), "--gpus", "2", "--parallel", "slabs", "--L", str(L),
+           "--master-port", str(_free_port()), os.path.join(ROOT, "bench.py"), "--gpus", "2", "--parallel", parallel, "--L", str(L),
            "--sweeps-per-step", str(S), "--steps", str(K), "--warmup", str(W), "--no-cpu", "--no-e2e"]
     r = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=600, cwd=ROOT)
     assert r.returncode == 0, r.stderr[-3000:]
     lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
     assert len(lines) == 1                                             # rank 0 alone prints
     d = json.loads(lines[0])
-    assert d["n_gpus"] == 2 and d["scaling"] == "strong" and d["config"]["launch"]["slabs"] == 2 and d["gpu_launches"] == 2 * S * K + K
+    sharded = parallel == "slabs"
+    assert d["n_gpus"] == 2 and d["scaling"] == ("strong" if sharded else "weak")
+    assert d["config"]["launch"]["slabs"] == (2 if sharded else 1)
+    if sharded:
+        assert d["gpu_launches"] == 2 * S * K + K
     cfg = wl.config(2)
     n = (W + K) * S
     s, tl = _oracle_run(cfg.model, L, cfg.beta, cfg.D, cfg.seed, n)
     assert (d["last_observables"]["bond_sum"], d["last_observables"]["M"], d["last_observables"]["sweeps_done"]) == (tl[0], tl[1], n)
-    assert d["value"] == pytest.approx(L * L * S / (d["ms_per_step"] * 1e6), rel=1e-9)     # ONE lattice's updates
+    lattices = 1 if sharded else 2
+    assert d["value"] == pytest.approx(lattices * L * L * S / (d["ms_per_step"] * 1e6), rel=1e-9)
