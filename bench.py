@@ -2,7 +2,8 @@
 """bench.py -- spin updates/ns of the checkerboard Metropolis hot path on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--L L] [--sweeps-per-step S] [--model ising|bc]
+                    [--config 0..4] [--L L] [--sweeps-per-step S] [--model ising|bc|lut|bc2]
+                    [--slabs S] [--parallel replicas|slabs] [--tally] [--workload sweep|corr]
 
 A "step" = S full sweeps (black + white update kernels)
 followed by one observables pass (A8: E, M every S sweeps as in BASELINE.json
@@ -11,10 +12,12 @@ Ising L = 2^18, T = 0.9 Tc, seed 1 (32 GiB packed, far larger than L2, so no L2
 flush is needed between iterations).  Prints ONE JSON line (rank 0).
 
 value     = L^2 * S * K / (device time of the K steps), lattice resident in HBM
-e2e       = same through the C ABI with HOST buffers: every step uploads the packed
-            lattice from pinned host memory (ising_write_packed), runs S sweeps and
-            reads the observables back; two handles on two streams alternate so that
-            the next step's upload overlaps this step's sweeps (serial figure beside it)
+e2e       = same through the C ABI with HOST buffers: every step uploads the lattice from
+            pinned host memory in the compact transport format (ising_write_bits: 1 bit per
+            Ising spin, 2 per Blume-Capel spin, expanded on the device), runs S sweeps and
+            reads the observables back; two handles on two streams alternate so that the
+            next step's upload overlaps this step's sweeps (serial figure beside it); the
+            observables of every e2e step are asserted equal to a device-resident run's
 roofline  = the update kernel against the bound that actually limits it: the integer
             ALU ("one Philox4x32-10 number per site" = 9.25 dispatch slots per site,
             DESIGN.md Sec. 5.1); peak derived from unit counts and the max SM clock, with
