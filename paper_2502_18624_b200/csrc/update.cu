@@ -320,17 +320,17 @@ __device__ __forceinline__ void tally_half(uint32_t x, uint32_t y, uint32_t up, 
         dB += 4 * (int)nibble_sum32(d & (F * 15u)) - 8 * cnt;
         dM += 2 * cnt - 4 * cnt_up;
     } else {
-        // codes 0, 1, 2 <-> s = -1, 0, +1: bit 0 marks s = 0, bit 1 marks s = +1.  Word level:
-        // sum (s1 - s0) = sum (c1 - c0) from four POPCs, s^2 = 1 unless bit 0, and per site
-        // c * S = (S where bit 0) + 2 (S where bit 1), so sum (c1 - c0)(S - 4) is four masked nibble sums.
-        const uint32_t S = up + dn + sm + sd;                      // h + 4 per nibble, <= 8
-        const uint32_t x0 = x & ONES, x1 = (x >> 1) & ONES, y0 = y & ONES, y1 = (y >> 1) & ONES;
-        const int px0 = __popc(x0), py0 = __popc(y0);
-        const int m = py0 + 2 * __popc(y1) - px0 - 2 * __popc(x1);
+        // codes c = s + 1 in {0, 1, 2}; S = h + 4.  Word level, by 4-way byte dot products (IDP4A) on the nibbles spread
+        // to bytes (as in observe.cu): with m = sum (c1 - c0),
+        //   dM = m,   dB = sum (c1 - c0)(S - 4) = sum c1 S - sum c0 S - 4 m,   dQ = sum (c1 - 1)^2 - (c0 - 1)^2 = sum c1^2 - sum c0^2 - 2 m.
+        const uint32_t S = up + dn + sm + sd, lo = 0x0F0F0F0Fu, one = 0x01010101u;
+        const uint32_t Se = S & lo, So = (S >> 4) & lo, xe = x & lo, xo = (x >> 4) & lo, ye = y & lo, yo = (y >> 4) & lo;
+        const uint32_t by = __dp4a(yo, So, __dp4a(ye, Se, 0u)), bx = __dp4a(xo, So, __dp4a(xe, Se, 0u));
+        const uint32_t qy = __dp4a(yo, yo, __dp4a(ye, ye, 0u)), qx = __dp4a(xo, xo, __dp4a(xe, xe, 0u));
+        const int m = (int)__dp4a(ye + yo, one, 0u) - (int)__dp4a(xe + xo, one, 0u);
         dM += m;
-        dQ += px0 - py0;
-        dB += (int)nibble_sum32(S & (y0 * 15u)) + 2 * (int)nibble_sum32(S & (y1 * 15u))
-            - (int)nibble_sum32(S & (x0 * 15u)) - 2 * (int)nibble_sum32(S & (x1 * 15u)) - 4 * m;
+        dB += (int)by - (int)bx - 4 * m;
+        dQ += (int)qy - (int)qx - 2 * m;
     }
 }
 
