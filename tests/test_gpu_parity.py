@@ -712,6 +712,31 @@ def test_run_protocol_schedule_matches_oracle(eng, model):
         assert sim.observables().sweeps_done == 9                # nothing was swept
 
 
+@pytest.mark.parametrize("model,L,tally", [(ISING, 4096, False), (BC, 2048, True), (wl.BLUME_CAPEL_2BIT, 2048, False), (wl.ISING_LUT, 4096, False)])
+def test_protocol_schedule_equals_one_call_per_time(eng, model, L, tally):
+    """ising_run_protocol_schedule over many closely spaced times, a repeated time (no sweep in between), a second call
+    with a longer list, with and without the observables, all four layouts -- every row equals what one sweep call + one
+    ising_correlation_protocol call per time give on a twin handle, and the empty schedule is a no-op."""
+    beta, D = (1 / 1.4, 1.0) if model in (BC, wl.BLUME_CAPEL_2BIT) else (wl.BETA_C / 0.5, 0.0)
+    first, second = [1, 2, 2, 3, 5, 6, 40], [41, 43, 44, 44, 45, 47, 50, 51, 52, 90]
+    with eng.IsingSim(model, L, beta, D, 8) as sim, eng.IsingSim(model, L, beta, D, 8) as twin:
+        if tally:
+            sim.set_tally(True)
+        for times, with_obs in ((first, True), (second, False)):
+            rows, obs = sim.run_protocol_schedule(times, with_observables=with_obs)
+            assert len(rows) == len(times) and (obs is None) == (not with_obs)
+            for k, t in enumerate(times):
+                twin.sweep(t - twin.observables().sweeps_done)
+                r, sx, sy, ns = twin.correlation_protocol()
+                assert all((a == b).all() for a, b in zip(rows[k], (r, sx, sy, ns))), (t, k)
+                assert len(rows[k][0]) == len(eng.protocol_distances(L, t)[0])
+                if with_obs:
+                    o = twin.observables()
+                    assert (obs[k].bond_sum, obs[k].M, obs[k].Q, obs[k].sweeps_done) == (o.bond_sum, o.M, o.Q, t)
+        assert (sim.read_lattice(0, 64) == twin.read_lattice(0, 64)).all()
+        assert sim.run_protocol_schedule([]) == ([], [])
+
+
 @pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("model,L,beta,D", [(ISING, 192, 0.0, 0.0), (ISING, 384, wl.BETA_C, 0.0), (ISING, 128, 3.0, 0.0), (ISING, 64, 40.0, 0.0),
                                             (BC, 128, 1 / 1.4, 1.0), (BC, 448, 0.0, 1.0), (BC, 192, 12.0, 0.5), (BC, 512, 1 / 1.4, 1.0)])
