@@ -308,6 +308,10 @@ __device__ __forceinline__ uint32_t nibble_sum32(uint32_t v)
     return (t * 0x01010101u) >> 24;
 }
 
+#ifndef TALLY_BY_ROW
+#define TALLY_BY_ROW 1
+#endif
+
 template <int MODEL>
 __device__ __forceinline__ void tally_half(uint32_t x, uint32_t y, uint32_t up, uint32_t dn, uint32_t sm, uint32_t sd,
                                            int &dB, int &dM, int &dQ)
@@ -340,6 +344,27 @@ __device__ __forceinline__ void tally_row(const uint4 &x, const uint4 &y, const 
 {
     uint32_t sd[4];
     side_words<MODEL, P>(sm, edge, sd);
+    if (MODEL == ISING_MODEL_ISING && TALLY_BY_ROW) {
+        // the four halves of the row together: their flip bits sit at bit 0 of every nibble, so F0 + 2 F1 + 4 F2 + 8 F3
+        // holds all of them and one POPC counts the row; the masked counts d (<= 4) of two halves share a nibble
+        const uint32_t xs[4] = {x.x, x.y, x.z, x.w}, ys[4] = {y.x, y.y, y.z, y.w};
+        const uint32_t us[4] = {up.x, up.y, up.z, up.w}, ds[4] = {dn.x, dn.y, dn.z, dn.w}, ss[4] = {sm.x, sm.y, sm.z, sm.w};
+        uint32_t Fc = 0, Xc = 0, v[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const uint32_t F = xs[k] ^ ys[k], n = us[k] + ds[k] + ss[k] + sd[k];
+            const uint32_t d = (n ^ (xs[k] * 7u)) - xs[k] * 3u;   // unequal neighbours before the flip
+            Fc += F << k;
+            Xc += (F & xs[k]) << k;
+            v[k] = d & (F * 15u);
+        }
+        const uint32_t lo = 0x0F0F0F0Fu, v01 = v[0] + v[1], v23 = v[2] + v[3];                  // <= 8 per nibble
+        const uint32_t bytes = (v01 & lo) + ((v01 >> 4) & lo) + (v23 & lo) + ((v23 >> 4) & lo);  // <= 32 per byte
+        const int cnt = __popc(Fc), cnt_up = __popc(Xc);
+        dB += 4 * (int)((bytes * 0x01010101u) >> 24) - 8 * cnt;
+        dM += 2 * cnt - 4 * cnt_up;
+        return;
+    }
     tally_half<MODEL>(x.x, y.x, up.x, dn.x, sm.x, sd[0], dB, dM, dQ);
     tally_half<MODEL>(x.y, y.y, up.y, dn.y, sm.y, sd[1], dB, dM, dQ);
     tally_half<MODEL>(x.z, y.z, up.z, dn.z, sm.z, sd[2], dB, dM, dQ);
