@@ -117,6 +117,44 @@ struct DeviceGuard {
     ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
 };
 
+// Programmatic dependent launch (PTX griddepcontrol).  An update kernel lets the next launch of its stream be
+// scheduled as soon as all of its own blocks have started (launch_dependents at the top), and touches the lattice
+// only after the launch before it has completed and its writes are visible (wait, after the table load): the next
+// phase's blocks are resident, tables loaded, when the last block of this phase retires.  Plain launches only
+// (measured, profiles/r02_README.md: L = 4096 815 -> 967 updates/ns, 2^14 1291 -> 1316, Blume-Capel 2^15 1139 -> 1146):
+// inside a captured CUDA graph the programmatic edges are slower than the graph's ordinary ones (L = 4096 1056 -> 991,
+// 2048 619 -> 328), so launches under capture go without the attribute and both instructions are no-ops there.
+#ifndef UPDATE_PDL
+#define UPDATE_PDL 1
+#endif
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_launch_dependents()
+{
+#if UPDATE_PDL
+    asm volatile("griddepcontrol.launch_dependents;");
+#endif
+}
+__device__ __forceinline__ void pdl_wait()
+{
+#if UPDATE_PDL
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
+}
+
+template <typename Kernel, typename Params>
+static inline cudaError_t launch_with_pdl(Kernel kernel, unsigned grid, int block, size_t smem, cudaStream_t stream, const Params &p,
+                                          bool allow)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = (UPDATE_PDL && allow) ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, p);
+}
+#endif
+
 // host-only arithmetic (host_logic.cu)
 int host_threshold_table(int model, double beta, double D, uint64_t *T);     // returns the number of entries (<= 54)
 void host_time_grid(uint64_t tmax, std::vector<uint64_t> &times);

@@ -197,7 +197,7 @@ template <int C, int V, int TALLY>
 __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const __grid_constant__ LutParams p)
 {
     int dB = 0, dM = 0;
-    const uint32_t t_eff = p.t + __ldg(p.t_base);
+    pdl_launch_dependents();
     __shared__ uint32_t s_tree[16];
     extern __shared__ __align__(16) unsigned char s_buckets[];          // V = 0: 4096 x 8 bytes
     if (threadIdx.x < 16) s_tree[threadIdx.x] = p.tree[threadIdx.x];
@@ -207,6 +207,8 @@ __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const _
         for (int i = threadIdx.x; i < (8 << LUT_BUCKET_BITS) / 16; i += blockDim.x) dst4[i] = src4[i];
     }
     __syncthreads();
+    pdl_wait();                        // tables (written at create / set_beta) are in; the phase before this one is complete from here on
+    const uint32_t t_eff = p.t + __ldg(p.t_base);
     const uint32_t c_root = s_tree[1];
     const BucketTable bk = {(uint32_t)__cvta_generic_to_shared(s_buckets), p.bucket_stride};
     const int cols = p.cols, L = p.L;
@@ -293,7 +295,8 @@ cudaError_t launch_lut_update(ising_sim *h, int slab, int colour, uint32_t t)
     const size_t smem = 8 << LUT_BUCKET_BITS;
     p.tally = sl.d_acc + 40;
     p.t_base = reinterpret_cast<const uint32_t *>(sl.d_acc + 48) + (h->graph_capture ? 1 : 0);
-#define LUT_LAUNCH(C, V, T, SM) lut_update_kernel<C, V, T><<<grid, block, SM, sl.stream>>>(p)
+    cudaError_t le = cudaSuccess;
+#define LUT_LAUNCH(C, V, T, SM) le = launch_with_pdl(lut_update_kernel<C, V, T>, grid, block, SM, sl.stream, p, !h->graph_capture)
     // variant 0 = automatic: the bucket table pays once its 32 KB fill per block is amortised over several
     // waves (L >= 8192); a single-wave launch starts faster with the table-free binary search.
     // 1 = binary search, 2 = bucket table
@@ -313,7 +316,7 @@ cudaError_t launch_lut_update(ising_sim *h, int slab, int colour, uint32_t t)
     }
 #undef LUT_LAUNCH
     h->launches++;
-    return cudaGetLastError();
+    return le != cudaSuccess ? le : cudaGetLastError();
 }
 
 // Resident blocks per SM of the kernel launch_lut_update picks for this handle (0 if the query fails).
