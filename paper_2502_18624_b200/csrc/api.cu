@@ -226,6 +226,7 @@ static int finish_create(ising_sim *h, ising_t **out)
         DeviceGuard g(h->device);
         tune_rows_for_waves(h);
     }
+    h->pdl_in_graph = h->model == ISING_MODEL_ISING_LUT || h->L <= 1536 || (h->model == ISING_MODEL_ISING && h->L <= 3072);
     const Slab &s0 = h->slabs[0];
     h->lat[0] = s0.lat[0]; h->lat[1] = s0.lat[1]; h->d_acc = s0.d_acc; h->d_bc_table = s0.d_table;
     *out = h;

@@ -86,6 +86,7 @@ struct ising_sim {
     int graph_key[2][5] = {{0, 0, 0, 0, 0}, {0, 0, 0, 0, 0}};  // rows_per_thread, block_threads, variant, tally_on, sweeps in the graph
     int64_t last_short_n = 0;                                 // the previous call's n when it was too short for graph [0]
     bool tally_on = false;                                    // A7: update kernels keep running B, M, Q at d_acc[40..42]
+    bool pdl_in_graph = false;                                // programmatic edges inside captured graphs (see launch_with_pdl)
     int sweep_mode = 0;                                       // small lattices (ising_set_sweep_mode): 0 auto, 1 graph, 2 plain, 3 persistent, 4 cluster
     int corr_path = 0;                                        // ising_set_corr_path: 0 auto, 1 bit planes, 2-4 tensor cores
     long long *d_corr = nullptr; size_t d_corr_bytes = 0;
@@ -120,10 +121,14 @@ struct DeviceGuard {
 // Programmatic dependent launch (PTX griddepcontrol).  An update kernel lets the next launch of its stream be
 // scheduled as soon as all of its own blocks have started (launch_dependents at the top), and touches the lattice
 // only after the launch before it has completed and its writes are visible (wait, after the table load): the next
-// phase's blocks are resident, tables loaded, when the last block of this phase retires.  Plain launches only
-// (measured, profiles/r02_README.md: L = 4096 815 -> 967 updates/ns, 2^14 1291 -> 1316, Blume-Capel 2^15 1139 -> 1146):
-// inside a captured CUDA graph the programmatic edges are slower than the graph's ordinary ones (L = 4096 1056 -> 991,
-// 2048 619 -> 328), so launches under capture go without the attribute and both instructions are no-ops there.
+// phase's blocks are resident, tables loaded, when the last block of this phase retires.  launch_dependents comes
+// AFTER the wait: issued at the top, every kernel of a captured graph triggers the one after it at once and the
+// whole chain piles up on the SMs, each generation waiting for the one before (L = 2048: 619 -> 328 updates/ns).
+// Plain launches always carry the attribute (measured, profiles/r02_README.md: L = 4096 815 -> 967, 2^14 1291 ->
+// 1316, Blume-Capel 2^15 1139 -> 1146).  Inside a captured graph the programmatic edges win where the launch latency
+// or the table load dominates -- the 1-bit kernel at every size (+2..7 %), the 4-bit Ising kernel up to L = 3072
+// (+4..7 %), everything up to L = 1536 (+5..14 %) -- and lose 7-11 % at L = 4096 / 8192 (the greedy placement of
+// the early blocks packs a partial wave onto the SMs that free up first): ising_sim::pdl_in_graph, set at create.
 #ifndef UPDATE_PDL
 #define UPDATE_PDL 1
 #endif

@@ -197,7 +197,6 @@ template <int C, int V, int TALLY>
 __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const __grid_constant__ LutParams p)
 {
     int dB = 0, dM = 0;
-    pdl_launch_dependents();
     __shared__ uint32_t s_tree[16];
     extern __shared__ __align__(16) unsigned char s_buckets[];          // V = 0: 4096 x 8 bytes
     if (threadIdx.x < 16) s_tree[threadIdx.x] = p.tree[threadIdx.x];
@@ -208,6 +207,7 @@ __global__ void __launch_bounds__(256, LUT_MIN_BLOCKS) lut_update_kernel(const _
     }
     __syncthreads();
     pdl_wait();                        // tables (written at create / set_beta) are in; the phase before this one is complete from here on
+    pdl_launch_dependents();           // after the wait: at most one later phase sits resident and waiting
     const uint32_t t_eff = p.t + __ldg(p.t_base);
     const uint32_t c_root = s_tree[1];
     const BucketTable bk = {(uint32_t)__cvta_generic_to_shared(s_buckets), p.bucket_stride};
@@ -296,7 +296,7 @@ cudaError_t launch_lut_update(ising_sim *h, int slab, int colour, uint32_t t)
     p.tally = sl.d_acc + 40;
     p.t_base = reinterpret_cast<const uint32_t *>(sl.d_acc + 48) + (h->graph_capture ? 1 : 0);
     cudaError_t le = cudaSuccess;
-#define LUT_LAUNCH(C, V, T, SM) le = launch_with_pdl(lut_update_kernel<C, V, T>, grid, block, SM, sl.stream, p, !h->graph_capture)
+#define LUT_LAUNCH(C, V, T, SM) le = launch_with_pdl(lut_update_kernel<C, V, T>, grid, block, SM, sl.stream, p, h->pdl_in_graph || !h->graph_capture)
     // variant 0 = automatic: the bucket table pays once its 32 KB fill per block is amortised over several
     // waves (L >= 8192); a single-wave launch starts faster with the table-free binary search.
     // 1 = binary search, 2 = bucket table

@@ -463,10 +463,10 @@ template <int MODEL, int C, int V, int TALLY>
 __global__ void __launch_bounds__(256) update_kernel(const __grid_constant__ UpdParams p)
 {
     int dB = 0, dM = 0, dQ = 0;                            // TALLY: this thread's share of the changes
-    pdl_launch_dependents();
     __shared__ __align__(16) uint32_t s_tab[80 + 132];
     const uint64_t always = load_tables<MODEL>(p, s_tab);  // thresholds and tables: written at create / set_beta, not by a sweep
     pdl_wait();                                            // the phase before this one is complete from here on
+    pdl_launch_dependents();                               // after the wait: at most one later phase sits resident and waiting
     const uint32_t t_eff = p.t + __ldg(p.t_base);
     update_chunk<MODEL, C, V, TALLY>(p, blockIdx.x * blockDim.x + threadIdx.x, t_eff, s_tab, always, dB, dM, dQ);
     if (TALLY) {            // warp sums fit 32 bits (<= 32 lanes x R rows x 32 sites x 8); threads past the lattice add zeros
@@ -562,7 +562,7 @@ cudaError_t launch_update(ising_sim *h, int slab, int colour, uint32_t t)
     const unsigned grid = (unsigned)((threads + block - 1) / block);
     const int v = effective_variant(h);
     cudaError_t le = cudaSuccess;
-#define LAUNCH_UPD(MODEL, C, V, T) le = launch_with_pdl(update_kernel<MODEL, C, V, T>, grid, block, 0, sl.stream, p, !h->graph_capture)
+#define LAUNCH_UPD(MODEL, C, V, T) le = launch_with_pdl(update_kernel<MODEL, C, V, T>, grid, block, 0, sl.stream, p, h->pdl_in_graph || !h->graph_capture)
 #define PICK_T(MODEL, C, V) do { if (h->tally_on) LAUNCH_UPD(MODEL, C, V, 1); else LAUNCH_UPD(MODEL, C, V, 0); } while (0)
 #define PICK_V(MODEL, C) do { if (v == 0) PICK_T(MODEL, C, 0); else PICK_T(MODEL, C, 1); } while (0)
     if (h->model == ISING_MODEL_ISING) { if (colour == 0) PICK_V(ISING_MODEL_ISING, 0); else PICK_V(ISING_MODEL_ISING, 1); }
