@@ -44,7 +44,7 @@ def test_lattice_and_observables_every_sweep(eng, L, beta, seed, n):
     s = oracle.lut_init(L, seed)
     tl = oracle.observables(s)
     with eng.IsingSim(LUT, L, beta, 0.0, seed) as sim:
-        sim.set_variant(2)                                   # the bucket-table kernel (automatic from L = 8192)
+        sim.set_variant(2)                                   # the bucket-table kernel (automatic from L = 6144)
         assert (sim.read_lattice() == s).all()
         for t in range(n):
             sim.sweep(1)
