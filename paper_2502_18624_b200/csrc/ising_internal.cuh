@@ -118,10 +118,10 @@ struct DeviceGuard {
     ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
 };
 
-// Programmatic dependent launch (PTX griddepcontrol).  An update kernel lets the next launch of its stream be
-// scheduled as soon as all of its own blocks have started (launch_dependents at the top), and touches the lattice
-// only after the launch before it has completed and its writes are visible (wait, after the table load): the next
-// phase's blocks are resident, tables loaded, when the last block of this phase retires.  launch_dependents comes
+// Programmatic dependent launch (PTX griddepcontrol).  An update kernel loads its tables, then waits until the launch
+// before it has completed and its writes are visible (griddepcontrol.wait: every lattice access comes after it), then
+// lets the next launch of its stream be scheduled (griddepcontrol.launch_dependents): the next phase's blocks take the
+// SM slots as they free up and sit ready, tables loaded, when the last block of this phase retires.  The trigger comes
 // AFTER the wait: issued at the top, every kernel of a captured graph triggers the one after it at once and the
 // whole chain piles up on the SMs, each generation waiting for the one before (L = 2048: 619 -> 328 updates/ns).
 // Plain launches always carry the attribute (measured, profiles/r02_README.md: L = 4096 815 -> 967, 2^14 1291 ->
