@@ -88,7 +88,12 @@ static void tune_rows_for_waves(ising_sim *h)
     int64_t rows = 0;
     for (const Slab &sl : h->slabs) rows = std::max(rows, sl.rows);
     auto blocks = [&](int64_t r) { return (((rows + r - 1) / r) * cols + block - 1) / block; };
-    if (blocks(rmax) > 16 * capacity) return;                   // many waves: the tail is a few per cent at most
+    if (blocks(rmax) > 16 * capacity) {                         // many waves: the tail is a few per cent at most
+        // 4-bit Ising kernel: longer columns re-read fewer halo rows (2 per R) -- L = 2^18: R = 32 1450.9, 64 1454.5,
+        // 128 1455.5, 512 1449.0 updates/ns (profiles/r02_README.md); the table kernels lose with long columns
+        if (h->model == ISING_MODEL_ISING && blocks(128) > 16 * capacity) h->rows_per_thread = 128;
+        return;
+    }
     double best = 0.0;
     int64_t best_r = h->rows_per_thread;
     for (int64_t r = 2; r <= rmax; r += 2) {
