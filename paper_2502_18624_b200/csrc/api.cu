@@ -94,11 +94,15 @@ static void tune_rows_for_waves(ising_sim *h)
         if (h->model == ISING_MODEL_ISING && blocks(128) > 16 * capacity) h->rows_per_thread = 128;
         return;
     }
+    const double wave_slack = is_blume_capel(h->model) ? 0.5 : 0.0;
     double best = 0.0;
     int64_t best_r = h->rows_per_thread;
     for (int64_t r = 2; r <= rmax; r += 2) {
         const int64_t waves = (blocks(r) + capacity - 1) / capacity;
-        const double cost = (double)waves * ((double)r + 0.7);      // two halo rows cost about a third of a row each
+        // two halo rows cost about a third of a row each.  Blume-Capel: half a wave on top -- its blocks (random table
+        // look-ups) finish unevenly, and one wave of long blocks loses to four waves of short ones (L = 2^14: R = 32
+        // 990, R = 8 1100 updates/ns); the Ising kernels lose with that term (measured, profiles/r02_README.md)
+        const double cost = ((double)waves + wave_slack) * ((double)r + 0.7);
         if (best == 0.0 || cost <= best) { best = cost; best_r = r; }
     }
     h->rows_per_thread = (int)best_r;
